@@ -1,0 +1,148 @@
+/*
+ * ctqmc.h — C ABI of the B200-native CT-HYB local-trace library (libctqmc_b200.so).
+ *
+ * The library evaluates, for many Monte-Carlo configurations per call, the local impurity trace of the
+ * hybridisation-expansion solver of arXiv:2010.08482 (ComCTQMC),
+ *
+ *     w_loc(C) = sum_{q0} Tr P_{beta-tau_L}(q_L) F_{alpha_L}(q_{L-1}) ... F_{alpha_1}(q_0) P_{tau_1}(q_0)      (Eq. 65)
+ *
+ * with P_tau(q) = diag(exp(-tau E_q[n])) the propagator in the eigenbasis of H_loc, F_alpha(q) the dense
+ * sector-to-sector blocks of c_f / c^dag_f, and s_alpha(q) the sector map with its "zero sector"
+ * (PAPER.md:534); and the lazy-trace upper bound built from submultiplicative norms of the factors.
+ *
+ * Everything on the path runs in sm_100a CUDA kernels; there is no CPU fallback.  All functions return 0 on success or
+ * a negative CTQMC_ERR_* code; on error nothing has been written to the outputs.  `ctqmc_last_error()` gives the text.
+ *
+ * Pointer conventions are stated per argument: HOST = ordinary host memory, DEVICE = device memory of the GPU the
+ * impurity was loaded on (e.g. a torch tensor's data_ptr()).
+ */
+#ifndef CTQMC_H
+#define CTQMC_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define CTQMC_OK               0
+#define CTQMC_ERR_ARG         -1   /* null pointer, bad size, inconsistent description */
+#define CTQMC_ERR_OOM         -2   /* device or host allocation failed */
+#define CTQMC_ERR_CUDA        -3   /* a CUDA call or kernel launch failed */
+#define CTQMC_ERR_UNSUPPORTED -4   /* valid request the library does not implement (e.g. spectral norm with segment_len != 1) */
+
+/* Per-configuration status values written to `status[b]`. */
+#define CTQMC_STATUS_OK        0
+#define CTQMC_STATUS_VANISHING 1   /* no start sector survives the sector map: w_loc = 0 structurally */
+#define CTQMC_STATUS_INVALID   2   /* symbol out of range, tau decreasing or outside [0, beta): outputs are NaN */
+
+/* Schedules for ctqmc_set_option(CTQMC_OPT_SCHEDULE, ...). */
+#define CTQMC_SCHEDULE_THIN    0   /* default: start each string at its smallest sector (exact by cyclicity of the trace) */
+#define CTQMC_SCHEDULE_LITERAL 1   /* start at q0 and carry dim(q0) columns, the literal order of Eq. 65 */
+
+#define CTQMC_OPT_SCHEDULE     1
+#define CTQMC_OPT_PANEL_WIDTH  2   /* columns carried per work unit: 8, 16, 32 (0 = automatic) */
+
+typedef struct ctqmc_impurity ctqmc_impurity;   /* opaque; created by ctqmc_load_impurity, destroyed by ctqmc_free_impurity */
+
+/*
+ * Description of the impurity in the eigenbasis of H_loc (sector decomposition and per-sector
+ * diagonalisation are done once at initialisation, by the caller).  All pointers are HOST memory; the library copies
+ * what it needs and the caller keeps ownership.
+ */
+typedef struct {
+  int32_t        n_sectors;    /* Q >= 1 (Eq. 64) */
+  const int32_t* dim;          /* [Q] sector dimensions, each >= 1 */
+  const double*  energy;       /* [sum dim] eigenvalues of H_loc, sector-major; any finite values */
+  int32_t        n_symbols;    /* A: number of operator symbols alpha; for c / c^dag: alpha = 2*flavour + (1 if creation) */
+  int32_t        is_complex;   /* 0: block data are doubles; 1: interleaved (re, im) pairs of doubles */
+  int64_t        n_blocks;     /* number of non-zero sector-to-sector blocks; at most one per (symbol, src) */
+  const int32_t* blk_symbol;   /* [n_blocks] alpha */
+  const int32_t* blk_src;      /* [n_blocks] q          */
+  const int32_t* blk_dst;      /* [n_blocks] s_alpha(q);  (symbol, src) pairs without a block map to the zero sector */
+  const int64_t* blk_offset;   /* [n_blocks] element offset of the block inside blk_data */
+  const void*    blk_data;     /* per block: column-major dim[dst] x dim[src]; element (m,n) = < m in dst | O_alpha | n in src > */
+} ctqmc_impurity_desc;
+
+/*
+ * A batch of configurations in CSR form.  A configuration is a time-ordered operator string
+ * (alpha_1, tau_1), ..., (alpha_L, tau_L) with 0 <= tau_1 <= ... <= tau_L < beta; index 0 acts first (rightmost in
+ * PAPER.md:519, Eq. 63).  The library applies no time-ordering sign (the caller passes ordered operators).
+ * L = 0 is legal and yields Z = sum_n exp(-beta E_n).
+ */
+typedef struct {
+  int64_t        n_configs;    /* B >= 0 */
+  const int64_t* offset;       /* [B+1], offset[0] = 0, non-decreasing */
+  const int32_t* symbol;       /* [offset[B]] */
+  const double*  tau;          /* [offset[B]] */
+} ctqmc_batch;
+
+/* Load an impurity onto CUDA device `device`: copies dims / energies, builds the routing table s_alpha(q), the padded
+ * row-major operator store and the per-block norm tables (row-norm^2, Frobenius, spectral) with device kernels.
+ * Errors: CTQMC_ERR_ARG for Q < 1, dim < 1, non-finite energy, block indices out of range, duplicate (symbol, src). */
+int ctqmc_load_impurity(const ctqmc_impurity_desc* desc, int device, ctqmc_impurity** out);
+
+void ctqmc_free_impurity(ctqmc_impurity* imp);
+
+/* Tuning knobs (CTQMC_OPT_*); affects subsequent batch calls on this handle.  Results are independent of them up to
+ * floating-point rounding. */
+int ctqmc_set_option(ctqmc_impurity* imp, int option, int64_t value);
+
+/*
+ * Evaluate w_loc (Eq. 65) for every configuration of the batch.  `batch` fields and all outputs are DEVICE pointers.
+ * The call only enqueues work on `cuda_stream` (a cudaStream_t, NULL = default stream) and returns; outputs are valid
+ * once the stream reaches that point.  The scratch arena is (re)allocated before enqueueing if the batch needs more
+ * than any previous call did (allocation synchronises the device, hence it never happens mid-call).
+ *
+ *   mant    [B][2]  (re, im) mantissa; im = 0 for real impurities; max(|re|,|im|) in [1,2), or (0,0) for an exact zero,
+ *                   or (NaN, NaN) for status 2
+ *   exp2    [B]     w_loc = (mant_re + i mant_im) * 2^exp2   (running exponent: long chains neither overflow nor underflow)
+ *   survive [B][Q]  or NULL: 1 iff the sector string starting at q0 never hits the zero sector
+ *   status  [B]     CTQMC_STATUS_*
+ */
+int ctqmc_trace_batch(ctqmc_impurity* imp, double beta, const ctqmc_batch* batch,
+                      double* mant, int64_t* exp2, uint8_t* survive, int32_t* status, void* cuda_stream);
+
+/*
+ * Upper bounds on |w_loc| from submultiplicative norms.  With the cyclic factorisation
+ * A_i = P_{Delta_i}(q_i) F_{alpha_i}(q_{i-1}), Delta_i = tau_{i+1} - tau_i, Delta_L = beta - tau_L + tau_1, and segments
+ * G_j of `segment_len` consecutive factors (0 = the whole chain, i.e. one segment):
+ *
+ *   norm_kind 0 (Frobenius):  B(q0) = sqrt(d_min) * prod_j ||G_j||_F
+ *   norm_kind 1 (spectral):   B(q0) = d_min * prod_i exp(-Delta_i Emin(q_i)) sigma_max(F_{alpha_i}(q_{i-1}))   (segment_len 1 only)
+ *
+ * with d_min the smallest sector dimension along the string; the configuration's bound is sum_{q0} B(q0).  All values
+ * are rounded outward by (1 + 2^-40), so bound >= |w_loc| holds for the returned numbers.
+ *
+ *   bound_mant [B], bound_exp2 [B]                   bound = mant * 2^exp2, mant in [1,2) or 0
+ *   sector_bound_mant [B][Q], sector_bound_exp2 [B][Q]   or NULL: B(q0), zero where q0 does not survive
+ *   status [B]                                        as for ctqmc_trace_batch
+ */
+int ctqmc_bound_batch(ctqmc_impurity* imp, double beta, const ctqmc_batch* batch, int norm_kind, int segment_len,
+                      double* bound_mant, int64_t* bound_exp2, double* sector_bound_mant, int64_t* sector_bound_exp2,
+                      int32_t* status, void* cuda_stream);
+
+/*
+ * Host-buffer convenience forms: identical results, but `batch` fields and all outputs are HOST pointers.  The library
+ * copies the batch to the device, runs the same kernels, copies the results back and synchronises the stream before
+ * returning (this is the end-to-end path bench.py times).
+ */
+int ctqmc_trace_batch_host(ctqmc_impurity* imp, double beta, const ctqmc_batch* batch,
+                           double* mant, int64_t* exp2, uint8_t* survive, int32_t* status, void* cuda_stream);
+int ctqmc_bound_batch_host(ctqmc_impurity* imp, double beta, const ctqmc_batch* batch, int norm_kind, int segment_len,
+                           double* bound_mant, int64_t* bound_exp2, double* sector_bound_mant, int64_t* sector_bound_exp2,
+                           int32_t* status, void* cuda_stream);
+
+/* Counters of the most recent batch call on this handle (HOST outputs; synchronises the stream it ran on):
+ * stats[0] = surviving strings, stats[1] = work units, stats[2] = kernels launched by the call,
+ * stats[3] = real multiply-adds executed by the chain kernel (padded tiles included),
+ * stats[4] = algorithmic real flops of the schedule executed (2 per real MAC, 8 per complex MAC, unpadded dims). */
+int ctqmc_last_stats(ctqmc_impurity* imp, int64_t stats[8]);
+
+/* Thread-local description of the last error on this thread ("" if none). */
+const char* ctqmc_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CTQMC_H */

@@ -1,0 +1,605 @@
+// C ABI of libctqmc_b200 (include/ctqmc.h): host-side validation, device store construction, scratch arena and the
+// kernel sequence of ctqmc_trace_batch / ctqmc_bound_batch.  sm_100a only; there is no CPU fallback anywhere.
+#include "../../include/ctqmc.h"
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "chain.cuh"
+#include "chain_large.cuh"
+#include "common.cuh"
+#include "reduce.cuh"
+#include "route.cuh"
+#include "store.cuh"
+
+using namespace ctqmc;
+
+namespace {
+
+thread_local std::string g_err;
+
+int fail(int code, const char* fmt, ...) {
+  char buf[512];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof buf, fmt, ap);
+  va_end(ap);
+  g_err = buf;
+  return code;
+}
+
+#define CU(call)                                                                                   \
+  do {                                                                                             \
+    cudaError_t e_ = (call);                                                                       \
+    if (e_ != cudaSuccess)                                                                         \
+      return fail(e_ == cudaErrorMemoryAllocation ? CTQMC_ERR_OOM : CTQMC_ERR_CUDA, "%s: %s (%s:%d)", #call, \
+                  cudaGetErrorString(e_), __FILE__, __LINE__);                                     \
+  } while (0)
+
+template <class T>
+int upload(T** dst, const std::vector<T>& v) {
+  *dst = nullptr;
+  size_t bytes = (v.size() ? v.size() : 1) * sizeof(T);
+  CU(cudaMalloc((void**)dst, bytes));
+  if (!v.empty()) CU(cudaMemcpy(*dst, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice));
+  return 0;
+}
+
+struct Arena {
+  long long cap_strings = 0, cap_units = 0, cap_configs = 0;
+  int* status = nullptr;
+  uint8_t* survive = nullptr;
+  StringRec* strings = nullptr;
+  int2* units = nullptr;
+  Slot* slots = nullptr;
+  Scaled* sector = nullptr;
+  Counters* cnt = nullptr;
+  double* xscratch = nullptr;   // large-sector path: per-CTA global ping-pong panels
+  size_t xscratch_bytes = 0;
+  // host-variant staging
+  void* h_stage = nullptr; size_t h_stage_bytes = 0;
+  void* d_stage = nullptr; size_t d_stage_bytes = 0;
+};
+
+}  // namespace
+
+struct ctqmc_impurity {
+  int device = 0;
+  int sm_count = 0;
+  DevImp dev{};
+  int n_blocks = 0;
+  // owned device arrays
+  int* d_dim = nullptr; long long* d_eoff = nullptr; double* d_energy = nullptr; double* d_emin = nullptr;
+  int* d_blkof = nullptr; BlkDesc* d_blks = nullptr; double* d_store = nullptr; double* d_rownorm2 = nullptr;
+  double* d_sigma = nullptr;
+  // schedule
+  int schedule = CTQMC_SCHEDULE_THIN;
+  int nt = 0, team_warps = 8, ldx = 0, large = 0;
+  size_t smem_bytes = 0;
+  int grid = 0;
+  Arena arena;
+  cudaStream_t last_stream = nullptr;
+  long long last_launches = 0;
+};
+
+namespace {
+
+using KernelFn = void (*)(ChainParams);
+
+KernelFn pick_kernel(int cplx, int nt, int tw) {
+#define PICK(C, N, T) if (cplx == C && nt == N && tw == T) return chain_kernel<(C != 0), N, T>;
+  PICK(0, 1, 1) PICK(0, 2, 1) PICK(1, 1, 1) PICK(1, 2, 1)
+  PICK(0, 1, 8) PICK(0, 2, 8) PICK(0, 4, 8)
+  PICK(1, 1, 8) PICK(1, 2, 8) PICK(1, 4, 8)
+#undef PICK
+  return nullptr;
+}
+
+int pick_ldx(int cplx, int dmax) {
+  int l = (dmax + 7) / 8 * 8;
+  if (cplx) { while (l % 8 != 4) ++l; }       // 16-byte elements: conflict-free 128-bit fragment loads need ldx = 4 mod 8
+  else      { while (l % 16 != 8) ++l; }      // 8-byte elements, two per load: ldx = 8 mod 16
+  return l;
+}
+
+// Choose panel width / team size for this impurity and set up the persistent grid.
+int configure(ctqmc_impurity* h, int want_w) {
+  const int cplx = h->dev.cplx, es = cplx ? 2 : 1;
+  const size_t smem_max = 227 * 1024 - 2048;
+  h->ldx = pick_ldx(cplx, h->dev.dmax);
+  h->team_warps = h->dev.dmax <= 16 ? 1 : 8;
+  const int teams = kCtaWarps / h->team_warps;
+  int nt_try[3] = {4, 2, 1};
+  h->nt = 0;
+  for (int i = 0; i < 3; ++i) {
+    int nt = nt_try[i];
+    if (want_w && nt * 8 != want_w) continue;
+    if (!pick_kernel(cplx, nt, h->team_warps)) continue;
+    size_t bytes = (size_t)teams * 2 * (8 * nt) * h->ldx * es * sizeof(double);
+    if (bytes <= smem_max) { h->nt = nt; h->smem_bytes = bytes; break; }
+  }
+  h->large = (h->nt == 0);
+  if (h->large) return large_configure(h->dev, h->sm_count, &h->grid, &h->smem_bytes, &h->nt);
+  KernelFn fn = pick_kernel(cplx, h->nt, h->team_warps);
+  CU(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_bytes));
+  int occ = 0;
+  CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, kCtaThreads, h->smem_bytes));
+  if (occ < 1) return fail(CTQMC_ERR_CUDA, "chain kernel does not fit on an SM (smem %zu)", h->smem_bytes);
+  h->grid = occ * h->sm_count;
+  return 0;
+}
+
+int ensure_arena(ctqmc_impurity* h, long long B, long long units_per_string) {
+  Arena& a = h->arena;
+  const long long n_strings = B * h->dev.Q;
+  const long long n_units = n_strings * units_per_string;
+  if (!a.cnt) CU(cudaMalloc((void**)&a.cnt, sizeof(Counters)));
+  if (B > a.cap_configs) {
+    cudaFree(a.status);
+    CU(cudaMalloc((void**)&a.status, (size_t)(B ? B : 1) * sizeof(int)));
+    a.cap_configs = B;
+  }
+  if (n_strings > a.cap_strings) {
+    cudaFree(a.survive); cudaFree(a.strings); cudaFree(a.sector);
+    a.survive = nullptr; a.strings = nullptr; a.sector = nullptr; a.cap_strings = 0;
+    size_t n = (size_t)(n_strings ? n_strings : 1);
+    CU(cudaMalloc((void**)&a.survive, n));
+    CU(cudaMalloc((void**)&a.strings, n * sizeof(StringRec)));
+    CU(cudaMalloc((void**)&a.sector, n * sizeof(Scaled)));
+    a.cap_strings = n_strings;
+  }
+  if (n_units > a.cap_units) {
+    cudaFree(a.units); cudaFree(a.slots);
+    a.units = nullptr; a.slots = nullptr; a.cap_units = 0;
+    size_t n = (size_t)(n_units ? n_units : 1);
+    CU(cudaMalloc((void**)&a.units, n * sizeof(int2)));
+    CU(cudaMalloc((void**)&a.slots, n * sizeof(Slot)));
+    a.cap_units = n_units;
+  }
+  return 0;
+}
+
+int check_batch_args(const ctqmc_impurity* h, double beta, const ctqmc_batch* batch) {
+  if (!h || !batch) return fail(CTQMC_ERR_ARG, "null impurity or batch");
+  if (!(beta > 0.0) || !std::isfinite(beta)) return fail(CTQMC_ERR_ARG, "beta must be positive and finite");
+  if (batch->n_configs < 0) return fail(CTQMC_ERR_ARG, "n_configs < 0");
+  if (batch->n_configs > 0 && (!batch->offset)) return fail(CTQMC_ERR_ARG, "batch.offset is null");
+  if (batch->n_configs * (long long)h->dev.Q > 2000000000LL) return fail(CTQMC_ERR_ARG, "n_configs * n_sectors exceeds 2^31");
+  return 0;
+}
+
+// validate -> route -> class scan -> unit scatter; leaves strings / units / counters ready.
+int enqueue_routing(ctqmc_impurity* h, const BatchView& bv, uint8_t* survive_out, int mode, int segment_len, cudaStream_t st) {
+  Arena& a = h->arena;
+  const long long B = bv.B, nS = B * h->dev.Q;
+  CU(cudaMemsetAsync(a.cnt, 0, sizeof(Counters), st));
+  validate_kernel<<<(unsigned)((B + 255) / 256), 256, 0, st>>>(bv, h->dev.A, a.status);
+  RouteParams rp;
+  rp.imp = h->dev; rp.bv = bv; rp.status = a.status; rp.survive = a.survive; rp.survive_out = survive_out;
+  rp.strings = a.strings; rp.cnt = a.cnt; rp.W = 8 * h->nt; rp.kstep = h->dev.cplx ? 4 : 8;
+  rp.literal = (h->schedule == CTQMC_SCHEDULE_LITERAL); rp.flops_per_mac = h->dev.cplx ? 8 : 2;
+  rp.mode = mode; rp.segment_len = segment_len;
+  route_kernel<<<(unsigned)((nS + 255) / 256), 256, 0, st>>>(rp);
+  h->last_launches += 2;
+  if (mode != 2) {
+    class_scan_kernel<<<1, 32, 0, st>>>(a.cnt);
+    unit_scatter_kernel<<<(unsigned)((nS + 255) / 256), 256, 0, st>>>(a.strings, nS, a.cnt, a.units);
+    h->last_launches += 2;
+  }
+  CU(cudaGetLastError());
+  return 0;
+}
+
+int enqueue_chain(ctqmc_impurity* h, const BatchView& bv, int mode, int segment_len, cudaStream_t st) {
+  Arena& a = h->arena;
+  ChainParams cp;
+  cp.imp = h->dev; cp.bv = bv; cp.strings = a.strings; cp.units = a.units; cp.cnt = a.cnt; cp.slots = a.slots;
+  cp.ldx = h->ldx; cp.mode = mode; cp.segment_len = segment_len;
+  if (h->large) {
+    int rc = large_enqueue(cp, h->grid, h->smem_bytes, h->nt, a.xscratch, st);
+    if (rc) return fail(rc, "large-sector chain kernel launch failed");
+  } else {
+    KernelFn fn = pick_kernel(h->dev.cplx, h->nt, h->team_warps);
+    fn<<<h->grid, kCtaThreads, h->smem_bytes, st>>>(cp);
+  }
+  h->last_launches += 1;
+  CU(cudaGetLastError());
+  return 0;
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------------ load / free
+extern "C" int ctqmc_load_impurity(const ctqmc_impurity_desc* desc, int device, ctqmc_impurity** out) {
+  if (!desc || !out) return fail(CTQMC_ERR_ARG, "null desc or out");
+  *out = nullptr;
+  const int Q = desc->n_sectors, A = desc->n_symbols;
+  if (Q < 1 || A < 1 || !desc->dim || !desc->energy) return fail(CTQMC_ERR_ARG, "need n_sectors >= 1, n_symbols >= 1, dim, energy");
+  if (desc->n_blocks < 0 || desc->n_blocks > 65535) return fail(CTQMC_ERR_ARG, "n_blocks out of range [0, 65535]");
+  if (desc->n_blocks > 0 && (!desc->blk_symbol || !desc->blk_src || !desc->blk_dst || !desc->blk_offset || !desc->blk_data))
+    return fail(CTQMC_ERR_ARG, "null block arrays");
+  const int cplx = desc->is_complex ? 1 : 0, es = cplx ? 2 : 1;
+  std::vector<int> dim(desc->dim, desc->dim + Q);
+  std::vector<long long> eoff(Q);
+  long long ne = 0;
+  int dmax = 0;
+  for (int q = 0; q < Q; ++q) {
+    if (dim[q] < 1) return fail(CTQMC_ERR_ARG, "dim[%d] = %d < 1", q, dim[q]);
+    eoff[q] = ne; ne += dim[q];
+    if (dim[q] > dmax) dmax = dim[q];
+  }
+  std::vector<double> energy(desc->energy, desc->energy + ne), emin(Q);
+  for (int q = 0; q < Q; ++q) {
+    double m = INFINITY;
+    for (int n = 0; n < dim[q]; ++n) {
+      double e = energy[eoff[q] + n];
+      if (!std::isfinite(e)) return fail(CTQMC_ERR_ARG, "non-finite eigenvalue in sector %d", q);
+      if (e < m) m = e;
+    }
+    emin[q] = m;
+  }
+  const int nb = (int)desc->n_blocks;
+  std::vector<int> blkof((size_t)A * Q, -1);
+  std::vector<BlkDesc> blks(nb);
+  std::vector<long long> raw_off(nb), v_off(nb);
+  long long store_len = 0, rn_len = 0, v_len = 0, raw_len = 0;
+  int max_rows = 1, max_cols = 1;
+  for (int b = 0; b < nb; ++b) {
+    int a = desc->blk_symbol[b], s = desc->blk_src[b], d = desc->blk_dst[b];
+    if (a < 0 || a >= A || s < 0 || s >= Q || d < 0 || d >= Q) return fail(CTQMC_ERR_ARG, "block %d: symbol/src/dst out of range", b);
+    if (blkof[(size_t)a * Q + s] != -1) return fail(CTQMC_ERR_ARG, "block %d duplicates (symbol %d, src %d)", b, a, s);
+    if (desc->blk_offset[b] < 0) return fail(CTQMC_ERR_ARG, "block %d: negative offset", b);
+    blkof[(size_t)a * Q + s] = b;
+    BlkDesc& bd = blks[b];
+    bd.rows = dim[d]; bd.cols = dim[s]; bd.dst = d; bd.src = s; bd.pad = 0;
+    bd.ld = (bd.cols + (cplx ? 3 : 7)) / (cplx ? 4 : 8) * (cplx ? 4 : 8);
+    bd.off = store_len;
+    bd.rn_off = rn_len;
+    const long long rows_pad = (bd.rows + 7) / 8 * 8;
+    store_len += rows_pad * bd.ld * es;
+    rn_len += rows_pad;
+    v_off[b] = v_len; v_len += bd.ld;
+    raw_off[b] = desc->blk_offset[b];
+    long long end = desc->blk_offset[b] + (long long)bd.rows * bd.cols;
+    if (end > raw_len) raw_len = end;
+    if (bd.rows > max_rows) max_rows = bd.rows;
+    if (bd.cols > max_cols) max_cols = bd.cols;
+  }
+
+  CU(cudaSetDevice(device));
+  ctqmc_impurity* h = new (std::nothrow) ctqmc_impurity();
+  if (!h) return fail(CTQMC_ERR_OOM, "host allocation failed");
+  h->device = device;
+  cudaDeviceProp prop;
+  cudaError_t pe = cudaGetDeviceProperties(&prop, device);
+  if (pe != cudaSuccess) { delete h; return fail(CTQMC_ERR_CUDA, "cudaGetDeviceProperties: %s", cudaGetErrorString(pe)); }
+  if (prop.major != 10) { delete h; return fail(CTQMC_ERR_UNSUPPORTED, "device is sm_%d%d; this library is built for sm_100a only", prop.major, prop.minor); }
+  h->sm_count = prop.multiProcessorCount;
+  h->n_blocks = nb;
+
+  int rc = 0;
+  double* d_raw = nullptr; long long* d_rawoff = nullptr; long long* d_voff = nullptr; double* d_v = nullptr; double* d_u = nullptr;
+  auto cleanup_tmp = [&]() { cudaFree(d_raw); cudaFree(d_rawoff); cudaFree(d_voff); cudaFree(d_v); cudaFree(d_u); };
+#define TRY(x) do { rc = (x); if (rc) { cleanup_tmp(); ctqmc_free_impurity(h); return rc; } } while (0)
+#define TRYCU(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) { rc = fail(e_ == cudaErrorMemoryAllocation ? CTQMC_ERR_OOM : CTQMC_ERR_CUDA, "%s: %s", #x, cudaGetErrorString(e_)); cleanup_tmp(); ctqmc_free_impurity(h); return rc; } } while (0)
+  TRY(upload(&h->d_dim, dim));
+  TRY(upload(&h->d_eoff, eoff));
+  TRY(upload(&h->d_energy, energy));
+  TRY(upload(&h->d_emin, emin));
+  TRY(upload(&h->d_blkof, blkof));
+  TRY(upload(&h->d_blks, blks));
+  TRY(upload(&d_rawoff, raw_off));
+  TRY(upload(&d_voff, v_off));
+  TRYCU(cudaMalloc((void**)&h->d_store, (size_t)(store_len ? store_len : 1) * sizeof(double)));
+  TRYCU(cudaMemset(h->d_store, 0, (size_t)(store_len ? store_len : 1) * sizeof(double)));
+  TRYCU(cudaMalloc((void**)&h->d_rownorm2, (size_t)(rn_len ? rn_len : 1) * sizeof(double)));
+  TRYCU(cudaMemset(h->d_rownorm2, 0, (size_t)(rn_len ? rn_len : 1) * sizeof(double)));
+  TRYCU(cudaMalloc((void**)&h->d_sigma, (size_t)(nb ? nb : 1) * sizeof(double)));
+  if (nb > 0) {
+    TRYCU(cudaMalloc((void**)&d_raw, (size_t)raw_len * es * sizeof(double)));
+    TRYCU(cudaMemcpy(d_raw, desc->blk_data, (size_t)raw_len * es * sizeof(double), cudaMemcpyHostToDevice));
+    TRYCU(cudaMalloc((void**)&d_v, (size_t)v_len * es * sizeof(double)));
+    TRYCU(cudaMalloc((void**)&d_u, (size_t)rn_len * es * sizeof(double)));
+    dim3 tb(32, 8), tg((unsigned)std::min((max_cols + 31) / 32, 64), (unsigned)std::min((max_rows + 31) / 32, 64), (unsigned)nb);
+    dim3 rg((unsigned)std::min((max_rows + 7) / 8, 512), (unsigned)nb);
+    dim3 cg((unsigned)std::min((max_cols + 127) / 128, 64), (unsigned)nb);
+    const int iters = 16;
+    if (cplx) {
+      relayout_kernel<2><<<tg, tb>>>(d_raw, d_rawoff, h->d_blks, h->d_store);
+      rownorm_kernel<2><<<rg, 256>>>(h->d_blks, h->d_store, h->d_rownorm2);
+      pi_init_kernel<2><<<nb, 128>>>(h->d_blks, d_voff, d_v);
+      pi_norm_kernel<<<nb, 256>>>(h->d_blks, d_voff, 0, 2, d_v, 1, nullptr);
+      for (int it = 0; it < iters; ++it) {
+        pi_fv_kernel<2><<<rg, 256>>>(h->d_blks, h->d_store, d_voff, d_v, d_u);
+        pi_fhu_kernel<2><<<cg, 128>>>(h->d_blks, h->d_store, d_voff, d_u, d_v);
+        pi_norm_kernel<<<nb, 256>>>(h->d_blks, d_voff, 0, 2, d_v, 1, nullptr);
+      }
+      pi_fv_kernel<2><<<rg, 256>>>(h->d_blks, h->d_store, d_voff, d_v, d_u);
+      pi_norm_kernel<<<nb, 256>>>(h->d_blks, d_voff, 1, 2, d_u, 0, h->d_sigma);
+    } else {
+      relayout_kernel<1><<<tg, tb>>>(d_raw, d_rawoff, h->d_blks, h->d_store);
+      rownorm_kernel<1><<<rg, 256>>>(h->d_blks, h->d_store, h->d_rownorm2);
+      pi_init_kernel<1><<<nb, 128>>>(h->d_blks, d_voff, d_v);
+      pi_norm_kernel<<<nb, 256>>>(h->d_blks, d_voff, 0, 1, d_v, 1, nullptr);
+      for (int it = 0; it < iters; ++it) {
+        pi_fv_kernel<1><<<rg, 256>>>(h->d_blks, h->d_store, d_voff, d_v, d_u);
+        pi_fhu_kernel<1><<<cg, 128>>>(h->d_blks, h->d_store, d_voff, d_u, d_v);
+        pi_norm_kernel<<<nb, 256>>>(h->d_blks, d_voff, 0, 1, d_v, 1, nullptr);
+      }
+      pi_fv_kernel<1><<<rg, 256>>>(h->d_blks, h->d_store, d_voff, d_v, d_u);
+      pi_norm_kernel<<<nb, 256>>>(h->d_blks, d_voff, 1, 1, d_u, 0, h->d_sigma);
+    }
+    TRYCU(cudaGetLastError());
+    TRYCU(cudaDeviceSynchronize());
+  }
+  cleanup_tmp();
+  d_raw = nullptr; d_rawoff = nullptr; d_voff = nullptr; d_v = nullptr; d_u = nullptr;
+
+  h->dev.Q = Q; h->dev.A = A; h->dev.cplx = cplx; h->dev.dmax = dmax;
+  h->dev.dim = h->d_dim; h->dev.e_off = h->d_eoff; h->dev.energy = h->d_energy; h->dev.e_min = h->d_emin;
+  h->dev.blk_of = h->d_blkof; h->dev.blks = h->d_blks; h->dev.store = h->d_store; h->dev.rownorm2 = h->d_rownorm2;
+  h->dev.sigma = h->d_sigma;
+  TRY(configure(h, 0));
+#undef TRY
+#undef TRYCU
+  *out = h;
+  return 0;
+}
+
+extern "C" void ctqmc_free_impurity(ctqmc_impurity* h) {
+  if (!h) return;
+  cudaSetDevice(h->device);
+  cudaFree(h->d_dim); cudaFree(h->d_eoff); cudaFree(h->d_energy); cudaFree(h->d_emin); cudaFree(h->d_blkof);
+  cudaFree(h->d_blks); cudaFree(h->d_store); cudaFree(h->d_rownorm2); cudaFree(h->d_sigma);
+  Arena& a = h->arena;
+  cudaFree(a.status); cudaFree(a.survive); cudaFree(a.strings); cudaFree(a.units); cudaFree(a.slots); cudaFree(a.sector);
+  cudaFree(a.cnt); cudaFree(a.xscratch); cudaFree(a.d_stage);
+  if (a.h_stage) cudaFreeHost(a.h_stage);
+  delete h;
+}
+
+extern "C" int ctqmc_set_option(ctqmc_impurity* h, int option, int64_t value) {
+  if (!h) return fail(CTQMC_ERR_ARG, "null impurity");
+  CU(cudaSetDevice(h->device));
+  if (option == CTQMC_OPT_SCHEDULE) {
+    if (value != CTQMC_SCHEDULE_THIN && value != CTQMC_SCHEDULE_LITERAL) return fail(CTQMC_ERR_ARG, "unknown schedule %lld", (long long)value);
+    h->schedule = (int)value;
+    return 0;
+  }
+  if (option == CTQMC_OPT_PANEL_WIDTH) {
+    if (value != 0 && value != 8 && value != 16 && value != 32) return fail(CTQMC_ERR_ARG, "panel width must be 0, 8, 16 or 32");
+    if (h->large) return 0;
+    int nt = h->nt, tw = h->team_warps, ldx = h->ldx, grid = h->grid; size_t sm = h->smem_bytes;
+    int rc = configure(h, (int)value);
+    if (rc || h->large) { h->nt = nt; h->team_warps = tw; h->ldx = ldx; h->grid = grid; h->smem_bytes = sm; h->large = 0;
+                          return rc ? rc : fail(CTQMC_ERR_UNSUPPORTED, "panel width %lld does not fit in shared memory for this impurity", (long long)value); }
+    return 0;
+  }
+  return fail(CTQMC_ERR_ARG, "unknown option %d", option);
+}
+
+// ------------------------------------------------------------------------------------------------ batch calls
+extern "C" int ctqmc_trace_batch(ctqmc_impurity* h, double beta, const ctqmc_batch* batch, double* mant, int64_t* exp2,
+                                 uint8_t* survive, int32_t* status, void* cuda_stream) {
+  int rc = check_batch_args(h, beta, batch);
+  if (rc) return rc;
+  const long long B = batch->n_configs;
+  if (B == 0) return 0;
+  if (!mant || !exp2 || !status) return fail(CTQMC_ERR_ARG, "null output (mant, exp2 and status are required)");
+  CU(cudaSetDevice(h->device));
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const int W = 8 * h->nt;
+  rc = ensure_arena(h, B, (h->dev.dmax + W - 1) / W);
+  if (rc) return rc;
+  if (h->large) { rc = large_ensure_scratch(h->dev, h->grid, h->nt, &h->arena.xscratch, &h->arena.xscratch_bytes); if (rc) return fail(rc, "scratch allocation failed"); }
+  h->last_stream = st; h->last_launches = 0;
+  BatchView bv; bv.B = B; bv.offset = (const long long*)batch->offset; bv.symbol = batch->symbol; bv.tau = batch->tau; bv.beta = beta;
+  rc = enqueue_routing(h, bv, survive, 0, 0, st);
+  if (rc) return rc;
+  rc = enqueue_chain(h, bv, 0, 0, st);
+  if (rc) return rc;
+  TraceReduceParams tp;
+  tp.B = B; tp.Q = h->dev.Q; tp.status_in = h->arena.status; tp.survive = h->arena.survive; tp.strings = h->arena.strings;
+  tp.slots = h->arena.slots; tp.mant = mant; tp.exp2 = (long long*)exp2; tp.status = status;
+  trace_reduce_kernel<<<(unsigned)((B + 127) / 128), 128, 0, st>>>(tp);
+  h->last_launches += 1;
+  CU(cudaGetLastError());
+  return 0;
+}
+
+extern "C" int ctqmc_bound_batch(ctqmc_impurity* h, double beta, const ctqmc_batch* batch, int norm_kind, int segment_len,
+                                 double* bound_mant, int64_t* bound_exp2, double* sector_bound_mant,
+                                 int64_t* sector_bound_exp2, int32_t* status, void* cuda_stream) {
+  int rc = check_batch_args(h, beta, batch);
+  if (rc) return rc;
+  if (norm_kind != 0 && norm_kind != 1) return fail(CTQMC_ERR_ARG, "norm_kind must be 0 (Frobenius) or 1 (spectral)");
+  if (segment_len < 0) return fail(CTQMC_ERR_ARG, "segment_len < 0");
+  if (norm_kind == 1 && segment_len != 1)
+    return fail(CTQMC_ERR_UNSUPPORTED, "spectral norm is implemented for segment_len = 1 only");
+  if ((sector_bound_mant == nullptr) != (sector_bound_exp2 == nullptr)) return fail(CTQMC_ERR_ARG, "sector_bound_mant / _exp2 must both be given or both be null");
+  const long long B = batch->n_configs;
+  if (B == 0) return 0;
+  if (!bound_mant || !bound_exp2 || !status) return fail(CTQMC_ERR_ARG, "null output");
+  if (segment_len != 1 && h->large) return fail(CTQMC_ERR_UNSUPPORTED, "segment_len != 1 is not implemented for sectors that do not fit in shared memory");
+  CU(cudaSetDevice(h->device));
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const int W = 8 * h->nt;
+  const long long nS = B * h->dev.Q;
+  BatchView bv; bv.B = B; bv.offset = (const long long*)batch->offset; bv.symbol = batch->symbol; bv.tau = batch->tau; bv.beta = beta;
+  h->last_stream = st; h->last_launches = 0;
+  BoundParams bp;
+  if (segment_len == 1) {
+    rc = ensure_arena(h, B, 1);
+    if (rc) return rc;
+    rc = enqueue_routing(h, bv, nullptr, 2, 1, st);
+    if (rc) return rc;
+    bp.imp = h->dev; bp.bv = bv; bp.survive = h->arena.survive; bp.strings = h->arena.strings; bp.slots = h->arena.slots;
+    bp.sector = h->arena.sector; bp.norm_kind = norm_kind; bp.segment_len = 1; bp.W = W;
+    bound_s1_kernel<<<(unsigned)((nS * 32 + 255) / 256), 256, 0, st>>>(bp);
+    h->last_launches += 1;
+  } else {
+    // units per string depend on the chain lengths, which live on the device: one small read-back of the total
+    // operator count sizes the arena (the only host synchronisation in the library's device-pointer API).
+    long long n_ops = 0;
+    CU(cudaMemcpyAsync(&n_ops, batch->offset + B, sizeof(long long), cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    const int S = segment_len == 0 ? 1 << 30 : segment_len;
+    const long long panels = (h->dev.dmax + W - 1) / W;
+    long long max_units_per_string = (segment_len == 0) ? panels : ((n_ops / S) / (B ? 1 : 1) + 1) * panels;
+    // worst case: one configuration holds every operator
+    rc = ensure_arena(h, B, 1);
+    if (rc) return rc;
+    {
+      // exact sizing would need the per-configuration lengths; bound it by sum over configurations instead:
+      // sum_b Q * (L_b / S + 1) * panels <= Q * panels * (n_ops / S + B)
+      long long need = (long long)h->dev.Q * panels * ((segment_len == 0 ? 0 : n_ops / S) + B);
+      Arena& a = h->arena;
+      if (need > a.cap_units) {
+        cudaFree(a.units); cudaFree(a.slots); a.units = nullptr; a.slots = nullptr; a.cap_units = 0;
+        CU(cudaMalloc((void**)&a.units, (size_t)need * sizeof(int2)));
+        CU(cudaMalloc((void**)&a.slots, (size_t)need * sizeof(Slot)));
+        a.cap_units = need;
+      }
+      (void)max_units_per_string;
+    }
+    rc = enqueue_routing(h, bv, nullptr, 1, S, st);
+    if (rc) return rc;
+    rc = enqueue_chain(h, bv, 1, S, st);
+    if (rc) return rc;
+    bp.imp = h->dev; bp.bv = bv; bp.survive = h->arena.survive; bp.strings = h->arena.strings; bp.slots = h->arena.slots;
+    bp.sector = h->arena.sector; bp.norm_kind = 0; bp.segment_len = S; bp.W = W;
+    bound_segments_kernel<<<(unsigned)((nS + 127) / 128), 128, 0, st>>>(bp);
+    h->last_launches += 1;
+  }
+  BoundReduceParams rp;
+  rp.B = B; rp.Q = h->dev.Q; rp.status_in = h->arena.status; rp.survive = h->arena.survive; rp.sector = h->arena.sector;
+  rp.bound_mant = bound_mant; rp.bound_exp2 = (long long*)bound_exp2; rp.sector_mant = sector_bound_mant;
+  rp.sector_exp2 = (long long*)sector_bound_exp2; rp.status = status;
+  bound_reduce_kernel<<<(unsigned)((B + 127) / 128), 128, 0, st>>>(rp);
+  h->last_launches += 1;
+  CU(cudaGetLastError());
+  return 0;
+}
+
+// ------------------------------------------------------------------------------------------------ host-buffer forms
+namespace {
+
+struct Staged {
+  ctqmc_batch dev_batch;
+  char* d_out = nullptr;   // device outputs region
+  char* h_out = nullptr;   // pinned mirror
+};
+
+size_t align_up(size_t x) { return (x + 255) / 256 * 256; }
+
+int stage_in(ctqmc_impurity* h, const ctqmc_batch* hb, size_t out_bytes, Staged* sg, cudaStream_t st) {
+  const long long B = hb->n_configs;
+  if (!hb->offset) return fail(CTQMC_ERR_ARG, "batch.offset is null");
+  const long long n_ops = hb->offset[B];
+  if (n_ops < 0) return fail(CTQMC_ERR_ARG, "negative operator count");
+  if (n_ops > 0 && (!hb->symbol || !hb->tau)) return fail(CTQMC_ERR_ARG, "null symbol / tau");
+  const size_t b_off = align_up((size_t)(B + 1) * 8), b_sym = align_up((size_t)n_ops * 4), b_tau = align_up((size_t)n_ops * 8);
+  const size_t total = b_off + b_sym + b_tau + align_up(out_bytes);
+  Arena& a = h->arena;
+  if (total > a.d_stage_bytes) {
+    cudaFree(a.d_stage); a.d_stage = nullptr; a.d_stage_bytes = 0;
+    if (a.h_stage) cudaFreeHost(a.h_stage);
+    a.h_stage = nullptr; a.h_stage_bytes = 0;
+    CU(cudaMalloc(&a.d_stage, total));
+    CU(cudaMallocHost(&a.h_stage, total));
+    a.d_stage_bytes = total; a.h_stage_bytes = total;
+  }
+  char* hs = (char*)a.h_stage; char* ds = (char*)a.d_stage;
+  memcpy(hs, hb->offset, (size_t)(B + 1) * 8);
+  if (n_ops) { memcpy(hs + b_off, hb->symbol, (size_t)n_ops * 4); memcpy(hs + b_off + b_sym, hb->tau, (size_t)n_ops * 8); }
+  CU(cudaMemcpyAsync(ds, hs, b_off + b_sym + b_tau, cudaMemcpyHostToDevice, st));
+  sg->dev_batch.n_configs = B;
+  sg->dev_batch.offset = (const int64_t*)ds;
+  sg->dev_batch.symbol = (const int32_t*)(ds + b_off);
+  sg->dev_batch.tau = (const double*)(ds + b_off + b_sym);
+  sg->d_out = ds + b_off + b_sym + b_tau;
+  sg->h_out = hs + b_off + b_sym + b_tau;
+  return 0;
+}
+
+}  // namespace
+
+extern "C" int ctqmc_trace_batch_host(ctqmc_impurity* h, double beta, const ctqmc_batch* batch, double* mant, int64_t* exp2,
+                                      uint8_t* survive, int32_t* status, void* cuda_stream) {
+  int rc = check_batch_args(h, beta, batch);
+  if (rc) return rc;
+  const long long B = batch->n_configs;
+  if (B == 0) return 0;
+  if (!mant || !exp2 || !status) return fail(CTQMC_ERR_ARG, "null output (mant, exp2 and status are required)");
+  CU(cudaSetDevice(h->device));
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const size_t Q = h->dev.Q;
+  const size_t o_mant = 0, o_exp = align_up(B * 16), o_stat = o_exp + align_up(B * 8), o_surv = o_stat + align_up(B * 4);
+  const size_t out_bytes = o_surv + align_up(B * Q);
+  Staged sg;
+  rc = stage_in(h, batch, out_bytes, &sg, st);
+  if (rc) return rc;
+  rc = ctqmc_trace_batch(h, beta, &sg.dev_batch, (double*)(sg.d_out + o_mant), (int64_t*)(sg.d_out + o_exp),
+                         survive ? (uint8_t*)(sg.d_out + o_surv) : nullptr, (int32_t*)(sg.d_out + o_stat), cuda_stream);
+  if (rc) return rc;
+  CU(cudaMemcpyAsync(sg.h_out, sg.d_out, survive ? out_bytes : o_surv, cudaMemcpyDeviceToHost, st));
+  CU(cudaStreamSynchronize(st));
+  memcpy(mant, sg.h_out + o_mant, B * 16);
+  memcpy(exp2, sg.h_out + o_exp, B * 8);
+  memcpy(status, sg.h_out + o_stat, B * 4);
+  if (survive) memcpy(survive, sg.h_out + o_surv, B * Q);
+  return 0;
+}
+
+extern "C" int ctqmc_bound_batch_host(ctqmc_impurity* h, double beta, const ctqmc_batch* batch, int norm_kind, int segment_len,
+                                      double* bound_mant, int64_t* bound_exp2, double* sector_bound_mant,
+                                      int64_t* sector_bound_exp2, int32_t* status, void* cuda_stream) {
+  int rc = check_batch_args(h, beta, batch);
+  if (rc) return rc;
+  const long long B = batch->n_configs;
+  if (B == 0) return 0;
+  if (!bound_mant || !bound_exp2 || !status) return fail(CTQMC_ERR_ARG, "null output");
+  if ((sector_bound_mant == nullptr) != (sector_bound_exp2 == nullptr)) return fail(CTQMC_ERR_ARG, "sector_bound_mant / _exp2 must both be given or both be null");
+  CU(cudaSetDevice(h->device));
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const size_t Q = h->dev.Q;
+  const bool sec = sector_bound_mant != nullptr;
+  const size_t o_m = 0, o_e = align_up(B * 8), o_stat = o_e + align_up(B * 8), o_sm = o_stat + align_up(B * 4),
+               o_se = o_sm + align_up(B * Q * 8);
+  const size_t out_bytes = o_se + align_up(B * Q * 8);
+  Staged sg;
+  rc = stage_in(h, batch, out_bytes, &sg, st);
+  if (rc) return rc;
+  rc = ctqmc_bound_batch(h, beta, &sg.dev_batch, norm_kind, segment_len, (double*)(sg.d_out + o_m), (int64_t*)(sg.d_out + o_e),
+                         sec ? (double*)(sg.d_out + o_sm) : nullptr, sec ? (int64_t*)(sg.d_out + o_se) : nullptr,
+                         (int32_t*)(sg.d_out + o_stat), cuda_stream);
+  if (rc) return rc;
+  CU(cudaMemcpyAsync(sg.h_out, sg.d_out, sec ? out_bytes : o_sm, cudaMemcpyDeviceToHost, st));
+  CU(cudaStreamSynchronize(st));
+  memcpy(bound_mant, sg.h_out + o_m, B * 8);
+  memcpy(bound_exp2, sg.h_out + o_e, B * 8);
+  memcpy(status, sg.h_out + o_stat, B * 4);
+  if (sec) { memcpy(sector_bound_mant, sg.h_out + o_sm, B * Q * 8); memcpy(sector_bound_exp2, sg.h_out + o_se, B * Q * 8); }
+  return 0;
+}
+
+extern "C" int ctqmc_last_stats(ctqmc_impurity* h, int64_t stats[8]) {
+  if (!h || !stats) return fail(CTQMC_ERR_ARG, "null argument");
+  for (int i = 0; i < 8; ++i) stats[i] = 0;
+  if (!h->arena.cnt) return 0;
+  CU(cudaSetDevice(h->device));
+  Counters c;
+  CU(cudaStreamSynchronize(h->last_stream));
+  CU(cudaMemcpy(&c, h->arena.cnt, sizeof c, cudaMemcpyDeviceToHost));
+  stats[0] = (int64_t)c.n_strings; stats[1] = (int64_t)c.n_slots; stats[2] = h->last_launches;
+  stats[3] = (int64_t)c.macs; stats[4] = (int64_t)c.alg_flops;
+  stats[5] = h->nt * 8; stats[6] = h->team_warps; stats[7] = h->large;
+  return 0;
+}
+
+extern "C" const char* ctqmc_last_error(void) { return g_err.c_str(); }
