@@ -1,0 +1,239 @@
+"""ctypes binding of libctqmc_b200.so (include/ctqmc.h).  Argument marshalling only: every step of the path
+(routing, chain product, rescaling, trace, norms) runs in the library's CUDA kernels.  There is no CPU fallback: if the
+library cannot be loaded, importing this module's functions raises.
+
+The function names are the C names.  Device arrays are torch CUDA tensors (torch is used for device memory and streams
+only); host arrays are numpy arrays.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libctqmc_b200.so")
+
+CTQMC_OK, CTQMC_ERR_ARG, CTQMC_ERR_OOM, CTQMC_ERR_CUDA, CTQMC_ERR_UNSUPPORTED = 0, -1, -2, -3, -4
+CTQMC_STATUS_OK, CTQMC_STATUS_VANISHING, CTQMC_STATUS_INVALID = 0, 1, 2
+CTQMC_SCHEDULE_THIN, CTQMC_SCHEDULE_LITERAL = 0, 1
+CTQMC_OPT_SCHEDULE, CTQMC_OPT_PANEL_WIDTH = 1, 2
+
+EXPORTS = ["ctqmc_load_impurity", "ctqmc_free_impurity", "ctqmc_set_option", "ctqmc_trace_batch", "ctqmc_bound_batch",
+           "ctqmc_trace_batch_host", "ctqmc_bound_batch_host", "ctqmc_last_stats", "ctqmc_last_error"]
+
+
+class CtqmcError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"ctqmc error {code}: {msg}")
+        self.code = code
+
+
+class _Desc(C.Structure):
+    _fields_ = [("n_sectors", C.c_int32), ("dim", C.c_void_p), ("energy", C.c_void_p), ("n_symbols", C.c_int32),
+                ("is_complex", C.c_int32), ("n_blocks", C.c_int64), ("blk_symbol", C.c_void_p), ("blk_src", C.c_void_p),
+                ("blk_dst", C.c_void_p), ("blk_offset", C.c_void_p), ("blk_data", C.c_void_p)]
+
+
+class _Batch(C.Structure):
+    _fields_ = [("n_configs", C.c_int64), ("offset", C.c_void_p), ("symbol", C.c_void_p), ("tau", C.c_void_p)]
+
+
+_lib = None
+
+
+def library() -> C.CDLL:
+    """The loaded shared library; raises if it has not been built (python -m paper_2010_08482_b200.build)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_2010_08482_b200.build` "
+                              "(there is no CPU fallback)")
+        lib = C.CDLL(LIB_PATH)
+        vp, i32, i64, dbl = C.c_void_p, C.c_int32, C.c_int64, C.c_double
+        lib.ctqmc_load_impurity.argtypes = [C.POINTER(_Desc), C.c_int, C.POINTER(vp)]
+        lib.ctqmc_load_impurity.restype = C.c_int
+        lib.ctqmc_free_impurity.argtypes = [vp]
+        lib.ctqmc_free_impurity.restype = None
+        lib.ctqmc_set_option.argtypes = [vp, C.c_int, i64]
+        lib.ctqmc_set_option.restype = C.c_int
+        for name in ("ctqmc_trace_batch", "ctqmc_trace_batch_host"):
+            fn = getattr(lib, name)
+            fn.argtypes = [vp, dbl, C.POINTER(_Batch), vp, vp, vp, vp, vp]
+            fn.restype = C.c_int
+        for name in ("ctqmc_bound_batch", "ctqmc_bound_batch_host"):
+            fn = getattr(lib, name)
+            fn.argtypes = [vp, dbl, C.POINTER(_Batch), C.c_int, C.c_int, vp, vp, vp, vp, vp, vp]
+            fn.restype = C.c_int
+        lib.ctqmc_last_stats.argtypes = [vp, C.POINTER(i64 * 8)]
+        lib.ctqmc_last_stats.restype = C.c_int
+        lib.ctqmc_last_error.argtypes = []
+        lib.ctqmc_last_error.restype = C.c_char_p
+        _lib = lib
+    return _lib
+
+
+def ctqmc_last_error() -> str:
+    return library().ctqmc_last_error().decode()
+
+
+def _check(rc: int):
+    if rc != 0:
+        raise CtqmcError(rc, ctqmc_last_error())
+
+
+def _np(a, dtype):
+    return np.ascontiguousarray(np.asarray(a), dtype=dtype)
+
+
+class ImpurityHandle:
+    """Owns a `ctqmc_impurity*`.  Created by `ctqmc_load_impurity`."""
+
+    def __init__(self, ptr: int, n_sectors: int, is_complex: bool, device: int):
+        self._ptr = C.c_void_p(ptr)
+        self.n_sectors = n_sectors
+        self.is_complex = is_complex
+        self.device = device
+
+    @property
+    def ptr(self):
+        if not self._ptr:
+            raise CtqmcError(CTQMC_ERR_ARG, "impurity handle already freed")
+        return self._ptr
+
+    def free(self):
+        if self._ptr:
+            library().ctqmc_free_impurity(self._ptr)
+            self._ptr = C.c_void_p(None)
+
+    def __del__(self):
+        try:
+            self.free()
+        except Exception:
+            pass
+
+
+def ctqmc_load_impurity(desc, device: int = 0) -> ImpurityHandle:
+    """desc: any object with dims, energy, n_symbols, is_complex, blk_symbol, blk_src, blk_dst, blk_offset, blk_data
+    (host numpy arrays; e.g. workloads.Impurity).  Copies everything to `device`."""
+    dims = _np(desc.dims, np.int32)
+    energy = _np(desc.energy, np.float64)
+    cplx = bool(desc.is_complex)
+    bs, bsrc, bdst = _np(desc.blk_symbol, np.int32), _np(desc.blk_src, np.int32), _np(desc.blk_dst, np.int32)
+    boff = _np(desc.blk_offset, np.int64)
+    data = _np(desc.blk_data, np.complex128 if cplx else np.float64)
+    d = _Desc(len(dims), dims.ctypes.data, energy.ctypes.data, int(desc.n_symbols), int(cplx), len(bs),
+              bs.ctypes.data, bsrc.ctypes.data, bdst.ctypes.data, boff.ctypes.data, data.ctypes.data)
+    out = C.c_void_p(None)
+    _check(library().ctqmc_load_impurity(C.byref(d), int(device), C.byref(out)))
+    return ImpurityHandle(out.value, len(dims), cplx, int(device))
+
+
+def ctqmc_free_impurity(imp: ImpurityHandle):
+    imp.free()
+
+
+def ctqmc_set_option(imp: ImpurityHandle, option: int, value: int):
+    _check(library().ctqmc_set_option(imp.ptr, int(option), int(value)))
+
+
+def ctqmc_last_stats(imp: ImpurityHandle) -> dict:
+    buf = (C.c_int64 * 8)()
+    _check(library().ctqmc_last_stats(imp.ptr, C.byref(buf)))
+    keys = ["strings", "units", "launches", "macs", "alg_flops", "panel_width", "team_warps", "large"]
+    return dict(zip(keys, [int(x) for x in buf]))
+
+
+def _stream_ptr(stream, host: bool = False):
+    if stream is None:
+        if host:
+            return C.c_void_p(None)   # the legacy default stream
+        import torch
+        stream = torch.cuda.current_stream()
+    return C.c_void_p(int(stream.cuda_stream))
+
+
+def _dev_batch(offset, symbol, tau):
+    import torch
+    assert offset.is_cuda and offset.dtype == torch.int64 and offset.is_contiguous()
+    assert symbol.is_cuda and symbol.dtype == torch.int32 and symbol.is_contiguous()
+    assert tau.is_cuda and tau.dtype == torch.float64 and tau.is_contiguous()
+    return _Batch(offset.numel() - 1, offset.data_ptr(), symbol.data_ptr(), tau.data_ptr())
+
+
+def ctqmc_trace_batch(imp: ImpurityHandle, beta: float, offset, symbol, tau, want_survive: bool = True, stream=None,
+                      out=None):
+    """Device form.  offset int64[B+1], symbol int32[n], tau float64[n]: torch CUDA tensors.  Returns torch CUDA
+    tensors (mant[B,2], exp2[B], survive[B,Q] or None, status[B]); asynchronous on `stream` (default: current)."""
+    import torch
+    B = offset.numel() - 1
+    dev = offset.device
+    if out is None:
+        mant = torch.empty((B, 2), dtype=torch.float64, device=dev)
+        exp2 = torch.empty(B, dtype=torch.int64, device=dev)
+        surv = torch.empty((B, imp.n_sectors), dtype=torch.uint8, device=dev) if want_survive else None
+        status = torch.empty(B, dtype=torch.int32, device=dev)
+    else:
+        mant, exp2, surv, status = out
+    b = _dev_batch(offset, symbol, tau)
+    _check(library().ctqmc_trace_batch(imp.ptr, float(beta), C.byref(b), mant.data_ptr(), exp2.data_ptr(),
+                                       surv.data_ptr() if surv is not None else None, status.data_ptr(),
+                                       _stream_ptr(stream)))
+    return mant, exp2, surv, status
+
+
+def ctqmc_bound_batch(imp: ImpurityHandle, beta: float, offset, symbol, tau, norm_kind: int = 0, segment_len: int = 1,
+                      want_sector: bool = True, stream=None):
+    """Device form.  Returns (bound_mant[B], bound_exp2[B], sector_mant[B,Q] | None, sector_exp2[B,Q] | None, status[B])."""
+    import torch
+    B = offset.numel() - 1
+    dev = offset.device
+    bm = torch.empty(B, dtype=torch.float64, device=dev)
+    be = torch.empty(B, dtype=torch.int64, device=dev)
+    sm = torch.empty((B, imp.n_sectors), dtype=torch.float64, device=dev) if want_sector else None
+    se = torch.empty((B, imp.n_sectors), dtype=torch.int64, device=dev) if want_sector else None
+    status = torch.empty(B, dtype=torch.int32, device=dev)
+    b = _dev_batch(offset, symbol, tau)
+    _check(library().ctqmc_bound_batch(imp.ptr, float(beta), C.byref(b), int(norm_kind), int(segment_len),
+                                       bm.data_ptr(), be.data_ptr(), sm.data_ptr() if want_sector else None,
+                                       se.data_ptr() if want_sector else None, status.data_ptr(), _stream_ptr(stream)))
+    return bm, be, sm, se, status
+
+
+def _host_batch(offset, symbol, tau):
+    offset, symbol, tau = _np(offset, np.int64), _np(symbol, np.int32), _np(tau, np.float64)
+    keep = (offset, symbol, tau)
+    return _Batch(len(offset) - 1, offset.ctypes.data, symbol.ctypes.data if len(symbol) else None,
+                  tau.ctypes.data if len(tau) else None), keep
+
+
+def ctqmc_trace_batch_host(imp: ImpurityHandle, beta: float, offset, symbol, tau, want_survive: bool = True,
+                           stream=None):
+    """Host form: numpy in, numpy out; copies and synchronises inside the library."""
+    b, keep = _host_batch(offset, symbol, tau)
+    B = b.n_configs
+    mant = np.empty((B, 2), np.float64)
+    exp2 = np.empty(B, np.int64)
+    surv = np.empty((B, imp.n_sectors), np.uint8) if want_survive else None
+    status = np.empty(B, np.int32)
+    _check(library().ctqmc_trace_batch_host(imp.ptr, float(beta), C.byref(b), mant.ctypes.data, exp2.ctypes.data,
+                                            surv.ctypes.data if want_survive else None, status.ctypes.data,
+                                            _stream_ptr(stream, host=True)))
+    return mant, exp2, surv, status
+
+
+def ctqmc_bound_batch_host(imp: ImpurityHandle, beta: float, offset, symbol, tau, norm_kind: int = 0,
+                           segment_len: int = 1, want_sector: bool = True, stream=None):
+    b, keep = _host_batch(offset, symbol, tau)
+    B = b.n_configs
+    bm = np.empty(B, np.float64)
+    be = np.empty(B, np.int64)
+    sm = np.empty((B, imp.n_sectors), np.float64) if want_sector else None
+    se = np.empty((B, imp.n_sectors), np.int64) if want_sector else None
+    status = np.empty(B, np.int32)
+    _check(library().ctqmc_bound_batch_host(imp.ptr, float(beta), C.byref(b), int(norm_kind), int(segment_len),
+                                            bm.ctypes.data, be.ctypes.data, sm.ctypes.data if want_sector else None,
+                                            se.ctypes.data if want_sector else None, status.ctypes.data,
+                                            _stream_ptr(stream, host=True)))
+    return bm, be, sm, se, status

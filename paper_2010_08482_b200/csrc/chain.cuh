@@ -231,6 +231,11 @@ __global__ void __launch_bounds__(kCtaThreads) chain_kernel(ChainParams P) {
         Slot out; out.re = 0.0; out.im = 0.0; out.e2 = 0; out.pad = 0;
         if (!dead) {
           double re = 0.0, im = 0.0;
+          if (L == 0) {   // empty configuration: Tr P_beta(q0), the partition-function term (reading A7)
+            const double* E0 = P.imp.energy + P.imp.e_off[q];
+            const double em0 = P.imp.e_min[q];
+            for (int n = 0; n < ncols; ++n) re += exp(-P.bv.beta * (E0[c0 + n] - em0));
+          } else
           for (int n = 0; n < ncols; ++n) {
             if constexpr (CPLX) {
               const double2 v = *reinterpret_cast<const double2*>(X + ((size_t)n * ldx + c0 + n) * 2);

@@ -1,0 +1,291 @@
+"""Parity of the CUDA path (through the C ABI) with the CPU oracle on the same seeded inputs.  Run on a B200: -m gpu.
+
+Bars (BASELINE.json north_star):
+  * routing (`survive`) and the vanishing pattern (`status`): bit-exact;
+  * trace: |w_gpu - w_cpu| <= 1e-9 |w_cpu| at a common exponent (checks sign / phase too; reading A5), loosened only
+    by the cancellation rule A8 (tolerance 1e-9 * max(1, kappa * 1e-5));
+  * bound: relative 1e-9 against the oracle's bound, and bound >= |trace|.
+"""
+import math
+
+import numpy as np
+import pytest
+
+from util import rel_diff, scaled_ge
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-9
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    torch = pytest.importorskip("torch")
+    if not torch.cuda.is_available():
+        pytest.fail("no CUDA device: the gpu tests must run on the B200 box")
+    return torch
+
+
+@pytest.fixture(scope="module")
+def lib():
+    import paper_2010_08482_b200 as L
+    L.library()   # raises loudly if the extension is missing
+    return L
+
+
+@pytest.fixture(scope="module")
+def handles(lib, impurities, torch_cuda):
+    cache = {}
+
+    def get(cfg):
+        if cfg not in cache:
+            cache[cfg] = lib.ctqmc_load_impurity(impurities(cfg), 0)
+        return cache[cfg]
+    yield get
+    for h in cache.values():
+        h.free()
+
+
+def _dev(torch, batch):
+    return (torch.from_numpy(batch.offset).cuda(), torch.from_numpy(batch.symbol).cuda(), torch.from_numpy(batch.tau).cuda())
+
+
+def _check_trace(lib, torch, imp, handle, batch, label):
+    from oracle import trace_oracle as O
+    off, sym, tau = _dev(torch, batch)
+    mant, exp2, surv, status = lib.ctqmc_trace_batch(handle, batch.beta, off, sym, tau)
+    torch.cuda.synchronize()
+    mant, exp2, surv, status = mant.cpu().numpy(), exp2.cpu().numpy(), surv.cpu().numpy(), status.cpu().numpy()
+    worst = 0.0
+    loosened = 0
+    for b in range(batch.n_configs):
+        s, t = batch.config(b)
+        r = O.trace_config(imp, batch.beta, s, t)
+        assert status[b] == r["status"], f"{label} config {b}: status {status[b]} != oracle {r['status']}"
+        if r["status"] == 2:
+            assert math.isnan(mant[b, 0]) and math.isnan(mant[b, 1])
+            continue
+        assert np.array_equal(surv[b], r["survive"]), f"{label} config {b}: survive mask differs"
+        w = complex(mant[b, 0], mant[b, 1])
+        if r["mant"] == 0:
+            assert w == 0, f"{label} config {b}: oracle is exactly zero, gpu is {w}"
+            continue
+        mx = max(abs(w.real), abs(w.imag))
+        assert 1.0 <= mx < 2.0, f"{label} config {b}: mantissa {w} not normalised"
+        d = rel_diff(w, int(exp2[b]), r["mant"], r["exp2"])
+        tol = TOL * max(1.0, r["kappa"] * 1e-5)
+        if tol > TOL:
+            loosened += 1
+        assert d <= tol, f"{label} config {b}: rel diff {d:.3e} > {tol:.1e} (kappa {r['kappa']:.2e})"
+        worst = max(worst, d)
+    assert loosened <= max(1, batch.n_configs // 100), f"{label}: {loosened} configurations needed the A8 loosening"
+    return worst
+
+
+# --------------------------------------------------------------------------- trace parity on the BASELINE configs
+@pytest.mark.parametrize("cfg,n", [(1, 1024), (2, 512), (3, 24), (4, 4)])
+def test_trace_parity_baseline_configs(cfg, n, lib, torch_cuda, impurities, handles):
+    from workloads import make_batch
+    batch = make_batch(cfg, n)
+    worst = _check_trace(lib, torch_cuda, impurities(cfg), handles(cfg), batch, f"cfg{cfg}")
+    print(f"cfg{cfg}: worst relative difference {worst:.3e}")
+
+
+@pytest.mark.parametrize("cfg,n", [(1, 64), (2, 64), (3, 6), (4, 2)])
+def test_trace_parity_literal_schedule(cfg, n, lib, torch_cuda, impurities, handles):
+    """The literal order of Eq. 65 (start at q0, carry dim(q0) columns) must agree with the thin start."""
+    from workloads import make_batch
+    h = handles(cfg)
+    lib.ctqmc_set_option(h, lib.CTQMC_OPT_SCHEDULE, lib.CTQMC_SCHEDULE_LITERAL)
+    try:
+        _check_trace(lib, torch_cuda, impurities(cfg), h, make_batch(cfg, n, start=5000), f"cfg{cfg}-literal")
+    finally:
+        lib.ctqmc_set_option(h, lib.CTQMC_OPT_SCHEDULE, lib.CTQMC_SCHEDULE_THIN)
+
+
+@pytest.mark.parametrize("cfg,width", [(2, 8), (2, 16), (3, 8), (3, 16), (3, 32)])
+def test_trace_parity_panel_widths(cfg, width, lib, torch_cuda, impurities, handles):
+    from workloads import make_batch
+    h = handles(cfg)
+    try:
+        lib.ctqmc_set_option(h, lib.CTQMC_OPT_PANEL_WIDTH, width)
+    except lib.CtqmcError as e:
+        if e.code == -4:
+            pytest.skip(str(e))
+        raise
+    try:
+        lib.ctqmc_set_option(h, lib.CTQMC_OPT_SCHEDULE, lib.CTQMC_SCHEDULE_LITERAL)
+        _check_trace(lib, torch_cuda, impurities(cfg), h, make_batch(cfg, 6, start=7000), f"cfg{cfg}-W{width}")
+    finally:
+        lib.ctqmc_set_option(h, lib.CTQMC_OPT_SCHEDULE, lib.CTQMC_SCHEDULE_THIN)
+        lib.ctqmc_set_option(h, lib.CTQMC_OPT_PANEL_WIDTH, 0)
+
+
+# --------------------------------------------------------------------------- edge cases
+def test_empty_configuration_is_partition_function(lib, torch_cuda, impurities, handles):
+    """L = 0 gives Z = sum_n exp(-beta E_n) (north_star pin P1), here against the closed form directly."""
+    from workloads import Batch
+    for cfg in (1, 2, 3):
+        imp = impurities(cfg)
+        batch = Batch.from_lists(imp.beta, [([], []), ([], [])])
+        off, sym, tau = _dev(torch_cuda, batch)
+        mant, exp2, surv, status = lib.ctqmc_trace_batch(handles(cfg), imp.beta, off, sym, tau)
+        torch_cuda.cuda.synchronize()
+        emin = imp.energy.min()
+        z = math.fsum(np.exp(-imp.beta * (imp.energy - emin)))
+        lg = -imp.beta * emin / math.log(2.0)
+        k = math.floor(lg)
+        zm, ze = math.frexp(z * 2.0 ** (lg - k))
+        for b in range(2):
+            assert status[b].item() == 0 and surv[b].all().item()
+            assert rel_diff(complex(mant[b, 0].item(), mant[b, 1].item()), int(exp2[b].item()), zm, ze + k) < 1e-10
+
+
+def test_empty_batch_and_null_arguments(lib, torch_cuda, impurities, handles):
+    from workloads import Batch
+    imp = impurities(1)
+    batch = Batch.from_lists(imp.beta, [])
+    off, sym, tau = _dev(torch_cuda, batch)
+    mant, exp2, surv, status = lib.ctqmc_trace_batch(handles(1), imp.beta, off, sym, tau)
+    assert mant.shape == (0, 2)
+    with pytest.raises(lib.CtqmcError):
+        lib.ctqmc_trace_batch(handles(1), -1.0, off, sym, tau)
+    assert "beta" in lib.ctqmc_last_error()
+
+
+def test_vanishing_invalid_and_ragged(lib, torch_cuda, impurities, handles):
+    """Structurally vanishing strings (status 1, exact zero), invalid inputs (status 2, NaN) and valid ones of very
+    different lengths in one batch; neighbours must be unaffected."""
+    from workloads import Batch, make_batch
+    imp = impurities(2)
+    good = make_batch(2, 5, start=900)
+    c = [good.config(b) for b in range(5)]
+    beta = imp.beta
+    cfgs = [
+        c[0],
+        ([1, 1, 1, 1], [1.0, 2.0, 3.0, 4.0]),  # c^dag_0 four times: leaves the sector table from every start sector
+        ([1, 1], [1.0, 2.0]),                  # c^dag_0 twice: survives routing but q_L != q_0, contributes exactly 0
+        c[1],
+        ([1, 0], [3.0, 2.0]),                  # tau decreasing
+        ([1, 0], [1.0, beta]),                 # tau == beta is outside [0, beta)
+        ([99, 0], [1.0, 2.0]),                 # symbol out of range
+        ([1, 0], [1.0, float("nan")]),
+        c[2],
+        ([], []),
+        ([1, 0], [0.0, 0.0]),                  # equal times, tau = 0 (reading A7): legal
+        ([0, 1, 3, 2], [1.0, 1.0, 7.5, 7.5]),  # ties keep input order
+        c[3], c[4],
+    ]
+    batch = Batch.from_lists(beta, cfgs)
+    _check_trace(lib, torch_cuda, imp, handles(2), batch, "edge")
+    off, sym, tau = _dev(torch_cuda, batch)
+    mant, exp2, surv, status = lib.ctqmc_trace_batch(handles(2), beta, off, sym, tau)
+    st = status.cpu().numpy()
+    assert list(st) == [0, 1, 0, 0, 2, 2, 2, 2, 0, 0, 0, 0, 0, 0]
+    assert mant[1].abs().sum().item() == 0.0 and exp2[1].item() == 0 and surv[1].sum().item() == 0
+    assert mant[2].abs().sum().item() == 0.0 and exp2[2].item() == 0 and surv[2].sum().item() > 0
+
+
+def test_long_chain_exponent_range(lib, torch_cuda, impurities, handles):
+    """A long chain (L = 2000) at large beta: the running exponent must carry ~1e4 binary orders without overflow."""
+    from workloads import Batch
+    from workloads.rng import Stream
+    imp = impurities(2)
+    rng = Stream(77)
+    beta = 2000.0
+    cfgs = []
+    for _ in range(3):
+        ops = []
+        for f in range(6):
+            t = np.sort(beta * rng.uniforms(334))
+            first = rng.integer(2)
+            ops += [(t[i], 2 * f + ((first + i) & 1)) for i in range(len(t))]
+        ops.sort()
+        cfgs.append(([a for _, a in ops], [t for t, _ in ops]))
+    batch = Batch.from_lists(beta, cfgs)
+    _check_trace(lib, torch_cuda, imp, handles(2), batch, "long")
+
+
+def test_host_form_matches_device_form(lib, torch_cuda, impurities, handles):
+    from workloads import make_batch
+    for cfg, n in ((1, 200), (3, 5)):
+        batch = make_batch(cfg, n, start=300)
+        off, sym, tau = _dev(torch_cuda, batch)
+        d = lib.ctqmc_trace_batch(handles(cfg), batch.beta, off, sym, tau)
+        torch_cuda.cuda.synchronize()
+        h = lib.ctqmc_trace_batch_host(handles(cfg), batch.beta, batch.offset, batch.symbol, batch.tau)
+        for a, b in zip(d, h):
+            assert np.array_equal(a.cpu().numpy(), b, equal_nan=True)
+
+
+def test_repeatable_and_stream_ordered(lib, torch_cuda, impurities, handles):
+    """Same inputs twice, on a side stream, give bit-identical outputs (fixed summation order)."""
+    from workloads import make_batch
+    batch = make_batch(3, 8, start=40)
+    off, sym, tau = _dev(torch_cuda, batch)
+    a = lib.ctqmc_trace_batch(handles(3), batch.beta, off, sym, tau)
+    torch_cuda.cuda.synchronize()
+    st = torch_cuda.cuda.Stream()
+    with torch_cuda.cuda.stream(st):
+        b = lib.ctqmc_trace_batch(handles(3), batch.beta, off, sym, tau, stream=st)
+    st.synchronize()
+    for x, y in zip(a, b):
+        assert torch_cuda.equal(x, y)
+
+
+# --------------------------------------------------------------------------- bounds
+def _check_bound(lib, torch, imp, handle, batch, norm_kind, S, label):
+    from oracle import trace_oracle as O
+    off, sym, tau = _dev(torch, batch)
+    bm, be, sm, se, status = lib.ctqmc_bound_batch(handle, batch.beta, off, sym, tau, norm_kind, S)
+    mant, exp2, surv, tstatus = lib.ctqmc_trace_batch(handle, batch.beta, off, sym, tau)
+    torch.cuda.synchronize()
+    bm, be, sm, se, status = [x.cpu().numpy() for x in (bm, be, sm, se, status)]
+    mant, exp2 = mant.cpu().numpy(), exp2.cpu().numpy()
+    for b in range(batch.n_configs):
+        s, t = batch.config(b)
+        r = O.bound_config(imp, batch.beta, s, t, norm_kind, S)
+        assert status[b] == r["status"]
+        if r["status"] == 2:
+            assert math.isnan(bm[b])
+            continue
+        d = rel_diff(bm[b], int(be[b]), r["mant"], r["exp2"])
+        assert d <= TOL, f"{label} config {b}: bound rel diff {d:.3e}"
+        for q0, sec in enumerate(r["sector"]):
+            if sec is None:
+                assert sm[b, q0] == 0.0 and se[b, q0] == 0
+            else:
+                dq = rel_diff(sm[b, q0], int(se[b, q0]), sec[0], sec[1])
+                assert dq <= TOL, f"{label} config {b} sector {q0}: rel diff {dq:.3e}"
+        w = abs(complex(mant[b, 0], mant[b, 1]))
+        assert scaled_ge(bm[b], int(be[b]), w, int(exp2[b])), f"{label} config {b}: bound < |trace|"
+
+
+@pytest.mark.parametrize("cfg,n", [(1, 128), (2, 128), (3, 8), (4, 2)])
+@pytest.mark.parametrize("norm_kind", [0, 1])
+def test_bound_s1_parity(cfg, n, norm_kind, lib, torch_cuda, impurities, handles):
+    from workloads import make_batch
+    _check_bound(lib, torch_cuda, impurities(cfg), handles(cfg), make_batch(cfg, n, start=100), norm_kind, 1,
+                 f"cfg{cfg}-nk{norm_kind}-S1")
+
+
+@pytest.mark.parametrize("cfg,n", [(1, 64), (2, 64), (3, 4)])
+@pytest.mark.parametrize("S", [0, 2, 8, 37])
+def test_bound_segments_parity(cfg, n, S, lib, torch_cuda, impurities, handles):
+    from workloads import make_batch
+    _check_bound(lib, torch_cuda, impurities(cfg), handles(cfg), make_batch(cfg, n, start=200), 0, S,
+                 f"cfg{cfg}-S{S}")
+
+
+def test_bound_edge_cases(lib, torch_cuda, impurities, handles):
+    from workloads import Batch, make_batch
+    imp = impurities(2)
+    good = make_batch(2, 2, start=77)
+    cfgs = [good.config(0), ([], []), ([1, 1, 1, 1], [1.0, 2.0, 3.0, 4.0]), ([1, 0], [3.0, 2.0]), good.config(1)]
+    batch = Batch.from_lists(imp.beta, cfgs)
+    for nk, S in ((0, 1), (1, 1), (0, 0), (0, 3)):
+        _check_bound(lib, torch_cuda, imp, handles(2), batch, nk, S, f"edge-nk{nk}-S{S}")
+    off, sym, tau = _dev(torch_cuda, batch)
+    with pytest.raises(lib.CtqmcError) as ei:
+        lib.ctqmc_bound_batch(handles(2), imp.beta, off, sym, tau, 1, 4)
+    assert ei.value.code == -4
