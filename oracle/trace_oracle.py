@@ -13,10 +13,13 @@ What it computes (citations are PAPER.md line numbers):
   * `bound_config`   the lazy-trace upper bound (:542-548): product of submultiplicative norms of (segments of) the
                      factors, times a rank prefactor (readings A1, A2, A4, A9).
 
-Scaling (paper silent, reading A5): exp(-D E_n) is written exp(-D (E_n - Emin_q)) * 2**(-D Emin_q log2 e); the
-second factor goes into a running real exponent `lg`, and after every factor the matrix is divided by an exact power of
-two (frexp of its largest |component|) which goes into a running integer exponent.  Both are exact reorganisations of
-Eq. 65 apart from the rounding of `lg` (|lg| <~ 1e4, i.e. ~1e-12 relative in the value).
+Scaling (paper silent, reading A5): exp(-D E_n) is written 2**x_n * 2**(-D Emin_q log2 e) with
+x_n = -D (E_n - Emin_q) log2 e <= 0.  The second factor goes into a running real exponent `lg`.  Of the first, only the
+mantissa 2**(x_n - floor x_n) is multiplied into row n; the integers floor(x_n) are compared across rows, the largest
+(over non-zero rows) goes into a running integer exponent and the others are applied with ldexp relative to it
+(`_propagate`).  Both are exact reorganisations of Eq. 65 apart from the rounding of x_n and `lg` (|x|, |lg| <~ 1e4,
+i.e. ~1e-12 relative in the value), and neither can underflow: np.exp(-D (E_n - Emin)) would, for D (E_n - Emin) > 745,
+which the uniformly placed operators of BASELINE config 3 reach (pin: test_P5_coarse_sectors_do_not_underflow).
 
 Pins: tests/test_oracle_pins.py (Z closed form, cyclicity, brute force in the unblocked Fock space, gauge / shift /
 time-reversal invariances, Ising closed form, atomic Green function, bound >= |trace|, S-monotonicity, S=1 closed forms).
@@ -95,13 +98,32 @@ def _apply_lg(z: complex, e: int, lg: float):
     return _normalize(z * (2.0 ** (lg - k)), e + int(k))
 
 
-def _rescale(M: np.ndarray):
-    """Divide M by the power of two that brings its largest |component| into [0.5, 1); return (M, exponent)."""
-    mx = max(np.abs(M.real).max(), np.abs(M.imag).max()) if np.iscomplexobj(M) else np.abs(M).max()
-    if mx == 0.0:
-        return M, 0
-    _, ex = math.frexp(float(mx))
-    return M * math.ldexp(1.0, -ex), ex
+def _propagate(M: np.ndarray, delta: float, E: np.ndarray, Emin: float):
+    """diag(exp(-delta (E - Emin))) @ M, returned as (M', k) with the product equal to M' * 2**k and max|component| of
+    M' in [0.5, 1)  (M' = 0, k = 0 if the product vanishes).
+
+    Row n is multiplied by 2**x_n, x_n = -delta (E_n - Emin) log2(e) <= 0, which is split into the integer floor(x_n)
+    and the mantissa 2**(x_n - floor(x_n)) in [1, 2).  Only the mantissa is multiplied in; the integer parts are
+    compared across rows and applied with ldexp relative to the largest row.  So a row whose factor exp(-delta (E_n -
+    Emin)) is far below the smallest double keeps full precision whenever the rows with a larger factor are zero (e.g.
+    by a symmetry the sector labels do not resolve) -- np.exp would underflow there, although Eq. 65's value is
+    perfectly representable as mant * 2**exp2 (reading A5)."""
+    x = (-float(delta) * (E - Emin)) * LOG2E
+    k = np.floor(x)
+    M = np.exp2(x - k)[:, None] * M
+    k = k.astype(np.int64)
+    rowmax = np.maximum(np.abs(M.real), np.abs(M.imag)).max(axis=1) if np.iscomplexobj(M) else np.abs(M).max(axis=1)
+    nz = rowmax > 0.0
+    if not nz.any():
+        return M * 0.0, 0
+    _, ex = np.frexp(rowmax[nz])
+    kmax = int((k[nz] + ex).max())
+    shift = np.clip(k - kmax, -4000, 4000).astype(np.int32)[:, None]
+    if np.iscomplexobj(M):
+        M = np.ldexp(M.real, shift) + 1j * np.ldexp(M.imag, shift)
+    else:
+        M = np.ldexp(M, shift)
+    return M, kmax
 
 
 # --------------------------------------------------------------------------- routing (:532-534)
@@ -145,18 +167,15 @@ def _string_trace(imp: _Imp, beta: float, symbols, taus, visited):
     L = len(symbols)
     q0 = visited[0]
     tau1 = float(taus[0]) if L else float(beta)
-    M = np.diag(np.exp(-tau1 * (imp.E[q0] - imp.Emin[q0])))
-    if imp.is_complex:
-        M = M.astype(np.complex128)
+    M = np.eye(int(imp.dims[q0]), dtype=np.complex128 if imp.is_complex else np.float64)
+    M, e2 = _propagate(M, tau1, imp.E[q0], imp.Emin[q0])
     lg = -tau1 * imp.Emin[q0] * LOG2E
-    e2 = 0
     for i in range(L):
         q_prev, q = visited[i], visited[i + 1]
         M = imp.F[(int(symbols[i]), q_prev)] @ M
         delta = (float(taus[i + 1]) - float(taus[i])) if i + 1 < L else (float(beta) - float(taus[i]))
-        M = np.exp(-delta * (imp.E[q] - imp.Emin[q]))[:, None] * M
+        M, ex = _propagate(M, delta, imp.E[q], imp.Emin[q])
         lg += -delta * imp.Emin[q] * LOG2E
-        M, ex = _rescale(M)
         e2 += ex
     if visited[-1] != q0:       # off-diagonal block: no trace (never happens for balanced c^dag / c strings, :532)
         return 0j, 0, 0.0, 0.0
@@ -244,9 +263,8 @@ def _string_bound(imp: _Imp, beta: float, symbols, taus, visited, norm_kind: int
         for i in range(start, stop):
             q_prev, q = visited[i], visited[i + 1]
             M = imp.F[(int(symbols[i]), q_prev)] @ M
-            M = np.exp(-deltas[i] * (imp.E[q] - imp.Emin[q]))[:, None] * M
+            M, ex = _propagate(M, deltas[i], imp.E[q], imp.Emin[q])
             lg += -deltas[i] * imp.Emin[q] * LOG2E
-            M, ex = _rescale(M)
             e2 += ex
         if norm_kind == 0:
             nrm = math.sqrt(math.fsum((np.abs(M) ** 2).ravel()))

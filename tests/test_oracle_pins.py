@@ -187,6 +187,67 @@ def test_P5_ising_limit_closed_form():
         assert abs(O.to_log(r["mant"], r["exp2"]) + integral) < 1e-9 * max(1.0, abs(integral))
 
 
+def test_P5_coarse_sectors_do_not_underflow():
+    """Ising limit again, but with sectors labelled by N only (so d > 1 and E_n - Emin is large inside a sector) and
+    level splittings times time differences far beyond 745: exp(-Delta (E_n - Emin)) underflows a double, the value of
+    Eq. 65 does not.  Closed form per start sector: each Fock state is its own invariant subspace, so
+    t(q0) = sum over Fock states s in q0 that survive the operator sequence of sign(s) exp(-int E[n(tau)] dtau)."""
+    n, beta = 3, 60.0
+    eps = np.array([-2.0, 31.0, 75.0])
+    Umat = np.array([[0, 3.0, 1.0], [3.0, 0, 2.0], [1.0, 2.0, 0]])
+    u = np.zeros((n,) * 4)
+    for a in range(n):
+        for b_ in range(n):
+            if a != b_:
+                u[a, b_, b_, a] = Umat[a, b_]
+    imp = wi.build_impurity("ising-coarse", np.diag(eps), u, [(1,)] * n, beta=beta)
+    assert list(imp.dims) == [1, 3, 3, 1]
+
+    def energy(state):
+        occ = np.array([(state >> f) & 1 for f in range(n)], dtype=float)
+        return float(eps @ occ + 0.5 * occ @ Umat @ occ)
+
+    # flavour 2 (the expensive one) is created and kept for 40 time units; flavour 1 flips in between
+    configs = [([5, 3, 2, 4], [1.0, 7.0, 19.5, 41.0]),
+               ([5, 4], [3.0, 58.0]),
+               ([3, 5, 4, 2, 1, 0], [2.0, 2.5, 30.0, 44.0, 50.0, 59.0])]
+    for s, t in configs:
+        r = O.trace_config(imp, beta, s, t)
+        assert r["status"] == 0
+        for q0 in range(imp.n_sectors):
+            terms = []
+            for st0 in imp.sector_states[q0]:
+                state, sign, integral, t_prev, ok = int(st0), 1.0, 0.0, 0.0, True
+                for a, tt in zip(s, t):
+                    integral += (tt - t_prev) * energy(state)
+                    f, create = int(a) // 2, int(a) % 2
+                    if ((state >> f) & 1) == create:
+                        ok = False
+                        break
+                    sign *= (-1) ** bin(state & ((1 << f) - 1)).count("1")
+                    state ^= (1 << f)
+                    t_prev = tt
+                if ok and state == int(st0):
+                    terms.append((sign, integral + (beta - t_prev) * energy(state)))
+            if r["sector"][q0] is None:
+                assert not terms
+                continue
+            zs, es = r["sector"][q0]
+            if not terms:
+                assert zs == 0
+                continue
+            top = min(i for _, i in terms)
+            val = sum(sg * math.exp(-(i - top)) for sg, i in terms)
+            assert math.copysign(1.0, zs.real) == math.copysign(1.0, val)
+            assert abs(O.to_log(zs, es) - (math.log(abs(val)) - top)) < 1e-9 * max(1.0, abs(top))
+            assert (es * math.log(2.0) < -745.0) or top < 745.0   # at least some sectors are beyond exp()'s range
+            bd = O.bound_config(imp, beta, s, t, 0, 1)
+            assert scaled_ge(bd["sector"][q0][0], bd["sector"][q0][1], abs(zs), es)
+    # the middle configuration keeps flavour 2 for 55 time units: within the N=1 sector that is 77*55 = 4235 >> 745
+    r = O.trace_config(imp, beta, *configs[1])
+    assert r["sector"][0] is not None and r["sector"][0][0] != 0
+
+
 def test_P6_atomic_green_function():
     """One orbital: c^dag_up at 0+, c_up at tau:  w = e^{mu tau} + e^{-tau (U - 2 mu) + mu (beta - tau)}  (textbook)."""
     U, mu, beta, tau = 2.5, 0.9, 3.0, 1.234
