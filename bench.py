@@ -1,0 +1,278 @@
+"""bench.py -- one JSON line: local-trace evaluations per second of the CUDA path on a BASELINE.json workload.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--batch B] [--impl ours|reference]
+
+A *step* is one pass of the whole hot path (validate -> route -> bin -> fused propagate*operator chain -> trace
+reduction) over one batch of seeded synthetic configurations.  `value` is traces/s
+with the batch resident in HBM; `e2e` is the same through `ctqmc_trace_batch_host` (host buffers, copies inside the
+timed region).  L2 is flushed between timed steps.  `--impl reference` times the CPU oracle (oracle/) on a bounded
+sample of the same workload; it is the only code path here, besides `cpu_baseline`, that touches oracle/.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "local_trace_evaluations_per_s"
+UNIT = "traces/s"
+NOMINAL_FP64_TFLOPS = 40.0     # B200 FP64 (tensor) nominal; DESIGN.md §7
+NOMINAL_BF16_TFLOPS = 2250.0   # B200_PROFILING.md
+FALLBACK_HBM_GBS, FALLBACK_BF16_TFLOPS = 6650.0, 1590.0
+WORKLOADS = {
+    1: "cfg1: 2-orbital Kanamori (Q=9, d_max=4), L=40",
+    2: "cfg2: 3-orbital t2g Kanamori (Q=16, d_max=9), pairs~Poisson(60)",
+    3: "cfg3: 5-orbital d-shell Slater, N sectors (Q=11, d_max=252), pairs~Poisson(80)",
+    4: "cfg4: 7-orbital f-shell Slater+SOC, (N,Jz) sectors N in 4..6 (Q=70, d_max=295), complex, pairs~Poisson(100)",
+    5: "cfg5: 7-orbital f-shell + crystal field, N sectors 1001/2002/3003, complex, pairs~Poisson(100)",
+}
+REF_SAMPLE = {1: 1024, 2: 512, 3: 8, 4: 1, 5: 1}   # configurations per reference step (about a second or more each)
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as fh:
+            d = json.load(fh)
+        return dict(hbm_gbs=float(d["hbm_gbs"]), bf16=float(d["bf16_tflops"]), bf16_sustained=float(d.get("bf16_tflops_sustained", d["bf16_tflops"])), source="measured")
+    return dict(hbm_gbs=FALLBACK_HBM_GBS, bf16=FALLBACK_BF16_TFLOPS, bf16_sustained=1400.0, source="fallback")
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md)."""
+    Q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
+        "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, mx, reasons = [], None, set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx = float(r[1])
+            except (ValueError, IndexError):
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def oracle_rate(imp, batch, n_sample: int):
+    """traces/s of the oracle, as it stands, on the first n_sample configurations."""
+    from oracle import trace_oracle as O
+    sub = batch.subset(range(min(n_sample, batch.n_configs)))
+    t0 = time.perf_counter()
+    O.trace_batch(imp, sub.beta, sub.offset, sub.symbol, sub.tau)
+    dt = time.perf_counter() - t0
+    return sub.n_configs / dt, sub.n_configs, dt
+
+
+def blas_threads() -> int:
+    try:
+        from threadpoolctl import threadpool_info
+        return max([int(i.get("num_threads", 1)) for i in threadpool_info()] + [1])
+    except Exception:
+        return 1
+
+
+def run_reference(args, rank: int):
+    """--impl reference: the CPU oracle, as it stands, on a bounded sample per step (rank 0 only)."""
+    if rank != 0:
+        return
+    from workloads import build_config_impurity, make_batch
+    cfg = args.config
+    imp = build_config_impurity(cfg, keep_eigvecs=False)
+    n = REF_SAMPLE[cfg]
+    batch = make_batch(cfg, n)
+    for _ in range(min(args.warmup, 1)):
+        oracle_rate(imp, batch, max(1, n // 8))
+    t_tot, n_tot = 0.0, 0
+    for _ in range(args.steps):
+        _, k, dt = oracle_rate(imp, batch, n)
+        t_tot += dt
+        n_tot += k
+    val = n_tot / t_tot
+    cores = blas_threads()
+    sample = f"{n} configurations of {WORKLOADS[cfg]} per step, oracle.trace_oracle.trace_batch (numpy fp64)"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * t_tot / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": WORKLOADS[cfg], "batch": n},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }))
+
+
+def run_ours(args, rank: int, world: int, local_rank: int):
+    import numpy as np
+    import torch
+
+    import paper_2010_08482_b200 as L
+    from workloads import BASELINE_CONFIGS, build_config_impurity, make_batch
+
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    cfg = args.config
+    B = args.batch or BASELINE_CONFIGS[cfg]["batch"]
+    imp = build_config_impurity(cfg, keep_eigvecs=False)
+    t0 = time.perf_counter()
+    h = L.ctqmc_load_impurity(imp, local_rank)
+    load_s = time.perf_counter() - t0
+    if args.schedule == "literal":
+        L.ctqmc_set_option(h, L.CTQMC_OPT_SCHEDULE, L.CTQMC_SCHEDULE_LITERAL)
+    L.ctqmc_set_option(h, L.CTQMC_OPT_TIMING, 1)
+    batch = make_batch(cfg, B, start=rank * B)           # weak scaling: every rank its own B configurations
+    off, sym, tau = (torch.from_numpy(x).cuda() for x in (batch.offset, batch.symbol, batch.tau))
+    Q = imp.n_sectors
+    out = (torch.empty((B, 2), dtype=torch.float64, device="cuda"), torch.empty(B, dtype=torch.int64, device="cuda"),
+           torch.empty((B, Q), dtype=torch.uint8, device="cuda"), torch.empty(B, dtype=torch.int32, device="cuda"))
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")   # > 126 MB L2
+    stream = torch.cuda.current_stream()
+
+    def step():
+        L.ctqmc_trace_batch(h, batch.beta, off, sym, tau, stream=stream, out=out)
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    stats = L.ctqmc_last_stats(h)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    chain_ms, route_ms, reduce_ms = [], [], []
+    barrier()
+    for a, b in ev:
+        flush.zero_()
+        a.record(stream)
+        step()
+        b.record(stream)
+        tm = L.ctqmc_last_timing(h)      # synchronises; outside the event pair
+        chain_ms.append(tm["chain_ms"]); route_ms.append(tm["route_ms"]); reduce_ms.append(tm["reduce_ms"])
+    barrier()
+    step_ms = [a.elapsed_time(b) for a, b in ev]
+    total_ms = sum(step_ms)
+
+    # end to end through the host-buffer C call: H2D of the batch, kernels, D2H of the results, inside the timed region
+    for _ in range(2):
+        L.ctqmc_trace_batch_host(h, batch.beta, batch.offset, batch.symbol, batch.tau)
+    e2e_s = 0.0
+    barrier()
+    for _ in range(args.steps):
+        flush.zero_()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        L.ctqmc_trace_batch_host(h, batch.beta, batch.offset, batch.symbol, batch.tau)
+        e2e_s += time.perf_counter() - t0
+    barrier()
+    clocks = sampler.stop() if rank == 0 else None
+
+    t = torch.tensor([total_ms, e2e_s * 1e3], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    total_ms, e2e_ms = float(t[0]), float(t[1])
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    n_ops = int(batch.offset[-1])
+    pk = peaks()
+    fp64_peak = pk["bf16"] * NOMINAL_FP64_TFLOPS / NOMINAL_BF16_TFLOPS
+    chain_avg_ms = sum(chain_ms) / len(chain_ms)
+    achieved_tf = stats["alg_flops"] / (chain_avg_ms * 1e-3) / 1e12
+    alg_bytes = n_ops * 12 + (B + 1) * 8 + B * (16 + 8 + 4 + Q)
+    value = world * B * args.steps / (total_ms * 1e-3)
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+        "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": WORKLOADS[cfg], "batch_per_gpu": B, "operators_per_batch": n_ops, "schedule": args.schedule,
+                   "l2": "flushed between timed steps (256 MiB write)", "sharding": "batch split over ranks, no collective"},
+        "gflops": world * stats["alg_flops"] * args.steps / (total_ms * 1e-3) / 1e9,
+        "e2e": {"value": world * B * args.steps / (e2e_ms * 1e-3), "unit": UNIT,
+                "h2d_bytes_per_step": n_ops * 12 + (B + 1) * 8, "d2h_bytes_per_step": B * (16 + 8 + 4 + Q)},
+        "gpu_launches": stats["launches"] * args.steps,
+        "clocks": clocks,
+        "roofline": {"bound": "tensor", "kernel": "chain_kernel (fused propagate x operator, FP64 DMMA)",
+                     "achieved": achieved_tf, "peak": fp64_peak, "unit": "TFLOP/s", "frac": achieved_tf / fp64_peak,
+                     "traffic": None,
+                     "peak_source": f"{pk['source']} bf16 {pk['bf16']} TF/s x nominal fp64/bf16 ratio {NOMINAL_FP64_TFLOPS}/{NOMINAL_BF16_TFLOPS}",
+                     "kernel_ms": chain_avg_ms, "kernel_share_of_step": chain_avg_ms * args.steps / total_ms,
+                     "flops_per_launch": stats["alg_flops"], "executed_real_macs_padded": stats["macs"],
+                     "hbm_frac_algorithmic": alg_bytes / (total_ms / args.steps * 1e-3) / 1e9 / pk["hbm_gbs"]},
+        "phases_ms": {"route": sum(route_ms) / len(route_ms), "chain": chain_avg_ms, "reduce": sum(reduce_ms) / len(reduce_ms)},
+        "lib": {"strings": stats["strings"], "units": stats["units"], "panel_width": stats["panel_width"],
+                "team_warps": stats["team_warps"], "load_impurity_s": load_s},
+    }
+    if not args.no_cpu_baseline and world == 1:
+        n = REF_SAMPLE[cfg] * (4 if cfg <= 2 else 1)
+        rate, k, dt = oracle_rate(imp, batch, n)
+        line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": blas_threads(), "kind": "oracle",
+                                "sample": f"first {k} configurations of the same batch, {dt:.1f} s, oracle.trace_oracle.trace_batch (numpy fp64)"}
+    print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=2, choices=sorted(WORKLOADS))
+    ap.add_argument("--batch", type=int, default=0, help="configurations per GPU per step (default: BASELINE.json's batch)")
+    ap.add_argument("--schedule", default="thin", choices=["thin", "literal"])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank)
+    else:
+        run_ours(args, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()

@@ -42,6 +42,7 @@ extern "C" {
 
 #define CTQMC_OPT_SCHEDULE     1
 #define CTQMC_OPT_PANEL_WIDTH  2   /* columns carried per work unit: 8, 16, 32 (0 = automatic) */
+#define CTQMC_OPT_TIMING       3   /* 1: record CUDA events around the phases of every batch call (see ctqmc_last_timing) */
 
 typedef struct ctqmc_impurity ctqmc_impurity;   /* opaque; created by ctqmc_load_impurity, destroyed by ctqmc_free_impurity */
 
@@ -138,6 +139,13 @@ int ctqmc_bound_batch_host(ctqmc_impurity* imp, double beta, const ctqmc_batch* 
  * stats[3] = real multiply-adds executed by the chain kernel (padded tiles included),
  * stats[4] = algorithmic real flops of the schedule executed (2 per real MAC, 8 per complex MAC, unpadded dims). */
 int ctqmc_last_stats(ctqmc_impurity* imp, int64_t stats[8]);
+
+/* With CTQMC_OPT_TIMING = 1: device time in milliseconds of the phases of the most recent batch call on this handle,
+ * from CUDA events recorded on the call's stream (HOST output; synchronises that stream):
+ * ms[0] = validate + route + binning kernels, ms[1] = chain kernel(s) ("matrix multiplication ... kernels",
+ * with the propagator, rescale and trace fused), ms[2] = final reduction kernels, ms[3] = whole call.
+ * CTQMC_ERR_ARG if timing was not enabled when the call was made. */
+int ctqmc_last_timing(ctqmc_impurity* imp, double ms[4]);
 
 /* Thread-local description of the last error on this thread ("" if none). */
 const char* ctqmc_last_error(void);

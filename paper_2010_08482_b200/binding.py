@@ -18,10 +18,10 @@ LIB_PATH = os.path.join(HERE, "libctqmc_b200.so")
 CTQMC_OK, CTQMC_ERR_ARG, CTQMC_ERR_OOM, CTQMC_ERR_CUDA, CTQMC_ERR_UNSUPPORTED = 0, -1, -2, -3, -4
 CTQMC_STATUS_OK, CTQMC_STATUS_VANISHING, CTQMC_STATUS_INVALID = 0, 1, 2
 CTQMC_SCHEDULE_THIN, CTQMC_SCHEDULE_LITERAL = 0, 1
-CTQMC_OPT_SCHEDULE, CTQMC_OPT_PANEL_WIDTH = 1, 2
+CTQMC_OPT_SCHEDULE, CTQMC_OPT_PANEL_WIDTH, CTQMC_OPT_TIMING = 1, 2, 3
 
 EXPORTS = ["ctqmc_load_impurity", "ctqmc_free_impurity", "ctqmc_set_option", "ctqmc_trace_batch", "ctqmc_bound_batch",
-           "ctqmc_trace_batch_host", "ctqmc_bound_batch_host", "ctqmc_last_stats", "ctqmc_last_error"]
+           "ctqmc_trace_batch_host", "ctqmc_bound_batch_host", "ctqmc_last_stats", "ctqmc_last_timing", "ctqmc_last_error"]
 
 
 class CtqmcError(RuntimeError):
@@ -68,6 +68,8 @@ def library() -> C.CDLL:
             fn.restype = C.c_int
         lib.ctqmc_last_stats.argtypes = [vp, C.POINTER(i64 * 8)]
         lib.ctqmc_last_stats.restype = C.c_int
+        lib.ctqmc_last_timing.argtypes = [vp, C.POINTER(dbl * 4)]
+        lib.ctqmc_last_timing.restype = C.c_int
         lib.ctqmc_last_error.argtypes = []
         lib.ctqmc_last_error.restype = C.c_char_p
         _lib = lib
@@ -143,6 +145,12 @@ def ctqmc_last_stats(imp: ImpurityHandle) -> dict:
     _check(library().ctqmc_last_stats(imp.ptr, C.byref(buf)))
     keys = ["strings", "units", "launches", "macs", "alg_flops", "panel_width", "team_warps", "large"]
     return dict(zip(keys, [int(x) for x in buf]))
+
+
+def ctqmc_last_timing(imp: ImpurityHandle) -> dict:
+    buf = (C.c_double * 4)()
+    _check(library().ctqmc_last_timing(imp.ptr, C.byref(buf)))
+    return dict(zip(["route_ms", "chain_ms", "reduce_ms", "total_ms"], [float(x) for x in buf]))
 
 
 def _stream_ptr(stream, host: bool = False):

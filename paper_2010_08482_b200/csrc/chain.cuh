@@ -6,12 +6,16 @@
 //        X' = 2^-k * diag(exp(-Delta (E - Emin))) * F_alpha(q) * X
 // on the FP64 tensor cores (mma.sync m8n8k4, SASS DMMA.8x8x4).  The operator block streams from the device store
 // (L2 / HBM) straight into A fragments (each element is needed by exactly one warp, so staging it in shared memory would
-// buy no reuse), the propagator is applied in the epilogue of the same step (never as a separate pass), the largest
-// |component| of X' is reduced with warp shuffles and becomes the exact power-of-two rescale of the next step, and the
-// last step is followed by the diagonal sum (trace) or the sum of squares (Frobenius norm of a segment).
+// buy no reuse), the propagator is applied in the epilogue of the same step (never as a separate pass) as a mantissa in
+// [1, 2) per row plus an integer row exponent; the largest exponent over non-zero rows is reduced with warp shuffles, goes
+// into the running exponent, and the rows are brought to it by exact powers of two (so neither long chains nor
+// Delta (E - Emin) >> 745 can overflow or underflow).  The last step is followed by the diagonal sum (trace) or the
+// sum of squares (Frobenius norm of a segment).
 // Work units are independent, so there is no inter-CTA communication: a persistent grid pulls units from an atomic
 // counter, heaviest first.
 #pragma once
+#include <climits>
+
 #include "common.cuh"
 
 namespace ctqmc {
@@ -50,7 +54,8 @@ __global__ void __launch_bounds__(kCtaThreads) chain_kernel(ChainParams P) {
 
   extern __shared__ __align__(16) double smem[];
   __shared__ unsigned long long s_unit[TEAMS];
-  __shared__ double s_red[2][TEAMS][TEAM_WARPS];
+  __shared__ double s_red[TEAMS][TEAM_WARPS];
+  __shared__ int s_exp[2][TEAMS][TEAM_WARPS];
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int team = warp / TEAM_WARPS, tw = warp % TEAM_WARPS;
@@ -117,7 +122,6 @@ __global__ void __launch_bounds__(kCtaThreads) chain_kernel(ChainParams P) {
     double* X = Xbuf0;
     double* Xn = Xbuf1;
     long long e2 = 0;
-    int kprev = 0;
     bool dead = false;
 
     for (int j = 0; j < nsteps; ++j) {
@@ -129,11 +133,9 @@ __global__ void __launch_bounds__(kCtaThreads) chain_kernel(ChainParams P) {
       const double delta = (i + 1 < L) ? (tau[i + 1] - tau[i]) : (P.bv.beta - tau[i] + tau[0]);
       const double* E = P.imp.energy + P.imp.e_off[qn];
       const double emin = P.imp.e_min[qn];
-      const double scale = pow2i(-kprev);
-      e2 += kprev;
       const int MT = (dn + 7) >> 3;
       const int nk = round_up(d, KS) / KS;
-      double wmax = 0.0;
+      int wexp = INT_MIN;
 
       for (int mt = tw; mt < MT; mt += TEAM_WARPS) {
         const int row = mt * 8 + g;
@@ -189,37 +191,82 @@ __global__ void __launch_bounds__(kCtaThreads) chain_kernel(ChainParams P) {
           for (int uu = 0; uu < U; ++uu) a_cur[uu] = a_nxt[uu];
         }
 
-        // epilogue: propagator row scaling fused with the pending power-of-two rescale; track max |component|
-        const double pr = (row < dn) ? exp(-delta * (E[row] - emin)) * scale : 0.0;
+        // epilogue, phase 1: the propagator exp(-Delta (E_row - Emin)) = 2^x is split into the mantissa 2^(x - floor x),
+        // multiplied in here, and the integer floor(x), which only enters the row's binary exponent (so no row can
+        // underflow, whatever Delta (E - Emin) is); track the largest exponent of a non-zero row.
+        double mr = 0.0;
+        int kr = 0;
+        if (row < dn) {
+          const double x = (-delta * (E[row] - emin)) * kLog2e;
+          const double kf = floor(x);
+          mr = exp2(x - kf);
+          kr = (int)fmax(kf, -1.0e9);
+        }
+        double rmax = 0.0;
 #pragma unroll
         for (int nt = 0; nt < NT; ++nt) {
           if (nt < ntu) {
             const int n = nt * 8 + 2 * t;
             if constexpr (CPLX) {
-              const double2 v0 = make_double2(acc[nt][0] * pr, acc[nt][2] * pr);
-              const double2 v1 = make_double2(acc[nt][1] * pr, acc[nt][3] * pr);
+              const double2 v0 = make_double2(acc[nt][0] * mr, acc[nt][2] * mr);
+              const double2 v1 = make_double2(acc[nt][1] * mr, acc[nt][3] * mr);
               *reinterpret_cast<double2*>(Xn + ((size_t)n * ldx + row) * 2) = v0;
               *reinterpret_cast<double2*>(Xn + ((size_t)(n + 1) * ldx + row) * 2) = v1;
-              wmax = fmax(fmax(wmax, fmax(fabs(v0.x), fabs(v0.y))), fmax(fabs(v1.x), fabs(v1.y)));
+              rmax = fmax(fmax(rmax, fmax(fabs(v0.x), fabs(v0.y))), fmax(fabs(v1.x), fabs(v1.y)));
             } else {
-              const double v0 = acc[nt][0] * pr, v1 = acc[nt][1] * pr;
+              const double v0 = acc[nt][0] * mr, v1 = acc[nt][1] * mr;
               Xn[(size_t)n * ldx + row] = v0;
               Xn[(size_t)(n + 1) * ldx + row] = v1;
-              wmax = fmax(wmax, fmax(fabs(v0), fabs(v1)));
+              rmax = fmax(rmax, fmax(fabs(v0), fabs(v1)));
+            }
+          }
+        }
+        rmax = fmax(rmax, __shfl_xor_sync(0xffffffffu, rmax, 1));
+        rmax = fmax(rmax, __shfl_xor_sync(0xffffffffu, rmax, 2));
+        if (rmax > 0.0) wexp = max(wexp, kr + ilogb(rmax));
+      }
+
+      // running exponent: largest row exponent over the team
+      wexp = __reduce_max_sync(0xffffffffu, wexp);
+      if (lane == 0) s_exp[j & 1][team][tw] = wexp;
+      team_sync<TEAM_WARPS>(team);
+      int kmax = INT_MIN;
+#pragma unroll
+      for (int w = 0; w < TEAM_WARPS; ++w) kmax = max(kmax, s_exp[j & 1][team][w]);
+      if (kmax == INT_MIN) { dead = true; break; }
+      e2 += kmax;
+
+      // epilogue, phase 2: every thread brings the elements it wrote to the common exponent (exact power of two;
+      // rows more than 2^-1022 below the largest flush to zero)
+      for (int mt = tw; mt < MT; mt += TEAM_WARPS) {
+        const int row = mt * 8 + g;
+        if (row < dn) {
+          const double x = (-delta * (E[row] - emin)) * kLog2e;
+          const int sh = (int)fmax(floor(x), -1.0e9) - kmax;
+          const bool slow = sh > 1022;
+          const double f = (sh < -1022) ? 0.0 : pow2i(min(sh, 1022));
+#pragma unroll
+          for (int nt = 0; nt < NT; ++nt) {
+            if (nt < ntu) {
+              const int n = nt * 8 + 2 * t;
+              if constexpr (CPLX) {
+                double2* p0 = reinterpret_cast<double2*>(Xn + ((size_t)n * ldx + row) * 2);
+                double2* p1 = reinterpret_cast<double2*>(Xn + ((size_t)(n + 1) * ldx + row) * 2);
+                double2 v0 = *p0, v1 = *p1;
+                if (slow) { v0.x = scalbn(v0.x, sh); v0.y = scalbn(v0.y, sh); v1.x = scalbn(v1.x, sh); v1.y = scalbn(v1.y, sh); }
+                else { v0.x *= f; v0.y *= f; v1.x *= f; v1.y *= f; }
+                *p0 = v0; *p1 = v1;
+              } else {
+                double* p0 = Xn + (size_t)n * ldx + row;
+                double* p1 = Xn + (size_t)(n + 1) * ldx + row;
+                if (slow) { *p0 = scalbn(*p0, sh); *p1 = scalbn(*p1, sh); }
+                else { *p0 *= f; *p1 *= f; }
+              }
             }
           }
         }
       }
-
-      // running exponent: max over the team, exact power of two applied in the next step's epilogue
-      wmax = warp_max(wmax);
-      if (lane == 0) s_red[j & 1][team][tw] = wmax;
       team_sync<TEAM_WARPS>(team);
-      double mx = 0.0;
-#pragma unroll
-      for (int w = 0; w < TEAM_WARPS; ++w) mx = fmax(mx, s_red[j & 1][team][w]);
-      if (!(mx > 0.0)) { dead = true; break; }
-      kprev = max(-1000, min(1000, ilogb(mx)));
       double* tmp = X; X = Xn; Xn = tmp;
       q = qn;
       d = dn;
@@ -264,11 +311,11 @@ __global__ void __launch_bounds__(kCtaThreads) chain_kernel(ChainParams P) {
       }
       ss = warp_sum(ss);
       team_sync<TEAM_WARPS>(team);
-      if (lane == 0) s_red[0][team][tw] = ss;
+      if (lane == 0) s_red[team][tw] = ss;
       team_sync<TEAM_WARPS>(team);
       if (tt == 0) {
         double tot = 0.0;
-        for (int w = 0; w < TEAM_WARPS; ++w) tot += s_red[0][team][w];
+        for (int w = 0; w < TEAM_WARPS; ++w) tot += s_red[team][w];
         Slot out; out.re = tot; out.im = 0.0; out.e2 = dead ? 0 : e2; out.pad = 0;
         P.slots[sr.slot + un.y] = out;
       }

@@ -85,6 +85,8 @@ struct ctqmc_impurity {
   Arena arena;
   cudaStream_t last_stream = nullptr;
   long long last_launches = 0;
+  int timing = 0, timing_valid = 0;
+  cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
 };
 
 namespace {
@@ -162,6 +164,10 @@ int ensure_arena(ctqmc_impurity* h, long long B, long long units_per_string) {
     a.cap_units = n_units;
   }
   return 0;
+}
+
+inline void mark(ctqmc_impurity* h, int i, cudaStream_t st) {
+  if (h->timing) cudaEventRecord(h->ev[i], st);
 }
 
 int check_batch_args(const ctqmc_impurity* h, double beta, const ctqmc_batch* batch) {
@@ -360,6 +366,7 @@ extern "C" void ctqmc_free_impurity(ctqmc_impurity* h) {
   cudaFree(a.status); cudaFree(a.survive); cudaFree(a.strings); cudaFree(a.units); cudaFree(a.slots); cudaFree(a.sector);
   cudaFree(a.cnt); cudaFree(a.xscratch); cudaFree(a.d_stage);
   if (a.h_stage) cudaFreeHost(a.h_stage);
+  for (int i = 0; i < 4; ++i) if (h->ev[i]) cudaEventDestroy(h->ev[i]);
   delete h;
 }
 
@@ -378,6 +385,13 @@ extern "C" int ctqmc_set_option(ctqmc_impurity* h, int option, int64_t value) {
     int rc = configure(h, (int)value);
     if (rc || h->large) { h->nt = nt; h->team_warps = tw; h->ldx = ldx; h->grid = grid; h->smem_bytes = sm; h->large = 0;
                           return rc ? rc : fail(CTQMC_ERR_UNSUPPORTED, "panel width %lld does not fit in shared memory for this impurity", (long long)value); }
+    return 0;
+  }
+  if (option == CTQMC_OPT_TIMING) {
+    if (value && !h->ev[0])
+      for (int i = 0; i < 4; ++i) CU(cudaEventCreate(&h->ev[i]));
+    h->timing = value ? 1 : 0;
+    h->timing_valid = 0;
     return 0;
   }
   return fail(CTQMC_ERR_ARG, "unknown option %d", option);
@@ -399,15 +413,21 @@ extern "C" int ctqmc_trace_batch(ctqmc_impurity* h, double beta, const ctqmc_bat
   if (h->large) { rc = large_ensure_scratch(h->dev, h->grid, h->nt, &h->arena.xscratch, &h->arena.xscratch_bytes); if (rc) return fail(rc, "scratch allocation failed"); }
   h->last_stream = st; h->last_launches = 0;
   BatchView bv; bv.B = B; bv.offset = (const long long*)batch->offset; bv.symbol = batch->symbol; bv.tau = batch->tau; bv.beta = beta;
+  h->timing_valid = 0;
+  mark(h, 0, st);
   rc = enqueue_routing(h, bv, survive, 0, 0, st);
   if (rc) return rc;
+  mark(h, 1, st);
   rc = enqueue_chain(h, bv, 0, 0, st);
   if (rc) return rc;
+  mark(h, 2, st);
   TraceReduceParams tp;
   tp.B = B; tp.Q = h->dev.Q; tp.status_in = h->arena.status; tp.survive = h->arena.survive; tp.strings = h->arena.strings;
   tp.slots = h->arena.slots; tp.mant = mant; tp.exp2 = (long long*)exp2; tp.status = status;
   trace_reduce_kernel<<<(unsigned)((B + 127) / 128), 128, 0, st>>>(tp);
   h->last_launches += 1;
+  mark(h, 3, st);
+  h->timing_valid = h->timing;
   CU(cudaGetLastError());
   return 0;
 }
@@ -432,12 +452,15 @@ extern "C" int ctqmc_bound_batch(ctqmc_impurity* h, double beta, const ctqmc_bat
   const long long nS = B * h->dev.Q;
   BatchView bv; bv.B = B; bv.offset = (const long long*)batch->offset; bv.symbol = batch->symbol; bv.tau = batch->tau; bv.beta = beta;
   h->last_stream = st; h->last_launches = 0;
+  h->timing_valid = 0;
   BoundParams bp;
   if (segment_len == 1) {
     rc = ensure_arena(h, B, 1);
     if (rc) return rc;
+    mark(h, 0, st);
     rc = enqueue_routing(h, bv, nullptr, 2, 1, st);
     if (rc) return rc;
+    mark(h, 1, st);
     bp.imp = h->dev; bp.bv = bv; bp.survive = h->arena.survive; bp.strings = h->arena.strings; bp.slots = h->arena.slots;
     bp.sector = h->arena.sector; bp.norm_kind = norm_kind; bp.segment_len = 1; bp.W = W;
     bound_s1_kernel<<<(unsigned)((nS * 32 + 255) / 256), 256, 0, st>>>(bp);
@@ -467,8 +490,10 @@ extern "C" int ctqmc_bound_batch(ctqmc_impurity* h, double beta, const ctqmc_bat
       }
       (void)max_units_per_string;
     }
+    mark(h, 0, st);
     rc = enqueue_routing(h, bv, nullptr, 1, S, st);
     if (rc) return rc;
+    mark(h, 1, st);
     rc = enqueue_chain(h, bv, 1, S, st);
     if (rc) return rc;
     bp.imp = h->dev; bp.bv = bv; bp.survive = h->arena.survive; bp.strings = h->arena.strings; bp.slots = h->arena.slots;
@@ -476,12 +501,15 @@ extern "C" int ctqmc_bound_batch(ctqmc_impurity* h, double beta, const ctqmc_bat
     bound_segments_kernel<<<(unsigned)((nS + 127) / 128), 128, 0, st>>>(bp);
     h->last_launches += 1;
   }
+  mark(h, 2, st);
   BoundReduceParams rp;
   rp.B = B; rp.Q = h->dev.Q; rp.status_in = h->arena.status; rp.survive = h->arena.survive; rp.sector = h->arena.sector;
   rp.bound_mant = bound_mant; rp.bound_exp2 = (long long*)bound_exp2; rp.sector_mant = sector_bound_mant;
   rp.sector_exp2 = (long long*)sector_bound_exp2; rp.status = status;
   bound_reduce_kernel<<<(unsigned)((B + 127) / 128), 128, 0, st>>>(rp);
   h->last_launches += 1;
+  mark(h, 3, st);
+  h->timing_valid = h->timing;
   CU(cudaGetLastError());
   return 0;
 }
@@ -599,6 +627,22 @@ extern "C" int ctqmc_last_stats(ctqmc_impurity* h, int64_t stats[8]) {
   stats[0] = (int64_t)c.n_strings; stats[1] = (int64_t)c.n_slots; stats[2] = h->last_launches;
   stats[3] = (int64_t)c.macs; stats[4] = (int64_t)c.alg_flops;
   stats[5] = h->nt * 8; stats[6] = h->team_warps; stats[7] = h->large;
+  return 0;
+}
+
+extern "C" int ctqmc_last_timing(ctqmc_impurity* h, double ms[4]) {
+  if (!h || !ms) return fail(CTQMC_ERR_ARG, "null argument");
+  if (!h->timing_valid) return fail(CTQMC_ERR_ARG, "no timed batch call on this handle (set CTQMC_OPT_TIMING first)");
+  CU(cudaSetDevice(h->device));
+  CU(cudaEventSynchronize(h->ev[3]));
+  for (int i = 0; i < 3; ++i) {
+    float f = 0.f;
+    CU(cudaEventElapsedTime(&f, h->ev[i], h->ev[i + 1]));
+    ms[i] = f;
+  }
+  float f = 0.f;
+  CU(cudaEventElapsedTime(&f, h->ev[0], h->ev[3]));
+  ms[3] = f;
   return 0;
 }
 

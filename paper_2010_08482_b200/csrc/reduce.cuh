@@ -131,6 +131,7 @@ __global__ void bound_s1_kernel(BoundParams P) {
   const int L = (int)(P.bv.offset[b + 1] - lo);
   double val = P.norm_kind == 0 ? sqrt((double)rec.dmin) : (double)rec.dmin;
   long long e = 0;
+  double lgx = 0.0;
   int q = q0;
   if (L == 0) {
     if (P.norm_kind == 0) {
@@ -151,14 +152,24 @@ __global__ void bound_s1_kernel(BoundParams P) {
       const double* E = P.imp.energy + P.imp.e_off[bd.dst];
       const double emin = P.imp.e_min[bd.dst];
       const double* rn = P.imp.rownorm2 + bd.rn_off;
-      double ss = 0.0;
-      for (int m = lane; m < bd.rows; m += 32) { double p = exp(-delta * (E[m] - emin)); ss += p * p * rn[m]; }
-      val *= sqrt(warp_sum(ss));
+      // ||diag(2^x) F||_F^2 = sum_m 4^x_m r_m relative to the largest x_m of a non-zero row (cannot underflow)
+      double xmax = -INFINITY;
+      for (int m = lane; m < bd.rows; m += 32)
+        if (rn[m] > 0.0) xmax = fmax(xmax, (-delta * (E[m] - emin)) * kLog2e);
+      xmax = warp_max(xmax);
+      if (xmax == -INFINITY) { val = 0.0; }
+      else {
+        double ss = 0.0;
+        for (int m = lane; m < bd.rows; m += 32)
+          if (rn[m] > 0.0) ss += exp2(2.0 * ((-delta * (E[m] - emin)) * kLog2e - xmax)) * rn[m];
+        val *= sqrt(warp_sum(ss));
+        lgx += xmax;
+      }
     }
     if (val != 0.0) { int k = ilogb(val); val = scalbn(val, -k); e += k; }
     q = bd.dst;
   }
-  if (lane == 0) P.sector[s] = finish_sector_bound(val, e, rec.lg);
+  if (lane == 0) P.sector[s] = finish_sector_bound(val, e, rec.lg + lgx);
 }
 
 // segment_len != 1, Frobenius: the chain kernel (mode 1) left sum |X|^2 per (segment, panel) in the slots; combine

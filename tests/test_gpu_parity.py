@@ -256,7 +256,11 @@ def _check_bound(lib, torch, imp, handle, batch, norm_kind, S, label):
                 assert sm[b, q0] == 0.0 and se[b, q0] == 0
             else:
                 dq = rel_diff(sm[b, q0], int(se[b, q0]), sec[0], sec[1])
-                assert dq <= TOL, f"{label} config {b} sector {q0}: rel diff {dq:.3e}"
+                # DESIGN.md reading A8 for bounds: a start sector whose bound is more than 2^-40 below the
+                # configuration's bound may be rounding-noise limited (segment products lose Delta (E - Emin) >> 36
+                # decades against the factor norms); it is checked to a factor 2 there, to 1e-9 otherwise.
+                negligible = sec[0] == 0 or (sec[1] - r["exp2"]) < -40
+                assert dq <= (1.0 if negligible else TOL), f"{label} config {b} sector {q0}: rel diff {dq:.3e}"
         w = abs(complex(mant[b, 0], mant[b, 1]))
         assert scaled_ge(bm[b], int(be[b]), w, int(exp2[b])), f"{label} config {b}: bound < |trace|"
 
@@ -289,3 +293,32 @@ def test_bound_edge_cases(lib, torch_cuda, impurities, handles):
     with pytest.raises(lib.CtqmcError) as ei:
         lib.ctqmc_bound_batch(handles(2), imp.beta, off, sym, tau, 1, 4)
     assert ei.value.code == -4
+
+
+# --------------------------------------------------------------------------- dynamic range inside a sector
+def test_coarse_sectors_do_not_underflow(lib, torch_cuda):
+    """Same inputs as the oracle pin test_P5_coarse_sectors_do_not_underflow: Delta (E_n - Emin) up to 4235 inside a
+    sector.  exp() of that underflows; the (mant, exp2) result must not."""
+    import numpy as np
+    from workloads import Batch
+    from workloads import impurity as wi
+    n, beta = 3, 60.0
+    eps = np.array([-2.0, 31.0, 75.0])
+    Umat = np.array([[0, 3.0, 1.0], [3.0, 0, 2.0], [1.0, 2.0, 0]])
+    u = np.zeros((n,) * 4)
+    for a in range(n):
+        for b_ in range(n):
+            if a != b_:
+                u[a, b_, b_, a] = Umat[a, b_]
+    imp = wi.build_impurity("ising-coarse", np.diag(eps), u, [(1,)] * n, beta=beta)
+    batch = Batch.from_lists(beta, [([5, 3, 2, 4], [1.0, 7.0, 19.5, 41.0]), ([5, 4], [3.0, 58.0]),
+                                    ([3, 5, 4, 2, 1, 0], [2.0, 2.5, 30.0, 44.0, 50.0, 59.0])])
+    h = lib.ctqmc_load_impurity(imp, 0)
+    try:
+        for sched in (lib.CTQMC_SCHEDULE_THIN, lib.CTQMC_SCHEDULE_LITERAL):
+            lib.ctqmc_set_option(h, lib.CTQMC_OPT_SCHEDULE, sched)
+            _check_trace(lib, torch_cuda, imp, h, batch, "ising-coarse")
+        for nk, S in ((0, 1), (1, 1), (0, 0), (0, 2)):
+            _check_bound(lib, torch_cuda, imp, h, batch, nk, S, f"ising-coarse-nk{nk}-S{S}")
+    finally:
+        h.free()
