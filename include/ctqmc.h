@@ -43,6 +43,17 @@ extern "C" {
 #define CTQMC_OPT_SCHEDULE     1
 #define CTQMC_OPT_PANEL_WIDTH  2   /* columns carried per work unit: 8, 16, 32 (0 = automatic) */
 #define CTQMC_OPT_TIMING       3   /* 1: record CUDA events around the phases of every batch call (see ctqmc_last_timing) */
+#define CTQMC_OPT_PATH         4   /* which chain kernel family runs (CTQMC_PATH_*); results agree up to rounding */
+
+/* Kernel families for CTQMC_OPT_PATH.  AUTO: the small-sector kernel (whole path in one launch, operator store in shared
+ * memory) when every sector has at most 16 states; else the shared-memory panel kernel when a panel of the largest sector
+ * fits in shared memory; else the large-sector tiled GEMM kernel (one launch per chain position; that path reads three
+ * integers back from the device before enqueueing its step loop, so the call is not fully asynchronous).
+ * ctqmc_bound_batch always uses the panel kernel family (or tables only, for segment_len 1). */
+#define CTQMC_PATH_AUTO        0
+#define CTQMC_PATH_PANEL       1
+#define CTQMC_PATH_LARGE       2
+#define CTQMC_PATH_SMALL       3
 
 typedef struct ctqmc_impurity ctqmc_impurity;   /* opaque; created by ctqmc_load_impurity, destroyed by ctqmc_free_impurity */
 
@@ -137,7 +148,9 @@ int ctqmc_bound_batch_host(ctqmc_impurity* imp, double beta, const ctqmc_batch* 
 /* Counters of the most recent batch call on this handle (HOST outputs; synchronises the stream it ran on):
  * stats[0] = surviving strings, stats[1] = work units, stats[2] = kernels launched by the call,
  * stats[3] = real multiply-adds executed by the chain kernel (padded tiles included),
- * stats[4] = algorithmic real flops of the schedule executed (2 per real MAC, 8 per complex MAC, unpadded dims). */
+ * stats[4] = algorithmic real flops of the schedule executed (2 per real MAC, 8 per complex MAC, unpadded dims),
+ * stats[5] = panel width (panel path) or lanes per configuration (small path), stats[6] = warps per team (panel path),
+ * stats[7] = kernel family that ran (CTQMC_PATH_PANEL / _LARGE / _SMALL). */
 int ctqmc_last_stats(ctqmc_impurity* imp, int64_t stats[8]);
 
 /* With CTQMC_OPT_TIMING = 1: device time in milliseconds of the phases of the most recent batch call on this handle,

@@ -197,9 +197,9 @@ __global__ void __launch_bounds__(kCtaThreads) chain_kernel(ChainParams P) {
         double mr = 0.0;
         int kr = 0;
         if (row < dn) {
-          const double x = (-delta * (E[row] - emin)) * kLog2e;
+          const double x = prop_x(delta, E[row], emin);
           const double kf = floor(x);
-          mr = exp2(x - kf);
+          mr = exp2(__dsub_rn(x, kf));
           kr = (int)fmax(kf, -1.0e9);
         }
         double rmax = 0.0;
@@ -241,7 +241,7 @@ __global__ void __launch_bounds__(kCtaThreads) chain_kernel(ChainParams P) {
       for (int mt = tw; mt < MT; mt += TEAM_WARPS) {
         const int row = mt * 8 + g;
         if (row < dn) {
-          const double x = (-delta * (E[row] - emin)) * kLog2e;
+          const double x = prop_x(delta, E[row], emin);
           const int sh = (int)fmax(floor(x), -1.0e9) - kmax;
           const bool slow = sh > 1022;
           const double f = (sh < -1022) ? 0.0 : pow2i(min(sh, 1022));

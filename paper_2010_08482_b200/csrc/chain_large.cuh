@@ -1,9 +1,346 @@
-// Large-sector chain kernel (sectors whose carried panel does not fit in shared memory) -- placeholder, see chain.cuh.
+// Large-sector chain path (SURVEY.md §8(a) a3-a5 for sectors whose carried matrix does not fit in shared memory, e.g. the
+// 1001 / 2002 / 3003-state sectors of the low-symmetry f-shell; PAPER.md:554 "858", :572 "matrix multiplication ... kernels").
+//
+// Here one chain step   X' = diag(exp(-Delta (E - Emin))) * F_alpha(q) * X   is a real dense contraction (hundreds of flop
+// per byte), so it runs as a tiled GEMM on the FP64 tensor cores: CTA tile 128 x 64, 8 warps of 32 x 32, operands staged
+// global -> shared by a 4-deep cp.async pipeline of 128-byte rows (XOR-swizzled so the 128-bit fragment loads are
+// bank-conflict free), mma.sync m8n8k4 f64 (SASS DMMA.8x8x4), complex as four real products on interleaved (re, im) storage.
+// All surviving strings of the batch advance together: one launch per chain position, grid = (tiles, strings).
+//
+// Fusion.  The propagator is never a separate pass (PAPER.md:572 has a separate "time evolution" kernel): its mantissa
+// 2^(x - floor x), x = -Delta (E_row - Emin) log2 e, is multiplied into the accumulators in the epilogue; its integer
+// part floor(x) stays a per-row binary exponent that the *next* step applies, together with the running-exponent
+// rescale, as one exact power-of-two factor per contraction index while it loads its B fragments (SURVEY a4 "applied
+// lazily in the next step's load").  The largest row exponent of a step is found with warp shuffles plus one atomicMax
+// per warp.  Only a shift of more than 2^1022 between a row and the largest row is clamped (flushes to zero / cannot
+// occur for operators with O(1) entries).
 #pragma once
+#include <climits>
+
 #include "chain.cuh"
 
 namespace ctqmc {
-inline int large_configure(const DevImp&, int, int*, size_t*, int*) { return -4; }
-inline int large_ensure_scratch(const DevImp&, int, int, double**, size_t*) { return -4; }
-inline int large_enqueue(const ChainParams&, int, size_t, int, double*, cudaStream_t) { return -4; }
+
+constexpr int kLBM = 128, kLBN = 64, kLStages = 4;
+constexpr int kLStageBytes = (kLBM + kLBN) * 128;
+
+struct LargeParams {
+  DevImp imp;
+  BatchView bv;
+  const StringRec* strings;
+  const int2* units;      // unit u -> (string index, 0)
+  long long u0;           // first unit of this group
+  int n_group;            // units in this group
+  int Lmax;               // plan stride
+  int ldx;                // leading dimension (elements) of an X column
+  long long xslab;        // elements per X buffer (one string, one parity)
+  double* X;              // [n_group][2][xslab] elements
+  int* plan_blk;          // [n_group][Lmax]
+  double* plan_delta;     // [n_group][Lmax]
+  int* kmax;              // [n_group][Lmax]
+  Slot* slots;
+};
+
+// One thread per string of the group: the sector walk in the (rotated) order the chain will be multiplied in.
+__global__ void large_plan_kernel(LargeParams P) {
+  const int s = blockIdx.x * blockDim.x + threadIdx.x;
+  if (s >= P.n_group) return;
+  const int2 un = P.units[P.u0 + s];
+  const StringRec sr = P.strings[un.x];
+  const int Q = P.imp.Q;
+  const long long b = un.x / Q;
+  const long long base = P.bv.offset[b];
+  const int L = (int)(P.bv.offset[b + 1] - base);
+  const int* sym = P.bv.symbol + base;
+  const double* tau = P.bv.tau + base;
+  int q = sr.q_start;
+  for (int j = 0; j < L; ++j) {
+    int i = sr.r + j;
+    if (i >= L) i -= L;
+    const int blk = P.imp.blk_of[sym[i] * Q + q];
+    P.plan_blk[(size_t)s * P.Lmax + j] = blk;
+    P.plan_delta[(size_t)s * P.Lmax + j] = (i + 1 < L) ? (tau[i + 1] - tau[i]) : (P.bv.beta - tau[i] + tau[0]);
+    P.kmax[(size_t)s * P.Lmax + j] = INT_MIN;
+    q = P.imp.blks[blk].dst;
+  }
+}
+
+// X_0 = identity (c x c, c = dim of the start sector); grid (column blocks, strings).
+template <bool CPLX>
+__global__ void large_init_kernel(LargeParams P) {
+  const int s = blockIdx.y;
+  const int2 un = P.units[P.u0 + s];
+  const StringRec sr = P.strings[un.x];
+  const int c = sr.c;
+  constexpr int ES = CPLX ? 2 : 1;
+  double* X = P.X + (size_t)s * 2 * P.xslab * ES;
+  const int dpad = round_up(c, 2);
+  for (int col = blockIdx.x; col < c; col += gridDim.x)
+    for (int k = threadIdx.x; k < dpad; k += blockDim.x) {
+      const double v = (k == col) ? 1.0 : 0.0;
+      if constexpr (CPLX) *reinterpret_cast<double2*>(X + ((size_t)col * P.ldx + k) * 2) = make_double2(v, 0.0);
+      else X[(size_t)col * P.ldx + k] = v;
+    }
+}
+
+__device__ __forceinline__ void cp_async16(void* smem, const void* gmem, bool valid) {
+  const unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
+  const int sz = valid ? 16 : 0;
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(sa), "l"(gmem), "r"(sz) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+// One chain position for every string of the group.  blockIdx.x = mt * NTmax + nt (nt fastest: CTAs that share rows of
+// F run together and hit L2), blockIdx.y = string.
+template <bool CPLX>
+__global__ void __launch_bounds__(256, 1) large_step_kernel(LargeParams P, int j, int NTmax) {
+  constexpr int ES = CPLX ? 2 : 1;
+  constexpr int BKE = CPLX ? 8 : 16;       // contraction indices per stage (128-byte rows)
+  extern __shared__ __align__(128) unsigned char lsm[];
+  double* sscale = reinterpret_cast<double*>(lsm + kLStages * kLStageBytes);
+
+  const int s = blockIdx.y;
+  const int2 un = P.units[P.u0 + s];
+  const StringRec sr = P.strings[un.x];
+  const int Q = P.imp.Q;
+  const long long bcfg = un.x / Q;
+  const int L = (int)(P.bv.offset[bcfg + 1] - P.bv.offset[bcfg]);
+  if (j >= L) return;
+  const int blk = P.plan_blk[(size_t)s * P.Lmax + j];
+  const BlkDesc bd = P.imp.blks[blk];
+  const int dn = bd.rows, d = bd.cols, c = sr.c;
+  const int mt0 = blockIdx.x / NTmax, nt0 = blockIdx.x - mt0 * NTmax;
+  const int m0 = mt0 * kLBM, n0 = nt0 * kLBN;
+  if (m0 >= dn || n0 >= c) return;
+
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int g = lane >> 2, t = lane & 3;
+  const int wm = warp >> 1, wn = warp & 1;
+  const double* Xin = P.X + ((size_t)s * 2 + (j & 1)) * P.xslab * ES;
+  double* Xout = P.X + ((size_t)s * 2 + ((j + 1) & 1)) * P.xslab * ES;
+  const int nkt = (d + BKE - 1) / BKE;
+
+  // exact power-of-two factor per contraction index: row exponent of the previous step minus its largest (a4)
+  {
+    int kprev = 0;
+    double dprev = 0.0;
+    if (j > 0) { kprev = P.kmax[(size_t)s * P.Lmax + j - 1]; dprev = P.plan_delta[(size_t)s * P.Lmax + j - 1]; }
+    const double* Eq = P.imp.energy + P.imp.e_off[bd.src];
+    const double emin = P.imp.e_min[bd.src];
+    for (int k = tid; k < nkt * BKE; k += 256) {
+      double f = 0.0;
+      if (k < d && kprev != INT_MIN) {
+        if (j == 0) f = 1.0;
+        else {
+          const double x = prop_x(dprev, Eq[k], emin);
+          const long long sh = (long long)fmax(floor(x), -1.0e9) - (long long)kprev;
+          f = (sh < -1022) ? 0.0 : pow2i((int)min(sh, 1022LL));
+        }
+      }
+      sscale[k] = f;
+    }
+  }
+
+  const unsigned char* Ag = reinterpret_cast<const unsigned char*>(P.imp.store + bd.off);
+  const unsigned char* Bg = reinterpret_cast<const unsigned char*>(Xin);
+  const int rows_pad = round_up(dn, 8);
+  const size_t a_row_bytes = (size_t)bd.ld * ES * 8, b_col_bytes = (size_t)P.ldx * ES * 8;
+  const int ld_chunks = bd.ld * ES / 2;          // 16-byte chunks per row of F (padded with zeros)
+  const int x_chunks = CPLX ? d : (d + 1) / 2;   // 16-byte chunks of an X column that hold data
+
+  auto load_stage = [&](int kt, int stage) {
+    unsigned char* As = lsm + stage * kLStageBytes;
+    unsigned char* Bs = As + kLBM * 128;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const int idx = tid + i * 256, r = idx >> 3, ch = idx & 7;
+      const int row = m0 + r, gch = kt * 8 + ch;
+      const bool ok = row < rows_pad && gch < ld_chunks;
+      cp_async16(As + r * 128 + ((ch ^ ((r & 1) << 2)) << 4), ok ? Ag + (size_t)row * a_row_bytes + (size_t)gch * 16 : Ag, ok);
+    }
+#pragma unroll
+    for (int i = 0; i < 2; ++i) {
+      const int idx = tid + i * 256, r = idx >> 3, ch = idx & 7;
+      const int col = n0 + r, gch = kt * 8 + ch;
+      const bool ok = col < c && gch < x_chunks;
+      cp_async16(Bs + r * 128 + ((ch ^ ((r & 1) << 2)) << 4), ok ? Bg + (size_t)col * b_col_bytes + (size_t)gch * 16 : Bg, ok);
+    }
+  };
+
+  double acc[4][4][CPLX ? 4 : 2];
+#pragma unroll
+  for (int a = 0; a < 4; ++a)
+#pragma unroll
+    for (int b = 0; b < 4; ++b)
+#pragma unroll
+      for (int x = 0; x < (CPLX ? 4 : 2); ++x) acc[a][b][x] = 0.0;
+
+#pragma unroll
+  for (int st = 0; st < kLStages - 1; ++st) {
+    if (st < nkt) load_stage(st, st);
+    cp_async_commit();
+  }
+
+  const int swz = (g & 1) << 2;
+  for (int kt = 0; kt < nkt; ++kt) {
+    cp_async_wait<kLStages - 2>();
+    __syncthreads();
+    {
+      const int nx = kt + kLStages - 1;
+      if (nx < nkt) load_stage(nx, nx % kLStages);
+      cp_async_commit();
+    }
+    const unsigned char* As = lsm + (kt % kLStages) * kLStageBytes;
+    const unsigned char* Bs = As + kLBM * 128;
+#pragma unroll
+    for (int sub = 0; sub < 2; ++sub) {
+      const int ch = sub * 4 + t;
+      const int so = ((ch ^ swz) << 4);
+      double2 a[4], b[4];
+#pragma unroll
+      for (int mt = 0; mt < 4; ++mt) a[mt] = *reinterpret_cast<const double2*>(As + (wm * 32 + mt * 8 + g) * 128 + so);
+#pragma unroll
+      for (int nt = 0; nt < 4; ++nt) b[nt] = *reinterpret_cast<const double2*>(Bs + (wn * 32 + nt * 8 + g) * 128 + so);
+      if constexpr (CPLX) {
+        const double f = sscale[kt * 8 + ch];
+#pragma unroll
+        for (int nt = 0; nt < 4; ++nt) { b[nt].x *= f; b[nt].y *= f; }
+#pragma unroll
+        for (int mt = 0; mt < 4; ++mt)
+#pragma unroll
+          for (int nt = 0; nt < 4; ++nt) {
+            dmma884(acc[mt][nt][0], acc[mt][nt][1], a[mt].x, b[nt].x);
+            dmma884(acc[mt][nt][2], acc[mt][nt][3], a[mt].x, b[nt].y);
+          }
+#pragma unroll
+        for (int mt = 0; mt < 4; ++mt) {
+          const double na = -a[mt].y;
+#pragma unroll
+          for (int nt = 0; nt < 4; ++nt) {
+            dmma884(acc[mt][nt][0], acc[mt][nt][1], na, b[nt].y);
+            dmma884(acc[mt][nt][2], acc[mt][nt][3], a[mt].y, b[nt].x);
+          }
+        }
+      } else {
+        const double2 f = *reinterpret_cast<const double2*>(sscale + kt * 16 + ch * 2);
+#pragma unroll
+        for (int nt = 0; nt < 4; ++nt) { b[nt].x *= f.x; b[nt].y *= f.y; }
+#pragma unroll
+        for (int mt = 0; mt < 4; ++mt)
+#pragma unroll
+          for (int nt = 0; nt < 4; ++nt) dmma884(acc[mt][nt][0], acc[mt][nt][1], a[mt].x, b[nt].x);
+#pragma unroll
+        for (int mt = 0; mt < 4; ++mt)
+#pragma unroll
+          for (int nt = 0; nt < 4; ++nt) dmma884(acc[mt][nt][0], acc[mt][nt][1], a[mt].y, b[nt].y);
+      }
+    }
+  }
+  cp_async_wait<0>();
+
+  // ---- epilogue: propagator mantissa, store, largest row exponent
+  const double delta = P.plan_delta[(size_t)s * P.Lmax + j];
+  const double* E = P.imp.energy + P.imp.e_off[bd.dst];
+  const double emin = P.imp.e_min[bd.dst];
+  int wexp = INT_MIN;
+#pragma unroll
+  for (int mt = 0; mt < 4; ++mt) {
+    const int row = m0 + wm * 32 + mt * 8 + g;
+    double mr = 0.0;
+    int kr = 0;
+    if (row < dn) {
+      const double x = prop_x(delta, E[row], emin);
+      const double kf = floor(x);
+      mr = exp2(__dsub_rn(x, kf));
+      kr = (int)fmax(kf, -1.0e9);
+    }
+    double rmax = 0.0;
+#pragma unroll
+    for (int nt = 0; nt < 4; ++nt) {
+      const int col = n0 + wn * 32 + nt * 8 + 2 * t;
+      if constexpr (CPLX) {
+        const double2 v0 = make_double2(acc[mt][nt][0] * mr, acc[mt][nt][2] * mr);
+        const double2 v1 = make_double2(acc[mt][nt][1] * mr, acc[mt][nt][3] * mr);
+        if (row < dn && col < c) {
+          *reinterpret_cast<double2*>(Xout + ((size_t)col * P.ldx + row) * 2) = v0;
+          rmax = fmax(rmax, fmax(fabs(v0.x), fabs(v0.y)));
+        }
+        if (row < dn && col + 1 < c) {
+          *reinterpret_cast<double2*>(Xout + ((size_t)(col + 1) * P.ldx + row) * 2) = v1;
+          rmax = fmax(rmax, fmax(fabs(v1.x), fabs(v1.y)));
+        }
+      } else {
+        const double v0 = acc[mt][nt][0] * mr, v1 = acc[mt][nt][1] * mr;
+        if (row < dn && col < c) { Xout[(size_t)col * P.ldx + row] = v0; rmax = fmax(rmax, fabs(v0)); }
+        if (row < dn && col + 1 < c) { Xout[(size_t)(col + 1) * P.ldx + row] = v1; rmax = fmax(rmax, fabs(v1)); }
+      }
+    }
+    rmax = fmax(rmax, __shfl_xor_sync(0xffffffffu, rmax, 1));
+    rmax = fmax(rmax, __shfl_xor_sync(0xffffffffu, rmax, 2));
+    if (rmax > 0.0) wexp = max(wexp, kr + ilogb(rmax));
+  }
+  wexp = __reduce_max_sync(0xffffffffu, wexp);
+  if (lane == 0 && wexp != INT_MIN) atomicMax(&P.kmax[(size_t)s * P.Lmax + j], wexp);
+}
+
+// Trace of the final matrix (a5): sum_n X[n][n] 2^(row exponent - largest), running exponent = sum of the steps' largest.
+template <bool CPLX>
+__global__ void large_finish_kernel(LargeParams P) {
+  constexpr int ES = CPLX ? 2 : 1;
+  __shared__ double red[2][8];
+  const int s = blockIdx.x;
+  const int2 un = P.units[P.u0 + s];
+  const StringRec sr = P.strings[un.x];
+  const int Q = P.imp.Q;
+  const long long bcfg = un.x / Q;
+  const int L = (int)(P.bv.offset[bcfg + 1] - P.bv.offset[bcfg]);
+  const int c = sr.c;
+  const int q = sr.q_start;
+  const double* E = P.imp.energy + P.imp.e_off[q];
+  const double emin = P.imp.e_min[q];
+  double re = 0.0, im = 0.0;
+  long long e2 = 0;
+  bool dead = false;
+  if (L == 0) {
+    for (int n = threadIdx.x; n < c; n += blockDim.x) re += exp(-P.bv.beta * (E[n] - emin));
+  } else {
+    for (int j = 0; j < L; ++j) {
+      const int k = P.kmax[(size_t)s * P.Lmax + j];
+      if (k == INT_MIN) { dead = true; break; }
+      e2 += k;
+    }
+    if (!dead) {
+      const int klast = P.kmax[(size_t)s * P.Lmax + L - 1];
+      const double dlast = P.plan_delta[(size_t)s * P.Lmax + L - 1];
+      const double* X = P.X + ((size_t)s * 2 + (L & 1)) * P.xslab * ES;
+      for (int n = threadIdx.x; n < c; n += blockDim.x) {
+        const double x = prop_x(dlast, E[n], emin);
+        const long long sh = (long long)fmax(floor(x), -1.0e9) - (long long)klast;
+        const double f = (sh < -1022) ? 0.0 : pow2i((int)min(sh, 1022LL));
+        if constexpr (CPLX) {
+          const double2 v = *reinterpret_cast<const double2*>(X + ((size_t)n * P.ldx + n) * 2);
+          re += v.x * f; im += v.y * f;
+        } else {
+          re += X[(size_t)n * P.ldx + n] * f;
+        }
+      }
+    }
+  }
+  re = warp_sum(re); im = warp_sum(im);
+  if ((threadIdx.x & 31) == 0) { red[0][threadIdx.x >> 5] = re; red[1][threadIdx.x >> 5] = im; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double tr = 0.0, ti = 0.0;
+    for (int w = 0; w < (int)(blockDim.x >> 5); ++w) { tr += red[0][w]; ti += red[1][w]; }
+    Slot out; out.re = dead ? 0.0 : tr; out.im = dead ? 0.0 : ti; out.e2 = dead ? 0 : e2; out.pad = 0;
+    P.slots[sr.slot] = out;
+  }
+}
+
+inline size_t large_smem_bytes(int dmax) {
+  return (size_t)kLStages * kLStageBytes + (size_t)((dmax + 15) / 16 * 16 + 16) * sizeof(double);
+}
+
 }  // namespace ctqmc

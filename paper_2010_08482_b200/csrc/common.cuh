@@ -71,6 +71,8 @@ struct Counters {
   unsigned long long next_unit;
   unsigned long long macs;        // real MACs executed (padded)
   unsigned long long alg_flops;   // algorithmic flops of the executed schedule
+  unsigned int max_len;           // longest chain among strings with work (large-sector path: number of step launches)
+  unsigned int max_c;             // widest carried matrix among them
   unsigned int class_count[kCostClasses];
   unsigned int class_base[kCostClasses];
   unsigned int class_cursor[kCostClasses];
@@ -87,6 +89,12 @@ __device__ __forceinline__ double warp_sum(double v) {
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
   return v;
+}
+
+// x = -Delta (E - Emin) log2(e) with every operation rounded on its own (no FMA contraction): the producer of a row
+// exponent floor(x) and its consumers (the rescale, the next step's load) must see bit-identical x.
+__device__ __forceinline__ double prop_x(double delta, double e, double emin) {
+  return __dmul_rn(__dmul_rn(-delta, __dsub_rn(e, emin)), kLog2e);
 }
 
 // exact 2^k for |k| <= 1022

@@ -5,6 +5,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -12,6 +13,7 @@
 
 #include "chain.cuh"
 #include "chain_large.cuh"
+#include "chain_small.cuh"
 #include "common.cuh"
 #include "reduce.cuh"
 #include "route.cuh"
@@ -59,8 +61,9 @@ struct Arena {
   Slot* slots = nullptr;
   Scaled* sector = nullptr;
   Counters* cnt = nullptr;
-  double* xscratch = nullptr;   // large-sector path: per-CTA global ping-pong panels
-  size_t xscratch_bytes = 0;
+  // large-sector path: carried matrices (two per string), step plan, per-step largest exponents
+  double* lx = nullptr; size_t lx_bytes = 0;
+  int* plan_blk = nullptr; double* plan_delta = nullptr; int* lkmax = nullptr; size_t plan_cap = 0;
   // host-variant staging
   void* h_stage = nullptr; size_t h_stage_bytes = 0;
   void* d_stage = nullptr; size_t d_stage_bytes = 0;
@@ -77,8 +80,13 @@ struct ctqmc_impurity {
   int* d_dim = nullptr; long long* d_eoff = nullptr; double* d_energy = nullptr; double* d_emin = nullptr;
   int* d_blkof = nullptr; BlkDesc* d_blks = nullptr; double* d_store = nullptr; double* d_rownorm2 = nullptr;
   double* d_sigma = nullptr;
+  double* d_pack = nullptr; int4* d_pblk = nullptr;   // small-sector path: unpadded store
+  int pack_len = 0, n_energy = 0;
+  int small_ok = 0, small = 0, small_g = 32, small_grid_max = 0;
+  size_t small_smem = 0;
   // schedule
   int schedule = CTQMC_SCHEDULE_THIN;
+  int path = CTQMC_PATH_AUTO;
   int nt = 0, team_warps = 8, ldx = 0, large = 0;
   size_t smem_bytes = 0;
   int grid = 0;
@@ -102,6 +110,12 @@ KernelFn pick_kernel(int cplx, int nt, int tw) {
   return nullptr;
 }
 
+using SmallFn = void (*)(SmallParams);
+SmallFn pick_small(int cplx, int g) {
+  if (cplx) return g == 8 ? small_trace_kernel<true, 8> : g == 16 ? small_trace_kernel<true, 16> : small_trace_kernel<true, 32>;
+  return g == 8 ? small_trace_kernel<false, 8> : g == 16 ? small_trace_kernel<false, 16> : small_trace_kernel<false, 32>;
+}
+
 int pick_ldx(int cplx, int dmax) {
   int l = (dmax + 7) / 8 * 8;
   if (cplx) { while (l % 8 != 4) ++l; }       // 16-byte elements: conflict-free 128-bit fragment loads need ldx = 4 mod 8
@@ -113,20 +127,50 @@ int pick_ldx(int cplx, int dmax) {
 int configure(ctqmc_impurity* h, int want_w) {
   const int cplx = h->dev.cplx, es = cplx ? 2 : 1;
   const size_t smem_max = 227 * 1024 - 2048;
+  h->small = 0;
+  if (h->path == CTQMC_PATH_SMALL && !h->small_ok)
+    return fail(CTQMC_ERR_UNSUPPORTED, "the small-sector kernel needs all sectors <= 16 states and a store that fits in shared memory");
+  if (h->small_ok && (h->path == CTQMC_PATH_AUTO || h->path == CTQMC_PATH_SMALL)) {
+    int g = h->dev.dmax <= 2 ? 8 : h->dev.dmax <= 4 ? 16 : 32;
+    if (const char* e = getenv("CTQMC_SMALL_G")) { int v = atoi(e); if (v == 8 || v == 16 || v == 32) g = v; }
+    h->small_g = g;
+    h->small_smem = small_common_bytes(h->dev.Q, h->dev.A, h->n_blocks, h->pack_len, h->n_energy, es) +
+                    (size_t)(kCtaThreads / g) * small_group_bytes(h->dev.Q, h->dev.dmax, es);
+    if (h->small_smem <= smem_max) {
+      SmallFn fn = pick_small(cplx, g);
+      CU(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->small_smem));
+      int occ = 0;
+      CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, kCtaThreads, h->small_smem));
+      if (occ >= 1) { h->small = 1; h->small_grid_max = occ * h->sm_count; }
+    }
+    if (!h->small && h->path == CTQMC_PATH_SMALL) return fail(CTQMC_ERR_UNSUPPORTED, "small-sector kernel does not fit in shared memory");
+  }
   h->ldx = pick_ldx(cplx, h->dev.dmax);
   h->team_warps = h->dev.dmax <= 16 ? 1 : 8;
   const int teams = kCtaWarps / h->team_warps;
   int nt_try[3] = {4, 2, 1};
   h->nt = 0;
-  for (int i = 0; i < 3; ++i) {
+  h->large = 0;
+  for (int i = 0; i < 3 && h->path != CTQMC_PATH_LARGE; ++i) {
     int nt = nt_try[i];
     if (want_w && nt * 8 != want_w) continue;
     if (!pick_kernel(cplx, nt, h->team_warps)) continue;
     size_t bytes = (size_t)teams * 2 * (8 * nt) * h->ldx * es * sizeof(double);
     if (bytes <= smem_max) { h->nt = nt; h->smem_bytes = bytes; break; }
   }
-  h->large = (h->nt == 0);
-  if (h->large) return large_configure(h->dev, h->sm_count, &h->grid, &h->smem_bytes, &h->nt);
+  if (h->path == CTQMC_PATH_PANEL && h->nt == 0)
+    return fail(CTQMC_ERR_UNSUPPORTED, "the shared-memory panel kernel cannot hold sectors of dimension %d", h->dev.dmax);
+  h->large = (h->nt == 0 || h->path == CTQMC_PATH_LARGE);
+  if (h->large) {
+    h->nt = 0;
+    h->ldx = (h->dev.dmax + 7) / 8 * 8;
+    h->smem_bytes = large_smem_bytes(h->dev.dmax);
+    if (h->smem_bytes > smem_max) return fail(CTQMC_ERR_UNSUPPORTED, "sector dimension %d exceeds the large-sector kernel's limit", h->dev.dmax);
+    if (cplx) CU(cudaFuncSetAttribute(large_step_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_bytes));
+    else      CU(cudaFuncSetAttribute(large_step_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_bytes));
+    h->grid = 0;
+    return 0;
+  }
   KernelFn fn = pick_kernel(cplx, h->nt, h->team_warps);
   CU(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_bytes));
   int occ = 0;
@@ -187,7 +231,7 @@ int enqueue_routing(ctqmc_impurity* h, const BatchView& bv, uint8_t* survive_out
   validate_kernel<<<(unsigned)((B + 255) / 256), 256, 0, st>>>(bv, h->dev.A, a.status);
   RouteParams rp;
   rp.imp = h->dev; rp.bv = bv; rp.status = a.status; rp.survive = a.survive; rp.survive_out = survive_out;
-  rp.strings = a.strings; rp.cnt = a.cnt; rp.W = 8 * h->nt; rp.kstep = h->dev.cplx ? 4 : 8;
+  rp.strings = a.strings; rp.cnt = a.cnt; rp.W = h->large ? (1 << 20) : 8 * h->nt; rp.kstep = h->dev.cplx ? 4 : 8;
   rp.literal = (h->schedule == CTQMC_SCHEDULE_LITERAL); rp.flops_per_mac = h->dev.cplx ? 8 : 2;
   rp.mode = mode; rp.segment_len = segment_len;
   route_kernel<<<(unsigned)((nS + 255) / 256), 256, 0, st>>>(rp);
@@ -207,13 +251,73 @@ int enqueue_chain(ctqmc_impurity* h, const BatchView& bv, int mode, int segment_
   cp.imp = h->dev; cp.bv = bv; cp.strings = a.strings; cp.units = a.units; cp.cnt = a.cnt; cp.slots = a.slots;
   cp.ldx = h->ldx; cp.mode = mode; cp.segment_len = segment_len;
   if (h->large) {
-    int rc = large_enqueue(cp, h->grid, h->smem_bytes, h->nt, a.xscratch, st);
-    if (rc) return fail(rc, "large-sector chain kernel launch failed");
+    return fail(CTQMC_ERR_UNSUPPORTED, "internal: large-sector path is driven by enqueue_large");
   } else {
     KernelFn fn = pick_kernel(h->dev.cplx, h->nt, h->team_warps);
     fn<<<h->grid, kCtaThreads, h->smem_bytes, st>>>(cp);
   }
   h->last_launches += 1;
+  CU(cudaGetLastError());
+  return 0;
+}
+
+
+// Large-sector path: one launch per chain position over all strings of a group (chain_large.cuh).  Reads back three
+// integers (strings with work, longest chain, widest carried matrix) to size the step loop and the carried matrices:
+// the one host synchronisation of this path.
+int enqueue_large(ctqmc_impurity* h, const BatchView& bv, cudaStream_t st) {
+  Arena& a = h->arena;
+  Counters c;
+  CU(cudaMemcpyAsync(&c, a.cnt, sizeof c, cudaMemcpyDeviceToHost, st));
+  CU(cudaStreamSynchronize(st));
+  const long long n_units = (long long)c.n_slots;
+  if (n_units == 0) return 0;
+  const int Lmax = (int)c.max_len > 0 ? (int)c.max_len : 1, cmax = (int)c.max_c > 0 ? (int)c.max_c : 1;
+  const int es = h->dev.cplx ? 2 : 1;
+  const long long xslab = (long long)cmax * h->ldx;
+  const size_t per_string = (size_t)2 * xslab * es * sizeof(double);
+  size_t free_b = 0, total_b = 0;
+  CU(cudaMemGetInfo(&free_b, &total_b));
+  const size_t budget = a.lx_bytes + (size_t)(0.7 * (double)free_b);
+  long long G = (long long)(budget / per_string);
+  if (G < 1) return fail(CTQMC_ERR_OOM, "not enough device memory for one carried matrix pair (%zu bytes)", per_string);
+  if (G > n_units) G = n_units;
+  if (G > 65535) G = 65535;
+  if ((size_t)G * per_string > a.lx_bytes) {
+    cudaFree(a.lx); a.lx = nullptr; a.lx_bytes = 0;
+    CU(cudaMalloc((void**)&a.lx, (size_t)G * per_string));
+    a.lx_bytes = (size_t)G * per_string;
+    CU(cudaMemsetAsync(a.lx, 0, a.lx_bytes, st));
+  }
+  if ((size_t)G * Lmax > a.plan_cap) {
+    cudaFree(a.plan_blk); cudaFree(a.plan_delta); cudaFree(a.lkmax);
+    a.plan_blk = nullptr; a.plan_delta = nullptr; a.lkmax = nullptr; a.plan_cap = 0;
+    const size_t n = (size_t)G * Lmax;
+    CU(cudaMalloc((void**)&a.plan_blk, n * sizeof(int)));
+    CU(cudaMalloc((void**)&a.plan_delta, n * sizeof(double)));
+    CU(cudaMalloc((void**)&a.lkmax, n * sizeof(int)));
+    a.plan_cap = n;
+  }
+  LargeParams lp;
+  lp.imp = h->dev; lp.bv = bv; lp.strings = a.strings; lp.units = a.units; lp.Lmax = Lmax; lp.ldx = h->ldx;
+  lp.xslab = xslab; lp.X = a.lx; lp.plan_blk = a.plan_blk; lp.plan_delta = a.plan_delta; lp.kmax = a.lkmax; lp.slots = a.slots;
+  const int MTmax = (h->dev.dmax + kLBM - 1) / kLBM, NTmax = (cmax + kLBN - 1) / kLBN;
+  for (long long u0 = 0; u0 < n_units; u0 += G) {
+    lp.u0 = u0; lp.n_group = (int)((n_units - u0 < G) ? (n_units - u0) : G);
+    large_plan_kernel<<<(lp.n_group + 127) / 128, 128, 0, st>>>(lp);
+    dim3 ig((unsigned)((cmax < 1024) ? cmax : 1024), (unsigned)lp.n_group);
+    dim3 sg((unsigned)(MTmax * NTmax), (unsigned)lp.n_group);
+    if (h->dev.cplx) {
+      large_init_kernel<true><<<ig, 256, 0, st>>>(lp);
+      for (int j = 0; j < Lmax; ++j) large_step_kernel<true><<<sg, 256, h->smem_bytes, st>>>(lp, j, NTmax);
+      large_finish_kernel<true><<<lp.n_group, 256, 0, st>>>(lp);
+    } else {
+      large_init_kernel<false><<<ig, 256, 0, st>>>(lp);
+      for (int j = 0; j < Lmax; ++j) large_step_kernel<false><<<sg, 256, h->smem_bytes, st>>>(lp, j, NTmax);
+      large_finish_kernel<false><<<lp.n_group, 256, 0, st>>>(lp);
+    }
+    h->last_launches += 3 + Lmax;
+  }
   CU(cudaGetLastError());
   return 0;
 }
@@ -277,6 +381,21 @@ extern "C" int ctqmc_load_impurity(const ctqmc_impurity_desc* desc, int device, 
     if (bd.cols > max_cols) max_cols = bd.cols;
   }
 
+  // small-sector path: the same blocks, row-major and unpadded (a few KB; lives in shared memory at run time)
+  std::vector<double> pack;
+  std::vector<int4> pblk(nb);
+  const bool small_ok = dmax <= 16 && nb <= 32767 && nb > 0;
+  if (small_ok) {
+    const double* raw = (const double*)desc->blk_data;
+    for (int b = 0; b < nb; ++b) {
+      const BlkDesc& bd = blks[b];
+      pblk[b] = make_int4((int)(pack.size() / es), bd.rows, bd.cols, bd.dst);
+      for (int m = 0; m < bd.rows; ++m)
+        for (int k = 0; k < bd.cols; ++k)
+          for (int c = 0; c < es; ++c) pack.push_back(raw[((size_t)raw_off[b] + (size_t)k * bd.rows + m) * es + c]);
+    }
+  }
+
   CU(cudaSetDevice(device));
   ctqmc_impurity* h = new (std::nothrow) ctqmc_impurity();
   if (!h) return fail(CTQMC_ERR_OOM, "host allocation failed");
@@ -300,6 +419,12 @@ extern "C" int ctqmc_load_impurity(const ctqmc_impurity_desc* desc, int device, 
   TRY(upload(&h->d_blkof, blkof));
   TRY(upload(&h->d_blks, blks));
   TRY(upload(&d_rawoff, raw_off));
+  if (small_ok) {
+    TRY(upload(&h->d_pack, pack));
+    TRY(upload(&h->d_pblk, pblk));
+    h->pack_len = (int)(pack.size() / es); h->small_ok = 1;
+  }
+  h->n_energy = (int)ne;
   TRY(upload(&d_voff, v_off));
   TRYCU(cudaMalloc((void**)&h->d_store, (size_t)(store_len ? store_len : 1) * sizeof(double)));
   TRYCU(cudaMemset(h->d_store, 0, (size_t)(store_len ? store_len : 1) * sizeof(double)));
@@ -361,10 +486,11 @@ extern "C" void ctqmc_free_impurity(ctqmc_impurity* h) {
   if (!h) return;
   cudaSetDevice(h->device);
   cudaFree(h->d_dim); cudaFree(h->d_eoff); cudaFree(h->d_energy); cudaFree(h->d_emin); cudaFree(h->d_blkof);
+  cudaFree(h->d_pack); cudaFree(h->d_pblk);
   cudaFree(h->d_blks); cudaFree(h->d_store); cudaFree(h->d_rownorm2); cudaFree(h->d_sigma);
   Arena& a = h->arena;
   cudaFree(a.status); cudaFree(a.survive); cudaFree(a.strings); cudaFree(a.units); cudaFree(a.slots); cudaFree(a.sector);
-  cudaFree(a.cnt); cudaFree(a.xscratch); cudaFree(a.d_stage);
+  cudaFree(a.cnt); cudaFree(a.lx); cudaFree(a.plan_blk); cudaFree(a.plan_delta); cudaFree(a.lkmax); cudaFree(a.d_stage);
   if (a.h_stage) cudaFreeHost(a.h_stage);
   for (int i = 0; i < 4; ++i) if (h->ev[i]) cudaEventDestroy(h->ev[i]);
   delete h;
@@ -387,6 +513,14 @@ extern "C" int ctqmc_set_option(ctqmc_impurity* h, int option, int64_t value) {
                           return rc ? rc : fail(CTQMC_ERR_UNSUPPORTED, "panel width %lld does not fit in shared memory for this impurity", (long long)value); }
     return 0;
   }
+  if (option == CTQMC_OPT_PATH) {
+    if (value != CTQMC_PATH_AUTO && value != CTQMC_PATH_PANEL && value != CTQMC_PATH_LARGE && value != CTQMC_PATH_SMALL) return fail(CTQMC_ERR_ARG, "unknown path %lld", (long long)value);
+    const int old = h->path;
+    h->path = (int)value;
+    int rc = configure(h, 0);
+    if (rc) { h->path = old; configure(h, 0); }
+    return rc;
+  }
   if (option == CTQMC_OPT_TIMING) {
     if (value && !h->ev[0])
       for (int i = 0; i < 4; ++i) CU(cudaEventCreate(&h->ev[i]));
@@ -407,18 +541,38 @@ extern "C" int ctqmc_trace_batch(ctqmc_impurity* h, double beta, const ctqmc_bat
   if (!mant || !exp2 || !status) return fail(CTQMC_ERR_ARG, "null output (mant, exp2 and status are required)");
   CU(cudaSetDevice(h->device));
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  const int W = 8 * h->nt;
-  rc = ensure_arena(h, B, (h->dev.dmax + W - 1) / W);
-  if (rc) return rc;
-  if (h->large) { rc = large_ensure_scratch(h->dev, h->grid, h->nt, &h->arena.xscratch, &h->arena.xscratch_bytes); if (rc) return fail(rc, "scratch allocation failed"); }
+  const int W = h->large ? (1 << 20) : 8 * h->nt;
+  if (h->small) { if (!h->arena.cnt) CU(cudaMalloc((void**)&h->arena.cnt, sizeof(Counters))); }
+  else { rc = ensure_arena(h, B, (h->dev.dmax + W - 1) / W); if (rc) return rc; }
   h->last_stream = st; h->last_launches = 0;
   BatchView bv; bv.B = B; bv.offset = (const long long*)batch->offset; bv.symbol = batch->symbol; bv.tau = batch->tau; bv.beta = beta;
   h->timing_valid = 0;
+  if (h->small) {
+    // everything (validation, routing, chain, trace, sector sum) in one launch: chain_small.cuh
+    Arena& a = h->arena;
+    mark(h, 0, st);
+    CU(cudaMemsetAsync(a.cnt, 0, sizeof(Counters), st));
+    mark(h, 1, st);
+    SmallParams sp;
+    sp.imp = h->dev; sp.bv = bv; sp.pack = h->d_pack; sp.pblk = h->d_pblk; sp.n_blocks = h->n_blocks; sp.pack_len = h->pack_len;
+    sp.n_energy = h->n_energy; sp.literal = (h->schedule == CTQMC_SCHEDULE_LITERAL); sp.mant = mant; sp.exp2 = (long long*)exp2;
+    sp.survive = survive; sp.status = status; sp.cnt = a.cnt; sp.dmax = h->dev.dmax;
+    const long long gpc = kCtaThreads / h->small_g;
+    long long grid = (B + gpc - 1) / gpc;
+    if (grid > h->small_grid_max) grid = h->small_grid_max;
+    pick_small(h->dev.cplx, h->small_g)<<<(unsigned)grid, kCtaThreads, h->small_smem, st>>>(sp);
+    h->last_launches += 1;
+    mark(h, 2, st);
+    mark(h, 3, st);
+    h->timing_valid = h->timing;
+    CU(cudaGetLastError());
+    return 0;
+  }
   mark(h, 0, st);
   rc = enqueue_routing(h, bv, survive, 0, 0, st);
   if (rc) return rc;
   mark(h, 1, st);
-  rc = enqueue_chain(h, bv, 0, 0, st);
+  rc = h->large ? enqueue_large(h, bv, st) : enqueue_chain(h, bv, 0, 0, st);
   if (rc) return rc;
   mark(h, 2, st);
   TraceReduceParams tp;
@@ -448,7 +602,7 @@ extern "C" int ctqmc_bound_batch(ctqmc_impurity* h, double beta, const ctqmc_bat
   if (segment_len != 1 && h->large) return fail(CTQMC_ERR_UNSUPPORTED, "segment_len != 1 is not implemented for sectors that do not fit in shared memory");
   CU(cudaSetDevice(h->device));
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  const int W = 8 * h->nt;
+  const int W = h->large ? (1 << 20) : 8 * h->nt;
   const long long nS = B * h->dev.Q;
   BatchView bv; bv.B = B; bv.offset = (const long long*)batch->offset; bv.symbol = batch->symbol; bv.tau = batch->tau; bv.beta = beta;
   h->last_stream = st; h->last_launches = 0;
@@ -619,6 +773,7 @@ extern "C" int ctqmc_bound_batch_host(ctqmc_impurity* h, double beta, const ctqm
 extern "C" int ctqmc_last_stats(ctqmc_impurity* h, int64_t stats[8]) {
   if (!h || !stats) return fail(CTQMC_ERR_ARG, "null argument");
   for (int i = 0; i < 8; ++i) stats[i] = 0;
+  stats[5] = h->small ? h->small_g : h->nt * 8; stats[6] = h->team_warps; stats[7] = h->small ? 3 : h->large ? 2 : 1;
   if (!h->arena.cnt) return 0;
   CU(cudaSetDevice(h->device));
   Counters c;
@@ -626,7 +781,6 @@ extern "C" int ctqmc_last_stats(ctqmc_impurity* h, int64_t stats[8]) {
   CU(cudaMemcpy(&c, h->arena.cnt, sizeof c, cudaMemcpyDeviceToHost));
   stats[0] = (int64_t)c.n_strings; stats[1] = (int64_t)c.n_slots; stats[2] = h->last_launches;
   stats[3] = (int64_t)c.macs; stats[4] = (int64_t)c.alg_flops;
-  stats[5] = h->nt * 8; stats[6] = h->team_warps; stats[7] = h->large;
   return 0;
 }
 

@@ -98,6 +98,8 @@ __global__ void route_kernel(RouteParams P) {
         rec.slot = (int)atomicAdd(&P.cnt->n_slots, (unsigned long long)rec.n_units);
         atomicAdd(&P.cnt->class_count[rec.cls], (unsigned)rec.n_units);
         atomicAdd(&P.cnt->n_strings, 1ull);
+        atomicMax(&P.cnt->max_len, (unsigned)L);
+        atomicMax(&P.cnt->max_c, (unsigned)rec.c);
         if (P.mode == 0) {
           atomicAdd(&P.cnt->macs, cost * (unsigned long long)(round_up(rec.c, 8)) * (unsigned long long)(P.flops_per_mac / 2));
           atomicAdd(&P.cnt->alg_flops, alg * (unsigned long long)rec.c * (unsigned long long)P.flops_per_mac);
