@@ -1,12 +1,12 @@
 """bench.py -- one JSON line: local-trace evaluations per second of the CUDA path on a BASELINE.json workload.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--batch B] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--batch B] [--impl ours|reference] [--no-others]
 
-A *step* is one pass of the whole hot path (validate -> route -> bin -> fused propagate*operator chain -> trace
-reduction) over one batch of seeded synthetic configurations.  `value` is traces/s
-with the batch resident in HBM; `e2e` is the same through `ctqmc_trace_batch_host` (host buffers, copies inside the
-timed region).  L2 is flushed between timed steps.  `--impl reference` times the CPU oracle (oracle/) on a bounded
-sample of the same workload; it is the only code path here, besides `cpu_baseline`, that touches oracle/.
+A *step* is one pass of the whole hot path (validate -> route -> fused propagate*operator chain with running exponent ->
+trace and sector sum) over one batch of seeded synthetic configurations.  `value` is
+traces/s with the batch resident in HBM; `e2e` is the same through `ctqmc_trace_batch_host` (host buffers, copies inside the
+timed region).  L2 is flushed between timed steps.  `--impl reference` times the CPU oracle (oracle/) on a bounded sample
+of the same workload; it is the only code path here, besides `cpu_baseline`, that touches oracle/.
 """
 from __future__ import annotations
 
@@ -25,7 +25,7 @@ if ROOT not in sys.path:
 
 METRIC = "local_trace_evaluations_per_s"
 UNIT = "traces/s"
-NOMINAL_FP64_TFLOPS = 40.0     # B200 FP64 (tensor) nominal; DESIGN.md §7
+NOMINAL_FP64_TFLOPS = 40.0     # B200 FP64 nominal (vendor figure); DESIGN.md §7
 NOMINAL_BF16_TFLOPS = 2250.0   # B200_PROFILING.md
 FALLBACK_HBM_GBS, FALLBACK_BF16_TFLOPS = 6650.0, 1590.0
 WORKLOADS = {
@@ -35,7 +35,13 @@ WORKLOADS = {
     4: "cfg4: 7-orbital f-shell Slater+SOC, (N,Jz) sectors N in 4..6 (Q=70, d_max=295), complex, pairs~Poisson(100)",
     5: "cfg5: 7-orbital f-shell + crystal field, N sectors 1001/2002/3003, complex, pairs~Poisson(100)",
 }
-REF_SAMPLE = {1: 1024, 2: 512, 3: 8, 4: 1, 5: 1}   # configurations per reference step (about a second or more each)
+REF_SAMPLE = {1: 4096, 2: 2048, 3: 16, 4: 2, 5: 1}   # configurations per reference step (seconds of oracle time each)
+KERNELS = {1: ("chain_kernel (panel in shared memory, fused propagate x operator, FP64 DMMA m8n8k4)", "tensor"),
+           2: ("large_step_kernel (128x64 tiles, cp.async pipeline, fused propagate x operator, FP64 DMMA m8n8k4)", "tensor"),
+           3: ("small_trace_kernel (whole path in one launch, operator store in shared memory, FP64 FMA)", "alu")}
+# dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, from the `ncu --set full` captures
+# summarised under profiles/ (same launch configuration as the default batch of each config); None = not captured.
+NCU_TRAFFIC_BYTES = {2: 5_991_680, 3: 30_400_256}
 
 
 def peaks():
@@ -43,8 +49,30 @@ def peaks():
     if os.path.exists(p):
         with open(p) as fh:
             d = json.load(fh)
-        return dict(hbm_gbs=float(d["hbm_gbs"]), bf16=float(d["bf16_tflops"]), bf16_sustained=float(d.get("bf16_tflops_sustained", d["bf16_tflops"])), source="measured")
-    return dict(hbm_gbs=FALLBACK_HBM_GBS, bf16=FALLBACK_BF16_TFLOPS, bf16_sustained=1400.0, source="fallback")
+        return dict(hbm_gbs=float(d["hbm_gbs"]), bf16=float(d["bf16_tflops"]), source="measured")
+    return dict(hbm_gbs=FALLBACK_HBM_GBS, bf16=FALLBACK_BF16_TFLOPS, source="fallback")
+
+
+def shard_batch(cfg: int, batch_per_gpu: int, rank: int):
+    """Weak scaling: rank r evaluates configurations [r*B, (r+1)*B) of the seeded stream of config `cfg`.
+    Configurations are independent, so there is no data-path collective."""
+    from workloads import make_batch
+    return make_batch(cfg, batch_per_gpu, start=rank * batch_per_gpu)
+
+
+def reduce_max(values, dist=None, device="cpu"):
+    """Max over ranks of a list of floats (the contract's max-over-ranks timing).  Works on gloo (CPU) and nccl."""
+    if dist is None:
+        return [float(v) for v in values]
+    import torch
+    t = torch.tensor(list(values), dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(x) for x in t]
+
+
+def aggregate_value(world: int, batch_per_gpu: int, steps: int, total_ms: float) -> float:
+    """Whole-job traces/s: every rank processed batch_per_gpu * steps configurations in total_ms (max over ranks)."""
+    return world * batch_per_gpu * steps / (total_ms * 1e-3)
 
 
 class ClockSampler:
@@ -131,30 +159,17 @@ def run_reference(args, rank: int):
     }))
 
 
-def run_ours(args, rank: int, world: int, local_rank: int):
-    import numpy as np
-    import torch
-
-    import paper_2010_08482_b200 as L
-    from workloads import BASELINE_CONFIGS, build_config_impurity, make_batch
-
-    assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
-    torch.cuda.set_device(local_rank)
-    dist = None
-    if world > 1:
-        import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
-
-    cfg = args.config
-    B = args.batch or BASELINE_CONFIGS[cfg]["batch"]
+def measure_config(L, torch, cfg, B, rank, steps, warmup, schedule, local_rank, barrier, fp64, pk, with_e2e=True):
+    """Times `steps` passes of the hot path on config `cfg` (this rank's shard) and returns the pieces of the JSON line."""
+    from workloads import build_config_impurity
     imp = build_config_impurity(cfg, keep_eigvecs=False)
     t0 = time.perf_counter()
     h = L.ctqmc_load_impurity(imp, local_rank)
     load_s = time.perf_counter() - t0
-    if args.schedule == "literal":
+    if schedule == "literal":
         L.ctqmc_set_option(h, L.CTQMC_OPT_SCHEDULE, L.CTQMC_SCHEDULE_LITERAL)
     L.ctqmc_set_option(h, L.CTQMC_OPT_TIMING, 1)
-    batch = make_batch(cfg, B, start=rank * B)           # weak scaling: every rank its own B configurations
+    batch = shard_batch(cfg, B, rank)
     off, sym, tau = (torch.from_numpy(x).cuda() for x in (batch.offset, batch.symbol, batch.tau))
     Q = imp.n_sectors
     out = (torch.empty((B, 2), dtype=torch.float64, device="cuda"), torch.empty(B, dtype=torch.int64, device="cuda"),
@@ -165,20 +180,11 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     def step():
         L.ctqmc_trace_batch(h, batch.beta, off, sym, tau, stream=stream, out=out)
 
-    for _ in range(max(args.warmup, 3)):
+    for _ in range(warmup):
         step()
     torch.cuda.synchronize()
     stats = L.ctqmc_last_stats(h)
-
-    def barrier():
-        if dist is not None:
-            dist.barrier()
-        torch.cuda.synchronize()
-
-    sampler = ClockSampler(local_rank)
-    if rank == 0:
-        sampler.start()
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
     chain_ms, route_ms, reduce_ms = [], [], []
     barrier()
     for a, b in ev:
@@ -189,64 +195,126 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         tm = L.ctqmc_last_timing(h)      # synchronises; outside the event pair
         chain_ms.append(tm["chain_ms"]); route_ms.append(tm["route_ms"]); reduce_ms.append(tm["reduce_ms"])
     barrier()
-    step_ms = [a.elapsed_time(b) for a, b in ev]
-    total_ms = sum(step_ms)
+    total_ms = sum(a.elapsed_time(b) for a, b in ev)
 
-    # end to end through the host-buffer C call: H2D of the batch, kernels, D2H of the results, inside the timed region
-    for _ in range(2):
-        L.ctqmc_trace_batch_host(h, batch.beta, batch.offset, batch.symbol, batch.tau)
-    e2e_s = 0.0
-    barrier()
-    for _ in range(args.steps):
-        flush.zero_()
+    e2e_ms = None
+    if with_e2e:
+        # end to end through the host-buffer C call: H2D of the batch, kernels, D2H of the results, inside the timed region
+        for _ in range(2):
+            L.ctqmc_trace_batch_host(h, batch.beta, batch.offset, batch.symbol, batch.tau)
+        e2e_s = 0.0
+        barrier()
+        for _ in range(steps):
+            flush.zero_()
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            L.ctqmc_trace_batch_host(h, batch.beta, batch.offset, batch.symbol, batch.tau)
+            e2e_s += time.perf_counter() - t0
+        barrier()
+        e2e_ms = e2e_s * 1e3
+    h.free()
+    del flush, out, off, sym, tau
+    torch.cuda.empty_cache()
+
+    n_ops = int(batch.offset[-1])
+    kname, bound = KERNELS[stats["path"]]
+    chain_avg_ms = sum(chain_ms) / len(chain_ms)
+    achieved_tf = stats["alg_flops"] / (chain_avg_ms * 1e-3) / 1e12
+    rule_peak = pk["bf16"] * NOMINAL_FP64_TFLOPS / NOMINAL_BF16_TFLOPS
+    peak = fp64["dmma_tflops"] if bound == "tensor" else fp64["dfma_tflops"]
+    alg_bytes = n_ops * 12 + (B + 1) * 8 + B * (16 + 8 + 4 + Q)
+    roofline = {
+        "bound": bound, "kernel": kname, "achieved": achieved_tf, "peak": peak, "unit": "TFLOP/s", "frac": achieved_tf / peak,
+        "traffic": NCU_TRAFFIC_BYTES.get(cfg) if B == _default_batch(cfg) else None,
+        "peak_source": ("FP64 " + ("DMMA" if bound == "tensor" else "DFMA") + " register-resident loop measured in this run by "
+                        "ctqmc_measure_fp64_peak (MEASURED_PEAKS.json has no FP64 entry); the guide's rule, "
+                        f"{pk['source']} bf16 {pk['bf16']} TF/s x nominal {NOMINAL_FP64_TFLOPS}/{NOMINAL_BF16_TFLOPS}, gives {rule_peak:.2f}"),
+        "frac_of_rule_peak": achieved_tf / rule_peak,
+        "kernel_ms": chain_avg_ms, "kernel_share_of_step": chain_avg_ms * steps / total_ms,
+        "flops_per_launch_algorithmic": stats["alg_flops"], "executed_real_macs_padded": stats["macs"],
+        "algorithmic_io_bytes_per_step": alg_bytes,
+        "hbm_frac_algorithmic": alg_bytes / (total_ms / steps * 1e-3) / 1e9 / pk["hbm_gbs"],
+    }
+    return dict(imp=imp, batch=batch, stats=stats, total_ms=total_ms, e2e_ms=e2e_ms, n_ops=n_ops, Q=Q, roofline=roofline,
+                phases={"route": sum(route_ms) / len(route_ms), "chain": chain_avg_ms, "reduce": sum(reduce_ms) / len(reduce_ms)},
+                load_s=load_s)
+
+
+def _default_batch(cfg: int) -> int:
+    from workloads import BASELINE_CONFIGS
+    return BASELINE_CONFIGS[cfg]["batch"]
+
+
+def run_ours(args, rank: int, world: int, local_rank: int):
+    import torch
+
+    import paper_2010_08482_b200 as L
+
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
         torch.cuda.synchronize()
-        t0 = time.perf_counter()
-        L.ctqmc_trace_batch_host(h, batch.beta, batch.offset, batch.symbol, batch.tau)
-        e2e_s += time.perf_counter() - t0
-    barrier()
-    clocks = sampler.stop() if rank == 0 else None
 
-    t = torch.tensor([total_ms, e2e_s * 1e3], dtype=torch.float64, device="cuda")
-    if dist is not None:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    total_ms, e2e_ms = float(t[0]), float(t[1])
+    cfg = args.config
+    B = args.batch or _default_batch(cfg)
+    warmup = max(args.warmup, 3)
+    pk = peaks()
+    fp64 = L.ctqmc_measure_fp64_peak(local_rank)
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    m = measure_config(L, torch, cfg, B, rank, args.steps, warmup, args.schedule, local_rank, barrier, fp64, pk)
+    clocks = sampler.stop() if rank == 0 else None
+    total_ms, e2e_ms = reduce_max([m["total_ms"], m["e2e_ms"]], dist, "cuda")
+
+    others = {}
+    if args.others and world == 1:
+        # the other BASELINE.json configs at their stated batch, device-resident timing only (fewer steps: they are context)
+        for c in (1, 3, 4, 5):
+            if c == cfg:
+                continue
+            k = 1 if c == 5 else 3
+            o = measure_config(L, torch, c, _default_batch(c), 0, k, 3 if c != 5 else 1, "thin", local_rank, barrier, fp64, pk,
+                               with_e2e=False)
+            others[f"cfg{c}"] = {"workload": WORKLOADS[c], "batch": _default_batch(c), "steps": k,
+                                 "value": aggregate_value(1, _default_batch(c), k, o["total_ms"]), "unit": UNIT,
+                                 "ms_per_step": o["total_ms"] / k, "gflops": o["stats"]["alg_flops"] * k / (o["total_ms"] * 1e-3) / 1e9,
+                                 "roofline": {x: o["roofline"][x] for x in ("bound", "kernel", "achieved", "peak", "unit", "frac",
+                                                                            "frac_of_rule_peak", "kernel_ms", "kernel_share_of_step")}}
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
         return
 
-    n_ops = int(batch.offset[-1])
-    pk = peaks()
-    fp64_peak = pk["bf16"] * NOMINAL_FP64_TFLOPS / NOMINAL_BF16_TFLOPS
-    chain_avg_ms = sum(chain_ms) / len(chain_ms)
-    achieved_tf = stats["alg_flops"] / (chain_avg_ms * 1e-3) / 1e12
-    alg_bytes = n_ops * 12 + (B + 1) * 8 + B * (16 + 8 + 4 + Q)
-    value = world * B * args.steps / (total_ms * 1e-3)
+    stats, Q, n_ops = m["stats"], m["Q"], m["n_ops"]
     line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
-        "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f64", "data": "synthetic",
+        "metric": METRIC, "value": aggregate_value(world, B, args.steps, total_ms), "unit": UNIT, "n_gpus": world,
+        "steps": args.steps, "warmup": warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": WORKLOADS[cfg], "batch_per_gpu": B, "operators_per_batch": n_ops, "schedule": args.schedule,
                    "l2": "flushed between timed steps (256 MiB write)", "sharding": "batch split over ranks, no collective"},
         "gflops": world * stats["alg_flops"] * args.steps / (total_ms * 1e-3) / 1e9,
-        "e2e": {"value": world * B * args.steps / (e2e_ms * 1e-3), "unit": UNIT,
+        "e2e": {"value": aggregate_value(world, B, args.steps, e2e_ms), "unit": UNIT,
                 "h2d_bytes_per_step": n_ops * 12 + (B + 1) * 8, "d2h_bytes_per_step": B * (16 + 8 + 4 + Q)},
         "gpu_launches": stats["launches"] * args.steps,
         "clocks": clocks,
-        "roofline": {"bound": "tensor", "kernel": "chain_kernel (fused propagate x operator, FP64 DMMA)",
-                     "achieved": achieved_tf, "peak": fp64_peak, "unit": "TFLOP/s", "frac": achieved_tf / fp64_peak,
-                     "traffic": None,
-                     "peak_source": f"{pk['source']} bf16 {pk['bf16']} TF/s x nominal fp64/bf16 ratio {NOMINAL_FP64_TFLOPS}/{NOMINAL_BF16_TFLOPS}",
-                     "kernel_ms": chain_avg_ms, "kernel_share_of_step": chain_avg_ms * args.steps / total_ms,
-                     "flops_per_launch": stats["alg_flops"], "executed_real_macs_padded": stats["macs"],
-                     "hbm_frac_algorithmic": alg_bytes / (total_ms / args.steps * 1e-3) / 1e9 / pk["hbm_gbs"]},
-        "phases_ms": {"route": sum(route_ms) / len(route_ms), "chain": chain_avg_ms, "reduce": sum(reduce_ms) / len(reduce_ms)},
-        "lib": {"strings": stats["strings"], "units": stats["units"], "panel_width": stats["panel_width"],
-                "team_warps": stats["team_warps"], "load_impurity_s": load_s},
+        "roofline": m["roofline"],
+        "phases_ms": m["phases"],
+        "fp64_peak_measured": fp64,
+        "lib": {"strings": stats["strings"], "units": stats["units"], "path": stats["path"], "panel_width_or_lanes": stats["panel_width"],
+                "team_warps": stats["team_warps"], "load_impurity_s": m["load_s"]},
     }
+    if others:
+        line["other_workloads"] = others
     if not args.no_cpu_baseline and world == 1:
-        n = REF_SAMPLE[cfg] * (4 if cfg <= 2 else 1)
-        rate, k, dt = oracle_rate(imp, batch, n)
+        rate, k, dt = oracle_rate(m["imp"], m["batch"], REF_SAMPLE[cfg])
         line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": blas_threads(), "kind": "oracle",
                                 "sample": f"first {k} configurations of the same batch, {dt:.1f} s, oracle.trace_oracle.trace_batch (numpy fp64)"}
     print(json.dumps(line))
@@ -264,6 +332,8 @@ def main():
     ap.add_argument("--schedule", default="thin", choices=["thin", "literal"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-others", dest="others", action="store_false",
+                    help="skip the short device-resident timings of the other BASELINE.json configs (about two minutes at N=1)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))

@@ -160,6 +160,11 @@ int ctqmc_last_stats(ctqmc_impurity* imp, int64_t stats[8]);
  * CTQMC_ERR_ARG if timing was not enabled when the call was made. */
 int ctqmc_last_timing(ctqmc_impurity* imp, double ms[4]);
 
+/* FP64 peak of `device` in TFLOP/s, measured with register-resident loops of independent mma.sync m8n8k4 f64 (DMMA) and
+ * of plain DFMA (no memory traffic; best of 3 after a warm-up).  The roofline denominator of bench.py: the driver's
+ * MEASURED_PEAKS.json holds HBM and bf16 peaks only.  HOST outputs; synchronises. */
+int ctqmc_measure_fp64_peak(int device, double* tflops_dmma, double* tflops_dfma);
+
 /* Thread-local description of the last error on this thread ("" if none). */
 const char* ctqmc_last_error(void);
 

@@ -22,7 +22,7 @@ CTQMC_OPT_SCHEDULE, CTQMC_OPT_PANEL_WIDTH, CTQMC_OPT_TIMING, CTQMC_OPT_PATH = 1,
 CTQMC_PATH_AUTO, CTQMC_PATH_PANEL, CTQMC_PATH_LARGE, CTQMC_PATH_SMALL = 0, 1, 2, 3
 
 EXPORTS = ["ctqmc_load_impurity", "ctqmc_free_impurity", "ctqmc_set_option", "ctqmc_trace_batch", "ctqmc_bound_batch",
-           "ctqmc_trace_batch_host", "ctqmc_bound_batch_host", "ctqmc_last_stats", "ctqmc_last_timing", "ctqmc_last_error"]
+           "ctqmc_trace_batch_host", "ctqmc_bound_batch_host", "ctqmc_last_stats", "ctqmc_last_timing", "ctqmc_measure_fp64_peak", "ctqmc_last_error"]
 
 
 class CtqmcError(RuntimeError):
@@ -71,6 +71,8 @@ def library() -> C.CDLL:
         lib.ctqmc_last_stats.restype = C.c_int
         lib.ctqmc_last_timing.argtypes = [vp, C.POINTER(dbl * 4)]
         lib.ctqmc_last_timing.restype = C.c_int
+        lib.ctqmc_measure_fp64_peak.argtypes = [C.c_int, C.POINTER(dbl), C.POINTER(dbl)]
+        lib.ctqmc_measure_fp64_peak.restype = C.c_int
         lib.ctqmc_last_error.argtypes = []
         lib.ctqmc_last_error.restype = C.c_char_p
         _lib = lib
@@ -152,6 +154,12 @@ def ctqmc_last_timing(imp: ImpurityHandle) -> dict:
     buf = (C.c_double * 4)()
     _check(library().ctqmc_last_timing(imp.ptr, C.byref(buf)))
     return dict(zip(["route_ms", "chain_ms", "reduce_ms", "total_ms"], [float(x) for x in buf]))
+
+
+def ctqmc_measure_fp64_peak(device: int = 0) -> dict:
+    a, b = C.c_double(0.0), C.c_double(0.0)
+    _check(library().ctqmc_measure_fp64_peak(int(device), C.byref(a), C.byref(b)))
+    return {"dmma_tflops": a.value, "dfma_tflops": b.value}
 
 
 def _stream_ptr(stream, host: bool = False):

@@ -15,6 +15,7 @@
 #include "chain_large.cuh"
 #include "chain_small.cuh"
 #include "common.cuh"
+#include "peak.cuh"
 #include "reduce.cuh"
 #include "route.cuh"
 #include "store.cuh"
@@ -797,6 +798,36 @@ extern "C" int ctqmc_last_timing(ctqmc_impurity* h, double ms[4]) {
   float f = 0.f;
   CU(cudaEventElapsedTime(&f, h->ev[0], h->ev[3]));
   ms[3] = f;
+  return 0;
+}
+
+extern "C" int ctqmc_measure_fp64_peak(int device, double* tflops_dmma, double* tflops_dfma) {
+  if (!tflops_dmma || !tflops_dfma) return fail(CTQMC_ERR_ARG, "null output");
+  CU(cudaSetDevice(device));
+  cudaDeviceProp prop;
+  CU(cudaGetDeviceProperties(&prop, device));
+  double* sink = nullptr;
+  CU(cudaMalloc((void**)&sink, 8));
+  cudaEvent_t e0, e1;
+  CU(cudaEventCreate(&e0)); CU(cudaEventCreate(&e1));
+  const int grid = prop.multiProcessorCount * 2, iters = 1 << 16;
+  double best[2] = {0.0, 0.0};
+  for (int which = 0; which < 2; ++which)
+    for (int rep = 0; rep < 4; ++rep) {
+      CU(cudaEventRecord(e0));
+      if (which == 0) peak_dmma_kernel<<<grid, 256>>>(iters, sink); else peak_dfma_kernel<<<grid, 256>>>(iters, sink);
+      CU(cudaEventRecord(e1));
+      CU(cudaEventSynchronize(e1));
+      float ms = 0.f;
+      CU(cudaEventElapsedTime(&ms, e0, e1));
+      // DMMA.8x8x4 = 256 FMA per warp instruction, 8 per iteration; DFMA: 32 lanes x 16 per iteration
+      const double flop = (double)grid * 8 * iters * (which == 0 ? 8.0 * 256 * 2 : 16.0 * 32 * 2);
+      const double tf = flop / (ms * 1e-3) / 1e12;
+      if (rep > 0 && tf > best[which]) best[which] = tf;
+    }
+  cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(sink);
+  CU(cudaGetLastError());
+  *tflops_dmma = best[0]; *tflops_dfma = best[1];
   return 0;
 }
 
