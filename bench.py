@@ -38,7 +38,8 @@ WORKLOADS = {
 REF_SAMPLE = {1: 4096, 2: 2048, 3: 16, 4: 2, 5: 1}   # configurations per reference step (seconds of oracle time each)
 KERNELS = {1: ("chain_kernel (panel in shared memory, fused propagate x operator, FP64 DMMA m8n8k4)", "tensor"),
            2: ("large_step_kernel (128x64 tiles, cp.async pipeline, fused propagate x operator, FP64 DMMA m8n8k4)", "tensor"),
-           3: ("small_trace_kernel (whole path in one launch, operator store in shared memory, FP64 FMA)", "alu")}
+           3: ("small_trace_kernel (whole path in one launch, operator store in shared memory, FP64 FMA)", "alu"),
+           4: ("grouped_step_kernel (strings sharing a block share one GEMM per chain position, 64x64 tiles, FP64 DMMA m8n8k4)", "tensor")}
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, from the `ncu --set full` captures
 # summarised under profiles/ (same launch configuration as the default batch of each config); None = not captured.
 NCU_TRAFFIC_BYTES = {2: 5_991_680, 3: 30_400_256}
@@ -159,7 +160,7 @@ def run_reference(args, rank: int):
     }))
 
 
-def measure_config(L, torch, cfg, B, rank, steps, warmup, schedule, local_rank, barrier, fp64, pk, with_e2e=True):
+def measure_config(L, torch, cfg, B, rank, steps, warmup, schedule, local_rank, barrier, fp64, pk, with_e2e=True, path="auto"):
     """Times `steps` passes of the hot path on config `cfg` (this rank's shard) and returns the pieces of the JSON line."""
     from workloads import build_config_impurity
     imp = build_config_impurity(cfg, keep_eigvecs=False)
@@ -168,6 +169,8 @@ def measure_config(L, torch, cfg, B, rank, steps, warmup, schedule, local_rank, 
     load_s = time.perf_counter() - t0
     if schedule == "literal":
         L.ctqmc_set_option(h, L.CTQMC_OPT_SCHEDULE, L.CTQMC_SCHEDULE_LITERAL)
+    if path != "auto":
+        L.ctqmc_set_option(h, L.CTQMC_OPT_PATH, {"panel": 1, "large": 2, "small": 3, "grouped": 4}[path])
     L.ctqmc_set_option(h, L.CTQMC_OPT_TIMING, 1)
     batch = shard_batch(cfg, B, rank)
     off, sym, tau = (torch.from_numpy(x).cuda() for x in (batch.offset, batch.symbol, batch.tau))
@@ -270,7 +273,7 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     sampler = ClockSampler(local_rank)
     if rank == 0:
         sampler.start()
-    m = measure_config(L, torch, cfg, B, rank, args.steps, warmup, args.schedule, local_rank, barrier, fp64, pk)
+    m = measure_config(L, torch, cfg, B, rank, args.steps, warmup, args.schedule, local_rank, barrier, fp64, pk, path=args.path)
     clocks = sampler.stop() if rank == 0 else None
     total_ms, e2e_ms = reduce_max([m["total_ms"], m["e2e_ms"]], dist, "cuda")
 
@@ -330,6 +333,8 @@ def main():
     ap.add_argument("--config", type=int, default=2, choices=sorted(WORKLOADS))
     ap.add_argument("--batch", type=int, default=0, help="configurations per GPU per step (default: BASELINE.json's batch)")
     ap.add_argument("--schedule", default="thin", choices=["thin", "literal"])
+    ap.add_argument("--path", default="auto", choices=["auto", "panel", "large", "small", "grouped"],
+                    help="kernel family (CTQMC_OPT_PATH); auto is what a user of the library gets")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-others", dest="others", action="store_false",

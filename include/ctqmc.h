@@ -54,6 +54,7 @@ extern "C" {
 #define CTQMC_PATH_PANEL       1
 #define CTQMC_PATH_LARGE       2
 #define CTQMC_PATH_SMALL       3
+#define CTQMC_PATH_GROUPED     4   /* step-synchronous grouped GEMM: strings that apply the same block share one GEMM per chain position */
 
 typedef struct ctqmc_impurity ctqmc_impurity;   /* opaque; created by ctqmc_load_impurity, destroyed by ctqmc_free_impurity */
 

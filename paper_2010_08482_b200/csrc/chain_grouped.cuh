@@ -1,0 +1,438 @@
+// Step-synchronous grouped path (SURVEY.md §8(a) a3-a5 for the "many moderate-sized matrices" regime, PAPER.md:31, :71:
+// configs 3-4, sector dimensions 1..295, thousands of strings in flight).
+//
+// All surviving strings of the batch advance one chain position per launch.  At a given position many strings apply the
+// SAME operator block F_alpha(q) (there are only a few hundred blocks), so their carried matrices are concatenated column-
+// wise and multiplied by F in one GEMM per block:   [X'_s1 | X'_s2 | ...] = F * [X_s1 | X_s2 | ...].
+// F is then read once per group instead of once per string, the N dimension is filled with real columns instead of the
+// 1..30 columns a single thin-start string carries, and the work is a dense contraction on the FP64 tensor cores
+// (mma.sync m8n8k4 f64, 64 x 64 CTA tiles, 4 warps of 32 x 32, cp.async pipeline of swizzled 128-byte rows).
+// The schedule (which string sits in which column of which tile at which chain position) is a pure function of the
+// routing result and is built once per call by three small kernels.
+//
+// Fusion (a3/a4): each column belongs to a string with its own time difference, so the propagator mantissa
+// 2^(x - floor x), x = -Delta_s (E_row - Emin) log2 e, is applied per (row, string) in the epilogue, the integer row
+// exponents floor(x) stay implicit and are re-derived bit-exactly (prop_x) by the next step, which folds "row exponent
+// minus the string's largest" into the B fragments as an exact power of two.  The largest exponent per string and step
+// is reduced with shared-memory atomics per tile and one global atomicMax per string run.
+#pragma once
+#include <climits>
+
+#include "chain_large.cuh"
+#include "chain_small.cuh"
+
+namespace ctqmc {
+
+constexpr int kGBM = 64, kGBN = 64, kGStages = 4, kGThreads = 128;
+constexpr int kGStageBytes = (kGBM + kGBN) * 128;
+
+struct GroupedParams {
+  DevImp imp;
+  BatchView bv;
+  const StringRec* strings;
+  const int2* units;
+  int n_units, Lmax, ldx, nb;
+  long long xtot;            // elements per parity buffer
+  double* X;                 // [2][xtot] elements
+  long long* xoff;           // [n_units] element offset of the unit's carried matrix
+  int* plan_blk;             // [n_units][Lmax]
+  double* plan_delta;        // [n_units][Lmax]
+  int* kmax;                 // [n_units][Lmax]
+  int* coff;                 // [n_units][Lmax] first column of the unit inside its block group
+  int* ulen;                 // [n_units] chain length
+  int* ucols;                // [n_units] columns carried
+  int* colcnt;               // [Lmax][nb]
+  int* colbase;              // [Lmax][nb]
+  int4* tiles;               // [Lmax][tile_cap] {block, first column, columns, -}
+  int* ntiles;               // [Lmax]
+  int2* colmap;              // [Lmax][col_cap] (unit, column of the unit)
+  int tile_cap;
+  long long col_cap;
+  Slot* slots;
+};
+
+// One thread per unit: sector walk in multiplication order, per-unit sizes.
+__global__ void grouped_plan_kernel(GroupedParams P) {
+  const int u = blockIdx.x * blockDim.x + threadIdx.x;
+  if (u >= P.n_units) return;
+  const int2 un = P.units[u];
+  const StringRec sr = P.strings[un.x];
+  const int Q = P.imp.Q;
+  const long long b = un.x / Q;
+  const long long base = P.bv.offset[b];
+  const int L = (int)(P.bv.offset[b + 1] - base);
+  const int* sym = P.bv.symbol + base;
+  const double* tau = P.bv.tau + base;
+  P.ulen[u] = L;
+  P.ucols[u] = sr.c;
+  int q = sr.q_start;
+  for (int j = 0; j < L; ++j) {
+    int i = sr.r + j;
+    if (i >= L) i -= L;
+    const int blk = P.imp.blk_of[sym[i] * Q + q];
+    P.plan_blk[(size_t)u * P.Lmax + j] = blk;
+    P.plan_delta[(size_t)u * P.Lmax + j] = (i + 1 < L) ? (tau[i + 1] - tau[i]) : (P.bv.beta - tau[i] + tau[0]);
+    P.kmax[(size_t)u * P.Lmax + j] = INT_MIN;
+    q = P.imp.blks[blk].dst;
+  }
+}
+
+// Exclusive prefix sum of ucols * ldx -> xoff (one CTA; n_units is at most a few hundred thousand on this path).
+__global__ void grouped_xoff_kernel(GroupedParams P) {
+  __shared__ long long s_part[1024];
+  __shared__ long long s_run;
+  if (threadIdx.x == 0) s_run = 0;
+  __syncthreads();
+  for (int base = 0; base < P.n_units; base += 1024) {
+    const int u = base + threadIdx.x;
+    const long long v = (u < P.n_units) ? (long long)P.ucols[u] * P.ldx : 0;
+    s_part[threadIdx.x] = v;
+    __syncthreads();
+    for (int o = 1; o < 1024; o <<= 1) {
+      long long add = (threadIdx.x >= o) ? s_part[threadIdx.x - o] : 0;
+      __syncthreads();
+      s_part[threadIdx.x] += add;
+      __syncthreads();
+    }
+    if (u < P.n_units) P.xoff[u] = s_run + s_part[threadIdx.x] - v;
+    __syncthreads();
+    if (threadIdx.x == 0) s_run += s_part[1023];
+    __syncthreads();
+  }
+}
+
+// Schedule, pass 1: columns per (chain position, block); each unit reserves its column range inside the group.
+__global__ void grouped_count_kernel(GroupedParams P) {
+  const long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (idx >= (long long)P.n_units * P.Lmax) return;
+  const int u = (int)(idx / P.Lmax), j = (int)(idx - (long long)u * P.Lmax);
+  if (j >= P.ulen[u]) return;
+  const int blk = P.plan_blk[idx];
+  P.coff[idx] = atomicAdd(&P.colcnt[(size_t)j * P.nb + blk], P.ucols[u]);
+}
+
+// Schedule, pass 2: one CTA per chain position; block groups -> column bases and the tile list.
+__global__ void grouped_tiles_kernel(GroupedParams P) {
+  const int j = blockIdx.x;
+  if (threadIdx.x != 0) return;
+  int col = 0, nt = 0;
+  for (int blk = 0; blk < P.nb; ++blk) {
+    const int cnt = P.colcnt[(size_t)j * P.nb + blk];
+    P.colbase[(size_t)j * P.nb + blk] = col;
+    for (int c0 = 0; c0 < cnt; c0 += kGBN) {
+      if (nt < P.tile_cap) P.tiles[(size_t)j * P.tile_cap + nt] = make_int4(blk, col + c0, min(kGBN, cnt - c0), 0);
+      ++nt;
+    }
+    col += cnt;
+  }
+  P.ntiles[j] = min(nt, P.tile_cap);
+}
+
+// Schedule, pass 3: column -> (unit, column of the unit).
+__global__ void grouped_fill_kernel(GroupedParams P) {
+  const long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (idx >= (long long)P.n_units * P.Lmax) return;
+  const int u = (int)(idx / P.Lmax), j = (int)(idx - (long long)u * P.Lmax);
+  if (j >= P.ulen[u]) return;
+  const int blk = P.plan_blk[idx];
+  const int c = P.ucols[u];
+  int2* dst = P.colmap + (size_t)j * P.col_cap + P.colbase[(size_t)j * P.nb + blk] + P.coff[idx];
+  for (int i = 0; i < c; ++i) dst[i] = make_int2(u, i);
+}
+
+// X_0 = identity for every unit (grid: units).
+template <bool CPLX>
+__global__ void grouped_init_kernel(GroupedParams P) {
+  constexpr int ES = CPLX ? 2 : 1;
+  const int u = blockIdx.x;
+  const int c = P.ucols[u];
+  double* X = P.X + P.xoff[u] * ES;
+  const int dpad = round_up(c, 2);
+  for (int idx = threadIdx.x; idx < c * dpad; idx += blockDim.x) {
+    const int col = idx / dpad, k = idx - col * dpad;
+    const double v = (k == col) ? 1.0 : 0.0;
+    if constexpr (CPLX) *reinterpret_cast<double2*>(X + ((size_t)col * P.ldx + k) * 2) = make_double2(v, 0.0);
+    else X[(size_t)col * P.ldx + k] = v;
+  }
+}
+
+// One chain position for every string: blockIdx.x = tile of the step's tile list, blockIdx.y = 64-row slab of F.
+template <bool CPLX>
+__global__ void __launch_bounds__(kGThreads, 2) grouped_step_kernel(GroupedParams P, int j) {
+  constexpr int ES = CPLX ? 2 : 1;
+  constexpr int BKE = CPLX ? 8 : 16;
+  extern __shared__ __align__(128) unsigned char gsm[];
+  __shared__ const unsigned char* s_xin[kGBN];
+  __shared__ double* s_xout[kGBN];
+  __shared__ double s_dprev[kGBN], s_delta[kGBN];
+  __shared__ int s_kprev[kGBN], s_u[kGBN], s_kmax[kGBN];
+  double* sde = reinterpret_cast<double*>(gsm + kGStages * kGStageBytes);   // E[k] - Emin of the source sector
+
+  if ((int)blockIdx.x >= P.ntiles[j]) return;
+  const int4 tl = P.tiles[(size_t)j * P.tile_cap + blockIdx.x];
+  const BlkDesc bd = P.imp.blks[tl.x];
+  const int dn = bd.rows, d = bd.cols, ncols = tl.z;
+  const int m0 = blockIdx.y * kGBM;
+  if (m0 >= dn) return;
+
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int g = lane >> 2, t = lane & 3;
+  const int wm = warp >> 1, wn = warp & 1;
+  const int nkt = (d + BKE - 1) / BKE;
+  const size_t par_in = (size_t)(j & 1) * P.xtot, par_out = (size_t)((j + 1) & 1) * P.xtot;
+
+  if (tid < kGBN) {
+    const int n = tid;
+    if (n < ncols) {
+      const int2 ui = P.colmap[(size_t)j * P.col_cap + tl.y + n];
+      const size_t idx = (size_t)ui.x * P.Lmax + j;
+      const size_t col = (size_t)P.xoff[ui.x] + (size_t)ui.y * P.ldx;
+      s_xin[n] = reinterpret_cast<const unsigned char*>(P.X + (par_in + col) * ES);
+      s_xout[n] = P.X + (par_out + col) * ES;
+      s_delta[n] = P.plan_delta[idx];
+      int kp = 0;
+      double dp = 0.0;               // j == 0: x = 0, shift 0, factor 1 (X_0 is the identity)
+      if (j > 0) { kp = P.kmax[idx - 1]; dp = P.plan_delta[idx - 1]; }
+      s_kprev[n] = (kp == INT_MIN) ? (1 << 29) : kp;   // a dead string keeps multiplying zeros
+      s_dprev[n] = dp;
+      s_u[n] = ui.x;
+    } else {
+      s_xin[n] = nullptr; s_xout[n] = nullptr; s_delta[n] = 0.0; s_dprev[n] = 0.0; s_kprev[n] = 1 << 29; s_u[n] = -1;
+    }
+    s_kmax[n] = INT_MIN;
+  }
+  {
+    const double* Eq = P.imp.energy + P.imp.e_off[bd.src];
+    const double emin = P.imp.e_min[bd.src];
+    for (int k = tid; k < nkt * BKE; k += kGThreads) sde[k] = (k < d) ? __dsub_rn(Eq[k], emin) : 0.0;
+  }
+  __syncthreads();
+
+  const unsigned char* Ag = reinterpret_cast<const unsigned char*>(P.imp.store + bd.off);
+  const int rows_pad = round_up(dn, 8);
+  const size_t a_row_bytes = (size_t)bd.ld * ES * 8;
+  const int ld_chunks = bd.ld * ES / 2;
+  const int x_chunks = CPLX ? d : (d + 1) / 2;
+
+  auto load_stage = [&](int kt, int stage) {
+    unsigned char* As = gsm + stage * kGStageBytes;
+    unsigned char* Bs = As + kGBM * 128;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const int idx = tid + i * kGThreads, r = idx >> 3, ch = idx & 7;
+      const int row = m0 + r, gch = kt * 8 + ch;
+      const bool ok = row < rows_pad && gch < ld_chunks;
+      cp_async16(As + r * 128 + ((ch ^ ((r & 1) << 2)) << 4), ok ? Ag + (size_t)row * a_row_bytes + (size_t)gch * 16 : Ag, ok);
+    }
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const int idx = tid + i * kGThreads, r = idx >> 3, ch = idx & 7;
+      const int gch = kt * 8 + ch;
+      const unsigned char* src = s_xin[r];
+      const bool ok = src != nullptr && gch < x_chunks;
+      cp_async16(Bs + r * 128 + ((ch ^ ((r & 1) << 2)) << 4), ok ? src + (size_t)gch * 16 : Ag, ok);
+    }
+  };
+
+  double acc[4][4][CPLX ? 4 : 2];
+#pragma unroll
+  for (int a = 0; a < 4; ++a)
+#pragma unroll
+    for (int b = 0; b < 4; ++b)
+#pragma unroll
+      for (int x = 0; x < (CPLX ? 4 : 2); ++x) acc[a][b][x] = 0.0;
+
+  // this lane's B-fragment columns: n = wn*32 + nt*8 + g
+  double ndp[4];
+  int kpv[4];
+#pragma unroll
+  for (int nt = 0; nt < 4; ++nt) { ndp[nt] = -s_dprev[wn * 32 + nt * 8 + g]; kpv[nt] = s_kprev[wn * 32 + nt * 8 + g]; }
+
+#pragma unroll
+  for (int st = 0; st < kGStages - 1; ++st) {
+    if (st < nkt) load_stage(st, st);
+    cp_async_commit();
+  }
+  const int swz = (g & 1) << 2;
+  for (int kt = 0; kt < nkt; ++kt) {
+    cp_async_wait<kGStages - 2>();
+    __syncthreads();
+    {
+      const int nx = kt + kGStages - 1;
+      if (nx < nkt) load_stage(nx, nx % kGStages);
+      cp_async_commit();
+    }
+    const unsigned char* As = gsm + (kt % kGStages) * kGStageBytes;
+    const unsigned char* Bs = As + kGBM * 128;
+#pragma unroll
+    for (int sub = 0; sub < 2; ++sub) {
+      const int ch = sub * 4 + t;
+      const int so = ((ch ^ swz) << 4);
+      double2 a[4], b[4];
+#pragma unroll
+      for (int mt = 0; mt < 4; ++mt) a[mt] = *reinterpret_cast<const double2*>(As + (wm * 32 + mt * 8 + g) * 128 + so);
+#pragma unroll
+      for (int nt = 0; nt < 4; ++nt) b[nt] = *reinterpret_cast<const double2*>(Bs + (wn * 32 + nt * 8 + g) * 128 + so);
+      if constexpr (CPLX) {
+        const double de = sde[kt * 8 + ch];
+#pragma unroll
+        for (int nt = 0; nt < 4; ++nt) {
+          const double x = __dmul_rn(__dmul_rn(ndp[nt], de), kLog2e);
+          const int sh = (int)fmax(floor(x), -1.0e9) - kpv[nt];
+          const double f = (sh < -1022) ? 0.0 : pow2i(min(sh, 1022));
+          b[nt].x *= f; b[nt].y *= f;
+        }
+#pragma unroll
+        for (int mt = 0; mt < 4; ++mt)
+#pragma unroll
+          for (int nt = 0; nt < 4; ++nt) {
+            dmma884(acc[mt][nt][0], acc[mt][nt][1], a[mt].x, b[nt].x);
+            dmma884(acc[mt][nt][2], acc[mt][nt][3], a[mt].x, b[nt].y);
+          }
+#pragma unroll
+        for (int mt = 0; mt < 4; ++mt) {
+          const double na = -a[mt].y;
+#pragma unroll
+          for (int nt = 0; nt < 4; ++nt) {
+            dmma884(acc[mt][nt][0], acc[mt][nt][1], na, b[nt].y);
+            dmma884(acc[mt][nt][2], acc[mt][nt][3], a[mt].y, b[nt].x);
+          }
+        }
+      } else {
+        const double2 de = *reinterpret_cast<const double2*>(sde + kt * 16 + ch * 2);
+#pragma unroll
+        for (int nt = 0; nt < 4; ++nt) {
+          const double x0 = __dmul_rn(__dmul_rn(ndp[nt], de.x), kLog2e), x1 = __dmul_rn(__dmul_rn(ndp[nt], de.y), kLog2e);
+          const int sh0 = (int)fmax(floor(x0), -1.0e9) - kpv[nt], sh1 = (int)fmax(floor(x1), -1.0e9) - kpv[nt];
+          b[nt].x *= (sh0 < -1022) ? 0.0 : pow2i(min(sh0, 1022));
+          b[nt].y *= (sh1 < -1022) ? 0.0 : pow2i(min(sh1, 1022));
+        }
+#pragma unroll
+        for (int mt = 0; mt < 4; ++mt)
+#pragma unroll
+          for (int nt = 0; nt < 4; ++nt) dmma884(acc[mt][nt][0], acc[mt][nt][1], a[mt].x, b[nt].x);
+#pragma unroll
+        for (int mt = 0; mt < 4; ++mt)
+#pragma unroll
+          for (int nt = 0; nt < 4; ++nt) dmma884(acc[mt][nt][0], acc[mt][nt][1], a[mt].y, b[nt].y);
+      }
+    }
+  }
+  cp_async_wait<0>();
+
+  // ---- epilogue: per (row, string) propagator mantissa, scatter to the strings' matrices, largest exponent per column
+  const double* E = P.imp.energy + P.imp.e_off[bd.dst];
+  const double emin = P.imp.e_min[bd.dst];
+  double er[4];
+#pragma unroll
+  for (int mt = 0; mt < 4; ++mt) {
+    const int row = m0 + wm * 32 + mt * 8 + g;
+    er[mt] = (row < dn) ? E[row] : emin;
+  }
+  int cur_u = -2;
+  double mr[4];
+  int kr[4];
+#pragma unroll
+  for (int nt = 0; nt < 4; ++nt) {
+#pragma unroll
+    for (int half = 0; half < 2; ++half) {
+      const int n = wn * 32 + nt * 8 + 2 * t + half;
+      const int u = s_u[n];
+      if (u < 0) continue;
+      if (u != cur_u) {   // columns of one string are adjacent: its row factors are computed once
+        cur_u = u;
+        const double delta = s_delta[n];
+#pragma unroll
+        for (int mt = 0; mt < 4; ++mt) {
+          const double x = prop_x(delta, er[mt], emin);
+          const double kf = floor(x);
+          mr[mt] = exp2(__dsub_rn(x, kf));
+          kr[mt] = (int)fmax(kf, -1.0e9);
+        }
+      }
+      double* xo = s_xout[n];
+      int cexp = INT_MIN;
+#pragma unroll
+      for (int mt = 0; mt < 4; ++mt) {
+        const int row = m0 + wm * 32 + mt * 8 + g;
+        if (row < dn) {
+          if constexpr (CPLX) {
+            const double2 v = make_double2(acc[mt][nt][half] * mr[mt], acc[mt][nt][2 + half] * mr[mt]);
+            *reinterpret_cast<double2*>(xo + (size_t)row * 2) = v;
+            const double mx = fmax(fabs(v.x), fabs(v.y));
+            if (mx > 0.0) cexp = max(cexp, kr[mt] + ilogb_fast(mx));
+          } else {
+            const double v = acc[mt][nt][half] * mr[mt];
+            xo[row] = v;
+            if (v != 0.0) cexp = max(cexp, kr[mt] + ilogb_fast(v));
+          }
+        }
+      }
+      if (cexp != INT_MIN) atomicMax(&s_kmax[n], cexp);
+    }
+  }
+  __syncthreads();
+  if (tid < ncols) {
+    const int u = s_u[tid];
+    if (tid == 0 || s_u[tid - 1] != u) {   // leader of a run of columns of the same string
+      int k = INT_MIN;
+      for (int n = tid; n < ncols && s_u[n] == u; ++n) k = max(k, s_kmax[n]);
+      if (k != INT_MIN) atomicMax(&P.kmax[(size_t)u * P.Lmax + j], k);
+    }
+  }
+}
+
+// Trace of each string's final matrix (a5); one CTA per unit.
+template <bool CPLX>
+__global__ void grouped_finish_kernel(GroupedParams P) {
+  constexpr int ES = CPLX ? 2 : 1;
+  __shared__ double red[2][8];
+  const int u = blockIdx.x;
+  const int2 un = P.units[u];
+  const StringRec sr = P.strings[un.x];
+  const int L = P.ulen[u], c = sr.c, q = sr.q_start;
+  const double* E = P.imp.energy + P.imp.e_off[q];
+  const double emin = P.imp.e_min[q];
+  double re = 0.0, im = 0.0;
+  long long e2 = 0;
+  bool dead = false;
+  if (L == 0) {
+    for (int n = threadIdx.x; n < c; n += blockDim.x) re += exp(-P.bv.beta * (E[n] - emin));
+  } else {
+    for (int j = 0; j < L; ++j) {
+      const int k = P.kmax[(size_t)u * P.Lmax + j];
+      if (k == INT_MIN) { dead = true; break; }
+      e2 += k;
+    }
+    if (!dead) {
+      const int klast = P.kmax[(size_t)u * P.Lmax + L - 1];
+      const double dlast = P.plan_delta[(size_t)u * P.Lmax + L - 1];
+      const double* X = P.X + ((size_t)(L & 1) * P.xtot + P.xoff[u]) * ES;
+      for (int n = threadIdx.x; n < c; n += blockDim.x) {
+        const long long sh = (long long)fmax(floor(prop_x(dlast, E[n], emin)), -1.0e9) - (long long)klast;
+        const double f = (sh < -1022) ? 0.0 : pow2i((int)min(sh, 1022LL));
+        if constexpr (CPLX) {
+          const double2 v = *reinterpret_cast<const double2*>(X + ((size_t)n * P.ldx + n) * 2);
+          re += v.x * f; im += v.y * f;
+        } else {
+          re += X[(size_t)n * P.ldx + n] * f;
+        }
+      }
+    }
+  }
+  re = warp_sum(re); im = warp_sum(im);
+  if ((threadIdx.x & 31) == 0) { red[0][threadIdx.x >> 5] = re; red[1][threadIdx.x >> 5] = im; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double tr = 0.0, ti = 0.0;
+    for (int w = 0; w < (int)(blockDim.x >> 5); ++w) { tr += red[0][w]; ti += red[1][w]; }
+    Slot out; out.re = dead ? 0.0 : tr; out.im = dead ? 0.0 : ti; out.e2 = dead ? 0 : e2; out.pad = 0;
+    P.slots[sr.slot] = out;
+  }
+}
+
+inline size_t grouped_smem_bytes(int dmax) {
+  return (size_t)kGStages * kGStageBytes + (size_t)((dmax + 15) / 16 * 16 + 16) * sizeof(double);
+}
+
+}  // namespace ctqmc

@@ -73,6 +73,7 @@ struct Counters {
   unsigned long long alg_flops;   // algorithmic flops of the executed schedule
   unsigned int max_len;           // longest chain among strings with work (large-sector path: number of step launches)
   unsigned int max_c;             // widest carried matrix among them
+  unsigned long long sum_c;       // total carried columns (grouped path: columns per chain position)
   unsigned int class_count[kCostClasses];
   unsigned int class_base[kCostClasses];
   unsigned int class_cursor[kCostClasses];

@@ -12,6 +12,7 @@
 #include <vector>
 
 #include "chain.cuh"
+#include "chain_grouped.cuh"
 #include "chain_large.cuh"
 #include "chain_small.cuh"
 #include "common.cuh"
@@ -53,6 +54,12 @@ int upload(T** dst, const std::vector<T>& v) {
   return 0;
 }
 
+struct DevBuf {   // grow-only device buffer
+  void* p = nullptr;
+  size_t cap = 0;
+  bool grew = false;
+};
+
 struct Arena {
   long long cap_strings = 0, cap_units = 0, cap_configs = 0;
   int* status = nullptr;
@@ -65,6 +72,8 @@ struct Arena {
   // large-sector path: carried matrices (two per string), step plan, per-step largest exponents
   double* lx = nullptr; size_t lx_bytes = 0;
   int* plan_blk = nullptr; double* plan_delta = nullptr; int* lkmax = nullptr; size_t plan_cap = 0;
+  // grouped path
+  DevBuf gx, gxoff, gplan_blk, gplan_delta, gkmax, gcoff, gulen, gucols, gcolcnt, gcolbase, gtiles, gntiles, gcolmap;
   // host-variant staging
   void* h_stage = nullptr; size_t h_stage_bytes = 0;
   void* d_stage = nullptr; size_t d_stage_bytes = 0;
@@ -88,7 +97,8 @@ struct ctqmc_impurity {
   // schedule
   int schedule = CTQMC_SCHEDULE_THIN;
   int path = CTQMC_PATH_AUTO;
-  int nt = 0, team_warps = 8, ldx = 0, large = 0;
+  int nt = 0, team_warps = 8, ldx = 0, large = 0, grouped = 0;
+  size_t grouped_smem = 0;
   size_t smem_bytes = 0;
   int grid = 0;
   Arena arena;
@@ -161,6 +171,14 @@ int configure(ctqmc_impurity* h, int want_w) {
   }
   if (h->path == CTQMC_PATH_PANEL && h->nt == 0)
     return fail(CTQMC_ERR_UNSUPPORTED, "the shared-memory panel kernel cannot hold sectors of dimension %d", h->dev.dmax);
+  h->grouped = 0;
+  if (h->path == CTQMC_PATH_GROUPED) {
+    h->grouped_smem = grouped_smem_bytes(h->dev.dmax);
+    if (h->grouped_smem > smem_max) return fail(CTQMC_ERR_UNSUPPORTED, "sector dimension %d exceeds the grouped kernel's limit", h->dev.dmax);
+    if (cplx) CU(cudaFuncSetAttribute(grouped_step_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->grouped_smem));
+    else      CU(cudaFuncSetAttribute(grouped_step_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->grouped_smem));
+    h->grouped = 1;
+  }
   h->large = (h->nt == 0 || h->path == CTQMC_PATH_LARGE);
   if (h->large) {
     h->nt = 0;
@@ -232,7 +250,7 @@ int enqueue_routing(ctqmc_impurity* h, const BatchView& bv, uint8_t* survive_out
   validate_kernel<<<(unsigned)((B + 255) / 256), 256, 0, st>>>(bv, h->dev.A, a.status);
   RouteParams rp;
   rp.imp = h->dev; rp.bv = bv; rp.status = a.status; rp.survive = a.survive; rp.survive_out = survive_out;
-  rp.strings = a.strings; rp.cnt = a.cnt; rp.W = h->large ? (1 << 20) : 8 * h->nt; rp.kstep = h->dev.cplx ? 4 : 8;
+  rp.strings = a.strings; rp.cnt = a.cnt; rp.W = (h->large || (h->grouped && mode == 0)) ? (1 << 20) : 8 * h->nt; rp.kstep = h->dev.cplx ? 4 : 8;
   rp.literal = (h->schedule == CTQMC_SCHEDULE_LITERAL); rp.flops_per_mac = h->dev.cplx ? 8 : 2;
   rp.mode = mode; rp.segment_len = segment_len;
   route_kernel<<<(unsigned)((nS + 255) / 256), 256, 0, st>>>(rp);
@@ -262,6 +280,71 @@ int enqueue_chain(ctqmc_impurity* h, const BatchView& bv, int mode, int segment_
   return 0;
 }
 
+
+int grow(DevBuf& b, size_t bytes) {
+  b.grew = false;
+  if (bytes <= b.cap) return 0;
+  cudaFree(b.p); b.p = nullptr; b.cap = 0;
+  const size_t want = bytes + bytes / 8;
+  CU(cudaMalloc(&b.p, want));
+  b.cap = want; b.grew = true;
+  return 0;
+}
+
+// Grouped path (chain_grouped.cuh): schedule for all chain positions, then one GEMM launch per position.  Like the
+// large path it reads the routing counters back once to size its buffers and the step loop.
+int enqueue_grouped(ctqmc_impurity* h, const BatchView& bv, cudaStream_t st) {
+  Arena& a = h->arena;
+  Counters c;
+  CU(cudaMemcpyAsync(&c, a.cnt, sizeof c, cudaMemcpyDeviceToHost, st));
+  CU(cudaStreamSynchronize(st));
+  const long long n_units = (long long)c.n_slots;
+  if (n_units == 0) return 0;
+  if (n_units > 2000000000LL / ((long long)c.max_len + 1)) return fail(CTQMC_ERR_UNSUPPORTED, "batch too large for the grouped path");
+  const int Lmax = (int)c.max_len > 0 ? (int)c.max_len : 1;
+  const long long sum_c = (long long)c.sum_c > 0 ? (long long)c.sum_c : 1;
+  const int es = h->dev.cplx ? 2 : 1, nb = h->n_blocks;
+  const int ldx = (h->dev.dmax + 7) / 8 * 8;
+  const long long xtot = sum_c * ldx;
+  const int tile_cap = (int)(sum_c / kGBN + (n_units < nb ? n_units : nb) + 1);
+  const size_t nul = (size_t)n_units * Lmax;
+  int rc;
+  if ((rc = grow(a.gx, (size_t)2 * xtot * es * sizeof(double)))) return rc;
+  if (a.gx.grew) CU(cudaMemsetAsync(a.gx.p, 0, a.gx.cap, st));
+  if ((rc = grow(a.gxoff, n_units * sizeof(long long))) || (rc = grow(a.gplan_blk, nul * sizeof(int))) ||
+      (rc = grow(a.gplan_delta, nul * sizeof(double))) || (rc = grow(a.gkmax, nul * sizeof(int))) ||
+      (rc = grow(a.gcoff, nul * sizeof(int))) || (rc = grow(a.gulen, n_units * sizeof(int))) ||
+      (rc = grow(a.gucols, n_units * sizeof(int))) || (rc = grow(a.gcolcnt, (size_t)Lmax * nb * sizeof(int))) ||
+      (rc = grow(a.gcolbase, (size_t)Lmax * nb * sizeof(int))) || (rc = grow(a.gtiles, (size_t)Lmax * tile_cap * sizeof(int4))) ||
+      (rc = grow(a.gntiles, (size_t)Lmax * sizeof(int))) || (rc = grow(a.gcolmap, (size_t)Lmax * sum_c * sizeof(int2))))
+    return rc;
+  GroupedParams gp;
+  gp.imp = h->dev; gp.bv = bv; gp.strings = a.strings; gp.units = a.units; gp.n_units = (int)n_units; gp.Lmax = Lmax; gp.ldx = ldx;
+  gp.nb = nb; gp.xtot = xtot; gp.X = (double*)a.gx.p; gp.xoff = (long long*)a.gxoff.p; gp.plan_blk = (int*)a.gplan_blk.p;
+  gp.plan_delta = (double*)a.gplan_delta.p; gp.kmax = (int*)a.gkmax.p; gp.coff = (int*)a.gcoff.p; gp.ulen = (int*)a.gulen.p;
+  gp.ucols = (int*)a.gucols.p; gp.colcnt = (int*)a.gcolcnt.p; gp.colbase = (int*)a.gcolbase.p; gp.tiles = (int4*)a.gtiles.p;
+  gp.ntiles = (int*)a.gntiles.p; gp.colmap = (int2*)a.gcolmap.p; gp.tile_cap = tile_cap; gp.col_cap = sum_c; gp.slots = a.slots;
+  CU(cudaMemsetAsync(gp.colcnt, 0, (size_t)Lmax * nb * sizeof(int), st));
+  const unsigned g_ul = (unsigned)((nul + 255) / 256);
+  grouped_plan_kernel<<<(unsigned)((n_units + 127) / 128), 128, 0, st>>>(gp);
+  grouped_xoff_kernel<<<1, 1024, 0, st>>>(gp);
+  grouped_count_kernel<<<g_ul, 256, 0, st>>>(gp);
+  grouped_tiles_kernel<<<Lmax, 32, 0, st>>>(gp);
+  grouped_fill_kernel<<<g_ul, 256, 0, st>>>(gp);
+  dim3 sg((unsigned)tile_cap, (unsigned)((h->dev.dmax + kGBM - 1) / kGBM));
+  if (h->dev.cplx) {
+    grouped_init_kernel<true><<<(unsigned)n_units, 128, 0, st>>>(gp);
+    for (int j = 0; j < Lmax; ++j) grouped_step_kernel<true><<<sg, kGThreads, h->grouped_smem, st>>>(gp, j);
+    grouped_finish_kernel<true><<<(unsigned)n_units, 256, 0, st>>>(gp);
+  } else {
+    grouped_init_kernel<false><<<(unsigned)n_units, 128, 0, st>>>(gp);
+    for (int j = 0; j < Lmax; ++j) grouped_step_kernel<false><<<sg, kGThreads, h->grouped_smem, st>>>(gp, j);
+    grouped_finish_kernel<false><<<(unsigned)n_units, 256, 0, st>>>(gp);
+  }
+  h->last_launches += 7 + Lmax;
+  CU(cudaGetLastError());
+  return 0;
+}
 
 // Large-sector path: one launch per chain position over all strings of a group (chain_large.cuh).  Reads back three
 // integers (strings with work, longest chain, widest carried matrix) to size the step loop and the carried matrices:
@@ -491,6 +574,8 @@ extern "C" void ctqmc_free_impurity(ctqmc_impurity* h) {
   cudaFree(h->d_blks); cudaFree(h->d_store); cudaFree(h->d_rownorm2); cudaFree(h->d_sigma);
   Arena& a = h->arena;
   cudaFree(a.status); cudaFree(a.survive); cudaFree(a.strings); cudaFree(a.units); cudaFree(a.slots); cudaFree(a.sector);
+  for (DevBuf* b : {&a.gx, &a.gxoff, &a.gplan_blk, &a.gplan_delta, &a.gkmax, &a.gcoff, &a.gulen, &a.gucols, &a.gcolcnt, &a.gcolbase,
+                     &a.gtiles, &a.gntiles, &a.gcolmap}) cudaFree(b->p);
   cudaFree(a.cnt); cudaFree(a.lx); cudaFree(a.plan_blk); cudaFree(a.plan_delta); cudaFree(a.lkmax); cudaFree(a.d_stage);
   if (a.h_stage) cudaFreeHost(a.h_stage);
   for (int i = 0; i < 4; ++i) if (h->ev[i]) cudaEventDestroy(h->ev[i]);
@@ -515,7 +600,7 @@ extern "C" int ctqmc_set_option(ctqmc_impurity* h, int option, int64_t value) {
     return 0;
   }
   if (option == CTQMC_OPT_PATH) {
-    if (value != CTQMC_PATH_AUTO && value != CTQMC_PATH_PANEL && value != CTQMC_PATH_LARGE && value != CTQMC_PATH_SMALL) return fail(CTQMC_ERR_ARG, "unknown path %lld", (long long)value);
+    if (value != CTQMC_PATH_AUTO && value != CTQMC_PATH_PANEL && value != CTQMC_PATH_LARGE && value != CTQMC_PATH_SMALL && value != CTQMC_PATH_GROUPED) return fail(CTQMC_ERR_ARG, "unknown path %lld", (long long)value);
     const int old = h->path;
     h->path = (int)value;
     int rc = configure(h, 0);
@@ -542,7 +627,7 @@ extern "C" int ctqmc_trace_batch(ctqmc_impurity* h, double beta, const ctqmc_bat
   if (!mant || !exp2 || !status) return fail(CTQMC_ERR_ARG, "null output (mant, exp2 and status are required)");
   CU(cudaSetDevice(h->device));
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  const int W = h->large ? (1 << 20) : 8 * h->nt;
+  const int W = (h->large || h->grouped) ? (1 << 20) : 8 * h->nt;
   if (h->small) { if (!h->arena.cnt) CU(cudaMalloc((void**)&h->arena.cnt, sizeof(Counters))); }
   else { rc = ensure_arena(h, B, (h->dev.dmax + W - 1) / W); if (rc) return rc; }
   h->last_stream = st; h->last_launches = 0;
@@ -573,7 +658,7 @@ extern "C" int ctqmc_trace_batch(ctqmc_impurity* h, double beta, const ctqmc_bat
   rc = enqueue_routing(h, bv, survive, 0, 0, st);
   if (rc) return rc;
   mark(h, 1, st);
-  rc = h->large ? enqueue_large(h, bv, st) : enqueue_chain(h, bv, 0, 0, st);
+  rc = h->grouped ? enqueue_grouped(h, bv, st) : h->large ? enqueue_large(h, bv, st) : enqueue_chain(h, bv, 0, 0, st);
   if (rc) return rc;
   mark(h, 2, st);
   TraceReduceParams tp;
@@ -774,7 +859,7 @@ extern "C" int ctqmc_bound_batch_host(ctqmc_impurity* h, double beta, const ctqm
 extern "C" int ctqmc_last_stats(ctqmc_impurity* h, int64_t stats[8]) {
   if (!h || !stats) return fail(CTQMC_ERR_ARG, "null argument");
   for (int i = 0; i < 8; ++i) stats[i] = 0;
-  stats[5] = h->small ? h->small_g : h->nt * 8; stats[6] = h->team_warps; stats[7] = h->small ? 3 : h->large ? 2 : 1;
+  stats[5] = h->small ? h->small_g : h->nt * 8; stats[6] = h->team_warps; stats[7] = h->small ? 3 : h->grouped ? 4 : h->large ? 2 : 1;
   if (!h->arena.cnt) return 0;
   CU(cudaSetDevice(h->device));
   Counters c;

@@ -100,6 +100,7 @@ __global__ void route_kernel(RouteParams P) {
         atomicAdd(&P.cnt->n_strings, 1ull);
         atomicMax(&P.cnt->max_len, (unsigned)L);
         atomicMax(&P.cnt->max_c, (unsigned)rec.c);
+        atomicAdd(&P.cnt->sum_c, (unsigned long long)rec.c);
         if (P.mode == 0) {
           atomicAdd(&P.cnt->macs, cost * (unsigned long long)(round_up(rec.c, 8)) * (unsigned long long)(P.flops_per_mac / 2));
           atomicAdd(&P.cnt->alg_flops, alg * (unsigned long long)rec.c * (unsigned long long)P.flops_per_mac);

@@ -231,6 +231,54 @@ def test_trace_parity_large_path_forced(cfg, n, schedule, lib, torch_cuda, impur
         lib.ctqmc_set_option(h, lib.CTQMC_OPT_PATH, lib.CTQMC_PATH_AUTO)
 
 
+@pytest.mark.parametrize("cfg,n", [(1, 64), (2, 64), (3, 24), (4, 4)])
+@pytest.mark.parametrize("schedule", ["thin", "literal"])
+def test_trace_parity_grouped_path(cfg, n, schedule, lib, torch_cuda, impurities, handles):
+    """Step-synchronous grouped GEMM path: strings sharing a block share a GEMM; columns gathered from / scattered to the
+    strings' own matrices.  Ragged tiles, real and complex, both schedules, element-wise against the oracle."""
+    from workloads import make_batch
+    h = handles(cfg)
+    lib.ctqmc_set_option(h, lib.CTQMC_OPT_PATH, lib.CTQMC_PATH_GROUPED)
+    try:
+        if schedule == "literal":
+            lib.ctqmc_set_option(h, lib.CTQMC_OPT_SCHEDULE, lib.CTQMC_SCHEDULE_LITERAL)
+        worst = _check_trace(lib, torch_cuda, impurities(cfg), h, make_batch(cfg, n, start=13000), f"cfg{cfg}-grouped-{schedule}")
+        assert lib.ctqmc_last_stats(h)["path"] == lib.CTQMC_PATH_GROUPED
+        print(f"cfg{cfg} grouped path {schedule}: worst relative difference {worst:.3e}")
+    finally:
+        lib.ctqmc_set_option(h, lib.CTQMC_OPT_SCHEDULE, lib.CTQMC_SCHEDULE_THIN)
+        lib.ctqmc_set_option(h, lib.CTQMC_OPT_PATH, lib.CTQMC_PATH_AUTO)
+
+
+def test_grouped_path_edge_cases_and_repeatability(lib, torch_cuda, impurities, handles):
+    from workloads import Batch, make_batch
+    imp = impurities(2)
+    h = handles(2)
+    good = make_batch(2, 3, start=960)
+    cfgs = [good.config(0), ([], []), ([1, 1, 1, 1], [1.0, 2.0, 3.0, 4.0]), ([1, 1], [1.0, 2.0]), ([1, 0], [3.0, 2.0]),
+            good.config(1), ([1, 0], [0.0, 0.0]), good.config(2)]
+    batch = Batch.from_lists(imp.beta, cfgs)
+    lib.ctqmc_set_option(h, lib.CTQMC_OPT_PATH, lib.CTQMC_PATH_GROUPED)
+    try:
+        _check_trace(lib, torch_cuda, imp, h, batch, "grouped-edge")
+    finally:
+        lib.ctqmc_set_option(h, lib.CTQMC_OPT_PATH, lib.CTQMC_PATH_AUTO)
+    # column order inside a group comes from atomics, the values must not depend on it
+    h3 = handles(3)
+    b3 = make_batch(3, 16, start=14000)
+    off, sym, tau = _dev(torch_cuda, b3)
+    lib.ctqmc_set_option(h3, lib.CTQMC_OPT_PATH, lib.CTQMC_PATH_GROUPED)
+    try:
+        a = lib.ctqmc_trace_batch(h3, b3.beta, off, sym, tau)
+        torch_cuda.cuda.synchronize()
+        b = lib.ctqmc_trace_batch(h3, b3.beta, off, sym, tau)
+        torch_cuda.cuda.synchronize()
+        for x, y in zip(a, b):
+            assert torch_cuda.equal(x, y)
+    finally:
+        lib.ctqmc_set_option(h3, lib.CTQMC_OPT_PATH, lib.CTQMC_PATH_AUTO)
+
+
 def test_large_path_edge_cases(lib, torch_cuda, impurities, handles):
     """Empty, vanishing, invalid and off-diagonal configurations through the large-sector path."""
     from workloads import Batch, make_batch
