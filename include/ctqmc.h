@@ -46,9 +46,10 @@ extern "C" {
 #define CTQMC_OPT_PATH         4   /* which chain kernel family runs (CTQMC_PATH_*); results agree up to rounding */
 
 /* Kernel families for CTQMC_OPT_PATH.  AUTO: the small-sector kernel (whole path in one launch, operator store in shared
- * memory) when every sector has at most 16 states; else the shared-memory panel kernel when a panel of the largest sector
- * fits in shared memory; else the large-sector tiled GEMM kernel (one launch per chain position; that path reads three
- * integers back from the device before enqueueing its step loop, so the call is not fully asynchronous).
+ * memory) when every sector has at most 16 states; else, when a panel of the largest sector fits in shared memory, the
+ * step-synchronous grouped GEMM kernel for batches of 32 configurations or more and the persistent shared-memory panel
+ * kernel for smaller ones; else the large-sector tiled GEMM kernel (one launch per chain position).  The grouped and the large path read the
+ * routing counters back from the device before enqueueing their step loop, so those calls are not fully asynchronous.
  * ctqmc_bound_batch always uses the panel kernel family (or tables only, for segment_len 1). */
 #define CTQMC_PATH_AUTO        0
 #define CTQMC_PATH_PANEL       1

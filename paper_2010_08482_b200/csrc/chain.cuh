@@ -200,7 +200,7 @@ __global__ void __launch_bounds__(kCtaThreads) chain_kernel(ChainParams P) {
           const double x = prop_x(delta, E[row], emin);
           const double kf = floor(x);
           mr = exp2(__dsub_rn(x, kf));
-          kr = (int)fmax(kf, -1.0e9);
+          kr = row_exp(x);
         }
         double rmax = 0.0;
 #pragma unroll
@@ -242,7 +242,7 @@ __global__ void __launch_bounds__(kCtaThreads) chain_kernel(ChainParams P) {
         const int row = mt * 8 + g;
         if (row < dn) {
           const double x = prop_x(delta, E[row], emin);
-          const int sh = (int)fmax(floor(x), -1.0e9) - kmax;
+          const int sh = row_exp(x) - kmax;
           const bool slow = sh > 1022;
           const double f = (sh < -1022) ? 0.0 : pow2i(min(sh, 1022));
 #pragma unroll

@@ -17,6 +17,7 @@
 // is reduced with shared-memory atomics per tile and one global atomicMax per string run.
 #pragma once
 #include <climits>
+#include <type_traits>
 
 #include "chain_large.cuh"
 #include "chain_small.cuh"
@@ -116,7 +117,8 @@ __global__ void grouped_tiles_kernel(GroupedParams P) {
   const int j = blockIdx.x;
   if (threadIdx.x != 0) return;
   int col = 0, nt = 0;
-  for (int blk = 0; blk < P.nb; ++blk) {
+  for (int o = 0; o < P.nb; ++o) {   // heaviest blocks first: the launch's tail is made of short tiles
+    const int blk = P.imp.blk_order[o];
     const int cnt = P.colcnt[(size_t)j * P.nb + blk];
     P.colbase[(size_t)j * P.nb + blk] = col;
     for (int c0 = 0; c0 < cnt; c0 += kGBN) {
@@ -156,9 +158,9 @@ __global__ void grouped_init_kernel(GroupedParams P) {
   }
 }
 
-// One chain position for every string: blockIdx.x = tile of the step's tile list, blockIdx.y = 64-row slab of F.
+// One chain position for every string: blockIdx.x = (tile of the step's tile list, 64-row slab of F).
 template <bool CPLX>
-__global__ void __launch_bounds__(kGThreads, 2) grouped_step_kernel(GroupedParams P, int j) {
+__global__ void __launch_bounds__(kGThreads, CPLX ? 2 : 3) grouped_step_kernel(GroupedParams P, int j, int MTmax) {
   constexpr int ES = CPLX ? 2 : 1;
   constexpr int BKE = CPLX ? 8 : 16;
   extern __shared__ __align__(128) unsigned char gsm[];
@@ -168,17 +170,22 @@ __global__ void __launch_bounds__(kGThreads, 2) grouped_step_kernel(GroupedParam
   __shared__ int s_kprev[kGBN], s_u[kGBN], s_kmax[kGBN];
   double* sde = reinterpret_cast<double*>(gsm + kGStages * kGStageBytes);   // E[k] - Emin of the source sector
 
-  if ((int)blockIdx.x >= P.ntiles[j]) return;
-  const int4 tl = P.tiles[(size_t)j * P.tile_cap + blockIdx.x];
+  const int tile_id = blockIdx.x / MTmax, slab = blockIdx.x - tile_id * MTmax;   // slabs of a tile are neighbours in launch order
+  if (tile_id >= P.ntiles[j]) return;
+  const int4 tl = P.tiles[(size_t)j * P.tile_cap + tile_id];
   const BlkDesc bd = P.imp.blks[tl.x];
   const int dn = bd.rows, d = bd.cols, ncols = tl.z;
-  const int m0 = blockIdx.y * kGBM;
+  const int m0 = slab * kGBM;
   if (m0 >= dn) return;
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int g = lane >> 2, t = lane & 3;
   const int wm = warp >> 1, wn = warp & 1;
   const int nkt = (d + BKE - 1) / BKE;
+  // 8-row / 8-column blocks are dealt to the warps round-robin, and blocks that are all padding are skipped: the tensor
+  // work is quantised to 8 x 8 although the CTA stages 64 x 64 tiles
+  const int mtu = ((min(kGBM, dn - m0) + 7) / 8 - wm + 1) / 2;
+  const int ntu = ((ncols + 7) / 8 - wn + 1) / 2;
   const size_t par_in = (size_t)(j & 1) * P.xtot, par_out = (size_t)((j + 1) & 1) * P.xtot;
 
   if (tid < kGBN) {
@@ -246,78 +253,94 @@ __global__ void __launch_bounds__(kGThreads, 2) grouped_step_kernel(GroupedParam
   double ndp[4];
   int kpv[4];
 #pragma unroll
-  for (int nt = 0; nt < 4; ++nt) { ndp[nt] = -s_dprev[wn * 32 + nt * 8 + g]; kpv[nt] = s_kprev[wn * 32 + nt * 8 + g]; }
+  for (int nt = 0; nt < 4; ++nt) { ndp[nt] = -s_dprev[(nt * 2 + wn) * 8 + g]; kpv[nt] = s_kprev[(nt * 2 + wn) * 8 + g]; }
 
-#pragma unroll
-  for (int st = 0; st < kGStages - 1; ++st) {
-    if (st < nkt) load_stage(st, st);
-    cp_async_commit();
-  }
-  const int swz = (g & 1) << 2;
-  for (int kt = 0; kt < nkt; ++kt) {
-    cp_async_wait<kGStages - 2>();
-    __syncthreads();
-    {
-      const int nx = kt + kGStages - 1;
-      if (nx < nkt) load_stage(nx, nx % kGStages);
+  // the main loop is instantiated for every (row blocks, column blocks) count of a warp, so partial tiles issue only the
+  // DMMAs they need and the loops stay fully unrolled
+  auto mainloop = [&](auto mtc, auto ntc) {
+    constexpr int MTU = decltype(mtc)::value, NTU = decltype(ntc)::value;
+  #pragma unroll
+    for (int st = 0; st < kGStages - 1; ++st) {
+      if (st < nkt) load_stage(st, st);
       cp_async_commit();
     }
-    const unsigned char* As = gsm + (kt % kGStages) * kGStageBytes;
-    const unsigned char* Bs = As + kGBM * 128;
-#pragma unroll
-    for (int sub = 0; sub < 2; ++sub) {
-      const int ch = sub * 4 + t;
-      const int so = ((ch ^ swz) << 4);
-      double2 a[4], b[4];
-#pragma unroll
-      for (int mt = 0; mt < 4; ++mt) a[mt] = *reinterpret_cast<const double2*>(As + (wm * 32 + mt * 8 + g) * 128 + so);
-#pragma unroll
-      for (int nt = 0; nt < 4; ++nt) b[nt] = *reinterpret_cast<const double2*>(Bs + (wn * 32 + nt * 8 + g) * 128 + so);
-      if constexpr (CPLX) {
-        const double de = sde[kt * 8 + ch];
-#pragma unroll
-        for (int nt = 0; nt < 4; ++nt) {
-          const double x = __dmul_rn(__dmul_rn(ndp[nt], de), kLog2e);
-          const int sh = (int)fmax(floor(x), -1.0e9) - kpv[nt];
-          const double f = (sh < -1022) ? 0.0 : pow2i(min(sh, 1022));
-          b[nt].x *= f; b[nt].y *= f;
-        }
-#pragma unroll
-        for (int mt = 0; mt < 4; ++mt)
-#pragma unroll
-          for (int nt = 0; nt < 4; ++nt) {
-            dmma884(acc[mt][nt][0], acc[mt][nt][1], a[mt].x, b[nt].x);
-            dmma884(acc[mt][nt][2], acc[mt][nt][3], a[mt].x, b[nt].y);
+    const int swz = (g & 1) << 2;
+    for (int kt = 0; kt < nkt; ++kt) {
+      cp_async_wait<kGStages - 2>();
+      __syncthreads();
+      {
+        const int nx = kt + kGStages - 1;
+        if (nx < nkt) load_stage(nx, nx % kGStages);
+        cp_async_commit();
+      }
+      const unsigned char* As = gsm + (kt % kGStages) * kGStageBytes;
+      const unsigned char* Bs = As + kGBM * 128;
+  #pragma unroll
+      for (int sub = 0; sub < 2; ++sub) {
+        const int ch = sub * 4 + t;
+        const int so = ((ch ^ swz) << 4);
+        double2 a[MTU > 0 ? MTU : 1], b[NTU > 0 ? NTU : 1];
+  #pragma unroll
+        for (int mt = 0; mt < MTU; ++mt) a[mt] = *reinterpret_cast<const double2*>(As + ((mt * 2 + wm) * 8 + g) * 128 + so);
+  #pragma unroll
+        for (int nt = 0; nt < NTU; ++nt) b[nt] = *reinterpret_cast<const double2*>(Bs + ((nt * 2 + wn) * 8 + g) * 128 + so);
+        if constexpr (CPLX) {
+          const double de = sde[kt * 8 + ch];
+  #pragma unroll
+          for (int nt = 0; nt < NTU; ++nt) {
+            const double x = __dmul_rn(__dmul_rn(ndp[nt], de), kLog2e);
+            const int sh = row_exp(x) - kpv[nt];
+            const double f = (sh < -1022) ? 0.0 : pow2i(min(sh, 1022));
+            b[nt].x *= f; b[nt].y *= f;
           }
-#pragma unroll
-        for (int mt = 0; mt < 4; ++mt) {
-          const double na = -a[mt].y;
-#pragma unroll
-          for (int nt = 0; nt < 4; ++nt) {
-            dmma884(acc[mt][nt][0], acc[mt][nt][1], na, b[nt].y);
-            dmma884(acc[mt][nt][2], acc[mt][nt][3], a[mt].y, b[nt].x);
+  #pragma unroll
+          for (int mt = 0; mt < MTU; ++mt)
+  #pragma unroll
+            for (int nt = 0; nt < NTU; ++nt)
+              {
+                dmma884(acc[mt][nt][0], acc[mt][nt][1], a[mt].x, b[nt].x);
+                dmma884(acc[mt][nt][2], acc[mt][nt][3], a[mt].x, b[nt].y);
+              }
+  #pragma unroll
+          for (int mt = 0; mt < MTU; ++mt) {
+            const double na = -a[mt].y;
+  #pragma unroll
+            for (int nt = 0; nt < NTU; ++nt)
+              {
+                dmma884(acc[mt][nt][0], acc[mt][nt][1], na, b[nt].y);
+                dmma884(acc[mt][nt][2], acc[mt][nt][3], a[mt].y, b[nt].x);
+              }
           }
+        } else {
+          const double2 de = *reinterpret_cast<const double2*>(sde + kt * 16 + ch * 2);
+  #pragma unroll
+          for (int nt = 0; nt < NTU; ++nt) {
+            const double x0 = __dmul_rn(__dmul_rn(ndp[nt], de.x), kLog2e), x1 = __dmul_rn(__dmul_rn(ndp[nt], de.y), kLog2e);
+            const int sh0 = row_exp(x0) - kpv[nt], sh1 = row_exp(x1) - kpv[nt];
+            b[nt].x *= (sh0 < -1022) ? 0.0 : pow2i(min(sh0, 1022));
+            b[nt].y *= (sh1 < -1022) ? 0.0 : pow2i(min(sh1, 1022));
+          }
+  #pragma unroll
+          for (int mt = 0; mt < MTU; ++mt)
+  #pragma unroll
+            for (int nt = 0; nt < NTU; ++nt)
+              dmma884(acc[mt][nt][0], acc[mt][nt][1], a[mt].x, b[nt].x);
+  #pragma unroll
+          for (int mt = 0; mt < MTU; ++mt)
+  #pragma unroll
+            for (int nt = 0; nt < NTU; ++nt)
+              dmma884(acc[mt][nt][0], acc[mt][nt][1], a[mt].y, b[nt].y);
         }
-      } else {
-        const double2 de = *reinterpret_cast<const double2*>(sde + kt * 16 + ch * 2);
-#pragma unroll
-        for (int nt = 0; nt < 4; ++nt) {
-          const double x0 = __dmul_rn(__dmul_rn(ndp[nt], de.x), kLog2e), x1 = __dmul_rn(__dmul_rn(ndp[nt], de.y), kLog2e);
-          const int sh0 = (int)fmax(floor(x0), -1.0e9) - kpv[nt], sh1 = (int)fmax(floor(x1), -1.0e9) - kpv[nt];
-          b[nt].x *= (sh0 < -1022) ? 0.0 : pow2i(min(sh0, 1022));
-          b[nt].y *= (sh1 < -1022) ? 0.0 : pow2i(min(sh1, 1022));
-        }
-#pragma unroll
-        for (int mt = 0; mt < 4; ++mt)
-#pragma unroll
-          for (int nt = 0; nt < 4; ++nt) dmma884(acc[mt][nt][0], acc[mt][nt][1], a[mt].x, b[nt].x);
-#pragma unroll
-        for (int mt = 0; mt < 4; ++mt)
-#pragma unroll
-          for (int nt = 0; nt < 4; ++nt) dmma884(acc[mt][nt][0], acc[mt][nt][1], a[mt].y, b[nt].y);
       }
     }
+  };
+#define CTQMC_GD(M, N) case (M) * 8 + (N): mainloop(std::integral_constant<int, M>{}, std::integral_constant<int, N>{}); break;
+  switch ((mtu > 0 && ntu > 0) ? mtu * 8 + ntu : 0) {
+    CTQMC_GD(1, 1) CTQMC_GD(1, 2) CTQMC_GD(1, 3) CTQMC_GD(1, 4) CTQMC_GD(2, 1) CTQMC_GD(2, 2) CTQMC_GD(2, 3) CTQMC_GD(2, 4)
+    CTQMC_GD(3, 1) CTQMC_GD(3, 2) CTQMC_GD(3, 3) CTQMC_GD(3, 4) CTQMC_GD(4, 1) CTQMC_GD(4, 2) CTQMC_GD(4, 3) CTQMC_GD(4, 4)
+    default: mainloop(std::integral_constant<int, 0>{}, std::integral_constant<int, 0>{}); break;
   }
+#undef CTQMC_GD
   cp_async_wait<0>();
 
   // ---- epilogue: per (row, string) propagator mantissa, scatter to the strings' matrices, largest exponent per column
@@ -326,7 +349,7 @@ __global__ void __launch_bounds__(kGThreads, 2) grouped_step_kernel(GroupedParam
   double er[4];
 #pragma unroll
   for (int mt = 0; mt < 4; ++mt) {
-    const int row = m0 + wm * 32 + mt * 8 + g;
+    const int row = m0 + (mt * 2 + wm) * 8 + g;
     er[mt] = (row < dn) ? E[row] : emin;
   }
   int cur_u = -2;
@@ -336,7 +359,7 @@ __global__ void __launch_bounds__(kGThreads, 2) grouped_step_kernel(GroupedParam
   for (int nt = 0; nt < 4; ++nt) {
 #pragma unroll
     for (int half = 0; half < 2; ++half) {
-      const int n = wn * 32 + nt * 8 + 2 * t + half;
+      const int n = (nt * 2 + wn) * 8 + 2 * t + half;
       const int u = s_u[n];
       if (u < 0) continue;
       if (u != cur_u) {   // columns of one string are adjacent: its row factors are computed once
@@ -347,14 +370,14 @@ __global__ void __launch_bounds__(kGThreads, 2) grouped_step_kernel(GroupedParam
           const double x = prop_x(delta, er[mt], emin);
           const double kf = floor(x);
           mr[mt] = exp2(__dsub_rn(x, kf));
-          kr[mt] = (int)fmax(kf, -1.0e9);
+          kr[mt] = row_exp(x);
         }
       }
       double* xo = s_xout[n];
       int cexp = INT_MIN;
 #pragma unroll
       for (int mt = 0; mt < 4; ++mt) {
-        const int row = m0 + wm * 32 + mt * 8 + g;
+        const int row = m0 + (mt * 2 + wm) * 8 + g;
         if (row < dn) {
           if constexpr (CPLX) {
             const double2 v = make_double2(acc[mt][nt][half] * mr[mt], acc[mt][nt][2 + half] * mr[mt]);
@@ -409,7 +432,7 @@ __global__ void grouped_finish_kernel(GroupedParams P) {
       const double dlast = P.plan_delta[(size_t)u * P.Lmax + L - 1];
       const double* X = P.X + ((size_t)(L & 1) * P.xtot + P.xoff[u]) * ES;
       for (int n = threadIdx.x; n < c; n += blockDim.x) {
-        const long long sh = (long long)fmax(floor(prop_x(dlast, E[n], emin)), -1.0e9) - (long long)klast;
+        const long long sh = (long long)row_exp(prop_x(dlast, E[n], emin)) - (long long)klast;
         const double f = (sh < -1022) ? 0.0 : pow2i((int)min(sh, 1022LL));
         if constexpr (CPLX) {
           const double2 v = *reinterpret_cast<const double2*>(X + ((size_t)n * P.ldx + n) * 2);

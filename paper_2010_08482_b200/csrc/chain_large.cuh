@@ -135,7 +135,7 @@ __global__ void __launch_bounds__(256, 1) large_step_kernel(LargeParams P, int j
         if (j == 0) f = 1.0;
         else {
           const double x = prop_x(dprev, Eq[k], emin);
-          const long long sh = (long long)fmax(floor(x), -1.0e9) - (long long)kprev;
+          const long long sh = (long long)row_exp(x) - (long long)kprev;
           f = (sh < -1022) ? 0.0 : pow2i((int)min(sh, 1022LL));
         }
       }
@@ -254,7 +254,7 @@ __global__ void __launch_bounds__(256, 1) large_step_kernel(LargeParams P, int j
       const double x = prop_x(delta, E[row], emin);
       const double kf = floor(x);
       mr = exp2(__dsub_rn(x, kf));
-      kr = (int)fmax(kf, -1.0e9);
+      kr = row_exp(x);
     }
     double rmax = 0.0;
 #pragma unroll
@@ -317,7 +317,7 @@ __global__ void large_finish_kernel(LargeParams P) {
       const double* X = P.X + ((size_t)s * 2 + (L & 1)) * P.xslab * ES;
       for (int n = threadIdx.x; n < c; n += blockDim.x) {
         const double x = prop_x(dlast, E[n], emin);
-        const long long sh = (long long)fmax(floor(x), -1.0e9) - (long long)klast;
+        const long long sh = (long long)row_exp(x) - (long long)klast;
         const double f = (sh < -1022) ? 0.0 : pow2i((int)min(sh, 1022LL));
         if constexpr (CPLX) {
           const double2 v = *reinterpret_cast<const double2*>(X + ((size_t)n * P.ldx + n) * 2);

@@ -188,7 +188,7 @@ __global__ void __launch_bounds__(256) small_trace_kernel(SmallParams P) {
             const double x = prop_x(delta, E[m], emin);
             const double kf = floor(x);
             const double mr = exp2(__dsub_rn(x, kf));
-            const int kr = (int)fmax(kf, -1.0e9);
+            const int kr = row_exp(x);
             if (e == lg) kr0 = kr;
             const double* Fr = F + (size_t)m * d * ES;
             if constexpr (CPLX) {
@@ -217,7 +217,7 @@ __global__ void __launch_bounds__(256) small_trace_kernel(SmallParams P) {
           if (kmax == INT_MIN) { dead = true; break; }
           e2 += kmax;
           for (int e = lg; e < nel; e += G) {
-            const int sh = ((e == lg) ? kr0 : (int)fmax(floor(prop_x(delta, E[e / c], emin)), -1.0e9)) - kmax;
+            const int sh = ((e == lg) ? kr0 : row_exp(prop_x(delta, E[e / c], emin))) - kmax;
             if (sh > 1022 || sh < -1022) {
               Xn[e * ES] = scalbn(Xn[e * ES], max(sh, -2200));
               if constexpr (CPLX) Xn[e * ES + 1] = scalbn(Xn[e * ES + 1], max(sh, -2200));

@@ -35,6 +35,7 @@ struct DevImp {
   const double* store;       // operator store
   const double* rownorm2;    // per block row: sum_k |F_mk|^2
   const double* sigma;       // [n_blocks] spectral norm
+  const int* blk_order;      // [n_blocks] block indices, heaviest (rows x cols) first: tile order of the grouped path
 };
 
 struct BatchView {
@@ -97,6 +98,10 @@ __device__ __forceinline__ double warp_sum(double v) {
 __device__ __forceinline__ double prop_x(double delta, double e, double emin) {
   return __dmul_rn(__dmul_rn(-delta, __dsub_rn(e, emin)), kLog2e);
 }
+
+// integer part of the row exponent, floor(x), saturated; one instruction (cvt.rmi.s32.f64).  Every producer and consumer of
+// a row exponent uses this function so that they agree bit for bit.
+__device__ __forceinline__ int row_exp(double x) { return max(__double2int_rd(x), -(1 << 30)); }
 
 // exact 2^k for |k| <= 1022
 __device__ __forceinline__ double pow2i(int k) { return __longlong_as_double((long long)(k + 1023) << 52); }

@@ -7,6 +7,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <algorithm>
 #include <new>
 #include <string>
 #include <vector>
@@ -90,6 +91,7 @@ struct ctqmc_impurity {
   int* d_dim = nullptr; long long* d_eoff = nullptr; double* d_energy = nullptr; double* d_emin = nullptr;
   int* d_blkof = nullptr; BlkDesc* d_blks = nullptr; double* d_store = nullptr; double* d_rownorm2 = nullptr;
   double* d_sigma = nullptr;
+  int* d_blkorder = nullptr;
   double* d_pack = nullptr; int4* d_pblk = nullptr;   // small-sector path: unpadded store
   int pack_len = 0, n_energy = 0;
   int small_ok = 0, small = 0, small_g = 32, small_grid_max = 0;
@@ -97,7 +99,7 @@ struct ctqmc_impurity {
   // schedule
   int schedule = CTQMC_SCHEDULE_THIN;
   int path = CTQMC_PATH_AUTO;
-  int nt = 0, team_warps = 8, ldx = 0, large = 0, grouped = 0;
+  int nt = 0, team_warps = 8, ldx = 0, large = 0, grouped = 0, grouped_ok = 0, grouped_now = 0, last_path = 0;
   size_t grouped_smem = 0;
   size_t smem_bytes = 0;
   int grid = 0;
@@ -109,6 +111,8 @@ struct ctqmc_impurity {
 };
 
 namespace {
+
+constexpr long long kGroupedMinBatch = 32;
 
 using KernelFn = void (*)(ChainParams);
 
@@ -171,13 +175,18 @@ int configure(ctqmc_impurity* h, int want_w) {
   }
   if (h->path == CTQMC_PATH_PANEL && h->nt == 0)
     return fail(CTQMC_ERR_UNSUPPORTED, "the shared-memory panel kernel cannot hold sectors of dimension %d", h->dev.dmax);
-  h->grouped = 0;
-  if (h->path == CTQMC_PATH_GROUPED) {
+  h->grouped = 0; h->grouped_ok = 0;
+  if (h->path == CTQMC_PATH_GROUPED || (h->path == CTQMC_PATH_AUTO && h->nt != 0 && !h->small)) {
     h->grouped_smem = grouped_smem_bytes(h->dev.dmax);
-    if (h->grouped_smem > smem_max) return fail(CTQMC_ERR_UNSUPPORTED, "sector dimension %d exceeds the grouped kernel's limit", h->dev.dmax);
-    if (cplx) CU(cudaFuncSetAttribute(grouped_step_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->grouped_smem));
-    else      CU(cudaFuncSetAttribute(grouped_step_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->grouped_smem));
-    h->grouped = 1;
+    if (h->grouped_smem <= smem_max) {
+      if (cplx) CU(cudaFuncSetAttribute(grouped_step_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->grouped_smem));
+      else      CU(cudaFuncSetAttribute(grouped_step_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->grouped_smem));
+      h->grouped_ok = 1;
+    }
+    if (h->path == CTQMC_PATH_GROUPED) {
+      if (!h->grouped_ok) return fail(CTQMC_ERR_UNSUPPORTED, "sector dimension %d exceeds the grouped kernel's limit", h->dev.dmax);
+      h->grouped = 1;
+    }
   }
   h->large = (h->nt == 0 || h->path == CTQMC_PATH_LARGE);
   if (h->large) {
@@ -250,7 +259,7 @@ int enqueue_routing(ctqmc_impurity* h, const BatchView& bv, uint8_t* survive_out
   validate_kernel<<<(unsigned)((B + 255) / 256), 256, 0, st>>>(bv, h->dev.A, a.status);
   RouteParams rp;
   rp.imp = h->dev; rp.bv = bv; rp.status = a.status; rp.survive = a.survive; rp.survive_out = survive_out;
-  rp.strings = a.strings; rp.cnt = a.cnt; rp.W = (h->large || (h->grouped && mode == 0)) ? (1 << 20) : 8 * h->nt; rp.kstep = h->dev.cplx ? 4 : 8;
+  rp.strings = a.strings; rp.cnt = a.cnt; rp.W = (h->large || (h->grouped_now && mode == 0)) ? (1 << 20) : 8 * h->nt; rp.kstep = h->dev.cplx ? 4 : 8;
   rp.literal = (h->schedule == CTQMC_SCHEDULE_LITERAL); rp.flops_per_mac = h->dev.cplx ? 8 : 2;
   rp.mode = mode; rp.segment_len = segment_len;
   route_kernel<<<(unsigned)((nS + 255) / 256), 256, 0, st>>>(rp);
@@ -331,14 +340,15 @@ int enqueue_grouped(ctqmc_impurity* h, const BatchView& bv, cudaStream_t st) {
   grouped_count_kernel<<<g_ul, 256, 0, st>>>(gp);
   grouped_tiles_kernel<<<Lmax, 32, 0, st>>>(gp);
   grouped_fill_kernel<<<g_ul, 256, 0, st>>>(gp);
-  dim3 sg((unsigned)tile_cap, (unsigned)((h->dev.dmax + kGBM - 1) / kGBM));
+  const int MTmax = (h->dev.dmax + kGBM - 1) / kGBM;
+  const unsigned sg = (unsigned)tile_cap * (unsigned)MTmax;
   if (h->dev.cplx) {
     grouped_init_kernel<true><<<(unsigned)n_units, 128, 0, st>>>(gp);
-    for (int j = 0; j < Lmax; ++j) grouped_step_kernel<true><<<sg, kGThreads, h->grouped_smem, st>>>(gp, j);
+    for (int j = 0; j < Lmax; ++j) grouped_step_kernel<true><<<sg, kGThreads, h->grouped_smem, st>>>(gp, j, MTmax);
     grouped_finish_kernel<true><<<(unsigned)n_units, 256, 0, st>>>(gp);
   } else {
     grouped_init_kernel<false><<<(unsigned)n_units, 128, 0, st>>>(gp);
-    for (int j = 0; j < Lmax; ++j) grouped_step_kernel<false><<<sg, kGThreads, h->grouped_smem, st>>>(gp, j);
+    for (int j = 0; j < Lmax; ++j) grouped_step_kernel<false><<<sg, kGThreads, h->grouped_smem, st>>>(gp, j, MTmax);
     grouped_finish_kernel<false><<<(unsigned)n_units, 256, 0, st>>>(gp);
   }
   h->last_launches += 7 + Lmax;
@@ -502,6 +512,13 @@ extern "C" int ctqmc_load_impurity(const ctqmc_impurity_desc* desc, int device, 
   TRY(upload(&h->d_emin, emin));
   TRY(upload(&h->d_blkof, blkof));
   TRY(upload(&h->d_blks, blks));
+  {
+    std::vector<int> order(nb);
+    for (int b = 0; b < nb; ++b) order[b] = b;
+    std::stable_sort(order.begin(), order.end(), [&](int x, int y) {
+      return (long long)blks[x].rows * blks[x].cols > (long long)blks[y].rows * blks[y].cols; });
+    TRY(upload(&h->d_blkorder, order));
+  }
   TRY(upload(&d_rawoff, raw_off));
   if (small_ok) {
     TRY(upload(&h->d_pack, pack));
@@ -558,7 +575,7 @@ extern "C" int ctqmc_load_impurity(const ctqmc_impurity_desc* desc, int device, 
   h->dev.Q = Q; h->dev.A = A; h->dev.cplx = cplx; h->dev.dmax = dmax;
   h->dev.dim = h->d_dim; h->dev.e_off = h->d_eoff; h->dev.energy = h->d_energy; h->dev.e_min = h->d_emin;
   h->dev.blk_of = h->d_blkof; h->dev.blks = h->d_blks; h->dev.store = h->d_store; h->dev.rownorm2 = h->d_rownorm2;
-  h->dev.sigma = h->d_sigma;
+  h->dev.sigma = h->d_sigma; h->dev.blk_order = h->d_blkorder;
   TRY(configure(h, 0));
 #undef TRY
 #undef TRYCU
@@ -570,7 +587,7 @@ extern "C" void ctqmc_free_impurity(ctqmc_impurity* h) {
   if (!h) return;
   cudaSetDevice(h->device);
   cudaFree(h->d_dim); cudaFree(h->d_eoff); cudaFree(h->d_energy); cudaFree(h->d_emin); cudaFree(h->d_blkof);
-  cudaFree(h->d_pack); cudaFree(h->d_pblk);
+  cudaFree(h->d_pack); cudaFree(h->d_pblk); cudaFree(h->d_blkorder);
   cudaFree(h->d_blks); cudaFree(h->d_store); cudaFree(h->d_rownorm2); cudaFree(h->d_sigma);
   Arena& a = h->arena;
   cudaFree(a.status); cudaFree(a.survive); cudaFree(a.strings); cudaFree(a.units); cudaFree(a.slots); cudaFree(a.sector);
@@ -627,7 +644,11 @@ extern "C" int ctqmc_trace_batch(ctqmc_impurity* h, double beta, const ctqmc_bat
   if (!mant || !exp2 || !status) return fail(CTQMC_ERR_ARG, "null output (mant, exp2 and status are required)");
   CU(cudaSetDevice(h->device));
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  const int W = (h->large || h->grouped) ? (1 << 20) : 8 * h->nt;
+  // AUTO: batches of at least kGroupedMinBatch configurations take the step-synchronous grouped path (one launch per chain
+  // position pays off once many strings share blocks); smaller ones the persistent panel kernel
+  h->grouped_now = h->grouped || (h->path == CTQMC_PATH_AUTO && h->grouped_ok && !h->small && !h->large && B >= kGroupedMinBatch);
+  h->last_path = h->small ? CTQMC_PATH_SMALL : h->grouped_now ? CTQMC_PATH_GROUPED : h->large ? CTQMC_PATH_LARGE : CTQMC_PATH_PANEL;
+  const int W = (h->large || h->grouped_now) ? (1 << 20) : 8 * h->nt;
   if (h->small) { if (!h->arena.cnt) CU(cudaMalloc((void**)&h->arena.cnt, sizeof(Counters))); }
   else { rc = ensure_arena(h, B, (h->dev.dmax + W - 1) / W); if (rc) return rc; }
   h->last_stream = st; h->last_launches = 0;
@@ -658,7 +679,7 @@ extern "C" int ctqmc_trace_batch(ctqmc_impurity* h, double beta, const ctqmc_bat
   rc = enqueue_routing(h, bv, survive, 0, 0, st);
   if (rc) return rc;
   mark(h, 1, st);
-  rc = h->grouped ? enqueue_grouped(h, bv, st) : h->large ? enqueue_large(h, bv, st) : enqueue_chain(h, bv, 0, 0, st);
+  rc = h->grouped_now ? enqueue_grouped(h, bv, st) : h->large ? enqueue_large(h, bv, st) : enqueue_chain(h, bv, 0, 0, st);
   if (rc) return rc;
   mark(h, 2, st);
   TraceReduceParams tp;
@@ -693,6 +714,7 @@ extern "C" int ctqmc_bound_batch(ctqmc_impurity* h, double beta, const ctqmc_bat
   BatchView bv; bv.B = B; bv.offset = (const long long*)batch->offset; bv.symbol = batch->symbol; bv.tau = batch->tau; bv.beta = beta;
   h->last_stream = st; h->last_launches = 0;
   h->timing_valid = 0;
+  h->grouped_now = 0; h->last_path = h->large ? CTQMC_PATH_LARGE : CTQMC_PATH_PANEL;
   BoundParams bp;
   if (segment_len == 1) {
     rc = ensure_arena(h, B, 1);
@@ -859,7 +881,7 @@ extern "C" int ctqmc_bound_batch_host(ctqmc_impurity* h, double beta, const ctqm
 extern "C" int ctqmc_last_stats(ctqmc_impurity* h, int64_t stats[8]) {
   if (!h || !stats) return fail(CTQMC_ERR_ARG, "null argument");
   for (int i = 0; i < 8; ++i) stats[i] = 0;
-  stats[5] = h->small ? h->small_g : h->nt * 8; stats[6] = h->team_warps; stats[7] = h->small ? 3 : h->grouped ? 4 : h->large ? 2 : 1;
+  stats[5] = h->small ? h->small_g : h->nt * 8; stats[6] = h->team_warps; stats[7] = h->last_path ? h->last_path : (h->small ? 3 : h->grouped ? 4 : h->large ? 2 : 1);
   if (!h->arena.cnt) return 0;
   CU(cudaSetDevice(h->device));
   Counters c;

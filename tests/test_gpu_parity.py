@@ -250,6 +250,19 @@ def test_trace_parity_grouped_path(cfg, n, schedule, lib, torch_cuda, impurities
         lib.ctqmc_set_option(h, lib.CTQMC_OPT_PATH, lib.CTQMC_PATH_AUTO)
 
 
+def test_auto_path_by_batch_size(lib, torch_cuda, impurities, handles):
+    """AUTO: batches of >= 32 configurations of a mid-size impurity take the grouped path, smaller ones the panel kernel;
+    both agree with the oracle (checked on the larger batch here, on the smaller ones by the baseline-config tests)."""
+    from workloads import make_batch
+    h = handles(3)
+    batch = make_batch(3, 40, start=15000)
+    _check_trace(lib, torch_cuda, impurities(3), h, batch, "cfg3-auto-40")
+    assert lib.ctqmc_last_stats(h)["path"] == lib.CTQMC_PATH_GROUPED
+    off, sym, tau = _dev(torch_cuda, make_batch(3, 8, start=15000))
+    lib.ctqmc_trace_batch(h, batch.beta, off, sym, tau)
+    assert lib.ctqmc_last_stats(h)["path"] == lib.CTQMC_PATH_PANEL
+
+
 def test_grouped_path_edge_cases_and_repeatability(lib, torch_cuda, impurities, handles):
     from workloads import Batch, make_batch
     imp = impurities(2)
