@@ -38,6 +38,11 @@ struct LargeParams {
   int* plan_blk;          // [n_group][Lmax]
   double* plan_delta;     // [n_group][Lmax]
   int* kmax;              // [n_group][Lmax]
+  int* u_q;               // [n_group] sector the unit's chain starts in
+  int* u_n;               // [n_group] chain positions to multiply
+  int* u_c;               // [n_group] columns carried
+  int mode;               // 0 trace of the whole (rotated) chain, 1 Frobenius norm^2 of one segment per unit
+  int segment_len;        // mode 1
   Slot* slots;
 };
 
@@ -53,9 +58,16 @@ __global__ void large_plan_kernel(LargeParams P) {
   const int L = (int)(P.bv.offset[b + 1] - base);
   const int* sym = P.bv.symbol + base;
   const double* tau = P.bv.tau + base;
-  int q = sr.q_start;
-  for (int j = 0; j < L; ++j) {
-    int i = sr.r + j;
+  int q = sr.q_start, i0 = sr.r, n = L, c = sr.c;
+  if (P.mode == 1) {   // unit = segment un.y of the literal chain: starts from the identity of the sector it begins in
+    i0 = un.y * P.segment_len;
+    for (int i = 0; i < i0; ++i) q = P.imp.blks[P.imp.blk_of[sym[i] * Q + q]].dst;
+    n = min(P.segment_len, L - i0);
+    c = P.imp.dim[q];
+  }
+  P.u_q[s] = q; P.u_n[s] = n; P.u_c[s] = c;
+  for (int j = 0; j < n; ++j) {
+    int i = i0 + j;
     if (i >= L) i -= L;
     const int blk = P.imp.blk_of[sym[i] * Q + q];
     P.plan_blk[(size_t)s * P.Lmax + j] = blk;
@@ -69,9 +81,7 @@ __global__ void large_plan_kernel(LargeParams P) {
 template <bool CPLX>
 __global__ void large_init_kernel(LargeParams P) {
   const int s = blockIdx.y;
-  const int2 un = P.units[P.u0 + s];
-  const StringRec sr = P.strings[un.x];
-  const int c = sr.c;
+  const int c = P.u_c[s];
   constexpr int ES = CPLX ? 2 : 1;
   double* X = P.X + (size_t)s * 2 * P.xslab * ES;
   const int dpad = round_up(c, 2);
@@ -102,15 +112,10 @@ __global__ void __launch_bounds__(256, 1) large_step_kernel(LargeParams P, int j
   double* sscale = reinterpret_cast<double*>(lsm + kLStages * kLStageBytes);
 
   const int s = blockIdx.y;
-  const int2 un = P.units[P.u0 + s];
-  const StringRec sr = P.strings[un.x];
-  const int Q = P.imp.Q;
-  const long long bcfg = un.x / Q;
-  const int L = (int)(P.bv.offset[bcfg + 1] - P.bv.offset[bcfg]);
-  if (j >= L) return;
+  if (j >= P.u_n[s]) return;
   const int blk = P.plan_blk[(size_t)s * P.Lmax + j];
   const BlkDesc bd = P.imp.blks[blk];
-  const int dn = bd.rows, d = bd.cols, c = sr.c;
+  const int dn = bd.rows, d = bd.cols, c = P.u_c[s];
   const int mt0 = blockIdx.x / NTmax, nt0 = blockIdx.x - mt0 * NTmax;
   const int m0 = mt0 * kLBM, n0 = nt0 * kLBN;
   if (m0 >= dn || n0 >= c) return;
@@ -285,7 +290,8 @@ __global__ void __launch_bounds__(256, 1) large_step_kernel(LargeParams P, int j
   if (lane == 0 && wexp != INT_MIN) atomicMax(&P.kmax[(size_t)s * P.Lmax + j], wexp);
 }
 
-// Trace of the final matrix (a5): sum_n X[n][n] 2^(row exponent - largest), running exponent = sum of the steps' largest.
+// Mode 0: trace of the final matrix (a5): sum_n X[n][n] 2^(row exponent - largest).  Mode 1: squared Frobenius norm of the
+// segment product (a6).  Running exponent = sum of the steps' largest row exponents.
 template <bool CPLX>
 __global__ void large_finish_kernel(LargeParams P) {
   constexpr int ES = CPLX ? 2 : 1;
@@ -293,37 +299,52 @@ __global__ void large_finish_kernel(LargeParams P) {
   const int s = blockIdx.x;
   const int2 un = P.units[P.u0 + s];
   const StringRec sr = P.strings[un.x];
-  const int Q = P.imp.Q;
-  const long long bcfg = un.x / Q;
-  const int L = (int)(P.bv.offset[bcfg + 1] - P.bv.offset[bcfg]);
-  const int c = sr.c;
-  const int q = sr.q_start;
-  const double* E = P.imp.energy + P.imp.e_off[q];
-  const double emin = P.imp.e_min[q];
+  const int n_steps = P.u_n[s], c = P.u_c[s];
   double re = 0.0, im = 0.0;
   long long e2 = 0;
   bool dead = false;
-  if (L == 0) {
+  if (n_steps == 0) {   // empty configuration, trace mode only: Tr P_beta(q0)
+    const int q = P.u_q[s];
+    const double* E = P.imp.energy + P.imp.e_off[q];
+    const double emin = P.imp.e_min[q];
     for (int n = threadIdx.x; n < c; n += blockDim.x) re += exp(-P.bv.beta * (E[n] - emin));
   } else {
-    for (int j = 0; j < L; ++j) {
+    for (int j = 0; j < n_steps; ++j) {
       const int k = P.kmax[(size_t)s * P.Lmax + j];
       if (k == INT_MIN) { dead = true; break; }
       e2 += k;
     }
     if (!dead) {
-      const int klast = P.kmax[(size_t)s * P.Lmax + L - 1];
-      const double dlast = P.plan_delta[(size_t)s * P.Lmax + L - 1];
-      const double* X = P.X + ((size_t)s * 2 + (L & 1)) * P.xslab * ES;
-      for (int n = threadIdx.x; n < c; n += blockDim.x) {
-        const double x = prop_x(dlast, E[n], emin);
-        const long long sh = (long long)row_exp(x) - (long long)klast;
-        const double f = (sh < -1022) ? 0.0 : pow2i((int)min(sh, 1022LL));
-        if constexpr (CPLX) {
-          const double2 v = *reinterpret_cast<const double2*>(X + ((size_t)n * P.ldx + n) * 2);
-          re += v.x * f; im += v.y * f;
-        } else {
-          re += X[(size_t)n * P.ldx + n] * f;
+      const BlkDesc bl = P.imp.blks[P.plan_blk[(size_t)s * P.Lmax + n_steps - 1]];
+      const double* E = P.imp.energy + P.imp.e_off[bl.dst];
+      const double emin = P.imp.e_min[bl.dst];
+      const int klast = P.kmax[(size_t)s * P.Lmax + n_steps - 1];
+      const double dlast = P.plan_delta[(size_t)s * P.Lmax + n_steps - 1];
+      const double* X = P.X + ((size_t)s * 2 + (n_steps & 1)) * P.xslab * ES;
+      if (P.mode == 0) {
+        for (int n = threadIdx.x; n < c; n += blockDim.x) {
+          const long long sh = (long long)row_exp(prop_x(dlast, E[n], emin)) - (long long)klast;
+          const double f = (sh < -1022) ? 0.0 : pow2i((int)min(sh, 1022LL));
+          if constexpr (CPLX) {
+            const double2 v = *reinterpret_cast<const double2*>(X + ((size_t)n * P.ldx + n) * 2);
+            re += v.x * f; im += v.y * f;
+          } else {
+            re += X[(size_t)n * P.ldx + n] * f;
+          }
+        }
+      } else {
+        const int rows = bl.rows;
+        for (long long idx = threadIdx.x; idx < (long long)rows * c; idx += blockDim.x) {
+          const int col = (int)(idx / rows), row = (int)(idx - (long long)col * rows);
+          const long long sh = (long long)row_exp(prop_x(dlast, E[row], emin)) - (long long)klast;
+          const double f = (sh < -1022) ? 0.0 : pow2i((int)min(sh, 1022LL));
+          if constexpr (CPLX) {
+            const double2 v = *reinterpret_cast<const double2*>(X + ((size_t)col * P.ldx + row) * 2);
+            re += (v.x * f) * (v.x * f) + (v.y * f) * (v.y * f);
+          } else {
+            const double v = X[(size_t)col * P.ldx + row] * f;
+            re += v * v;
+          }
         }
       }
     }
@@ -335,7 +356,7 @@ __global__ void large_finish_kernel(LargeParams P) {
     double tr = 0.0, ti = 0.0;
     for (int w = 0; w < (int)(blockDim.x >> 5); ++w) { tr += red[0][w]; ti += red[1][w]; }
     Slot out; out.re = dead ? 0.0 : tr; out.im = dead ? 0.0 : ti; out.e2 = dead ? 0 : e2; out.pad = 0;
-    P.slots[sr.slot] = out;
+    P.slots[sr.slot + (P.mode == 1 ? un.y : 0)] = out;
   }
 }
 

@@ -73,6 +73,7 @@ struct Arena {
   // large-sector path: carried matrices (two per string), step plan, per-step largest exponents
   double* lx = nullptr; size_t lx_bytes = 0;
   int* plan_blk = nullptr; double* plan_delta = nullptr; int* lkmax = nullptr; size_t plan_cap = 0;
+  DevBuf lunit;   // u_q, u_n, u_c
   // grouped path
   DevBuf gx, gxoff, gplan_blk, gplan_delta, gkmax, gcoff, gulen, gucols, gcolcnt, gcolbase, gtiles, gntiles, gcolmap;
   // host-variant staging
@@ -359,14 +360,16 @@ int enqueue_grouped(ctqmc_impurity* h, const BatchView& bv, cudaStream_t st) {
 // Large-sector path: one launch per chain position over all strings of a group (chain_large.cuh).  Reads back three
 // integers (strings with work, longest chain, widest carried matrix) to size the step loop and the carried matrices:
 // the one host synchronisation of this path.
-int enqueue_large(ctqmc_impurity* h, const BatchView& bv, cudaStream_t st) {
+int enqueue_large(ctqmc_impurity* h, const BatchView& bv, int mode, int segment_len, cudaStream_t st) {
   Arena& a = h->arena;
   Counters c;
   CU(cudaMemcpyAsync(&c, a.cnt, sizeof c, cudaMemcpyDeviceToHost, st));
   CU(cudaStreamSynchronize(st));
   const long long n_units = (long long)c.n_slots;
   if (n_units == 0) return 0;
-  const int Lmax = (int)c.max_len > 0 ? (int)c.max_len : 1, cmax = (int)c.max_c > 0 ? (int)c.max_c : 1;
+  const int Lmax = (int)c.max_len > 0 ? (int)c.max_len : 1;
+  const int cmax = mode == 1 ? h->dev.dmax : ((int)c.max_c > 0 ? (int)c.max_c : 1);   // segments start from full identities
+  const int n_launch = mode == 1 ? (segment_len < Lmax ? segment_len : Lmax) : Lmax;
   const int es = h->dev.cplx ? 2 : 1;
   const long long xslab = (long long)cmax * h->ldx;
   const size_t per_string = (size_t)2 * xslab * es * sizeof(double);
@@ -392,7 +395,9 @@ int enqueue_large(ctqmc_impurity* h, const BatchView& bv, cudaStream_t st) {
     CU(cudaMalloc((void**)&a.lkmax, n * sizeof(int)));
     a.plan_cap = n;
   }
+  { int rc = grow(a.lunit, (size_t)3 * G * sizeof(int)); if (rc) return rc; }
   LargeParams lp;
+  lp.u_q = (int*)a.lunit.p; lp.u_n = lp.u_q + G; lp.u_c = lp.u_n + G; lp.mode = mode; lp.segment_len = segment_len;
   lp.imp = h->dev; lp.bv = bv; lp.strings = a.strings; lp.units = a.units; lp.Lmax = Lmax; lp.ldx = h->ldx;
   lp.xslab = xslab; lp.X = a.lx; lp.plan_blk = a.plan_blk; lp.plan_delta = a.plan_delta; lp.kmax = a.lkmax; lp.slots = a.slots;
   const int MTmax = (h->dev.dmax + kLBM - 1) / kLBM, NTmax = (cmax + kLBN - 1) / kLBN;
@@ -403,14 +408,14 @@ int enqueue_large(ctqmc_impurity* h, const BatchView& bv, cudaStream_t st) {
     dim3 sg((unsigned)(MTmax * NTmax), (unsigned)lp.n_group);
     if (h->dev.cplx) {
       large_init_kernel<true><<<ig, 256, 0, st>>>(lp);
-      for (int j = 0; j < Lmax; ++j) large_step_kernel<true><<<sg, 256, h->smem_bytes, st>>>(lp, j, NTmax);
+      for (int j = 0; j < n_launch; ++j) large_step_kernel<true><<<sg, 256, h->smem_bytes, st>>>(lp, j, NTmax);
       large_finish_kernel<true><<<lp.n_group, 256, 0, st>>>(lp);
     } else {
       large_init_kernel<false><<<ig, 256, 0, st>>>(lp);
-      for (int j = 0; j < Lmax; ++j) large_step_kernel<false><<<sg, 256, h->smem_bytes, st>>>(lp, j, NTmax);
+      for (int j = 0; j < n_launch; ++j) large_step_kernel<false><<<sg, 256, h->smem_bytes, st>>>(lp, j, NTmax);
       large_finish_kernel<false><<<lp.n_group, 256, 0, st>>>(lp);
     }
-    h->last_launches += 3 + Lmax;
+    h->last_launches += 3 + n_launch;
   }
   CU(cudaGetLastError());
   return 0;
@@ -593,7 +598,7 @@ extern "C" void ctqmc_free_impurity(ctqmc_impurity* h) {
   cudaFree(a.status); cudaFree(a.survive); cudaFree(a.strings); cudaFree(a.units); cudaFree(a.slots); cudaFree(a.sector);
   for (DevBuf* b : {&a.gx, &a.gxoff, &a.gplan_blk, &a.gplan_delta, &a.gkmax, &a.gcoff, &a.gulen, &a.gucols, &a.gcolcnt, &a.gcolbase,
                      &a.gtiles, &a.gntiles, &a.gcolmap}) cudaFree(b->p);
-  cudaFree(a.cnt); cudaFree(a.lx); cudaFree(a.plan_blk); cudaFree(a.plan_delta); cudaFree(a.lkmax); cudaFree(a.d_stage);
+  cudaFree(a.lunit.p); cudaFree(a.cnt); cudaFree(a.lx); cudaFree(a.plan_blk); cudaFree(a.plan_delta); cudaFree(a.lkmax); cudaFree(a.d_stage);
   if (a.h_stage) cudaFreeHost(a.h_stage);
   for (int i = 0; i < 4; ++i) if (h->ev[i]) cudaEventDestroy(h->ev[i]);
   delete h;
@@ -679,7 +684,7 @@ extern "C" int ctqmc_trace_batch(ctqmc_impurity* h, double beta, const ctqmc_bat
   rc = enqueue_routing(h, bv, survive, 0, 0, st);
   if (rc) return rc;
   mark(h, 1, st);
-  rc = h->grouped_now ? enqueue_grouped(h, bv, st) : h->large ? enqueue_large(h, bv, st) : enqueue_chain(h, bv, 0, 0, st);
+  rc = h->grouped_now ? enqueue_grouped(h, bv, st) : h->large ? enqueue_large(h, bv, 0, 0, st) : enqueue_chain(h, bv, 0, 0, st);
   if (rc) return rc;
   mark(h, 2, st);
   TraceReduceParams tp;
@@ -706,7 +711,6 @@ extern "C" int ctqmc_bound_batch(ctqmc_impurity* h, double beta, const ctqmc_bat
   const long long B = batch->n_configs;
   if (B == 0) return 0;
   if (!bound_mant || !bound_exp2 || !status) return fail(CTQMC_ERR_ARG, "null output");
-  if (segment_len != 1 && h->large) return fail(CTQMC_ERR_UNSUPPORTED, "segment_len != 1 is not implemented for sectors that do not fit in shared memory");
   CU(cudaSetDevice(h->device));
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const int W = h->large ? (1 << 20) : 8 * h->nt;
@@ -756,7 +760,7 @@ extern "C" int ctqmc_bound_batch(ctqmc_impurity* h, double beta, const ctqmc_bat
     rc = enqueue_routing(h, bv, nullptr, 1, S, st);
     if (rc) return rc;
     mark(h, 1, st);
-    rc = enqueue_chain(h, bv, 1, S, st);
+    rc = h->large ? enqueue_large(h, bv, 1, S, st) : enqueue_chain(h, bv, 1, S, st);
     if (rc) return rc;
     bp.imp = h->dev; bp.bv = bv; bp.survive = h->arena.survive; bp.strings = h->arena.strings; bp.slots = h->arena.slots;
     bp.sector = h->arena.sector; bp.norm_kind = 0; bp.segment_len = S; bp.W = W;

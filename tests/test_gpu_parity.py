@@ -318,6 +318,7 @@ def test_trace_parity_cfg5_crystal_field(lib, torch_cuda, impurities):
         assert lib.ctqmc_last_stats(h)["path"] == lib.CTQMC_PATH_LARGE
         worst = _check_trace(lib, torch_cuda, imp, h, make_batch(5, 1), "cfg5")
         print(f"cfg5: worst relative difference {worst:.3e}")
+        _check_bound(lib, torch_cuda, imp, h, make_batch(5, 1), 0, 1, "cfg5-frobenius-S1")
     finally:
         h.free()
 
@@ -480,6 +481,20 @@ def test_bound_segments_parity(cfg, n, S, lib, torch_cuda, impurities, handles):
     from workloads import make_batch
     _check_bound(lib, torch_cuda, impurities(cfg), handles(cfg), make_batch(cfg, n, start=200), 0, S,
                  f"cfg{cfg}-S{S}")
+
+
+@pytest.mark.parametrize("cfg,n", [(1, 32), (2, 32), (3, 4), (4, 1)])
+@pytest.mark.parametrize("S", [0, 3, 16])
+def test_bound_segments_parity_large_path(cfg, n, S, lib, torch_cuda, impurities, handles):
+    """Segment Frobenius norms through the large-sector kernel family (what config 5 uses), forced onto the small
+    impurities so that the oracle can check every segment."""
+    from workloads import make_batch
+    h = handles(cfg)
+    lib.ctqmc_set_option(h, lib.CTQMC_OPT_PATH, lib.CTQMC_PATH_LARGE)
+    try:
+        _check_bound(lib, torch_cuda, impurities(cfg), h, make_batch(cfg, n, start=250), 0, S, f"cfg{cfg}-large-S{S}")
+    finally:
+        lib.ctqmc_set_option(h, lib.CTQMC_OPT_PATH, lib.CTQMC_PATH_AUTO)
 
 
 def test_bound_edge_cases(lib, torch_cuda, impurities, handles):
