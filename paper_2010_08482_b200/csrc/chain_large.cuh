@@ -16,6 +16,7 @@
 // occur for operators with O(1) entries).
 #pragma once
 #include <climits>
+#include <cuda.h>
 
 #include "chain.cuh"
 
@@ -43,6 +44,8 @@ struct LargeParams {
   int* u_c;               // [n_group] columns carried
   int mode;               // 0 trace of the whole (rotated) chain, 1 Frobenius norm^2 of one segment per unit
   int segment_len;        // mode 1
+  const CUtensorMap* amaps;   // [n_blocks] tensor maps of the operator blocks (TMA variant)
+  const CUtensorMap* xmaps;   // [n_group][2] tensor maps of the carried matrices
   Slot* slots;
 };
 
@@ -102,13 +105,34 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
+// ---- TMA (cp.async.bulk.tensor) + mbarrier primitives: the Blackwell-native way to stage the operand tiles.  One elected
+// thread arms the stage's barrier with the byte count and issues four 2-D box copies (two k-halves of F rows and of X
+// columns); the copy engine writes shared memory and completes the transaction on the barrier; all threads wait on it.
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
+  asm volatile(
+      "{\n.reg .pred P1;\nLAB_WAIT:\nmbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n@P1 bra DONE;\nbra LAB_WAIT;\nDONE:\n}"
+      ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* map, unsigned long long* bar, int c0, int c1) {
+  asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+               ::"r"(smem_u32(dst)), "l"(map), "r"(c0), "r"(c1), "r"(smem_u32(bar)) : "memory");
+}
+
 // One chain position for every string of the group.  blockIdx.x = mt * NTmax + nt (nt fastest: CTAs that share rows of
 // F run together and hit L2), blockIdx.y = string.
-template <bool CPLX>
+template <bool CPLX, bool TMA>
 __global__ void __launch_bounds__(256, 1) large_step_kernel(LargeParams P, int j, int NTmax) {
   constexpr int ES = CPLX ? 2 : 1;
   constexpr int BKE = CPLX ? 8 : 16;       // contraction indices per stage (128-byte rows)
   extern __shared__ __align__(128) unsigned char lsm[];
+  __shared__ __align__(8) unsigned long long full_bar[kLStages];
   double* sscale = reinterpret_cast<double*>(lsm + kLStages * kLStageBytes);
 
   const int s = blockIdx.y;
@@ -154,23 +178,39 @@ __global__ void __launch_bounds__(256, 1) large_step_kernel(LargeParams P, int j
   const size_t a_row_bytes = (size_t)bd.ld * ES * 8, b_col_bytes = (size_t)P.ldx * ES * 8;
   const int ld_chunks = bd.ld * ES / 2;          // 16-byte chunks per row of F (padded with zeros)
   const int x_chunks = CPLX ? d : (d + 1) / 2;   // 16-byte chunks of an X column that hold data
+  const CUtensorMap* amap = P.amaps + blk;
+  const CUtensorMap* xmap = P.xmaps + (size_t)s * 2 + (j & 1);
 
+  // cp.async variant: 128-byte rows, 16-byte chunks XOR-swizzled by the row parity.
+  // TMA variant: per k-half a dense box of 64-byte rows (two adjacent rows = one 128-byte line, so the 128-bit fragment loads
+  // of a quarter warp are conflict free without any swizzle); out-of-range rows / k are zero-filled by the copy engine.
   auto load_stage = [&](int kt, int stage) {
     unsigned char* As = lsm + stage * kLStageBytes;
-    unsigned char* Bs = As + kLBM * 128;
+    if constexpr (TMA) {
+      if (tid == 0) {
+        mbar_expect_tx(&full_bar[stage], kLStageBytes);
 #pragma unroll
-    for (int i = 0; i < 4; ++i) {
-      const int idx = tid + i * 256, r = idx >> 3, ch = idx & 7;
-      const int row = m0 + r, gch = kt * 8 + ch;
-      const bool ok = row < rows_pad && gch < ld_chunks;
-      cp_async16(As + r * 128 + ((ch ^ ((r & 1) << 2)) << 4), ok ? Ag + (size_t)row * a_row_bytes + (size_t)gch * 16 : Ag, ok);
-    }
+        for (int sub = 0; sub < 2; ++sub) {
+          tma_load_2d(As + sub * (kLBM * 64), amap, &full_bar[stage], kt * 16 + sub * 8, m0);
+          tma_load_2d(As + 2 * (kLBM * 64) + sub * (kLBN * 64), xmap, &full_bar[stage], kt * 16 + sub * 8, n0);
+        }
+      }
+    } else {
+      unsigned char* Bs = As + kLBM * 128;
 #pragma unroll
-    for (int i = 0; i < 2; ++i) {
-      const int idx = tid + i * 256, r = idx >> 3, ch = idx & 7;
-      const int col = n0 + r, gch = kt * 8 + ch;
-      const bool ok = col < c && gch < x_chunks;
-      cp_async16(Bs + r * 128 + ((ch ^ ((r & 1) << 2)) << 4), ok ? Bg + (size_t)col * b_col_bytes + (size_t)gch * 16 : Bg, ok);
+      for (int i = 0; i < 4; ++i) {
+        const int idx = tid + i * 256, r = idx >> 3, ch = idx & 7;
+        const int row = m0 + r, gch = kt * 8 + ch;
+        const bool ok = row < rows_pad && gch < ld_chunks;
+        cp_async16(As + r * 128 + ((ch ^ ((r & 1) << 2)) << 4), ok ? Ag + (size_t)row * a_row_bytes + (size_t)gch * 16 : Ag, ok);
+      }
+#pragma unroll
+      for (int i = 0; i < 2; ++i) {
+        const int idx = tid + i * 256, r = idx >> 3, ch = idx & 7;
+        const int col = n0 + r, gch = kt * 8 + ch;
+        const bool ok = col < c && gch < x_chunks;
+        cp_async16(Bs + r * 128 + ((ch ^ ((r & 1) << 2)) << 4), ok ? Bg + (size_t)col * b_col_bytes + (size_t)gch * 16 : Bg, ok);
+      }
     }
   };
 
@@ -182,32 +222,50 @@ __global__ void __launch_bounds__(256, 1) large_step_kernel(LargeParams P, int j
 #pragma unroll
       for (int x = 0; x < (CPLX ? 4 : 2); ++x) acc[a][b][x] = 0.0;
 
+  if constexpr (TMA) {
+    if (tid == 0) {
+#pragma unroll
+      for (int st = 0; st < kLStages; ++st) mbar_init(&full_bar[st], 1);
+      asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+  }
 #pragma unroll
   for (int st = 0; st < kLStages - 1; ++st) {
     if (st < nkt) load_stage(st, st);
-    cp_async_commit();
+    if constexpr (!TMA) cp_async_commit();
   }
 
   const int swz = (g & 1) << 2;
   for (int kt = 0; kt < nkt; ++kt) {
-    cp_async_wait<kLStages - 2>();
+    if constexpr (TMA) mbar_wait(&full_bar[kt % kLStages], (kt / kLStages) & 1);
+    else cp_async_wait<kLStages - 2>();
     __syncthreads();
     {
       const int nx = kt + kLStages - 1;
       if (nx < nkt) load_stage(nx, nx % kLStages);
-      cp_async_commit();
+      if constexpr (!TMA) cp_async_commit();
     }
     const unsigned char* As = lsm + (kt % kLStages) * kLStageBytes;
-    const unsigned char* Bs = As + kLBM * 128;
 #pragma unroll
     for (int sub = 0; sub < 2; ++sub) {
       const int ch = sub * 4 + t;
-      const int so = ((ch ^ swz) << 4);
       double2 a[4], b[4];
+      if constexpr (TMA) {
+        const unsigned char* Ah = As + sub * (kLBM * 64) + t * 16;
+        const unsigned char* Bh = As + 2 * (kLBM * 64) + sub * (kLBN * 64) + t * 16;
 #pragma unroll
-      for (int mt = 0; mt < 4; ++mt) a[mt] = *reinterpret_cast<const double2*>(As + (wm * 32 + mt * 8 + g) * 128 + so);
+        for (int mt = 0; mt < 4; ++mt) a[mt] = *reinterpret_cast<const double2*>(Ah + (wm * 32 + mt * 8 + g) * 64);
 #pragma unroll
-      for (int nt = 0; nt < 4; ++nt) b[nt] = *reinterpret_cast<const double2*>(Bs + (wn * 32 + nt * 8 + g) * 128 + so);
+        for (int nt = 0; nt < 4; ++nt) b[nt] = *reinterpret_cast<const double2*>(Bh + (wn * 32 + nt * 8 + g) * 64);
+      } else {
+        const unsigned char* Bs = As + kLBM * 128;
+        const int so = ((ch ^ swz) << 4);
+#pragma unroll
+        for (int mt = 0; mt < 4; ++mt) a[mt] = *reinterpret_cast<const double2*>(As + (wm * 32 + mt * 8 + g) * 128 + so);
+#pragma unroll
+        for (int nt = 0; nt < 4; ++nt) b[nt] = *reinterpret_cast<const double2*>(Bs + (wn * 32 + nt * 8 + g) * 128 + so);
+      }
       if constexpr (CPLX) {
         const double f = sscale[kt * 8 + ch];
 #pragma unroll
@@ -243,7 +301,7 @@ __global__ void __launch_bounds__(256, 1) large_step_kernel(LargeParams P, int j
       }
     }
   }
-  cp_async_wait<0>();
+  if constexpr (!TMA) cp_async_wait<0>();
 
   // ---- epilogue: propagator mantissa, store, largest row exponent
   const double delta = P.plan_delta[(size_t)s * P.Lmax + j];

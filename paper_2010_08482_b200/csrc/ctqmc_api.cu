@@ -74,6 +74,7 @@ struct Arena {
   double* lx = nullptr; size_t lx_bytes = 0;
   int* plan_blk = nullptr; double* plan_delta = nullptr; int* lkmax = nullptr; size_t plan_cap = 0;
   DevBuf lunit;   // u_q, u_n, u_c
+  DevBuf xmaps; const void* xmaps_base = nullptr; long long xmaps_g = 0, xmaps_slab = 0; int xmaps_cmax = 0;
   // grouped path
   DevBuf gx, gxoff, gplan_blk, gplan_delta, gkmax, gcoff, gulen, gucols, gcolcnt, gcolbase, gtiles, gntiles, gcolmap;
   // host-variant staging
@@ -93,6 +94,9 @@ struct ctqmc_impurity {
   int* d_blkof = nullptr; BlkDesc* d_blks = nullptr; double* d_store = nullptr; double* d_rownorm2 = nullptr;
   double* d_sigma = nullptr;
   int* d_blkorder = nullptr;
+  std::vector<BlkDesc> h_blks;        // host copy (tensor-map construction)
+  CUtensorMap* d_amaps = nullptr;     // large path, TMA variant: one tensor map per operator block
+  int use_tma = 1;
   double* d_pack = nullptr; int4* d_pblk = nullptr;   // small-sector path: unpadded store
   int pack_len = 0, n_energy = 0;
   int small_ok = 0, small = 0, small_g = 32, small_grid_max = 0;
@@ -124,6 +128,35 @@ KernelFn pick_kernel(int cplx, int nt, int tw) {
   PICK(1, 1, 8) PICK(1, 2, 8) PICK(1, 4, 8)
 #undef PICK
   return nullptr;
+}
+
+// cuTensorMapEncodeTiled through the runtime's driver entry point (no link against libcuda)
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn encode_tiled_fn() {
+  static EncodeTiledFn fn = nullptr;
+  if (!fn) {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess && q == cudaDriverEntryPointSuccess)
+      fn = (EncodeTiledFn)p;
+  }
+  return fn;
+}
+
+// 2-D FP64 tensor map: `inner` doubles contiguous, `outer` rows of `stride_bytes`; box = 8 doubles (64 B) x box_outer rows,
+// no swizzle, out-of-range elements read as zero.
+int encode_2d(CUtensorMap* m, const void* base, unsigned long long inner, unsigned long long outer, unsigned long long stride_bytes,
+              unsigned box_outer) {
+  EncodeTiledFn fn = encode_tiled_fn();
+  if (!fn) return fail(CTQMC_ERR_CUDA, "cuTensorMapEncodeTiled is not available from this driver");
+  const cuuint64_t dims[2] = {inner, outer}, strides[1] = {stride_bytes};
+  const cuuint32_t box[2] = {8, box_outer}, estr[2] = {1, 1};
+  CUresult r = fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<void*>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                  CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return fail(CTQMC_ERR_CUDA, "cuTensorMapEncodeTiled failed (%d): inner %llu outer %llu stride %llu", (int)r, inner, outer, stride_bytes);
+  return 0;
 }
 
 using SmallFn = void (*)(SmallParams);
@@ -195,8 +228,25 @@ int configure(ctqmc_impurity* h, int want_w) {
     h->ldx = (h->dev.dmax + 7) / 8 * 8;
     h->smem_bytes = large_smem_bytes(h->dev.dmax);
     if (h->smem_bytes > smem_max) return fail(CTQMC_ERR_UNSUPPORTED, "sector dimension %d exceeds the large-sector kernel's limit", h->dev.dmax);
-    if (cplx) CU(cudaFuncSetAttribute(large_step_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_bytes));
-    else      CU(cudaFuncSetAttribute(large_step_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_bytes));
+    if (const char* e = getenv("CTQMC_LARGE_TMA")) h->use_tma = atoi(e) != 0;
+    if (cplx) {
+      CU(cudaFuncSetAttribute(large_step_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_bytes));
+      CU(cudaFuncSetAttribute(large_step_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_bytes));
+    } else {
+      CU(cudaFuncSetAttribute(large_step_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_bytes));
+      CU(cudaFuncSetAttribute(large_step_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_bytes));
+    }
+    if (h->use_tma && !h->d_amaps && h->n_blocks > 0) {   // tensor maps of the operator blocks, once
+      std::vector<CUtensorMap> maps(h->n_blocks);
+      for (int b = 0; b < h->n_blocks; ++b) {
+        const BlkDesc& bd = h->h_blks[b];
+        int rc = encode_2d(&maps[b], h->d_store + bd.off, (unsigned long long)bd.ld * es, (unsigned long long)((bd.rows + 7) / 8 * 8),
+                           (unsigned long long)bd.ld * es * 8, kLBM);
+        if (rc) return rc;
+      }
+      CU(cudaMalloc((void**)&h->d_amaps, maps.size() * sizeof(CUtensorMap)));
+      CU(cudaMemcpy(h->d_amaps, maps.data(), maps.size() * sizeof(CUtensorMap), cudaMemcpyHostToDevice));
+    }
     h->grid = 0;
     return 0;
   }
@@ -400,6 +450,23 @@ int enqueue_large(ctqmc_impurity* h, const BatchView& bv, int mode, int segment_
   lp.u_q = (int*)a.lunit.p; lp.u_n = lp.u_q + G; lp.u_c = lp.u_n + G; lp.mode = mode; lp.segment_len = segment_len;
   lp.imp = h->dev; lp.bv = bv; lp.strings = a.strings; lp.units = a.units; lp.Lmax = Lmax; lp.ldx = h->ldx;
   lp.xslab = xslab; lp.X = a.lx; lp.plan_blk = a.plan_blk; lp.plan_delta = a.plan_delta; lp.kmax = a.lkmax; lp.slots = a.slots;
+  lp.amaps = h->d_amaps; lp.xmaps = nullptr;
+  const bool tma = h->use_tma && h->d_amaps;
+  if (tma) {   // tensor maps of the carried matrices (two per string slot); rebuilt only when the arena changed
+    if (a.xmaps_base != a.lx || a.xmaps_g < G || a.xmaps_slab != xslab || a.xmaps_cmax != cmax) {
+      std::vector<CUtensorMap> maps((size_t)2 * G);
+      for (long long i = 0; i < 2 * G; ++i) {
+        int rc = encode_2d(&maps[i], a.lx + (size_t)i * xslab * es, (unsigned long long)h->ldx * es, (unsigned long long)cmax,
+                           (unsigned long long)h->ldx * es * 8, kLBN);
+        if (rc) return rc;
+      }
+      { int rc = grow(a.xmaps, maps.size() * sizeof(CUtensorMap)); if (rc) return rc; }
+      CU(cudaMemcpyAsync(a.xmaps.p, maps.data(), maps.size() * sizeof(CUtensorMap), cudaMemcpyHostToDevice, st));
+      CU(cudaStreamSynchronize(st));   // `maps` is a pageable host vector
+      a.xmaps_base = a.lx; a.xmaps_g = G; a.xmaps_slab = xslab; a.xmaps_cmax = cmax;
+    }
+    lp.xmaps = (const CUtensorMap*)a.xmaps.p;
+  }
   const int MTmax = (h->dev.dmax + kLBM - 1) / kLBM, NTmax = (cmax + kLBN - 1) / kLBN;
   for (long long u0 = 0; u0 < n_units; u0 += G) {
     lp.u0 = u0; lp.n_group = (int)((n_units - u0 < G) ? (n_units - u0) : G);
@@ -408,11 +475,17 @@ int enqueue_large(ctqmc_impurity* h, const BatchView& bv, int mode, int segment_
     dim3 sg((unsigned)(MTmax * NTmax), (unsigned)lp.n_group);
     if (h->dev.cplx) {
       large_init_kernel<true><<<ig, 256, 0, st>>>(lp);
-      for (int j = 0; j < n_launch; ++j) large_step_kernel<true><<<sg, 256, h->smem_bytes, st>>>(lp, j, NTmax);
+      for (int j = 0; j < n_launch; ++j) {
+        if (tma) large_step_kernel<true, true><<<sg, 256, h->smem_bytes, st>>>(lp, j, NTmax);
+        else     large_step_kernel<true, false><<<sg, 256, h->smem_bytes, st>>>(lp, j, NTmax);
+      }
       large_finish_kernel<true><<<lp.n_group, 256, 0, st>>>(lp);
     } else {
       large_init_kernel<false><<<ig, 256, 0, st>>>(lp);
-      for (int j = 0; j < n_launch; ++j) large_step_kernel<false><<<sg, 256, h->smem_bytes, st>>>(lp, j, NTmax);
+      for (int j = 0; j < n_launch; ++j) {
+        if (tma) large_step_kernel<false, true><<<sg, 256, h->smem_bytes, st>>>(lp, j, NTmax);
+        else     large_step_kernel<false, false><<<sg, 256, h->smem_bytes, st>>>(lp, j, NTmax);
+      }
       large_finish_kernel<false><<<lp.n_group, 256, 0, st>>>(lp);
     }
     h->last_launches += 3 + n_launch;
@@ -505,6 +578,7 @@ extern "C" int ctqmc_load_impurity(const ctqmc_impurity_desc* desc, int device, 
   if (prop.major != 10) { delete h; return fail(CTQMC_ERR_UNSUPPORTED, "device is sm_%d%d; this library is built for sm_100a only", prop.major, prop.minor); }
   h->sm_count = prop.multiProcessorCount;
   h->n_blocks = nb;
+  h->h_blks = blks;
 
   int rc = 0;
   double* d_raw = nullptr; long long* d_rawoff = nullptr; long long* d_voff = nullptr; double* d_v = nullptr; double* d_u = nullptr;
@@ -598,7 +672,7 @@ extern "C" void ctqmc_free_impurity(ctqmc_impurity* h) {
   cudaFree(a.status); cudaFree(a.survive); cudaFree(a.strings); cudaFree(a.units); cudaFree(a.slots); cudaFree(a.sector);
   for (DevBuf* b : {&a.gx, &a.gxoff, &a.gplan_blk, &a.gplan_delta, &a.gkmax, &a.gcoff, &a.gulen, &a.gucols, &a.gcolcnt, &a.gcolbase,
                      &a.gtiles, &a.gntiles, &a.gcolmap}) cudaFree(b->p);
-  cudaFree(a.lunit.p); cudaFree(a.cnt); cudaFree(a.lx); cudaFree(a.plan_blk); cudaFree(a.plan_delta); cudaFree(a.lkmax); cudaFree(a.d_stage);
+  cudaFree(a.lunit.p); cudaFree(a.xmaps.p); cudaFree(h->d_amaps); cudaFree(a.cnt); cudaFree(a.lx); cudaFree(a.plan_blk); cudaFree(a.plan_delta); cudaFree(a.lkmax); cudaFree(a.d_stage);
   if (a.h_stage) cudaFreeHost(a.h_stage);
   for (int i = 0; i < 4; ++i) if (h->ev[i]) cudaEventDestroy(h->ev[i]);
   delete h;
