@@ -115,6 +115,9 @@ __device__ __forceinline__ void mbar_init(unsigned long long* bar, int count) {
 __device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned bytes) {
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
 }
+__device__ __forceinline__ void mbar_arrive(unsigned long long* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
 __device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
   asm volatile(
       "{\n.reg .pred P1;\nLAB_WAIT:\nmbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n@P1 bra DONE;\nbra LAB_WAIT;\nDONE:\n}"
@@ -132,7 +135,7 @@ __global__ void __launch_bounds__(256, 1) large_step_kernel(LargeParams P, int j
   constexpr int ES = CPLX ? 2 : 1;
   constexpr int BKE = CPLX ? 8 : 16;       // contraction indices per stage (128-byte rows)
   extern __shared__ __align__(128) unsigned char lsm[];
-  __shared__ __align__(8) unsigned long long full_bar[kLStages];
+  __shared__ __align__(8) unsigned long long full_bar[kLStages], empty_bar[kLStages];
   double* sscale = reinterpret_cast<double*>(lsm + kLStages * kLStageBytes);
 
   const int s = blockIdx.y;
@@ -225,26 +228,35 @@ __global__ void __launch_bounds__(256, 1) large_step_kernel(LargeParams P, int j
   if constexpr (TMA) {
     if (tid == 0) {
 #pragma unroll
-      for (int st = 0; st < kLStages; ++st) mbar_init(&full_bar[st], 1);
+      for (int st = 0; st < kLStages; ++st) { mbar_init(&full_bar[st], 1); mbar_init(&empty_bar[st], 8); }
       asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
   }
+  // TMA variant: full/empty barrier ring, no CTA-wide barrier in the loop.  The producer (thread 0) refills the slot that was
+  // consumed TWO iterations ago, so a warp may run a whole k-tile ahead of the slowest one before anybody waits.
+  constexpr int kAhead = TMA ? kLStages - 2 : kLStages - 1;
 #pragma unroll
-  for (int st = 0; st < kLStages - 1; ++st) {
+  for (int st = 0; st < kAhead; ++st) {
     if (st < nkt) load_stage(st, st);
     if constexpr (!TMA) cp_async_commit();
   }
 
   const int swz = (g & 1) << 2;
   for (int kt = 0; kt < nkt; ++kt) {
-    if constexpr (TMA) mbar_wait(&full_bar[kt % kLStages], (kt / kLStages) & 1);
-    else cp_async_wait<kLStages - 2>();
-    __syncthreads();
-    {
+    if constexpr (TMA) {
+      const int nx = kt + kAhead;
+      if (nx < nkt) {
+        if (tid == 0 && nx >= kLStages) mbar_wait(&empty_bar[nx % kLStages], ((nx / kLStages) - 1) & 1);
+        load_stage(nx, nx % kLStages);
+      }
+      mbar_wait(&full_bar[kt % kLStages], (kt / kLStages) & 1);
+    } else {
+      cp_async_wait<kLStages - 2>();
+      __syncthreads();
       const int nx = kt + kLStages - 1;
       if (nx < nkt) load_stage(nx, nx % kLStages);
-      if constexpr (!TMA) cp_async_commit();
+      cp_async_commit();
     }
     const unsigned char* As = lsm + (kt % kLStages) * kLStageBytes;
 #pragma unroll
@@ -299,6 +311,10 @@ __global__ void __launch_bounds__(256, 1) large_step_kernel(LargeParams P, int j
 #pragma unroll
           for (int nt = 0; nt < 4; ++nt) dmma884(acc[mt][nt][0], acc[mt][nt][1], a[mt].y, b[nt].y);
       }
+    }
+    if constexpr (TMA) {   // this warp is done reading the slot
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&empty_bar[kt % kLStages]);
     }
   }
   if constexpr (!TMA) cp_async_wait<0>();
