@@ -1,0 +1,271 @@
+// Small-sector path, uniform variant (real impurities, all sectors <= 16 states): same single-launch fusion as
+// chain_small.cuh (validation, routing a2, chain a3/a4, trace and sector sum a5), but instruction-lean:
+//   * every sector is padded to DP states (DP = 2, 4, 6, 9, 12 or 16 >= d_max) and every operator block to DP x DP with
+//     zeros, stored TRANSPOSED in shared memory, so a chain step is the same fully unrolled DP-term dot product for every
+//     string whatever sectors it is in -- no data-dependent loop bounds, no index arithmetic;
+//   * a group of DP lanes owns one configuration (lane = row of the carried matrix), 32/DP configurations per warp.
+// Padded rows carry exact zeros (their operator rows are zero), so results are those of the unpadded product.
+#pragma once
+#include <climits>
+
+#include "chain_small.cuh"
+
+namespace ctqmc {
+
+struct Small2Params {
+  DevImp imp;
+  BatchView bv;
+  const double* ftpad;      // [n_blocks][DP][DP]: ftpad[b][k][r] = F_b[r][k], zero padded
+  const int2* binfo;        // [n_blocks] {dst sector, rows << 16 | cols}
+  int n_blocks;
+  int literal;
+  double* mant; long long* exp2; uint8_t* survive; int* status;
+  Counters* cnt;
+};
+
+__host__ __device__ inline size_t small2_common_bytes(int Q, int A, int nb, int DP) {
+  size_t b = ((size_t)nb * DP * DP * 8 + (size_t)Q * DP * 8 + (size_t)Q * 8 + 15) / 16 * 16;
+  b += (size_t)nb * 8 + (size_t)Q * 4 + (size_t)A * Q * 2;
+  return (b + 15) / 16 * 16;
+}
+__host__ __device__ inline size_t small2_group_bytes(int Q, int DP) {
+  size_t b = (size_t)2 * DP * DP * 8 + (size_t)Q * (8 * 3) + (size_t)Q * 4 * 4 + 16;
+  return (b + 15) / 16 * 16;
+}
+
+template <int DP>
+__global__ void __launch_bounds__(512) small2_trace_kernel(Small2Params P) {
+  constexpr int GPW = 32 / DP;                       // groups (configurations) per warp
+  extern __shared__ __align__(16) unsigned char ssm2[];
+  const int Q = P.imp.Q, A = P.imp.A, nb = P.n_blocks;
+  double* s_ft = reinterpret_cast<double*>(ssm2);
+  double* s_de = s_ft + (size_t)nb * DP * DP;        // [Q][DP]  E - Emin (0 on padded rows)
+  double* s_emin = s_de + (size_t)Q * DP;
+  int2* s_binfo = reinterpret_cast<int2*>(ssm2 + ((size_t)(nb * DP * DP + Q * DP + Q) * 8 + 15) / 16 * 16);
+  int* s_dim = reinterpret_cast<int*>(s_binfo + nb);
+  short* s_blkof = reinterpret_cast<short*>(s_dim + Q);
+  unsigned char* s_groups = ssm2 + small2_common_bytes(Q, A, nb, DP);
+  for (int i = threadIdx.x; i < nb * DP * DP; i += blockDim.x) s_ft[i] = P.ftpad[i];
+  for (int i = threadIdx.x; i < Q * DP; i += blockDim.x) {
+    const int q = i / DP, r = i - q * DP;
+    s_de[i] = (r < P.imp.dim[q]) ? __dsub_rn(P.imp.energy[P.imp.e_off[q] + r], P.imp.e_min[q]) : 0.0;
+  }
+  for (int i = threadIdx.x; i < Q; i += blockDim.x) { s_emin[i] = P.imp.e_min[i]; s_dim[i] = P.imp.dim[i]; }
+  for (int i = threadIdx.x; i < nb; i += blockDim.x) s_binfo[i] = P.binfo[i];
+  for (int i = threadIdx.x; i < A * Q; i += blockDim.x) s_blkof[i] = (short)P.imp.blk_of[i];
+  __syncthreads();
+
+  const int lane = threadIdx.x & 31, grp = lane / DP;
+  if (grp >= GPW) return;                            // spare lanes of the warp (32 is not a multiple of DP)
+  const int lg = lane - grp * DP;
+  const unsigned mask = (DP == 32 ? 0xffffffffu : ((1u << DP) - 1u)) << (grp * DP);
+  const int grp_in_cta = (threadIdx.x >> 5) * GPW + grp;
+  const int groups_per_cta = (blockDim.x >> 5) * GPW;
+  const size_t gbytes = small2_group_bytes(Q, DP);
+  double* Xa = reinterpret_cast<double*>(s_groups + (size_t)grp_in_cta * gbytes);
+  double* Xb = Xa + DP * DP;
+  double* t_re = Xb + DP * DP;
+  double* t_lg = t_re + Q;
+  long long* t_e = reinterpret_cast<long long*>(t_lg + Q);
+  int* s_c = reinterpret_cast<int*>(t_e + Q);
+  int* s_r = s_c + Q;
+  int* s_qs = s_r + Q;
+  int* s_sv = s_qs + Q;   // [Q + 1]: start sectors with a chain to multiply, then their count
+
+  const long long n_groups = (long long)gridDim.x * groups_per_cta;
+  unsigned long long st_strings = 0, st_flops = 0;
+  for (long long b = (long long)blockIdx.x * groups_per_cta + grp_in_cta; b < P.bv.B; b += n_groups) {
+    const long long lo = P.bv.offset[b];
+    const int L = (int)(P.bv.offset[b + 1] - lo);
+    const int* sym = P.bv.symbol + lo;
+    const double* tau = P.bv.tau + lo;
+    const double beta = P.bv.beta;
+
+    // ---- validation (reading A7)
+    bool ok = L >= 0;
+    for (int i = lg; i < L; i += DP) {
+      const int a = __ldg(sym + i);
+      const double t = __ldg(tau + i);
+      const double prev = i ? __ldg(tau + i - 1) : 0.0;
+      ok = ok && (a >= 0) && (a < A) && (t >= prev) && (t < beta);
+    }
+    ok = __all_sync(mask, ok);
+    if (!ok) {
+      if (lg == 0) {
+        const double nan = __longlong_as_double(0x7ff8000000000000LL);
+        P.mant[2 * b] = nan; P.mant[2 * b + 1] = nan; P.exp2[b] = 0; P.status[b] = 2;
+      }
+      if (P.survive) for (int q0 = lg; q0 < Q; q0 += DP) P.survive[b * Q + q0] = 0;
+      continue;
+    }
+
+    // ---- routing (a2): start sectors dealt to the lanes of the group
+    bool any_surv = false;
+    for (int q0 = lg; q0 < Q; q0 += DP) {
+      int q = q0, dmin = s_dim[q0], rpos = 0, qmin = q0;
+      double lgv = 0.0;
+      bool alive = true;
+      const double t0 = L ? __ldg(tau) : 0.0;
+      double tcur = t0;
+      // operator string one step ahead in registers: the loads overlap the table look-ups of the current step
+      int sym_nx = L ? __ldg(sym) : 0;
+      double tau_nx = (L > 1) ? __ldg(tau + 1) : 0.0;
+      for (int i = 0; i < L; ++i) {
+        const int sym_c = sym_nx;
+        const double tau_c1 = tau_nx;
+        if (i + 1 < L) sym_nx = __ldg(sym + i + 1);
+        if (i + 2 < L) tau_nx = __ldg(tau + i + 2);
+        const int blk = s_blkof[sym_c * Q + q];
+        if (blk < 0) { alive = false; break; }
+        const int qn = s_binfo[blk].x;
+        const int dn = s_dim[qn];
+        const double tnext = (i + 1 < L) ? tau_c1 : beta + t0;
+        lgv -= (tnext - tcur) * s_emin[qn] * kLog2e;
+        tcur = tnext;
+        if (i + 1 < L && dn < dmin) { dmin = dn; rpos = i + 1; qmin = qn; }
+        q = qn;
+      }
+      if (L == 0) lgv = -beta * s_emin[q0] * kLog2e;
+      int c = -1;
+      if (alive) {
+        c = 0;
+        if (q == q0) {
+          if (P.literal) { c = s_dim[q0]; s_r[q0] = 0; s_qs[q0] = q0; }
+          else { c = dmin; s_r[q0] = rpos; s_qs[q0] = qmin; }
+        }
+      }
+      s_c[q0] = c; t_lg[q0] = lgv; t_re[q0] = 0.0; t_e[q0] = 0;
+      if (P.survive) P.survive[b * Q + q0] = alive ? 1 : 0;
+      any_surv = any_surv || alive;
+    }
+    any_surv = __any_sync(mask, any_surv);
+    __syncwarp(mask);
+    if (lg == 0) {   // compact list of the start sectors that have a chain: every group of the warp then runs its
+      int ns = 0;    // si-th chain at the same time (a `continue` over q0 would serialise the groups of a warp)
+      for (int q0 = 0; q0 < Q; ++q0) if (s_c[q0] > 0) s_sv[ns++] = q0;
+      s_sv[Q] = ns;
+    }
+    __syncwarp(mask);
+    const int n_chain = s_sv[Q];
+
+    // ---- chains of the surviving start sectors (a3, a4, a5)
+    for (int si = 0; si < n_chain; ++si) {
+      const int q0 = s_sv[si];
+      const int c = s_c[q0];
+      int q = s_qs[q0];
+      const int r = s_r[q0];
+      double* X = Xa;      // X[n * DP + k]: column n of the carried matrix, padded rows are zero
+      double* Xn = Xb;
+      double tr = 0.0;
+      long long e2 = 0;
+      bool dead = false;
+      if (L == 0) {        // empty configuration: Tr P_beta(q0) (reading A7)
+        if (lg == 0) for (int n = 0; n < c; ++n) tr += exp(-beta * s_de[q * DP + n]);
+      } else {
+        for (int n = 0; n < c; ++n) X[n * DP + lg] = (lg == n) ? 1.0 : 0.0;
+        __syncwarp(mask);
+        unsigned long long macs = 0;
+        int i = r;
+        int sym_nx = __ldg(sym + i);
+        double ta_nx = __ldg(tau + i), tb_nx = __ldg(tau + ((i + 1 < L) ? i + 1 : 0));
+        for (int j = 0; j < L; ++j) {
+          const int sym_c = sym_nx;
+          const double ta = ta_nx, tb = tb_nx;
+          const bool wrap = i + 1 >= L;
+          i = wrap ? 0 : i + 1;
+          sym_nx = __ldg(sym + i);                     // next step's operator, in flight during this step
+          ta_nx = __ldg(tau + i); tb_nx = __ldg(tau + ((i + 1 < L) ? i + 1 : 0));
+          const int blk = s_blkof[sym_c * Q + q];
+          const int2 bi = s_binfo[blk];
+          const int qn = bi.x;
+          const double delta = wrap ? (beta - ta + tb) : (tb - ta);
+          // this lane's row of F (transposed store: consecutive lanes read consecutive doubles)
+          const double* ft = s_ft + (size_t)blk * (DP * DP) + lg;
+          double f[DP];
+#pragma unroll
+          for (int k = 0; k < DP; ++k) f[k] = ft[k * DP];
+          // propagator of this row: 2^x = mantissa in [1, 2) times 2^kr  (prop_x with the pre-subtracted energy)
+          const double x = __dmul_rn(__dmul_rn(-delta, s_de[qn * DP + lg]), kLog2e);
+          const double mr = exp2(__dsub_rn(x, floor(x)));
+          const int kr = row_exp(x);
+          int wexp = INT_MIN;
+          for (int n = 0; n < c; ++n) {
+            const double* xs = X + n * DP;
+            double a0 = 0.0, a1 = 0.0;
+#pragma unroll
+            for (int k = 0; k + 1 < DP; k += 2) { a0 = fma(f[k], xs[k], a0); a1 = fma(f[k + 1], xs[k + 1], a1); }
+            if (DP & 1) a0 = fma(f[DP - 1], xs[DP - 1], a0);
+            const double v = (a0 + a1) * mr;
+            Xn[n * DP + lg] = v;
+            if (v != 0.0) wexp = max(wexp, kr + ilogb_fast(v));
+          }
+          const int kmax = __reduce_max_sync(mask, wexp);
+          if (kmax == INT_MIN) { dead = true; break; }
+          e2 += kmax;
+          const int sh = kr - kmax;
+          if (sh > 1022 || sh < -1022) {
+            for (int n = 0; n < c; ++n) Xn[n * DP + lg] = scalbn(Xn[n * DP + lg], max(sh, -2200));
+          } else {
+            const double sc = pow2i(sh);
+            for (int n = 0; n < c; ++n) Xn[n * DP + lg] *= sc;
+          }
+          __syncwarp(mask);
+          double* tmp = X; X = Xn; Xn = tmp;
+          macs += (unsigned long long)(bi.y >> 16) * (unsigned long long)(bi.y & 0xffff);
+          q = qn;
+        }
+        if (lg == 0) {
+          if (!dead) for (int n = 0; n < c; ++n) tr += X[n * DP + n];
+          st_strings += 1; st_flops += macs * (unsigned long long)c * 2ull;
+        }
+        __syncwarp(mask);
+      }
+      if (lg == 0) { t_re[q0] = dead ? 0.0 : tr; t_e[q0] = dead ? 0 : e2; }
+    }
+    __syncwarp(mask);
+
+    // ---- sector sum with exponent alignment (a5): q0 ascending, Neumaier-compensated, normalised to [1, 2)
+    if (lg == 0) {
+      bool any_nz = false;
+      long long emax = 0;
+      for (int q0 = 0; q0 < Q; ++q0) {
+        if (s_c[q0] <= 0) continue;
+        const double kf = floor(t_lg[q0]);
+        const double mx = fabs(t_re[q0]) * exp2(t_lg[q0] - kf);
+        if (mx > 0.0) {
+          const long long e = t_e[q0] + (long long)kf + ilogb(mx);
+          emax = any_nz ? max(emax, e) : e;
+          any_nz = true;
+        }
+      }
+      double re = 0.0, cre = 0.0;
+      if (any_nz) {
+        for (int q0 = 0; q0 < Q; ++q0) {
+          if (s_c[q0] <= 0) continue;
+          const double kf = floor(t_lg[q0]);
+          long long sh = t_e[q0] + (long long)kf - emax;
+          double xr = 0.0;
+          if (sh >= -1100) { if (sh > 1000) sh = 1000; xr = scalbn(t_re[q0] * exp2(t_lg[q0] - kf), (int)sh); }
+          const double t2 = re + xr; cre += (fabs(re) >= fabs(xr)) ? (re - t2) + xr : (xr - t2) + re; re = t2;
+        }
+        re += cre;
+      }
+      if (re != 0.0) {
+        const int k = ilogb(re);
+        P.mant[2 * b] = scalbn(re, -k); P.mant[2 * b + 1] = 0.0; P.exp2[b] = emax + k;
+      } else {
+        P.mant[2 * b] = 0.0; P.mant[2 * b + 1] = 0.0; P.exp2[b] = 0;
+      }
+      P.status[b] = any_surv ? 0 : 1;
+    }
+    __syncwarp(mask);
+  }
+  if (lg == 0 && st_strings) {
+    atomicAdd(&P.cnt->n_strings, st_strings);
+    atomicAdd(&P.cnt->n_slots, st_strings);
+    atomicAdd(&P.cnt->alg_flops, st_flops);
+    atomicAdd(&P.cnt->macs, st_flops / 2);
+  }
+}
+
+}  // namespace ctqmc

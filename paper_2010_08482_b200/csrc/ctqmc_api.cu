@@ -16,6 +16,7 @@
 #include "chain_grouped.cuh"
 #include "chain_large.cuh"
 #include "chain_small.cuh"
+#include "chain_small2.cuh"
 #include "common.cuh"
 #include "peak.cuh"
 #include "reduce.cuh"
@@ -100,6 +101,10 @@ struct ctqmc_impurity {
   double* d_pack = nullptr; int4* d_pblk = nullptr;   // small-sector path: unpadded store
   int pack_len = 0, n_energy = 0;
   int small_ok = 0, small = 0, small_g = 32, small_grid_max = 0;
+  double* d_ftpad = nullptr; int2* d_binfo = nullptr;   // uniform small-sector variant (real): padded transposed blocks
+  int small2 = 0, small2_dp = 0, small2_threads = 512;
+  int small2_occ[17] = {0};
+  size_t small2_smem = 0;
   size_t small_smem = 0;
   // schedule
   int schedule = CTQMC_SCHEDULE_THIN;
@@ -165,6 +170,16 @@ SmallFn pick_small(int cplx, int g) {
   return g == 8 ? small_trace_kernel<false, 8> : g == 16 ? small_trace_kernel<false, 16> : small_trace_kernel<false, 32>;
 }
 
+using Small2Fn = void (*)(Small2Params);
+Small2Fn pick_small2(int dp) {
+  switch (dp) {
+    case 2: return small2_trace_kernel<2>;   case 4: return small2_trace_kernel<4>;   case 6: return small2_trace_kernel<6>;
+    case 9: return small2_trace_kernel<9>;   case 12: return small2_trace_kernel<12>; case 16: return small2_trace_kernel<16>;
+  }
+  return nullptr;
+}
+int small2_dp_for(int dmax) { const int c[6] = {2, 4, 6, 9, 12, 16}; for (int v : c) if (v >= dmax) return v; return 0; }
+
 int pick_ldx(int cplx, int dmax) {
   int l = (dmax + 7) / 8 * 8;
   if (cplx) { while (l % 8 != 4) ++l; }       // 16-byte elements: conflict-free 128-bit fragment loads need ldx = 4 mod 8
@@ -193,6 +208,23 @@ int configure(ctqmc_impurity* h, int want_w) {
       if (occ >= 1) { h->small = 1; h->small_grid_max = occ * h->sm_count; }
     }
     if (!h->small && h->path == CTQMC_PATH_SMALL) return fail(CTQMC_ERR_UNSUPPORTED, "small-sector kernel does not fit in shared memory");
+    // uniform variant for real impurities (chain_small2.cuh) unless CTQMC_SMALL_V1=1
+    h->small2 = 0;
+    const char* v1 = getenv("CTQMC_SMALL_V1");
+    if (h->small && h->d_ftpad && !(v1 && atoi(v1))) {
+      const int dp = h->small2_dp;
+      Small2Fn fn = pick_small2(dp);
+      for (int threads : {512, 256}) {
+        const size_t bytes = small2_common_bytes(h->dev.Q, h->dev.A, h->n_blocks, dp) +
+                             (size_t)(threads / 32) * (32 / dp) * small2_group_bytes(h->dev.Q, dp);
+        if (fn && bytes <= smem_max) {
+          CU(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+          int occ = 0;
+          CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, threads, bytes));
+          if (occ >= 1) { h->small2 = 1; h->small2_threads = threads; h->small2_smem = bytes; h->small_grid_max = occ * h->sm_count; break; }
+        }
+      }
+    }
   }
   h->ldx = pick_ldx(cplx, h->dev.dmax);
   h->team_warps = h->dev.dmax <= 16 ? 1 : 8;
@@ -568,6 +600,21 @@ extern "C" int ctqmc_load_impurity(const ctqmc_impurity_desc* desc, int device, 
     }
   }
 
+  std::vector<double> ftpad;
+  std::vector<int2> binfo(nb);
+  const int dp2 = (small_ok && !cplx) ? small2_dp_for(dmax) : 0;
+  if (dp2) {
+    const double* raw = (const double*)desc->blk_data;
+    ftpad.assign((size_t)nb * dp2 * dp2, 0.0);
+    for (int b = 0; b < nb; ++b) {
+      const BlkDesc& bd = blks[b];
+      binfo[b] = make_int2(bd.dst, (bd.rows << 16) | bd.cols);
+      for (int m = 0; m < bd.rows; ++m)
+        for (int k = 0; k < bd.cols; ++k)
+          ftpad[((size_t)b * dp2 + k) * dp2 + m] = raw[(size_t)raw_off[b] + (size_t)k * bd.rows + m];
+    }
+  }
+
   CU(cudaSetDevice(device));
   ctqmc_impurity* h = new (std::nothrow) ctqmc_impurity();
   if (!h) return fail(CTQMC_ERR_OOM, "host allocation failed");
@@ -603,6 +650,11 @@ extern "C" int ctqmc_load_impurity(const ctqmc_impurity_desc* desc, int device, 
     TRY(upload(&h->d_pack, pack));
     TRY(upload(&h->d_pblk, pblk));
     h->pack_len = (int)(pack.size() / es); h->small_ok = 1;
+  }
+  if (dp2) {
+    TRY(upload(&h->d_ftpad, ftpad));
+    TRY(upload(&h->d_binfo, binfo));
+    h->small2_dp = dp2;
   }
   h->n_energy = (int)ne;
   TRY(upload(&d_voff, v_off));
@@ -666,6 +718,7 @@ extern "C" void ctqmc_free_impurity(ctqmc_impurity* h) {
   if (!h) return;
   cudaSetDevice(h->device);
   cudaFree(h->d_dim); cudaFree(h->d_eoff); cudaFree(h->d_energy); cudaFree(h->d_emin); cudaFree(h->d_blkof);
+  cudaFree(h->d_ftpad); cudaFree(h->d_binfo);
   cudaFree(h->d_pack); cudaFree(h->d_pblk); cudaFree(h->d_blkorder);
   cudaFree(h->d_blks); cudaFree(h->d_store); cudaFree(h->d_rownorm2); cudaFree(h->d_sigma);
   Arena& a = h->arena;
@@ -743,10 +796,35 @@ extern "C" int ctqmc_trace_batch(ctqmc_impurity* h, double beta, const ctqmc_bat
     sp.imp = h->dev; sp.bv = bv; sp.pack = h->d_pack; sp.pblk = h->d_pblk; sp.n_blocks = h->n_blocks; sp.pack_len = h->pack_len;
     sp.n_energy = h->n_energy; sp.literal = (h->schedule == CTQMC_SCHEDULE_LITERAL); sp.mant = mant; sp.exp2 = (long long*)exp2;
     sp.survive = survive; sp.status = status; sp.cnt = a.cnt; sp.dmax = h->dev.dmax;
-    const long long gpc = kCtaThreads / h->small_g;
-    long long grid = (B + gpc - 1) / gpc;
-    if (grid > h->small_grid_max) grid = h->small_grid_max;
-    pick_small(h->dev.cplx, h->small_g)<<<(unsigned)grid, kCtaThreads, h->small_smem, st>>>(sp);
+    if (h->small2) {
+      Small2Params s2;
+      s2.imp = h->dev; s2.bv = bv; s2.ftpad = h->d_ftpad; s2.binfo = h->d_binfo; s2.n_blocks = h->n_blocks; s2.literal = sp.literal;
+      s2.mant = mant; s2.exp2 = (long long*)exp2; s2.survive = survive; s2.status = status; s2.cnt = a.cnt;
+      // CTA size: small batches are latency-bound, so they are spread over all SMs in ONE wave: warps per CTA =
+      // ceil(configurations per SM / configurations per warp), at most the configured maximum
+      const int gpw = 32 / h->small2_dp, max_warps = h->small2_threads / 32;
+      long long per_sm = (B + h->sm_count - 1) / h->sm_count;
+      int warps = (int)((per_sm + gpw - 1) / gpw);
+      if (warps < 2) warps = 2;
+      if (warps > max_warps) warps = max_warps;
+      const int threads = 32 * warps;
+      const long long gpc = (long long)warps * gpw;
+      const size_t smem = small2_common_bytes(h->dev.Q, h->dev.A, h->n_blocks, h->small2_dp) + (size_t)gpc * small2_group_bytes(h->dev.Q, h->small2_dp);
+      if (h->small2_occ[warps] == 0) {
+        int occ = 0;
+        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, pick_small2(h->small2_dp), threads, smem));
+        h->small2_occ[warps] = occ > 0 ? occ : 1;
+      }
+      long long grid = (B + gpc - 1) / gpc;
+      const long long grid_max = (long long)h->small2_occ[warps] * h->sm_count;
+      if (grid > grid_max) grid = grid_max;
+      pick_small2(h->small2_dp)<<<(unsigned)grid, threads, smem, st>>>(s2);
+    } else {
+      const long long gpc = kCtaThreads / h->small_g;
+      long long grid = (B + gpc - 1) / gpc;
+      if (grid > h->small_grid_max) grid = h->small_grid_max;
+      pick_small(h->dev.cplx, h->small_g)<<<(unsigned)grid, kCtaThreads, h->small_smem, st>>>(sp);
+    }
     h->last_launches += 1;
     mark(h, 2, st);
     mark(h, 3, st);
@@ -959,7 +1037,7 @@ extern "C" int ctqmc_bound_batch_host(ctqmc_impurity* h, double beta, const ctqm
 extern "C" int ctqmc_last_stats(ctqmc_impurity* h, int64_t stats[8]) {
   if (!h || !stats) return fail(CTQMC_ERR_ARG, "null argument");
   for (int i = 0; i < 8; ++i) stats[i] = 0;
-  stats[5] = h->small ? h->small_g : h->nt * 8; stats[6] = h->team_warps; stats[7] = h->last_path ? h->last_path : (h->small ? 3 : h->grouped ? 4 : h->large ? 2 : 1);
+  stats[5] = h->small ? (h->small2 ? h->small2_dp : h->small_g) : h->nt * 8; stats[6] = h->team_warps; stats[7] = h->last_path ? h->last_path : (h->small ? 3 : h->grouped ? 4 : h->large ? 2 : 1);
   if (!h->arena.cnt) return 0;
   CU(cudaSetDevice(h->device));
   Counters c;

@@ -176,6 +176,24 @@ def test_trace_parity_panel_path_forced(cfg, n, schedule, lib, torch_cuda, impur
         lib.ctqmc_set_option(h, lib.CTQMC_OPT_PATH, lib.CTQMC_PATH_AUTO)
 
 
+@pytest.mark.parametrize("cfg,n", [(1, 300), (2, 200)])
+def test_small_path_first_variant_on_real_impurities(cfg, n, lib, torch_cuda, impurities, monkeypatch):
+    """Real small impurities default to the uniform (padded, DP lanes per configuration) variant; CTQMC_SMALL_V1=1 selects
+    the element-per-lane variant that complex impurities use.  Both against the oracle, both schedules."""
+    from workloads import make_batch
+    imp = impurities(cfg)
+    monkeypatch.setenv("CTQMC_SMALL_V1", "1")
+    h = lib.ctqmc_load_impurity(imp, 0)
+    try:
+        for sched in (lib.CTQMC_SCHEDULE_THIN, lib.CTQMC_SCHEDULE_LITERAL):
+            lib.ctqmc_set_option(h, lib.CTQMC_OPT_SCHEDULE, sched)
+            _check_trace(lib, torch_cuda, imp, h, make_batch(cfg, n, start=16000), f"cfg{cfg}-small-v1")
+            st = lib.ctqmc_last_stats(h)
+            assert st["path"] == lib.CTQMC_PATH_SMALL and st["panel_width"] in (8, 16, 32)   # lanes per configuration, not DP
+    finally:
+        h.free()
+
+
 @pytest.mark.parametrize("lanes", [8, 16, 32])
 def test_small_path_complex_and_group_sizes(lanes, lib, torch_cuda, monkeypatch):
     """Small path with complex blocks (config 1 with seeded eigenvector phases, reading A17) and every lanes-per-
