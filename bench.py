@@ -37,12 +37,12 @@ WORKLOADS = {
 }
 REF_SAMPLE = {1: 4096, 2: 2048, 3: 16, 4: 2, 5: 1}   # configurations per reference step (seconds of oracle time each)
 KERNELS = {1: ("chain_kernel (panel in shared memory, fused propagate x operator, FP64 DMMA m8n8k4)", "tensor"),
-           2: ("large_step_kernel (128x64 tiles, cp.async pipeline, fused propagate x operator, FP64 DMMA m8n8k4)", "tensor"),
-           3: ("small_trace_kernel (whole path in one launch, operator store in shared memory, FP64 FMA)", "alu"),
+           2: ("large_step_kernel (128x64 tiles, TMA + mbarrier ring, fused propagate x operator, FP64 DMMA m8n8k4)", "tensor"),
+           3: ("small2_trace_kernel / small_trace_kernel (whole path in one launch, operator store in shared memory, FP64 FMA)", "alu"),
            4: ("grouped_step_kernel (strings sharing a block share one GEMM per chain position, 64x64 tiles, FP64 DMMA m8n8k4)", "tensor")}
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, from the `ncu --set full` captures
 # summarised under profiles/ (same launch configuration as the default batch of each config); None = not captured.
-NCU_TRAFFIC_BYTES = {2: 5_991_680, 3: 30_400_256}
+NCU_TRAFFIC_BYTES = {2: 6_059_008, 4: 664_738_560}   # cfg 2: profiles/r01_cfg2_small_full.md; cfg 4: r01_cfg4_grouped_step_full.md (one chain position)
 
 
 def peaks():
