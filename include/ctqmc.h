@@ -57,6 +57,11 @@ extern "C" {
 #define CTQMC_PATH_SMALL       3
 #define CTQMC_PATH_GROUPED     4   /* step-synchronous grouped GEMM: strings that apply the same block share one GEMM per chain position */
 
+/* Diagnostic environment variables, read when an impurity is loaded or a path is selected (results do not depend on them
+ * beyond rounding): CTQMC_LARGE_TMA=0 stages the large-sector kernel's tiles with cp.async instead of TMA; CTQMC_SMALL_V1=1
+ * runs real small impurities on the element-per-lane small kernel that complex ones use; CTQMC_SMALL_G=8|16|32 sets that
+ * kernel's lanes per configuration. */
+
 typedef struct ctqmc_impurity ctqmc_impurity;   /* opaque; created by ctqmc_load_impurity, destroyed by ctqmc_free_impurity */
 
 /*
