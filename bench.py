@@ -162,6 +162,7 @@ def run_reference(args, rank: int):
 
 def measure_config(L, torch, cfg, B, rank, steps, warmup, schedule, local_rank, barrier, fp64, pk, with_e2e=True, path="auto"):
     """Times `steps` passes of the hot path on config `cfg` (this rank's shard) and returns the pieces of the JSON line."""
+    import numpy as np
     from workloads import build_config_impurity
     imp = build_config_impurity(cfg, keep_eigvecs=False)
     t0 = time.perf_counter()
@@ -202,16 +203,23 @@ def measure_config(L, torch, cfg, B, rank, steps, warmup, schedule, local_rank, 
 
     e2e_ms = None
     if with_e2e:
-        # end to end through the host-buffer C call: H2D of the batch, kernels, D2H of the results, inside the timed region
+        # end to end through the host-buffer C call, from / to PINNED host memory: H2D of the batch, kernels, D2H of the
+        # results, all inside the timed region
+        pin = [torch.from_numpy(x).pin_memory() for x in (batch.offset, batch.symbol, batch.tau)]
+        h_in = [t.numpy() for t in pin]
+        pout = [torch.empty((B, 2), dtype=torch.float64).pin_memory(), torch.empty(B, dtype=torch.int64).pin_memory(),
+                torch.empty((B, Q), dtype=torch.uint8).pin_memory(), torch.empty(B, dtype=torch.int32).pin_memory()]
+        h_out = tuple(t.numpy() for t in pout)
         for _ in range(2):
-            L.ctqmc_trace_batch_host(h, batch.beta, batch.offset, batch.symbol, batch.tau)
+            L.ctqmc_trace_batch_host(h, batch.beta, *h_in, out=h_out)
+        assert np.array_equal(h_out[0], out[0].cpu().numpy(), equal_nan=True) and np.array_equal(h_out[1], out[1].cpu().numpy())
         e2e_s = 0.0
         barrier()
         for _ in range(steps):
             flush.zero_()
             torch.cuda.synchronize()
             t0 = time.perf_counter()
-            L.ctqmc_trace_batch_host(h, batch.beta, batch.offset, batch.symbol, batch.tau)
+            L.ctqmc_trace_batch_host(h, batch.beta, *h_in, out=h_out)
             e2e_s += time.perf_counter() - t0
         barrier()
         e2e_ms = e2e_s * 1e3

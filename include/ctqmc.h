@@ -144,7 +144,10 @@ int ctqmc_bound_batch(ctqmc_impurity* imp, double beta, const ctqmc_batch* batch
 /*
  * Host-buffer convenience forms: identical results, but `batch` fields and all outputs are HOST pointers.  The library
  * copies the batch to the device, runs the same kernels, copies the results back and synchronises the stream before
- * returning (this is the end-to-end path bench.py times).
+ * returning (this is the end-to-end path bench.py times).  If every buffer passed to ctqmc_trace_batch_host is page-locked
+ * (cudaHostAlloc / cudaHostRegister / torch pin_memory) the copies go straight from / to the caller's memory, and on the
+ * small-sector path batches of 32768 configurations or more are cut into four chunks whose host-to-device copies (on an
+ * internal stream) overlap the previous chunk's kernel; pageable buffers go through the library's pinned staging area.
  */
 int ctqmc_trace_batch_host(ctqmc_impurity* imp, double beta, const ctqmc_batch* batch,
                            double* mant, int64_t* exp2, uint8_t* survive, int32_t* status, void* cuda_stream);

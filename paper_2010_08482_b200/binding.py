@@ -226,14 +226,21 @@ def _host_batch(offset, symbol, tau):
 
 
 def ctqmc_trace_batch_host(imp: ImpurityHandle, beta: float, offset, symbol, tau, want_survive: bool = True,
-                           stream=None):
-    """Host form: numpy in, numpy out; copies and synchronises inside the library."""
+                           stream=None, out=None):
+    """Host form: numpy in, numpy out; copies and synchronises inside the library.  `out` = (mant, exp2, survive, status)
+    numpy arrays to write into (e.g. views of page-locked torch tensors: with page-locked inputs too, the library skips its
+    staging copies and overlaps transfers with compute)."""
     b, keep = _host_batch(offset, symbol, tau)
     B = b.n_configs
-    mant = np.empty((B, 2), np.float64)
-    exp2 = np.empty(B, np.int64)
-    surv = np.empty((B, imp.n_sectors), np.uint8) if want_survive else None
-    status = np.empty(B, np.int32)
+    if out is not None:
+        mant, exp2, surv, status = out
+        assert mant.dtype == np.float64 and exp2.dtype == np.int64 and status.dtype == np.int32
+        want_survive = surv is not None
+    else:
+        mant = np.empty((B, 2), np.float64)
+        exp2 = np.empty(B, np.int64)
+        surv = np.empty((B, imp.n_sectors), np.uint8) if want_survive else None
+        status = np.empty(B, np.int32)
     _check(library().ctqmc_trace_batch_host(imp.ptr, float(beta), C.byref(b), mant.ctypes.data, exp2.ctypes.data,
                                             surv.ctypes.data if want_survive else None, status.ctypes.data,
                                             _stream_ptr(stream, host=True)))

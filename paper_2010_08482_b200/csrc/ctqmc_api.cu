@@ -118,6 +118,8 @@ struct ctqmc_impurity {
   long long last_launches = 0;
   int timing = 0, timing_valid = 0;
   cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
+  cudaStream_t copy_stream = nullptr;          // host form, pinned inputs: H2D of chunk k+1 overlaps the kernel of chunk k
+  cudaEvent_t ev_chunk[9] = {nullptr};
 };
 
 namespace {
@@ -728,6 +730,8 @@ extern "C" void ctqmc_free_impurity(ctqmc_impurity* h) {
   cudaFree(a.lunit.p); cudaFree(a.xmaps.p); cudaFree(h->d_amaps); cudaFree(a.cnt); cudaFree(a.lx); cudaFree(a.plan_blk); cudaFree(a.plan_delta); cudaFree(a.lkmax); cudaFree(a.d_stage);
   if (a.h_stage) cudaFreeHost(a.h_stage);
   for (int i = 0; i < 4; ++i) if (h->ev[i]) cudaEventDestroy(h->ev[i]);
+  for (int i = 0; i < 9; ++i) if (h->ev_chunk[i]) cudaEventDestroy(h->ev_chunk[i]);
+  if (h->copy_stream) cudaStreamDestroy(h->copy_stream);
   delete h;
 }
 
@@ -973,6 +977,77 @@ int stage_in(ctqmc_impurity* h, const ctqmc_batch* hb, size_t out_bytes, Staged*
   return 0;
 }
 
+bool is_pinned(const void* p) {
+  if (!p) return false;
+  cudaPointerAttributes at;
+  if (cudaPointerGetAttributes(&at, p) != cudaSuccess) { cudaGetLastError(); return false; }
+  return at.type == cudaMemoryTypeHost;
+}
+
+// Host form, fast path: the caller's buffers are page-locked, so the library copies straight from / to them (no staging
+// memcpy), and -- on the single-launch small-sector path -- cuts the batch into chunks whose host-to-device copies run on a
+// second stream while the previous chunk's kernel runs.
+int trace_host_pinned(ctqmc_impurity* h, double beta, const ctqmc_batch* hb, double* mant, int64_t* exp2, uint8_t* survive,
+                      int32_t* status, cudaStream_t st) {
+  const long long B = hb->n_configs;
+  const long long n_ops = hb->offset[B];
+  const size_t Q = h->dev.Q;
+  const size_t b_off = align_up((size_t)(B + 1) * 8), b_sym = align_up((size_t)n_ops * 4), b_tau = align_up((size_t)n_ops * 8);
+  const size_t o_mant = 0, o_exp = align_up(B * 16), o_stat = o_exp + align_up(B * 8), o_surv = o_stat + align_up(B * 4);
+  const size_t out_bytes = o_surv + align_up(B * Q);
+  const size_t total = b_off + b_sym + b_tau + out_bytes;
+  Arena& a = h->arena;
+  if (total > a.d_stage_bytes) {
+    cudaFree(a.d_stage); a.d_stage = nullptr; a.d_stage_bytes = 0;
+    if (a.h_stage) cudaFreeHost(a.h_stage);
+    a.h_stage = nullptr; a.h_stage_bytes = 0;
+    CU(cudaMalloc(&a.d_stage, total));
+    CU(cudaMallocHost(&a.h_stage, total));
+    a.d_stage_bytes = total; a.h_stage_bytes = total;
+  }
+  char* ds = (char*)a.d_stage;
+  long long* d_off = (long long*)ds;
+  int* d_sym = (int*)(ds + b_off);
+  double* d_tau = (double*)(ds + b_off + b_sym);
+  char* d_out = ds + b_off + b_sym + b_tau;
+  // chunking pays only when the kernel is throughput-bound; below ~3e4 configurations its duration is one configuration's
+  // dependency chain whatever the batch size, and chunks would just serialise that latency
+  const int n_chunk = (h->small && B >= 32768) ? 4 : 1;
+  if (n_chunk > 1 && !h->copy_stream) {
+    CU(cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking));
+    for (int i = 0; i < 9; ++i) CU(cudaEventCreateWithFlags(&h->ev_chunk[i], cudaEventDisableTiming));
+  }
+  cudaStream_t cs = n_chunk > 1 ? h->copy_stream : st;
+  if (n_chunk > 1) {   // the copy stream starts after everything already enqueued on the caller's stream
+    CU(cudaEventRecord(h->ev_chunk[8], st));
+    CU(cudaStreamWaitEvent(cs, h->ev_chunk[8], 0));
+  }
+  for (int k = 0; k < n_chunk; ++k) {
+    const long long b0 = B * k / n_chunk, b1 = B * (k + 1) / n_chunk;
+    const long long p0 = hb->offset[b0], p1 = hb->offset[b1];
+    CU(cudaMemcpyAsync(d_off + b0, hb->offset + b0, (size_t)(b1 - b0 + 1) * 8, cudaMemcpyHostToDevice, cs));
+    if (p1 > p0) {
+      CU(cudaMemcpyAsync(d_sym + p0, hb->symbol + p0, (size_t)(p1 - p0) * 4, cudaMemcpyHostToDevice, cs));
+      CU(cudaMemcpyAsync(d_tau + p0, hb->tau + p0, (size_t)(p1 - p0) * 8, cudaMemcpyHostToDevice, cs));
+    }
+    if (n_chunk > 1) {
+      CU(cudaEventRecord(h->ev_chunk[k], cs));
+      CU(cudaStreamWaitEvent(st, h->ev_chunk[k], 0));
+    }
+    ctqmc_batch sub;
+    sub.n_configs = b1 - b0; sub.offset = (const int64_t*)(d_off + b0); sub.symbol = d_sym; sub.tau = d_tau;
+    int rc = ctqmc_trace_batch(h, beta, &sub, (double*)(d_out + o_mant) + 2 * b0, (int64_t*)(d_out + o_exp) + b0,
+                               survive ? (uint8_t*)(d_out + o_surv) + b0 * Q : nullptr, (int32_t*)(d_out + o_stat) + b0, st);
+    if (rc) return rc;
+  }
+  CU(cudaMemcpyAsync(mant, d_out + o_mant, B * 16, cudaMemcpyDeviceToHost, st));
+  CU(cudaMemcpyAsync(exp2, d_out + o_exp, B * 8, cudaMemcpyDeviceToHost, st));
+  CU(cudaMemcpyAsync(status, d_out + o_stat, B * 4, cudaMemcpyDeviceToHost, st));
+  if (survive) CU(cudaMemcpyAsync(survive, d_out + o_surv, B * Q, cudaMemcpyDeviceToHost, st));
+  CU(cudaStreamSynchronize(st));
+  return 0;
+}
+
 }  // namespace
 
 extern "C" int ctqmc_trace_batch_host(ctqmc_impurity* h, double beta, const ctqmc_batch* batch, double* mant, int64_t* exp2,
@@ -985,6 +1060,10 @@ extern "C" int ctqmc_trace_batch_host(ctqmc_impurity* h, double beta, const ctqm
   CU(cudaSetDevice(h->device));
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const size_t Q = h->dev.Q;
+  if (batch->offset && batch->offset[B] >= 0 && (batch->offset[B] == 0 || (batch->symbol && batch->tau)) &&
+      is_pinned(batch->offset) && (batch->offset[B] == 0 || (is_pinned(batch->symbol) && is_pinned(batch->tau))) &&
+      is_pinned(mant) && is_pinned(exp2) && is_pinned(status) && (!survive || is_pinned(survive)))
+    return trace_host_pinned(h, beta, batch, mant, exp2, survive, status, st);
   const size_t o_mant = 0, o_exp = align_up(B * 16), o_stat = o_exp + align_up(B * 8), o_surv = o_stat + align_up(B * 4);
   const size_t out_bytes = o_surv + align_up(B * Q);
   Staged sg;

@@ -438,6 +438,25 @@ def test_host_form_matches_device_form(lib, torch_cuda, impurities, handles):
             assert np.array_equal(a.cpu().numpy(), b, equal_nan=True)
 
 
+@pytest.mark.parametrize("cfg,n", [(1, 40000), (2, 300), (3, 6)])
+def test_host_form_with_pinned_buffers(cfg, n, lib, torch_cuda, impurities, handles):
+    """Page-locked caller buffers: direct copies (and, for the large small-sector batch, chunked copy/compute overlap) must
+    give exactly the device form's results."""
+    from workloads import make_batch
+    torch = torch_cuda
+    batch = make_batch(cfg, n, start=500)
+    off, sym, tau = _dev(torch, batch)
+    d = lib.ctqmc_trace_batch(handles(cfg), batch.beta, off, sym, tau)
+    torch.cuda.synchronize()
+    pin = [torch.from_numpy(x).pin_memory() for x in (batch.offset, batch.symbol, batch.tau)]
+    Q = impurities(cfg).n_sectors
+    pout = [torch.full((n, 2), -7.0, dtype=torch.float64).pin_memory(), torch.zeros(n, dtype=torch.int64).pin_memory(),
+            torch.zeros((n, Q), dtype=torch.uint8).pin_memory(), torch.full((n,), -1, dtype=torch.int32).pin_memory()]
+    lib.ctqmc_trace_batch_host(handles(cfg), batch.beta, *[t.numpy() for t in pin], out=tuple(t.numpy() for t in pout))
+    for a, b in zip(d, pout):
+        assert torch.equal(a.cpu(), b)
+
+
 def test_repeatable_and_stream_ordered(lib, torch_cuda, impurities, handles):
     """Same inputs twice, on a side stream, give bit-identical outputs (fixed summation order)."""
     from workloads import make_batch
