@@ -35,7 +35,7 @@ WORKLOADS = {
     4: "cfg4: 7-orbital f-shell Slater+SOC, (N,Jz) sectors N in 4..6 (Q=70, d_max=295), complex, pairs~Poisson(100)",
     5: "cfg5: 7-orbital f-shell + crystal field, N sectors 1001/2002/3003, complex, pairs~Poisson(100)",
 }
-REF_SAMPLE = {1: 4096, 2: 2048, 3: 16, 4: 2, 5: 1}   # configurations per reference step (seconds of oracle time each)
+REF_SAMPLE = {1: 8192, 2: 4096, 3: 128, 4: 4, 5: 1}   # configurations per reference step (seconds of oracle time each)
 KERNELS = {1: ("chain_kernel (panel in shared memory, fused propagate x operator, FP64 DMMA m8n8k4)", "tensor"),
            2: ("large_step_kernel (128x64 tiles, TMA + mbarrier ring, fused propagate x operator, FP64 DMMA m8n8k4)", "tensor"),
            3: ("small2_trace_kernel / small_trace_kernel (whole path in one launch, operator store in shared memory, FP64 FMA)", "alu"),

@@ -44,6 +44,9 @@ extern "C" {
 #define CTQMC_OPT_PANEL_WIDTH  2   /* columns carried per work unit: 8, 16, 32 (0 = automatic) */
 #define CTQMC_OPT_TIMING       3   /* 1: record CUDA events around the phases of every batch call (see ctqmc_last_timing) */
 #define CTQMC_OPT_PATH         4   /* which chain kernel family runs (CTQMC_PATH_*); results agree up to rounding */
+#define CTQMC_OPT_SCRATCH_LIMIT 5  /* bytes the grouped path may allocate for its schedule and carried matrices (0 = no limit).
+                                      Above it, or when the allocation fails, AUTO falls back to the panel kernel and an explicit
+                                      CTQMC_PATH_GROUPED request returns CTQMC_ERR_OOM */
 
 /* Kernel families for CTQMC_OPT_PATH.  AUTO: the small-sector kernel (whole path in one launch, operator store in shared
  * memory) when every sector has at most 16 states; else, when a panel of the largest sector fits in shared memory, the

@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(HERE, "libctqmc_b200.so")
 CTQMC_OK, CTQMC_ERR_ARG, CTQMC_ERR_OOM, CTQMC_ERR_CUDA, CTQMC_ERR_UNSUPPORTED = 0, -1, -2, -3, -4
 CTQMC_STATUS_OK, CTQMC_STATUS_VANISHING, CTQMC_STATUS_INVALID = 0, 1, 2
 CTQMC_SCHEDULE_THIN, CTQMC_SCHEDULE_LITERAL = 0, 1
-CTQMC_OPT_SCHEDULE, CTQMC_OPT_PANEL_WIDTH, CTQMC_OPT_TIMING, CTQMC_OPT_PATH = 1, 2, 3, 4
+CTQMC_OPT_SCHEDULE, CTQMC_OPT_PANEL_WIDTH, CTQMC_OPT_TIMING, CTQMC_OPT_PATH, CTQMC_OPT_SCRATCH_LIMIT = 1, 2, 3, 4, 5
 CTQMC_PATH_AUTO, CTQMC_PATH_PANEL, CTQMC_PATH_LARGE, CTQMC_PATH_SMALL, CTQMC_PATH_GROUPED = 0, 1, 2, 3, 4
 
 EXPORTS = ["ctqmc_load_impurity", "ctqmc_free_impurity", "ctqmc_set_option", "ctqmc_trace_batch", "ctqmc_bound_batch",

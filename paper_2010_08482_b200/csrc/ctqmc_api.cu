@@ -109,6 +109,7 @@ struct ctqmc_impurity {
   // schedule
   int schedule = CTQMC_SCHEDULE_THIN;
   int path = CTQMC_PATH_AUTO;
+  long long scratch_limit = 0;   // bytes the grouped path may use for its schedule and carried matrices (0 = no limit)
   int nt = 0, team_warps = 8, ldx = 0, large = 0, grouped = 0, grouped_ok = 0, grouped_now = 0, last_path = 0;
   size_t grouped_smem = 0;
   size_t smem_bytes = 0;
@@ -403,6 +404,11 @@ int enqueue_grouped(ctqmc_impurity* h, const BatchView& bv, cudaStream_t st) {
   const int tile_cap = (int)(sum_c / kGBN + (n_units < nb ? n_units : nb) + 1);
   const size_t nul = (size_t)n_units * Lmax;
   int rc;
+  {
+    const double need = 2.0 * (double)xtot * es * 8.0 + (double)Lmax * (double)sum_c * 8.0 + (double)nul * 20.0;
+    if (h->scratch_limit > 0 && need > (double)h->scratch_limit)
+      return fail(CTQMC_ERR_OOM, "grouped path needs %.0f bytes of scratch, limit is %lld", need, h->scratch_limit);
+  }
   if ((rc = grow(a.gx, (size_t)2 * xtot * es * sizeof(double)))) return rc;
   if (a.gx.grew) CU(cudaMemsetAsync(a.gx.p, 0, a.gx.cap, st));
   if ((rc = grow(a.gxoff, n_units * sizeof(long long))) || (rc = grow(a.gplan_blk, nul * sizeof(int))) ||
@@ -760,6 +766,11 @@ extern "C" int ctqmc_set_option(ctqmc_impurity* h, int option, int64_t value) {
     if (rc) { h->path = old; configure(h, 0); }
     return rc;
   }
+  if (option == CTQMC_OPT_SCRATCH_LIMIT) {
+    if (value < 0) return fail(CTQMC_ERR_ARG, "scratch limit must be >= 0");
+    h->scratch_limit = (long long)value;
+    return 0;
+  }
   if (option == CTQMC_OPT_TIMING) {
     if (value && !h->ev[0])
       for (int i = 0; i < 4; ++i) CU(cudaEventCreate(&h->ev[i]));
@@ -841,6 +852,18 @@ extern "C" int ctqmc_trace_batch(ctqmc_impurity* h, double beta, const ctqmc_bat
   if (rc) return rc;
   mark(h, 1, st);
   rc = h->grouped_now ? enqueue_grouped(h, bv, st) : h->large ? enqueue_large(h, bv, 0, 0, st) : enqueue_chain(h, bv, 0, 0, st);
+  if (rc == CTQMC_ERR_OOM && h->grouped_now && h->path == CTQMC_PATH_AUTO && !h->large) {
+    // the grouped path's schedule (one column map per chain position) did not fit: AUTO falls back to the persistent
+    // panel kernel, which needs no per-position scratch.  Routing is redone with panel-sized work units.
+    cudaGetLastError();
+    h->grouped_now = 0; h->last_path = CTQMC_PATH_PANEL; h->last_launches = 0;
+    const int Wp = 8 * h->nt;
+    rc = ensure_arena(h, B, (h->dev.dmax + Wp - 1) / Wp);
+    if (rc) return rc;
+    rc = enqueue_routing(h, bv, survive, 0, 0, st);
+    if (rc) return rc;
+    rc = enqueue_chain(h, bv, 0, 0, st);
+  }
   if (rc) return rc;
   mark(h, 2, st);
   TraceReduceParams tp;

@@ -364,3 +364,34 @@ def test_PB2_whole_chain_frobenius_matches_trace_matrix(impurities):
                 M = np.diag(np.exp(-deltas[k] * (view.E[vis[k + 1]] - e0))) @ view.F[(int(a), vis[k])] @ M
             ln = 0.5 * math.log(min(int(imp.dims[q]) for q in vis)) + math.log(np.linalg.norm(M)) - imp.beta * e0
             assert abs(O.to_log(*bd["sector"][q0]) - ln) < 1e-9 * max(1, abs(ln))
+
+
+def test_A8_config3_coarse_sectors_are_ill_conditioned_in_fp64(impurities):
+    """DESIGN.md reading A8 (ii), established with the oracle alone: configuration 45 of BASELINE config 3 is not determined by
+    fp64 in the N-only sector basis (its value moves by orders of magnitude under the exact cyclic shifts of pin P2), while
+    the same Hamiltonian in (N, 2S_z, L_z) sectors gives a value stable to 1e-10 -- the trace itself is basis independent
+    (pin P4 (iii)).  A well-conditioned neighbour (configuration 1) agrees between the two bases to 1e-10."""
+    coarse = impurities(3)
+    u = wi.spin_orbital_tensor(wi.slater_orbital_tensor(2, [6.0, 8.4, 5.3]))
+    u[np.abs(u) < 1e-14] = 0
+    h1 = -wi.symmetric_mu(u) * np.eye(10)
+    fineqn = [(1, -1, m) for m in range(-2, 3)] + [(1, 1, m) for m in range(-2, 3)]
+    fine = wi.build_impurity("d-fine", h1, u, fineqn, beta=coarse.beta, keep_eigvecs=False)
+    b = make_batch(3, 46)
+
+    def spread(imp, s, t, r):
+        out = 0.0
+        for frac in (0.23, 0.52, 0.77):
+            t2 = (t + frac * imp.beta) % imp.beta
+            o = np.argsort(t2, kind="stable")
+            r2 = O.trace_config(imp, imp.beta, s[o], t2[o])
+            out = max(out, rel_diff(r2["mant"], r2["exp2"], r["mant"], r["exp2"]))
+        return out
+
+    s, t = b.config(45)
+    rc, rf = O.trace_config(coarse, coarse.beta, s, t), O.trace_config(fine, fine.beta, s, t)
+    assert spread(fine, s, t, rf) < 1e-10
+    assert spread(coarse, s, t, rc) > 1e-3
+    s, t = b.config(1)
+    rc, rf = O.trace_config(coarse, coarse.beta, s, t), O.trace_config(fine, fine.beta, s, t)
+    assert rel_diff(rc["mant"], rc["exp2"], rf["mant"], rf["exp2"]) < 1e-10
