@@ -259,6 +259,13 @@ def _default_batch(cfg: int) -> int:
 def run_ours(args, rank: int, world: int, local_rank: int):
     import torch
 
+    from paper_2010_08482_b200 import build as _build
+    if rank == 0:
+        _build.build()   # no-op when the in-tree library is newer than its sources
+    else:
+        t_wait = time.time()
+        while _build.needs_build() and time.time() - t_wait < 300:
+            time.sleep(1.0)
     import paper_2010_08482_b200 as L
 
     assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
