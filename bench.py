@@ -223,6 +223,21 @@ def measure_config(L, torch, cfg, B, rank, steps, warmup, schedule, local_rank, 
             e2e_s += time.perf_counter() - t0
         barrier()
         e2e_ms = e2e_s * 1e3
+    # the lazy-trace bounds (a6) on the same batch: Frobenius, S = 1 (tables only) and S = 8 (segment products), device-resident
+    bound_ms = {}
+    if with_e2e:
+        for S in (1, 8):
+            for _ in range(2):
+                L.ctqmc_bound_batch(h, batch.beta, off, sym, tau, 0, S, want_sector=False)
+            torch.cuda.synchronize()
+            ea, eb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            reps = max(1, min(steps, 5))
+            ea.record(stream)
+            for _ in range(reps):
+                L.ctqmc_bound_batch(h, batch.beta, off, sym, tau, 0, S, want_sector=False, stream=stream)
+            eb.record(stream)
+            torch.cuda.synchronize()
+            bound_ms[f"S{S}"] = ea.elapsed_time(eb) / reps
     h.free()
     del flush, out, off, sym, tau
     torch.cuda.empty_cache()
@@ -248,7 +263,7 @@ def measure_config(L, torch, cfg, B, rank, steps, warmup, schedule, local_rank, 
     }
     return dict(imp=imp, batch=batch, stats=stats, total_ms=total_ms, e2e_ms=e2e_ms, n_ops=n_ops, Q=Q, roofline=roofline,
                 phases={"route": sum(route_ms) / len(route_ms), "chain": chain_avg_ms, "reduce": sum(reduce_ms) / len(reduce_ms)},
-                load_s=load_s)
+                load_s=load_s, bound_ms=bound_ms)
 
 
 def _default_batch(cfg: int) -> int:
@@ -326,6 +341,8 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         "roofline": m["roofline"],
         "phases_ms": m["phases"],
         "fp64_peak_measured": fp64,
+        "bound_batch": {"norm": "frobenius", "ms_per_batch": m["bound_ms"],
+                        "bounds_per_s": {k: B / (v * 1e-3) for k, v in m["bound_ms"].items()}},
         "lib": {"strings": stats["strings"], "units": stats["units"], "path": stats["path"], "panel_width_or_lanes": stats["panel_width"],
                 "team_warps": stats["team_warps"], "load_impurity_s": m["load_s"]},
     }
