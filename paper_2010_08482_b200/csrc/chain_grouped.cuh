@@ -6,7 +6,8 @@
 // wise and multiplied by F in one GEMM per block:   [X'_s1 | X'_s2 | ...] = F * [X_s1 | X_s2 | ...].
 // F is then read once per group instead of once per string, the N dimension is filled with real columns instead of the
 // 1..30 columns a single thin-start string carries, and the work is a dense contraction on the FP64 tensor cores
-// (mma.sync m8n8k4 f64, 64 x 64 CTA tiles, 4 warps of 32 x 32, cp.async pipeline of swizzled 128-byte rows).
+// (mma.sync m8n8k4 f64, 64 x 64 CTA tiles, 8 warps of 32 x 16 -- small warp tiles keep the kernel at 128 registers so that
+// 16 warps per SM hide the per-tile latencies --, cp.async pipeline of swizzled 128-byte rows).
 // The schedule (which string sits in which column of which tile at which chain position) is a pure function of the
 // routing result and is built once per call by three small kernels.
 //
@@ -24,7 +25,11 @@
 
 namespace ctqmc {
 
-constexpr int kGBM = 64, kGBN = 64, kGStages = 4, kGThreads = 128;
+#ifndef CTQMC_GROUPED_WN
+#define CTQMC_GROUPED_WN 4
+#endif
+// CTA tile 64 x 64; warps: 2 along M x kGWN along N; a warp owns 4 row blocks x kGNT column blocks of 8 x 8
+constexpr int kGBM = 64, kGBN = 64, kGStages = 4, kGWN = CTQMC_GROUPED_WN, kGNT = 8 / kGWN, kGThreads = 64 * kGWN;
 constexpr int kGStageBytes = (kGBM + kGBN) * 128;
 
 struct GroupedParams {
@@ -160,7 +165,7 @@ __global__ void grouped_init_kernel(GroupedParams P) {
 
 // One chain position for every string: blockIdx.x = (tile of the step's tile list, 64-row slab of F).
 template <bool CPLX>
-__global__ void __launch_bounds__(kGThreads, CPLX ? 2 : 3) grouped_step_kernel(GroupedParams P, int j, int MTmax) {
+__global__ void __launch_bounds__(kGThreads, (kGWN == 2 && !CPLX) ? 3 : 2) grouped_step_kernel(GroupedParams P, int j, int MTmax) {
   constexpr int ES = CPLX ? 2 : 1;
   constexpr int BKE = CPLX ? 8 : 16;
   extern __shared__ __align__(128) unsigned char gsm[];
@@ -180,12 +185,12 @@ __global__ void __launch_bounds__(kGThreads, CPLX ? 2 : 3) grouped_step_kernel(G
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int g = lane >> 2, t = lane & 3;
-  const int wm = warp >> 1, wn = warp & 1;
+  const int wm = warp / kGWN, wn = warp % kGWN;
   const int nkt = (d + BKE - 1) / BKE;
   // 8-row / 8-column blocks are dealt to the warps round-robin, and blocks that are all padding are skipped: the tensor
   // work is quantised to 8 x 8 although the CTA stages 64 x 64 tiles
   const int mtu = ((min(kGBM, dn - m0) + 7) / 8 - wm + 1) / 2;
-  const int ntu = ((ncols + 7) / 8 - wn + 1) / 2;
+  const int ntu = ((ncols + 7) / 8 - wn + kGWN - 1) / kGWN;
   const size_t par_in = (size_t)(j & 1) * P.xtot, par_out = (size_t)((j + 1) & 1) * P.xtot;
 
   if (tid < kGBN) {
@@ -225,14 +230,14 @@ __global__ void __launch_bounds__(kGThreads, CPLX ? 2 : 3) grouped_step_kernel(G
     unsigned char* As = gsm + stage * kGStageBytes;
     unsigned char* Bs = As + kGBM * 128;
 #pragma unroll
-    for (int i = 0; i < 4; ++i) {
+    for (int i = 0; i < kGBM * 8 / kGThreads; ++i) {
       const int idx = tid + i * kGThreads, r = idx >> 3, ch = idx & 7;
       const int row = m0 + r, gch = kt * 8 + ch;
       const bool ok = row < rows_pad && gch < ld_chunks;
       cp_async16(As + r * 128 + ((ch ^ ((r & 1) << 2)) << 4), ok ? Ag + (size_t)row * a_row_bytes + (size_t)gch * 16 : Ag, ok);
     }
 #pragma unroll
-    for (int i = 0; i < 4; ++i) {
+    for (int i = 0; i < kGBN * 8 / kGThreads; ++i) {
       const int idx = tid + i * kGThreads, r = idx >> 3, ch = idx & 7;
       const int gch = kt * 8 + ch;
       const unsigned char* src = s_xin[r];
@@ -241,19 +246,19 @@ __global__ void __launch_bounds__(kGThreads, CPLX ? 2 : 3) grouped_step_kernel(G
     }
   };
 
-  double acc[4][4][CPLX ? 4 : 2];
+  double acc[4][kGNT][CPLX ? 4 : 2];
 #pragma unroll
   for (int a = 0; a < 4; ++a)
 #pragma unroll
-    for (int b = 0; b < 4; ++b)
+    for (int b = 0; b < kGNT; ++b)
 #pragma unroll
       for (int x = 0; x < (CPLX ? 4 : 2); ++x) acc[a][b][x] = 0.0;
 
   // this lane's B-fragment columns: n = wn*32 + nt*8 + g
-  double ndp[4];
-  int kpv[4];
+  double ndp[kGNT];
+  int kpv[kGNT];
 #pragma unroll
-  for (int nt = 0; nt < 4; ++nt) { ndp[nt] = -s_dprev[(nt * 2 + wn) * 8 + g]; kpv[nt] = s_kprev[(nt * 2 + wn) * 8 + g]; }
+  for (int nt = 0; nt < kGNT; ++nt) { ndp[nt] = -s_dprev[(nt * kGWN + wn) * 8 + g]; kpv[nt] = s_kprev[(nt * kGWN + wn) * 8 + g]; }
 
   // the main loop is instantiated for every (row blocks, column blocks) count of a warp, so partial tiles issue only the
   // DMMAs they need and the loops stay fully unrolled
@@ -283,7 +288,7 @@ __global__ void __launch_bounds__(kGThreads, CPLX ? 2 : 3) grouped_step_kernel(G
   #pragma unroll
         for (int mt = 0; mt < MTU; ++mt) a[mt] = *reinterpret_cast<const double2*>(As + ((mt * 2 + wm) * 8 + g) * 128 + so);
   #pragma unroll
-        for (int nt = 0; nt < NTU; ++nt) b[nt] = *reinterpret_cast<const double2*>(Bs + ((nt * 2 + wn) * 8 + g) * 128 + so);
+        for (int nt = 0; nt < NTU; ++nt) b[nt] = *reinterpret_cast<const double2*>(Bs + ((nt * kGWN + wn) * 8 + g) * 128 + so);
         if constexpr (CPLX) {
           const double de = sde[kt * 8 + ch];
   #pragma unroll
@@ -336,8 +341,13 @@ __global__ void __launch_bounds__(kGThreads, CPLX ? 2 : 3) grouped_step_kernel(G
   };
 #define CTQMC_GD(M, N) case (M) * 8 + (N): mainloop(std::integral_constant<int, M>{}, std::integral_constant<int, N>{}); break;
   switch ((mtu > 0 && ntu > 0) ? mtu * 8 + ntu : 0) {
-    CTQMC_GD(1, 1) CTQMC_GD(1, 2) CTQMC_GD(1, 3) CTQMC_GD(1, 4) CTQMC_GD(2, 1) CTQMC_GD(2, 2) CTQMC_GD(2, 3) CTQMC_GD(2, 4)
-    CTQMC_GD(3, 1) CTQMC_GD(3, 2) CTQMC_GD(3, 3) CTQMC_GD(3, 4) CTQMC_GD(4, 1) CTQMC_GD(4, 2) CTQMC_GD(4, 3) CTQMC_GD(4, 4)
+    CTQMC_GD(1, 1) CTQMC_GD(2, 1) CTQMC_GD(3, 1) CTQMC_GD(4, 1)
+#if CTQMC_GROUPED_WN <= 4
+    CTQMC_GD(1, 2) CTQMC_GD(2, 2) CTQMC_GD(3, 2) CTQMC_GD(4, 2)
+#endif
+#if CTQMC_GROUPED_WN <= 2
+    CTQMC_GD(1, 3) CTQMC_GD(1, 4) CTQMC_GD(2, 3) CTQMC_GD(2, 4) CTQMC_GD(3, 3) CTQMC_GD(3, 4) CTQMC_GD(4, 3) CTQMC_GD(4, 4)
+#endif
     default: mainloop(std::integral_constant<int, 0>{}, std::integral_constant<int, 0>{}); break;
   }
 #undef CTQMC_GD
@@ -356,10 +366,10 @@ __global__ void __launch_bounds__(kGThreads, CPLX ? 2 : 3) grouped_step_kernel(G
   double mr[4];
   int kr[4];
 #pragma unroll
-  for (int nt = 0; nt < 4; ++nt) {
+  for (int nt = 0; nt < kGNT; ++nt) {
 #pragma unroll
     for (int half = 0; half < 2; ++half) {
-      const int n = (nt * 2 + wn) * 8 + 2 * t + half;
+      const int n = (nt * kGWN + wn) * 8 + 2 * t + half;
       const int u = s_u[n];
       if (u < 0) continue;
       if (u != cur_u) {   // columns of one string are adjacent: its row factors are computed once
