@@ -173,6 +173,7 @@ __global__ void __launch_bounds__(kGThreads, (kGWN == 2 && !CPLX) ? 3 : 2) group
   __shared__ double* s_xout[kGBN];
   __shared__ double s_dprev[kGBN], s_delta[kGBN];
   __shared__ int s_kprev[kGBN], s_u[kGBN], s_kmax[kGBN];
+  __shared__ __align__(8) unsigned long long g_full[kGStages], g_empty[kGStages];
   double* sde = reinterpret_cast<double*>(gsm + kGStages * kGStageBytes);   // E[k] - Emin of the source sector
 
   const int tile_id = blockIdx.x / MTmax, slab = blockIdx.x - tile_id * MTmax;   // slabs of a tile are neighbours in launch order
@@ -193,6 +194,11 @@ __global__ void __launch_bounds__(kGThreads, (kGWN == 2 && !CPLX) ? 3 : 2) group
   const int ntu = ((ncols + 7) / 8 - wn + kGWN - 1) / kGWN;
   const size_t par_in = (size_t)(j & 1) * P.xtot, par_out = (size_t)((j + 1) & 1) * P.xtot;
 
+  if (tid == 0) {
+#pragma unroll
+    for (int st = 0; st < kGStages; ++st) { mbar_init(&g_full[st], kGThreads); mbar_init(&g_empty[st], kGThreads / 32); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
   if (tid < kGBN) {
     const int n = tid;
     if (n < ncols) {
@@ -264,20 +270,24 @@ __global__ void __launch_bounds__(kGThreads, (kGWN == 2 && !CPLX) ? 3 : 2) group
   // DMMAs they need and the loops stay fully unrolled
   auto mainloop = [&](auto mtc, auto ntc) {
     constexpr int MTU = decltype(mtc)::value, NTU = decltype(ntc)::value;
+    // full/empty mbarrier ring (as in the large-sector kernel), fed by cp.async: a thread's copies of a stage arrive on the
+    // stage's "full" barrier when they land (cp.async.mbarrier.arrive.noinc), a warp releases a slot on its "empty" barrier;
+    // the slot consumed two k-tiles ago is refilled, so there is no CTA-wide barrier in the loop
+    constexpr int kAhead = kGStages - 2;
   #pragma unroll
-    for (int st = 0; st < kGStages - 1; ++st) {
-      if (st < nkt) load_stage(st, st);
-      cp_async_commit();
-    }
+    for (int st = 0; st < kAhead; ++st)
+      if (st < nkt) { load_stage(st, st); cp_async_arrive(&g_full[st]); }
     const int swz = (g & 1) << 2;
     for (int kt = 0; kt < nkt; ++kt) {
-      cp_async_wait<kGStages - 2>();
-      __syncthreads();
       {
-        const int nx = kt + kGStages - 1;
-        if (nx < nkt) load_stage(nx, nx % kGStages);
-        cp_async_commit();
+        const int nx = kt + kAhead;
+        if (nx < nkt) {
+          if (nx >= kGStages) mbar_wait(&g_empty[nx % kGStages], ((nx / kGStages) - 1) & 1);
+          load_stage(nx, nx % kGStages);
+          cp_async_arrive(&g_full[nx % kGStages]);
+        }
       }
+      mbar_wait(&g_full[kt % kGStages], (kt / kGStages) & 1);
       const unsigned char* As = gsm + (kt % kGStages) * kGStageBytes;
       const unsigned char* Bs = As + kGBM * 128;
   #pragma unroll
@@ -337,6 +347,8 @@ __global__ void __launch_bounds__(kGThreads, (kGWN == 2 && !CPLX) ? 3 : 2) group
               dmma884(acc[mt][nt][0], acc[mt][nt][1], a[mt].y, b[nt].y);
         }
       }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&g_empty[kt % kGStages]);
     }
   };
 #define CTQMC_GD(M, N) case (M) * 8 + (N): mainloop(std::integral_constant<int, M>{}, std::integral_constant<int, N>{}); break;
@@ -351,7 +363,6 @@ __global__ void __launch_bounds__(kGThreads, (kGWN == 2 && !CPLX) ? 3 : 2) group
     default: mainloop(std::integral_constant<int, 0>{}, std::integral_constant<int, 0>{}); break;
   }
 #undef CTQMC_GD
-  cp_async_wait<0>();
 
   // ---- epilogue: per (row, string) propagator mantissa, scatter to the strings' matrices, largest exponent per column
   const double* E = P.imp.energy + P.imp.e_off[bd.dst];
