@@ -132,6 +132,10 @@ int ctqmc_trace_batch(ctqmc_impurity* imp, double beta, const ctqmc_batch* batch
  *
  *   norm_kind 0 (Frobenius):  B(q0) = sqrt(d_min) * prod_j ||G_j||_F
  *   norm_kind 1 (spectral):   B(q0) = d_min * prod_i exp(-Delta_i Emin(q_i)) sigma_max(F_{alpha_i}(q_{i-1}))   (segment_len 1 only)
+ *                             sigma_max comes from a power iteration at load time, which approaches it from below: where the
+ *                             iteration has not converged to 1e-10 (it converges exactly for c / c^dag blocks, whose F^H F is a
+ *                             projector) the rigorous upper estimate min(||F||_F, sqrt(||F||_1 ||F||_inf)) is used instead, so the
+ *                             result is always an upper bound
  *
  * with d_min the smallest sector dimension along the string; the configuration's bound is sum_{q0} B(q0).  All values
  * are rounded outward by (1 + 2^-40), so bound >= |w_loc| holds for the returned numbers.

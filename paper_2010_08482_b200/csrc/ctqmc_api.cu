@@ -637,7 +637,8 @@ extern "C" int ctqmc_load_impurity(const ctqmc_impurity_desc* desc, int device, 
 
   int rc = 0;
   double* d_raw = nullptr; long long* d_rawoff = nullptr; long long* d_voff = nullptr; double* d_v = nullptr; double* d_u = nullptr;
-  auto cleanup_tmp = [&]() { cudaFree(d_raw); cudaFree(d_rawoff); cudaFree(d_voff); cudaFree(d_v); cudaFree(d_u); };
+  double* d_w = nullptr; int* d_need = nullptr;
+  auto cleanup_tmp = [&]() { cudaFree(d_raw); cudaFree(d_rawoff); cudaFree(d_voff); cudaFree(d_v); cudaFree(d_u); cudaFree(d_w); cudaFree(d_need); };
 #define TRY(x) do { rc = (x); if (rc) { cleanup_tmp(); ctqmc_free_impurity(h); return rc; } } while (0)
 #define TRYCU(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) { rc = fail(e_ == cudaErrorMemoryAllocation ? CTQMC_ERR_OOM : CTQMC_ERR_CUDA, "%s: %s", #x, cudaGetErrorString(e_)); cleanup_tmp(); ctqmc_free_impurity(h); return rc; } } while (0)
   TRY(upload(&h->d_dim, dim));
@@ -676,6 +677,8 @@ extern "C" int ctqmc_load_impurity(const ctqmc_impurity_desc* desc, int device, 
     TRYCU(cudaMemcpy(d_raw, desc->blk_data, (size_t)raw_len * es * sizeof(double), cudaMemcpyHostToDevice));
     TRYCU(cudaMalloc((void**)&d_v, (size_t)v_len * es * sizeof(double)));
     TRYCU(cudaMalloc((void**)&d_u, (size_t)rn_len * es * sizeof(double)));
+    TRYCU(cudaMalloc((void**)&d_w, (size_t)v_len * es * sizeof(double)));
+    TRYCU(cudaMalloc((void**)&d_need, (size_t)nb * sizeof(int)));
     dim3 tb(32, 8), tg((unsigned)std::min((max_cols + 31) / 32, 64), (unsigned)std::min((max_rows + 31) / 32, 64), (unsigned)nb);
     dim3 rg((unsigned)std::min((max_rows + 7) / 8, 512), (unsigned)nb);
     dim3 cg((unsigned)std::min((max_cols + 127) / 128, 64), (unsigned)nb);
@@ -692,6 +695,9 @@ extern "C" int ctqmc_load_impurity(const ctqmc_impurity_desc* desc, int device, 
       }
       pi_fv_kernel<2><<<rg, 256>>>(h->d_blks, h->d_store, d_voff, d_v, d_u);
       pi_norm_kernel<<<nb, 256>>>(h->d_blks, d_voff, 1, 2, d_u, 0, h->d_sigma);
+      pi_fhu_kernel<2><<<cg, 128>>>(h->d_blks, h->d_store, d_voff, d_u, d_w);
+      sigma_check_kernel<2><<<nb, 256>>>(h->d_blks, d_voff, d_v, d_w, h->d_sigma, d_need);
+      sigma_upper_kernel<2><<<nb, 256>>>(h->d_blks, h->d_store, h->d_rownorm2, d_need, h->d_sigma);
     } else {
       relayout_kernel<1><<<tg, tb>>>(d_raw, d_rawoff, h->d_blks, h->d_store);
       rownorm_kernel<1><<<rg, 256>>>(h->d_blks, h->d_store, h->d_rownorm2);
@@ -704,12 +710,15 @@ extern "C" int ctqmc_load_impurity(const ctqmc_impurity_desc* desc, int device, 
       }
       pi_fv_kernel<1><<<rg, 256>>>(h->d_blks, h->d_store, d_voff, d_v, d_u);
       pi_norm_kernel<<<nb, 256>>>(h->d_blks, d_voff, 1, 1, d_u, 0, h->d_sigma);
+      pi_fhu_kernel<1><<<cg, 128>>>(h->d_blks, h->d_store, d_voff, d_u, d_w);
+      sigma_check_kernel<1><<<nb, 256>>>(h->d_blks, d_voff, d_v, d_w, h->d_sigma, d_need);
+      sigma_upper_kernel<1><<<nb, 256>>>(h->d_blks, h->d_store, h->d_rownorm2, d_need, h->d_sigma);
     }
     TRYCU(cudaGetLastError());
     TRYCU(cudaDeviceSynchronize());
   }
   cleanup_tmp();
-  d_raw = nullptr; d_rawoff = nullptr; d_voff = nullptr; d_v = nullptr; d_u = nullptr;
+  d_raw = nullptr; d_rawoff = nullptr; d_voff = nullptr; d_v = nullptr; d_u = nullptr; d_w = nullptr; d_need = nullptr;
 
   h->dev.Q = Q; h->dev.A = A; h->dev.cplx = cplx; h->dev.dmax = dmax;
   h->dev.dim = h->d_dim; h->dev.e_off = h->d_eoff; h->dev.energy = h->d_energy; h->dev.e_min = h->d_emin;

@@ -121,3 +121,70 @@ __global__ void pi_norm_kernel(const BlkDesc* __restrict__ blks, const long long
 }
 
 }  // namespace ctqmc
+
+namespace ctqmc {
+
+// Spectral-norm guard (reading A1).  Power iteration approaches sigma_max from BELOW; a bound built from an
+// under-estimate would not be a bound.  With v the normalised iterate, u = F v, sigma = ||u|| and w = F^H u, the iteration has
+// converged iff w = sigma^2 v.  One CTA per block: need[b] = 1 unless ||w - sigma^2 v|| <= 1e-10 sigma^2 (c / c^dag blocks
+// converge exactly after one step: F^H F is a projector, pin P10).
+template <int ES>
+__global__ void sigma_check_kernel(const BlkDesc* __restrict__ blks, const long long* __restrict__ v_off,
+                                   const double* __restrict__ v, const double* __restrict__ w,
+                                   const double* __restrict__ sigma, int* __restrict__ need) {
+  __shared__ double red[8];
+  const BlkDesc bd = blks[blockIdx.x];
+  const double s2 = sigma[blockIdx.x] * sigma[blockIdx.x];
+  const double* vb = v + v_off[blockIdx.x] * ES;
+  const double* wb = w + v_off[blockIdx.x] * ES;
+  double r2 = 0.0;
+  for (int i = threadIdx.x; i < bd.cols * ES; i += blockDim.x) { const double d = wb[i] - s2 * vb[i]; r2 += d * d; }
+  r2 = warp_sum(r2);
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = r2;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double t = 0.0;
+    for (int i = 0; i < (int)(blockDim.x >> 5); ++i) t += red[i];
+    need[blockIdx.x] = (s2 > 0.0 && !(sqrt(t) <= 1e-10 * s2)) ? 1 : 0;
+  }
+}
+
+// For blocks whose iteration has not converged: sigma <- max(sigma, min(||F||_F, sqrt(||F||_1 ||F||_inf))), a rigorous upper
+// bound of the spectral norm.  One CTA per block; converged blocks return at once.
+template <int ES>
+__global__ void sigma_upper_kernel(const BlkDesc* __restrict__ blks, const double* __restrict__ store,
+                                   const double* __restrict__ rownorm2, const int* __restrict__ need, double* __restrict__ sigma) {
+  __shared__ double red[3][8];
+  if (!need[blockIdx.x]) return;
+  const BlkDesc bd = blks[blockIdx.x];
+  const double* F = store + bd.off;
+  double fro2 = 0.0, ninf = 0.0, n1 = 0.0;
+  for (int m = threadIdx.x; m < bd.rows; m += blockDim.x) {
+    fro2 += rownorm2[bd.rn_off + m];
+    double s = 0.0;
+    for (int k = 0; k < bd.cols; ++k) {
+      const double* e = F + ((size_t)m * bd.ld + k) * ES;
+      s += (ES == 1) ? fabs(e[0]) : hypot(e[0], e[ES - 1]);
+    }
+    ninf = fmax(ninf, s);
+  }
+  for (int k = threadIdx.x; k < bd.cols; k += blockDim.x) {
+    double s = 0.0;
+    for (int m = 0; m < bd.rows; ++m) {
+      const double* e = F + ((size_t)m * bd.ld + k) * ES;
+      s += (ES == 1) ? fabs(e[0]) : hypot(e[0], e[ES - 1]);
+    }
+    n1 = fmax(n1, s);
+  }
+  fro2 = warp_sum(fro2); ninf = warp_max(ninf); n1 = warp_max(n1);
+  if ((threadIdx.x & 31) == 0) { red[0][threadIdx.x >> 5] = fro2; red[1][threadIdx.x >> 5] = ninf; red[2][threadIdx.x >> 5] = n1; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double a = 0.0, b = 0.0, c = 0.0;
+    for (int i = 0; i < (int)(blockDim.x >> 5); ++i) { a += red[0][i]; b = fmax(b, red[1][i]); c = fmax(c, red[2][i]); }
+    const double upper = fmin(sqrt(a), sqrt(b * c)) * (1.0 + 1e-12);
+    sigma[blockIdx.x] = fmax(sigma[blockIdx.x], upper);
+  }
+}
+
+}  // namespace ctqmc
