@@ -17,6 +17,7 @@
 #include "chain_large.cuh"
 #include "chain_small.cuh"
 #include "chain_small2.cuh"
+#include "bound_small2.cuh"
 #include "common.cuh"
 #include "peak.cuh"
 #include "reduce.cuh"
@@ -178,6 +179,14 @@ Small2Fn pick_small2(int dp) {
   switch (dp) {
     case 2: return small2_trace_kernel<2>;   case 4: return small2_trace_kernel<4>;   case 6: return small2_trace_kernel<6>;
     case 9: return small2_trace_kernel<9>;   case 12: return small2_trace_kernel<12>; case 16: return small2_trace_kernel<16>;
+  }
+  return nullptr;
+}
+using Small2BoundFn = void (*)(Small2BoundParams);
+Small2BoundFn pick_small2_bound(int dp) {
+  switch (dp) {
+    case 2: return small2_bound_kernel<2>;   case 4: return small2_bound_kernel<4>;   case 6: return small2_bound_kernel<6>;
+    case 9: return small2_bound_kernel<9>;   case 12: return small2_bound_kernel<12>; case 16: return small2_bound_kernel<16>;
   }
   return nullptr;
 }
@@ -908,6 +917,33 @@ extern "C" int ctqmc_bound_batch(ctqmc_impurity* h, double beta, const ctqmc_bat
   h->timing_valid = 0;
   h->grouped_now = 0; h->last_path = h->large ? CTQMC_PATH_LARGE : CTQMC_PATH_PANEL;
   BoundParams bp;
+  if (segment_len == 1 && h->small2) {
+    // small real impurities: validation, routing, norm products and the sector sum in one launch (bound_small2.cuh)
+    const int dp = h->small2_dp, gpw = 32 / dp;
+    long long per_sm = (B + h->sm_count - 1) / h->sm_count;
+    int warps = (int)((per_sm + gpw - 1) / gpw);
+    if (warps < 2) warps = 2;
+    if (warps > 16) warps = 16;
+    const long long gpc = (long long)warps * gpw;
+    const size_t smem = small2b_common_bytes(h->dev.Q, h->dev.A, h->n_blocks, dp) + (size_t)gpc * small2b_group_bytes(h->dev.Q, dp);
+    Small2BoundFn fn = pick_small2_bound(dp);
+    if (fn && smem <= 227 * 1024 - 2048) {
+      CU(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+      Small2BoundParams sb;
+      sb.imp = h->dev; sb.bv = bv; sb.binfo = h->d_binfo; sb.n_blocks = h->n_blocks; sb.norm_kind = norm_kind;
+      sb.bound_mant = bound_mant; sb.bound_exp2 = (long long*)bound_exp2; sb.sector_mant = sector_bound_mant;
+      sb.sector_exp2 = (long long*)sector_bound_exp2; sb.status = status;
+      long long grid = (B + gpc - 1) / gpc;
+      if (grid > 8LL * h->sm_count) grid = 8LL * h->sm_count;
+      mark(h, 0, st); mark(h, 1, st);
+      fn<<<(unsigned)grid, 32 * warps, smem, st>>>(sb);
+      h->last_launches += 1; h->last_path = CTQMC_PATH_SMALL;
+      mark(h, 2, st); mark(h, 3, st);
+      h->timing_valid = h->timing;
+      CU(cudaGetLastError());
+      return 0;
+    }
+  }
   if (segment_len == 1) {
     rc = ensure_arena(h, B, 1);
     if (rc) return rc;
