@@ -310,14 +310,17 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     others = {}
     if args.others and world == 1:
         # the other BASELINE.json configs at their stated batch, device-resident timing only (fewer steps: they are context)
-        for c in (1, 3, 4, 5):
-            if c == cfg:
+        # plus the default small-sector config at a scaled batch (same generator, 64 x BASELINE's 4096): at the stated batch
+        # that launch lasts as long as ONE configuration's dependency chain, whatever the kernel
+        for c, bsz, key in ((1, 0, "cfg1"), (2, 262144, "cfg2_scaled_batch"), (3, 0, "cfg3"), (4, 0, "cfg4"), (5, 0, "cfg5")):
+            if c == cfg and not bsz:
                 continue
+            bsz = bsz or _default_batch(c)
             k = 1 if c == 5 else 3
-            o = measure_config(L, torch, c, _default_batch(c), 0, k, 3 if c != 5 else 1, "thin", local_rank, barrier, fp64, pk,
+            o = measure_config(L, torch, c, bsz, 0, k, 3 if c != 5 else 1, "thin", local_rank, barrier, fp64, pk,
                                with_e2e=False)
-            others[f"cfg{c}"] = {"workload": WORKLOADS[c], "batch": _default_batch(c), "steps": k,
-                                 "value": aggregate_value(1, _default_batch(c), k, o["total_ms"]), "unit": UNIT,
+            others[key] = {"workload": WORKLOADS[c], "batch": bsz, "steps": k,
+                                 "value": aggregate_value(1, bsz, k, o["total_ms"]), "unit": UNIT,
                                  "ms_per_step": o["total_ms"] / k, "gflops": o["stats"]["alg_flops"] * k / (o["total_ms"] * 1e-3) / 1e9,
                                  "roofline": {x: o["roofline"][x] for x in ("bound", "kernel", "achieved", "peak", "unit", "frac",
                                                                             "frac_of_rule_peak", "kernel_ms", "kernel_share_of_step")}}
