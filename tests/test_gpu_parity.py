@@ -200,6 +200,53 @@ def test_small_path_first_variant_on_real_impurities(cfg, n, lib, torch_cuda, im
         h.free()
 
 
+@pytest.mark.parametrize("dims", [(2, 1), (6, 5), (12, 7), (16, 12)])
+def test_small_path_every_padded_size(dims, lib, torch_cuda):
+    """The uniform small-sector kernels are instantiated for DP = 2, 4, 6, 9, 12, 16 lanes per configuration; BASELINE's
+    impurities only reach 4 and 9.  Hand-built two-sector impurities with seeded random blocks (0 -> 1, 1 -> 0, 0 -> 0) and
+    random closed walks cover the rest, traces and S = 1 bounds against the oracle."""
+    import types
+    from workloads import Batch
+    from workloads.rng import Stream
+    rng = Stream(100 * dims[0] + dims[1])
+    d0, d1 = dims
+    blocks = [(0, 0, 1), (1, 1, 0), (2, 0, 0)]          # (symbol, src, dst)
+    data, off, pos = [], [], 0
+    for _, s_, d_ in blocks:
+        m, n = (d0, d1)[d_], (d0, d1)[s_]
+        data.append(np.array([rng.normal() for _ in range(m * n)]) * (0.9 / np.sqrt(max(m, n))))
+        off.append(pos); pos += m * n
+    energy = np.array([0.3 * rng.normal() for _ in range(d0 + d1)])
+    beta = 3.0
+    imp = types.SimpleNamespace(dims=np.array([d0, d1], np.int32), energy=energy, n_symbols=3, is_complex=False, n_sectors=2,
+                                beta=beta, blk_symbol=np.array([b[0] for b in blocks], np.int32),
+                                blk_src=np.array([b[1] for b in blocks], np.int32), blk_dst=np.array([b[2] for b in blocks], np.int32),
+                                blk_offset=np.array(off, np.int64), blk_data=np.concatenate(data))
+    cfgs = []
+    for _ in range(40):
+        q, syms = 0, []
+        for _ in range(2 + rng.integer(30)):             # random walk on the two sectors, closed at the end
+            a = (rng.integer(2) * 2) if q == 0 else 1     # from 0: symbol 0 (to 1) or 2 (stay); from 1: symbol 1 (back)
+            syms.append(a)
+            q = 1 if a == 0 else 0
+        if q == 1:
+            syms.append(1)
+        taus = np.sort(beta * rng.uniforms(len(syms)))
+        cfgs.append((syms, taus))
+    cfgs += [([], []), ([1, 0], [0.5, 1.0]), ([0, 0], [0.5, 1.0])]   # empty; closes from sector 1 only; hits the zero sector
+    batch = Batch.from_lists(beta, cfgs)
+    h = lib.ctqmc_load_impurity(imp, 0)
+    try:
+        for sched in (lib.CTQMC_SCHEDULE_THIN, lib.CTQMC_SCHEDULE_LITERAL):
+            lib.ctqmc_set_option(h, lib.CTQMC_OPT_SCHEDULE, sched)
+            _check_trace(lib, torch_cuda, imp, h, batch, f"pad{dims}")
+            st = lib.ctqmc_last_stats(h)
+            assert st["path"] == lib.CTQMC_PATH_SMALL and st["panel_width"] >= max(dims)
+        _check_bound(lib, torch_cuda, imp, h, batch, 0, 1, f"pad{dims}-frobenius")
+    finally:
+        h.free()
+
+
 @pytest.mark.parametrize("lanes", [8, 16, 32])
 def test_small_path_complex_and_group_sizes(lanes, lib, torch_cuda, monkeypatch):
     """Small path with complex blocks (config 1 with seeded eigenvector phases, reading A17) and every lanes-per-
