@@ -13,6 +13,9 @@
  * Everything on the path runs in sm_100a CUDA kernels; there is no CPU fallback.  All functions return 0 on success or
  * a negative CTQMC_ERR_* code; on error nothing has been written to the outputs.  `ctqmc_last_error()` gives the text.
  *
+ * Concurrency: a handle owns one scratch arena, so batch calls on the SAME handle must be issued one after the other (they may
+ * be on different streams as long as the second is enqueued after the first has completed); different handles are independent.
+ *
  * Pointer conventions are stated per argument: HOST = ordinary host memory, DEVICE = device memory of the GPU the
  * impurity was loaded on (e.g. a torch tensor's data_ptr()).
  */
