@@ -32,6 +32,10 @@ namespace ctqmc {
 constexpr int kGBM = 64, kGBN = 64, kGStages = 4, kGWN = CTQMC_GROUPED_WN, kGNT = 8 / kGWN, kGThreads = 64 * kGWN;
 constexpr int kGStageBytes = (kGBM + kGBN) * 128;
 
+// 2^(e - 1023) for a biased exponent e, built on the integer pipe: e <= 0 gives exactly 0.0 (the row is more than 2^1022
+// below the string's largest), e is capped at 2045 (= 2^1022).  Same values as `sh < -1022 ? 0 : pow2i(min(sh, 1022))`.
+__device__ __forceinline__ double pow2_biased(int e) { return __hiloint2double(min(max(e, 0), 2045) << 20, 0); }
+
 struct GroupedParams {
   DevImp imp;
   BatchView bv;
@@ -264,7 +268,7 @@ __global__ void __launch_bounds__(kGThreads, (kGWN == 2 && !CPLX) ? 3 : 2) group
   double ndp[kGNT];
   int kpv[kGNT];
 #pragma unroll
-  for (int nt = 0; nt < kGNT; ++nt) { ndp[nt] = -s_dprev[(nt * kGWN + wn) * 8 + g]; kpv[nt] = s_kprev[(nt * kGWN + wn) * 8 + g]; }
+  for (int nt = 0; nt < kGNT; ++nt) { ndp[nt] = -s_dprev[(nt * kGWN + wn) * 8 + g]; kpv[nt] = s_kprev[(nt * kGWN + wn) * 8 + g] - 1023; }   // biased
 
   // the main loop is instantiated for every (row blocks, column blocks) count of a warp, so partial tiles issue only the
   // DMMAs they need and the loops stay fully unrolled
@@ -303,9 +307,7 @@ __global__ void __launch_bounds__(kGThreads, (kGWN == 2 && !CPLX) ? 3 : 2) group
           const double de = sde[kt * 8 + ch];
   #pragma unroll
           for (int nt = 0; nt < NTU; ++nt) {
-            const double x = __dmul_rn(__dmul_rn(ndp[nt], de), kLog2e);
-            const int sh = row_exp(x) - kpv[nt];
-            const double f = (sh < -1022) ? 0.0 : pow2i(min(sh, 1022));
+            const double f = pow2_biased(__double2int_rd(__dmul_rn(__dmul_rn(ndp[nt], de), kLog2e)) - kpv[nt]);
             b[nt].x *= f; b[nt].y *= f;
           }
   #pragma unroll
@@ -330,10 +332,8 @@ __global__ void __launch_bounds__(kGThreads, (kGWN == 2 && !CPLX) ? 3 : 2) group
           const double2 de = *reinterpret_cast<const double2*>(sde + kt * 16 + ch * 2);
   #pragma unroll
           for (int nt = 0; nt < NTU; ++nt) {
-            const double x0 = __dmul_rn(__dmul_rn(ndp[nt], de.x), kLog2e), x1 = __dmul_rn(__dmul_rn(ndp[nt], de.y), kLog2e);
-            const int sh0 = row_exp(x0) - kpv[nt], sh1 = row_exp(x1) - kpv[nt];
-            b[nt].x *= (sh0 < -1022) ? 0.0 : pow2i(min(sh0, 1022));
-            b[nt].y *= (sh1 < -1022) ? 0.0 : pow2i(min(sh1, 1022));
+            b[nt].x *= pow2_biased(__double2int_rd(__dmul_rn(__dmul_rn(ndp[nt], de.x), kLog2e)) - kpv[nt]);
+            b[nt].y *= pow2_biased(__double2int_rd(__dmul_rn(__dmul_rn(ndp[nt], de.y), kLog2e)) - kpv[nt]);
           }
   #pragma unroll
           for (int mt = 0; mt < MTU; ++mt)
