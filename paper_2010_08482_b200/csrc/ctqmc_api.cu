@@ -404,7 +404,7 @@ int enqueue_grouped(ctqmc_impurity* h, const BatchView& bv, cudaStream_t st) {
   CU(cudaStreamSynchronize(st));
   const long long n_units = (long long)c.n_slots;
   if (n_units == 0) return 0;
-  if (n_units > 2000000000LL / ((long long)c.max_len + 1)) return fail(CTQMC_ERR_UNSUPPORTED, "batch too large for the grouped path");
+  if (n_units > 2000000000LL / ((long long)c.max_len + 1)) return fail(CTQMC_ERR_OOM, "batch too large for the grouped path's per-position schedule");   // AUTO falls back to the panel kernel
   const int Lmax = (int)c.max_len > 0 ? (int)c.max_len : 1;
   const long long sum_c = (long long)c.sum_c > 0 ? (long long)c.sum_c : 1;
   const int es = h->dev.cplx ? 2 : 1, nb = h->n_blocks;
