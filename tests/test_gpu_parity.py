@@ -71,7 +71,7 @@ def _oracle_self_spread(imp, beta, s, t, r):
     return spread
 
 
-def _check_trace(lib, torch, imp, handle, batch, label):
+def _check_trace(lib, torch, imp, handle, batch, label, sample=None):
     from oracle import trace_oracle as O
     off, sym, tau = _dev(torch, batch)
     mant, exp2, surv, status = lib.ctqmc_trace_batch(handle, batch.beta, off, sym, tau)
@@ -79,7 +79,8 @@ def _check_trace(lib, torch, imp, handle, batch, label):
     mant, exp2, surv, status = mant.cpu().numpy(), exp2.cpu().numpy(), surv.cpu().numpy(), status.cpu().numpy()
     worst = 0.0
     loosened = 0
-    for b in range(batch.n_configs):
+    checked = range(batch.n_configs) if sample is None else sample   # the GPU ran the whole batch; the oracle checks these
+    for b in checked:
         s, t = batch.config(b)
         r = O.trace_config(imp, batch.beta, s, t)
         assert status[b] == r["status"], f"{label} config {b}: status {status[b]} != oracle {r['status']}"
@@ -103,8 +104,10 @@ def _check_trace(lib, torch, imp, handle, batch, label):
         if tol > TOL:
             loosened += 1
         assert d <= tol, f"{label} config {b}: rel diff {d:.3e} > {tol:.1e} (kappa {r['kappa']:.2e})"
-        worst = max(worst, d)
-    allowed = max(1, batch.n_configs // 4) if label.startswith("cfg3") else max(1, batch.n_configs // 100)
+        if tol == TOL:
+            worst = max(worst, d)          # worst difference among the configurations held to 1e-9
+    n_checked = len(checked)
+    allowed = max(1, n_checked // 4) if label.startswith("cfg3") else max(1, n_checked // 100)
     assert loosened <= allowed, f"{label}: {loosened} configurations needed the A8 loosening"
     return worst
 
@@ -116,6 +119,18 @@ def test_trace_parity_baseline_configs(cfg, n, lib, torch_cuda, impurities, hand
     batch = make_batch(cfg, n)
     worst = _check_trace(lib, torch_cuda, impurities(cfg), handles(cfg), batch, f"cfg{cfg}")
     print(f"cfg{cfg}: worst relative difference {worst:.3e}")
+
+
+@pytest.mark.parametrize("cfg,n_sample", [(1, 1024), (2, 4096), (3, 48), (4, 12)])
+def test_trace_parity_full_baseline_batch_sampled(cfg, n_sample, lib, torch_cuda, impurities, handles):
+    """BASELINE.json's full batch in the launch configuration bench.py times (configs 1-2: every output; 3-4: evenly spaced
+    samples the oracle can afford; config 5: see test_trace_parity_cfg5_crystal_field)."""
+    from workloads import BASELINE_CONFIGS, make_batch
+    B = BASELINE_CONFIGS[cfg]["batch"]
+    batch = make_batch(cfg, B)
+    sample = list(range(B)) if n_sample >= B else [int(i * B / n_sample) for i in range(n_sample)]
+    worst = _check_trace(lib, torch_cuda, impurities(cfg), handles(cfg), batch, f"cfg{cfg}-full", sample=sample)
+    print(f"cfg{cfg} full batch {B}, {len(sample)} outputs checked: worst relative difference {worst:.3e}")
 
 
 @pytest.mark.parametrize("cfg,n", [(1, 64), (2, 64), (3, 6), (4, 2)])
@@ -409,7 +424,7 @@ def test_trace_parity_cfg5_crystal_field(lib, torch_cuda, impurities):
     h = lib.ctqmc_load_impurity(imp, 0)
     try:
         assert lib.ctqmc_last_stats(h)["path"] == lib.CTQMC_PATH_LARGE
-        worst = _check_trace(lib, torch_cuda, imp, h, make_batch(5, 1), "cfg5")
+        worst = _check_trace(lib, torch_cuda, imp, h, make_batch(5, 64), "cfg5", sample=[0])   # full BASELINE batch on the GPU
         print(f"cfg5: worst relative difference {worst:.3e}")
         _check_bound(lib, torch_cuda, imp, h, make_batch(5, 1), 0, 1, "cfg5-frobenius-S1")
     finally:
