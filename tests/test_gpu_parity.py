@@ -516,6 +516,36 @@ def test_long_chain_exponent_range(lib, torch_cuda, impurities, handles):
     _check_trace(lib, torch_cuda, imp, handles(2), batch, "long")
 
 
+@pytest.mark.parametrize("path", ["panel", "grouped", "large"])
+def test_long_and_single_configuration_mid_size_paths(path, lib, torch_cuda, impurities, handles):
+    """Chains of ~600 operators at beta = 200 on the d-shell impurity (running exponents of several 1e4 binary orders) and
+    a batch of ONE configuration, through the panel, grouped and large-sector kernel families."""
+    from workloads import Batch, make_batch
+    from workloads.rng import Stream
+    imp = impurities(3)
+    h = handles(3)
+    rng = Stream(991)
+    beta = 200.0
+    cfgs = []
+    for _ in range(3):
+        ops = []
+        for f in range(10):
+            t = np.sort(beta * rng.uniforms(60))
+            first = rng.integer(2)
+            ops += [(t[i], 2 * f + ((first + i) & 1)) for i in range(len(t))]
+        ops.sort()
+        cfgs.append(([a for _, a in ops], [t for t, _ in ops]))
+    long_batch = Batch.from_lists(beta, cfgs)
+    one = make_batch(3, 1, start=19000)
+    lib.ctqmc_set_option(h, lib.CTQMC_OPT_PATH, {"panel": lib.CTQMC_PATH_PANEL, "grouped": lib.CTQMC_PATH_GROUPED,
+                                                 "large": lib.CTQMC_PATH_LARGE}[path])
+    try:
+        _check_trace(lib, torch_cuda, imp, h, long_batch, f"cfg3-long-{path}")
+        _check_trace(lib, torch_cuda, imp, h, one, f"cfg3-one-{path}")
+    finally:
+        lib.ctqmc_set_option(h, lib.CTQMC_OPT_PATH, lib.CTQMC_PATH_AUTO)
+
+
 def test_host_form_matches_device_form(lib, torch_cuda, impurities, handles):
     from workloads import make_batch
     for cfg, n in ((1, 200), (3, 5)):
