@@ -56,7 +56,8 @@ extern "C" {
  * step-synchronous grouped GEMM kernel for batches of 32 configurations or more and the persistent shared-memory panel
  * kernel for smaller ones; else the large-sector tiled GEMM kernel (one launch per chain position).  The grouped and the large path read the
  * routing counters back from the device before enqueueing their step loop, so those calls are not fully asynchronous.
- * ctqmc_bound_batch always uses the panel kernel family (or tables only, for segment_len 1). */
+ * ctqmc_bound_batch: segment_len 1 uses tables only (one fused launch for small real impurities); other segment lengths run
+ * the panel kernel family, or the large-sector one when the sectors do not fit in shared memory. */
 #define CTQMC_PATH_AUTO        0
 #define CTQMC_PATH_PANEL       1
 #define CTQMC_PATH_LARGE       2
