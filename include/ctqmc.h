@@ -53,7 +53,7 @@ extern "C" {
 
 /* Kernel families for CTQMC_OPT_PATH.  AUTO: the small-sector kernel (whole path in one launch, operator store in shared
  * memory) when every sector has at most 16 states; else, when a panel of the largest sector fits in shared memory, the
- * step-synchronous grouped GEMM kernel for batches of 32 configurations or more and the persistent shared-memory panel
+ * step-synchronous grouped GEMM kernel for batches of 64 configurations or more and the persistent shared-memory panel
  * kernel for smaller ones; else the large-sector tiled GEMM kernel (one launch per chain position).  The grouped and the large path read the
  * routing counters back from the device before enqueueing their step loop, so those calls are not fully asynchronous.
  * ctqmc_bound_batch: segment_len 1 uses tables only (one fused launch for small real impurities); other segment lengths run

@@ -337,12 +337,12 @@ def test_trace_parity_grouped_path(cfg, n, schedule, lib, torch_cuda, impurities
 
 
 def test_auto_path_by_batch_size(lib, torch_cuda, impurities, handles):
-    """AUTO: batches of >= 32 configurations of a mid-size impurity take the grouped path, smaller ones the panel kernel;
+    """AUTO: batches of >= 64 configurations of a mid-size impurity take the grouped path, smaller ones the panel kernel;
     both agree with the oracle (checked on the larger batch here, on the smaller ones by the baseline-config tests)."""
     from workloads import make_batch
     h = handles(3)
-    batch = make_batch(3, 40, start=15000)
-    _check_trace(lib, torch_cuda, impurities(3), h, batch, "cfg3-auto-40")
+    batch = make_batch(3, 72, start=15000)
+    _check_trace(lib, torch_cuda, impurities(3), h, batch, "cfg3-auto-72")
     assert lib.ctqmc_last_stats(h)["path"] == lib.CTQMC_PATH_GROUPED
     off, sym, tau = _dev(torch_cuda, make_batch(3, 8, start=15000))
     lib.ctqmc_trace_batch(h, batch.beta, off, sym, tau)
@@ -354,7 +354,7 @@ def test_grouped_scratch_limit_falls_back_to_panel(lib, torch_cuda, impurities, 
     request for the grouped path reports CTQMC_ERR_OOM."""
     from workloads import make_batch
     h = handles(3)
-    batch = make_batch(3, 40, start=17000)
+    batch = make_batch(3, 72, start=17000)
     lib.ctqmc_set_option(h, lib.CTQMC_OPT_SCRATCH_LIMIT, 1 << 20)
     try:
         _check_trace(lib, torch_cuda, impurities(3), h, batch, "cfg3-auto-limited")
