@@ -27,6 +27,7 @@ METRIC = "local_trace_evaluations_per_s"
 UNIT = "traces/s"
 NOMINAL_FP64_TFLOPS = 40.0     # B200 FP64 nominal (vendor figure); DESIGN.md §7
 NOMINAL_BF16_TFLOPS = 2250.0   # B200_PROFILING.md
+EXP_FLOP_EQUIV = 25            # FP64 exp at its instruction cost (~12 DFMA + range reduction)
 FALLBACK_HBM_GBS, FALLBACK_BF16_TFLOPS = 6650.0, 1590.0
 WORKLOADS = {
     1: "cfg1: 2-orbital Kanamori (Q=9, d_max=4), L=40",
@@ -245,7 +246,11 @@ def measure_config(L, torch, cfg, B, rank, steps, warmup, schedule, local_rank, 
     n_ops = int(batch.offset[-1])
     kname, bound = KERNELS[stats["path"]]
     chain_avg_ms = sum(chain_ms) / len(chain_ms)
-    achieved_tf = stats["alg_flops"] / (chain_avg_ms * 1e-3) / 1e12
+    # small (alu-bound) path: the algorithmic work also holds one FP64 exp per row and chain step; SURVEY 8(d) D3 counts it at
+    # its instruction cost (~25 flop-equivalents), not as one flop
+    n_exp = stats["team_warps"] if stats["path"] == 3 else 0
+    alg_flop_equiv = stats["alg_flops"] + EXP_FLOP_EQUIV * n_exp
+    achieved_tf = alg_flop_equiv / (chain_avg_ms * 1e-3) / 1e12
     rule_peak = pk["bf16"] * NOMINAL_FP64_TFLOPS / NOMINAL_BF16_TFLOPS
     peak = fp64["dmma_tflops"] if bound == "tensor" else fp64["dfma_tflops"]
     alg_bytes = n_ops * 12 + (B + 1) * 8 + B * (16 + 8 + 4 + Q)
@@ -257,7 +262,7 @@ def measure_config(L, torch, cfg, B, rank, steps, warmup, schedule, local_rank, 
                         f"{pk['source']} bf16 {pk['bf16']} TF/s x nominal {NOMINAL_FP64_TFLOPS}/{NOMINAL_BF16_TFLOPS}, gives {rule_peak:.2f}"),
         "frac_of_rule_peak": achieved_tf / rule_peak,
         "kernel_ms": chain_avg_ms, "kernel_share_of_step": chain_avg_ms * steps / total_ms,
-        "flops_per_launch_algorithmic": stats["alg_flops"], "executed_real_macs_padded": stats["macs"],
+        "flops_per_launch_algorithmic": stats["alg_flops"], "exp_per_launch": n_exp, "flop_equivalents_per_launch": alg_flop_equiv, "executed_real_macs_padded": stats["macs"],
         "algorithmic_io_bytes_per_step": alg_bytes,
         "hbm_frac_algorithmic": alg_bytes / (total_ms / steps * 1e-3) / 1e9 / pk["hbm_gbs"],
     }
@@ -347,7 +352,7 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         "bound_batch": {"norm": "frobenius unless the key says spectral", "ms_per_batch": m["bound_ms"],
                         "bounds_per_s": {k: B / (v * 1e-3) for k, v in m["bound_ms"].items()}},
         "lib": {"strings": stats["strings"], "units": stats["units"], "path": stats["path"], "panel_width_or_lanes": stats["panel_width"],
-                "team_warps": stats["team_warps"], "load_impurity_s": m["load_s"]},
+                "team_warps": stats["team_warps"] if stats["path"] != 3 else None, "load_impurity_s": m["load_s"]},
     }
     if others:
         line["other_workloads"] = others

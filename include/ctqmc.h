@@ -170,7 +170,8 @@ int ctqmc_bound_batch_host(ctqmc_impurity* imp, double beta, const ctqmc_batch* 
  * stats[0] = surviving strings, stats[1] = work units, stats[2] = kernels launched by the call,
  * stats[3] = real multiply-adds executed by the chain kernel (padded tiles included),
  * stats[4] = algorithmic real flops of the schedule executed (2 per real MAC, 8 per complex MAC, unpadded dims),
- * stats[5] = panel width (panel path) or lanes per configuration (small path), stats[6] = warps per team (panel path),
+ * stats[5] = panel width (panel path) or lanes per configuration (small path), stats[6] = warps per team (panel path) or the
+ * number of propagator exponentials evaluated (small path: sum over chain steps of the sector dimension),
  * stats[7] = kernel family that ran (CTQMC_PATH_PANEL / _LARGE / _SMALL). */
 int ctqmc_last_stats(ctqmc_impurity* imp, int64_t stats[8]);
 

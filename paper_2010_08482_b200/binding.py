@@ -146,6 +146,7 @@ def ctqmc_set_option(imp: ImpurityHandle, option: int, value: int):
 def ctqmc_last_stats(imp: ImpurityHandle) -> dict:
     buf = (C.c_int64 * 8)()
     _check(library().ctqmc_last_stats(imp.ptr, C.byref(buf)))
+    # "team_warps" is the number of propagator exponentials evaluated when path == CTQMC_PATH_SMALL (include/ctqmc.h)
     keys = ["strings", "units", "launches", "macs", "alg_flops", "panel_width", "team_warps", "path"]
     return dict(zip(keys, [int(x) for x in buf]))
 

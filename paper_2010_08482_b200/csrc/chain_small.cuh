@@ -86,7 +86,7 @@ __global__ void __launch_bounds__(256) small_trace_kernel(SmallParams P) {
   int* s_qs = s_r + Q;
 
   const long long n_groups = (long long)gridDim.x * (blockDim.x / G);
-  unsigned long long st_strings = 0, st_flops = 0;
+  unsigned long long st_strings = 0, st_flops = 0, st_exp = 0;
   for (long long b = (long long)blockIdx.x * (blockDim.x / G) + grp_in_cta; b < P.bv.B; b += n_groups) {
     const long long lo = P.bv.offset[b];
     const int L = (int)(P.bv.offset[b + 1] - lo);
@@ -169,7 +169,7 @@ __global__ void __launch_bounds__(256) small_trace_kernel(SmallParams P) {
         }
         __syncwarp(mask);
         int d = c;
-        unsigned long long macs = 0;
+        unsigned long long macs = 0, nexp = 0;
         const int m_first = lg / c, n_first = lg - m_first * c;   // c is fixed along the chain
         for (int j = 0; j < L; ++j) {
           int i = r + j;
@@ -230,11 +230,12 @@ __global__ void __launch_bounds__(256) small_trace_kernel(SmallParams P) {
           __syncwarp(mask);
           double* tmp = X; X = Xn; Xn = tmp;
           macs += (unsigned long long)dn * d;
+          nexp += (unsigned long long)dn;
           q = qn; d = dn;
         }
         if (!dead)
           for (int n = lg; n < c; n += G) { re += X[(n * c + n) * ES]; if constexpr (CPLX) im += X[(n * c + n) * ES + 1]; }
-        if (lg == 0) { st_strings += 1; st_flops += macs * (unsigned long long)c * (CPLX ? 8ull : 2ull); }
+        if (lg == 0) { st_strings += 1; st_flops += macs * (unsigned long long)c * (CPLX ? 8ull : 2ull); st_exp += nexp; }
         __syncwarp(mask);
       }
 #pragma unroll
@@ -288,6 +289,7 @@ __global__ void __launch_bounds__(256) small_trace_kernel(SmallParams P) {
     atomicAdd(&P.cnt->n_slots, st_strings);
     atomicAdd(&P.cnt->alg_flops, st_flops);
     atomicAdd(&P.cnt->macs, st_flops / 2);
+    atomicAdd(&P.cnt->n_exp, st_exp);
   }
 }
 

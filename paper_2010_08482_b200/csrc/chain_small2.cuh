@@ -73,7 +73,7 @@ __global__ void __launch_bounds__(512) small2_trace_kernel(Small2Params P) {
   int* s_sv = s_qs + Q;   // [Q + 1]: start sectors with a chain to multiply, then their count
 
   const long long n_groups = (long long)gridDim.x * groups_per_cta;
-  unsigned long long st_strings = 0, st_flops = 0;
+  unsigned long long st_strings = 0, st_flops = 0, st_exp = 0;
   for (long long b = (long long)blockIdx.x * groups_per_cta + grp_in_cta; b < P.bv.B; b += n_groups) {
     const long long lo = P.bv.offset[b];
     const int L = (int)(P.bv.offset[b + 1] - lo);
@@ -164,7 +164,7 @@ __global__ void __launch_bounds__(512) small2_trace_kernel(Small2Params P) {
       } else {
         for (int n = 0; n < c; ++n) X[n * DP + lg] = (lg == n) ? 1.0 : 0.0;
         __syncwarp(mask);
-        unsigned long long macs = 0;
+        unsigned long long macs = 0, nexp = 0;
         int i = r;
         int sym_nx = __ldg(sym + i);
         double ta_nx = __ldg(tau + i), tb_nx = __ldg(tau + ((i + 1 < L) ? i + 1 : 0));
@@ -212,11 +212,12 @@ __global__ void __launch_bounds__(512) small2_trace_kernel(Small2Params P) {
           __syncwarp(mask);
           double* tmp = X; X = Xn; Xn = tmp;
           macs += (unsigned long long)(bi.y >> 16) * (unsigned long long)(bi.y & 0xffff);
+          nexp += (unsigned long long)(bi.y >> 16);
           q = qn;
         }
         if (lg == 0) {
           if (!dead) for (int n = 0; n < c; ++n) tr += X[n * DP + n];
-          st_strings += 1; st_flops += macs * (unsigned long long)c * 2ull;
+          st_strings += 1; st_flops += macs * (unsigned long long)c * 2ull; st_exp += nexp;
         }
         __syncwarp(mask);
       }
@@ -265,6 +266,7 @@ __global__ void __launch_bounds__(512) small2_trace_kernel(Small2Params P) {
     atomicAdd(&P.cnt->n_slots, st_strings);
     atomicAdd(&P.cnt->alg_flops, st_flops);
     atomicAdd(&P.cnt->macs, st_flops / 2);
+    atomicAdd(&P.cnt->n_exp, st_exp);
   }
 }
 

@@ -1192,6 +1192,7 @@ extern "C" int ctqmc_last_stats(ctqmc_impurity* h, int64_t stats[8]) {
   CU(cudaMemcpy(&c, h->arena.cnt, sizeof c, cudaMemcpyDeviceToHost));
   stats[0] = (int64_t)c.n_strings; stats[1] = (int64_t)c.n_slots; stats[2] = h->last_launches;
   stats[3] = (int64_t)c.macs; stats[4] = (int64_t)c.alg_flops;
+  if (h->last_path == CTQMC_PATH_SMALL) stats[6] = (int64_t)c.n_exp;
   return 0;
 }
 
