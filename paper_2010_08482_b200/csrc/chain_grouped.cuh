@@ -180,6 +180,10 @@ __global__ void __launch_bounds__(kGThreads, (kGWN == 2 && !CPLX) ? 3 : 2) group
   __shared__ __align__(8) unsigned long long g_full[kGStages], g_empty[kGStages];
   double* sde = reinterpret_cast<double*>(gsm + kGStages * kGStageBytes);   // E[k] - Emin of the source sector
 
+  // Programmatic dependent launch: the next chain position's grid may start as soon as every CTA of this one is resident, so
+  // its CTAs fill the SM slots this launch's tail leaves empty and run their prologue (tile list, column map, barrier
+  // set-up: nothing a previous step writes) there; they wait (griddepcontrol.wait, below) before touching the carried matrices.
+  asm volatile("griddepcontrol.launch_dependents;");
   const int tile_id = blockIdx.x / MTmax, slab = blockIdx.x - tile_id * MTmax;   // slabs of a tile are neighbours in launch order
   if (tile_id >= P.ntiles[j]) return;
   const int4 tl = P.tiles[(size_t)j * P.tile_cap + tile_id];
@@ -203,6 +207,12 @@ __global__ void __launch_bounds__(kGThreads, (kGWN == 2 && !CPLX) ? 3 : 2) group
     for (int st = 0; st < kGStages; ++st) { mbar_init(&g_full[st], kGThreads); mbar_init(&g_empty[st], kGThreads / 32); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
+  {   // source-sector energies: static data, still before the wait
+    const double* Eq = P.imp.energy + P.imp.e_off[bd.src];
+    const double emin = P.imp.e_min[bd.src];
+    for (int k = tid; k < nkt * BKE; k += kGThreads) sde[k] = (k < d) ? __dsub_rn(Eq[k], emin) : 0.0;
+  }
+  asm volatile("griddepcontrol.wait;" ::: "memory");   // the previous chain position is complete and its writes are visible
   if (tid < kGBN) {
     const int n = tid;
     if (n < ncols) {
@@ -222,11 +232,6 @@ __global__ void __launch_bounds__(kGThreads, (kGWN == 2 && !CPLX) ? 3 : 2) group
       s_xin[n] = nullptr; s_xout[n] = nullptr; s_delta[n] = 0.0; s_dprev[n] = 0.0; s_kprev[n] = 1 << 29; s_u[n] = -1;
     }
     s_kmax[n] = INT_MIN;
-  }
-  {
-    const double* Eq = P.imp.energy + P.imp.e_off[bd.src];
-    const double emin = P.imp.e_min[bd.src];
-    for (int k = tid; k < nkt * BKE; k += kGThreads) sde[k] = (k < d) ? __dsub_rn(Eq[k], emin) : 0.0;
   }
   __syncthreads();
 

@@ -442,13 +442,20 @@ int enqueue_grouped(ctqmc_impurity* h, const BatchView& bv, cudaStream_t st) {
   grouped_fill_kernel<<<g_ul, 256, 0, st>>>(gp);
   const int MTmax = (h->dev.dmax + kGBM - 1) / kGBM;
   const unsigned sg = (unsigned)tile_cap * (unsigned)MTmax;
+  // step launches use programmatic stream serialization (see the kernel): launch gaps and tails overlap the next step's prologue
+  cudaLaunchConfig_t lc = {};
+  lc.gridDim = dim3(sg); lc.blockDim = dim3(kGThreads); lc.dynamicSmemBytes = h->grouped_smem; lc.stream = st;
+  cudaLaunchAttribute lattr[1];
+  lattr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  lattr[0].val.programmaticStreamSerializationAllowed = 1;
+  lc.attrs = lattr; lc.numAttrs = 1;
   if (h->dev.cplx) {
     grouped_init_kernel<true><<<(unsigned)n_units, 128, 0, st>>>(gp);
-    for (int j = 0; j < Lmax; ++j) grouped_step_kernel<true><<<sg, kGThreads, h->grouped_smem, st>>>(gp, j, MTmax);
+    for (int j = 0; j < Lmax; ++j) CU(cudaLaunchKernelEx(&lc, grouped_step_kernel<true>, gp, j, MTmax));
     grouped_finish_kernel<true><<<(unsigned)n_units, 256, 0, st>>>(gp);
   } else {
     grouped_init_kernel<false><<<(unsigned)n_units, 128, 0, st>>>(gp);
-    for (int j = 0; j < Lmax; ++j) grouped_step_kernel<false><<<sg, kGThreads, h->grouped_smem, st>>>(gp, j, MTmax);
+    for (int j = 0; j < Lmax; ++j) CU(cudaLaunchKernelEx(&lc, grouped_step_kernel<false>, gp, j, MTmax));
     grouped_finish_kernel<false><<<(unsigned)n_units, 256, 0, st>>>(gp);
   }
   h->last_launches += 7 + Lmax;
