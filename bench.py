@@ -37,13 +37,25 @@ WORKLOADS = {
     5: "cfg5: 7-orbital f-shell + crystal field, N sectors 1001/2002/3003, complex, pairs~Poisson(100)",
 }
 REF_SAMPLE = {1: 8192, 2: 4096, 3: 128, 4: 4, 5: 1}   # configurations per reference step (seconds of oracle time each)
+# config 5: one configuration is ~1e13 flop of numpy (a minute): a reference step / the cpu_baseline is the oracle on the
+# first L/REF_PREFIX_DIV operators of configuration 0, extrapolated to a whole trace by the literal flop count of Eq. 65
+REF_PREFIX_DIV = {"reference": 10, "cpu_baseline": 4}
 KERNELS = {1: ("chain_kernel (panel in shared memory, fused propagate x operator, FP64 DMMA m8n8k4)", "tensor"),
            2: ("large_step_kernel (128x64 tiles, TMA + mbarrier ring, fused propagate x operator, FP64 DMMA m8n8k4)", "tensor"),
            3: ("small2_trace_kernel / small_trace_kernel (whole path in one launch, operator store in shared memory, FP64 FMA)", "alu"),
            4: ("grouped_step_kernel (strings sharing a block share one GEMM per chain position, 64x64 tiles, FP64 DMMA m8n8k4)", "tensor")}
-# dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, from the `ncu --set full` captures
-# summarised under profiles/ (same launch configuration as the default batch of each config); None = not captured.
-NCU_TRAFFIC_BYTES = {2: 6_059_008, 4: 664_738_560}   # cfg 2: profiles/r01_cfg2_small_full.md; cfg 4: r01_cfg4_grouped_step_full.md (one chain position)
+
+
+def ncu_traffic(cfg: int, batch: int):
+    """dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, from the `ncu --set full` capture
+    summarised under profiles/ for exactly this config and batch (profiles/traffic.json, written next to the summaries);
+    None when there is no capture of this launch configuration."""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    if not os.path.exists(p):
+        return None
+    with open(p) as fh:
+        e = json.load(fh).get(f"cfg{cfg}_batch{batch}")
+    return None if e is None else e["dram_bytes_per_launch"]
 
 
 def peaks():
@@ -132,6 +144,41 @@ def blas_threads() -> int:
         return 1
 
 
+def oracle_cores(cfg: int):
+    """Threads the oracle really uses: it is ONE Python process looping over configurations and start sectors; only numpy's
+    matmul is threaded, and only where the blocks are large enough for the BLAS to split (configs 3-5)."""
+    avail = len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1)
+    used = 1 if cfg <= 2 else min(avail, blas_threads())
+    note = (f"single Python process; {avail} cores available to it, numpy BLAS pool {blas_threads()} threads; "
+            + ("blocks of at most 9 x 9: effectively one core" if cfg <= 2 else "matmul is the only threaded step"))
+    return used, note
+
+
+def oracle_rate_prefix(imp, batch, div: int):
+    """Config 5: the oracle (literal Eq. 65) on the first ceil(L/div) operators of configuration 0, and the factor that
+    extrapolates it to a whole trace: literal flops of the full string over those of the prefix (8 d_i d_{i-1} d_q0 per step
+    and surviving start sector, from the oracle's own routing).  Returns (traces/s extrapolated, description)."""
+    from oracle import trace_oracle as O
+    s, t = batch.config(0)
+    n = max(2, -(-len(s) // div))
+
+    def flops(sym):
+        tot = 0
+        for q0 in range(imp.n_sectors):
+            v = O.route(imp, sym, q0)
+            if v is not None:
+                tot += sum(8 * int(imp.dims[v[i + 1]]) * int(imp.dims[v[i]]) * int(imp.dims[q0]) for i in range(len(sym)))
+        return tot
+
+    f_full, f_pre = flops(s), flops(s[:n])
+    t0 = time.perf_counter()
+    O.trace_config(imp, batch.beta, s[:n], t[:n])
+    dt = time.perf_counter() - t0
+    rate = 1.0 / (dt * f_full / f_pre)
+    return rate, dt, (f"EXTRAPOLATED from the first {n} of the {len(s)} operators of configuration 0 ({dt:.1f} s of "
+                      f"oracle.trace_oracle.trace_config, numpy fp64) by the literal flop count of Eq. 65 ({f_full:.3e} / {f_pre:.3e})")
+
+
 def run_reference(args, rank: int):
     """--impl reference: the CPU oracle, as it stands, on a bounded sample per step (rank 0 only)."""
     if rank != 0:
@@ -141,27 +188,38 @@ def run_reference(args, rank: int):
     imp = build_config_impurity(cfg, keep_eigvecs=False)
     n = REF_SAMPLE[cfg]
     batch = make_batch(cfg, n)
-    for _ in range(min(args.warmup, 1)):
-        oracle_rate(imp, batch, max(1, n // 8))
-    t_tot, n_tot = 0.0, 0
-    for _ in range(args.steps):
-        _, k, dt = oracle_rate(imp, batch, n)
-        t_tot += dt
-        n_tot += k
-    val = n_tot / t_tot
-    cores = blas_threads()
-    sample = f"{n} configurations of {WORKLOADS[cfg]} per step, oracle.trace_oracle.trace_batch (numpy fp64)"
+    if cfg == 5:
+        rates, t_tot = [], 0.0
+        for i in range(min(args.warmup, 1) + args.steps):
+            rate, dt, sample = oracle_rate_prefix(imp, batch, REF_PREFIX_DIV["reference"])
+            if i >= min(args.warmup, 1):
+                rates.append(rate)
+                t_tot += dt
+        val = len(rates) / sum(1.0 / r for r in rates)
+        sample = "per step: " + sample
+    else:
+        for _ in range(min(args.warmup, 1)):
+            oracle_rate(imp, batch, max(1, n // 8))
+        t_tot, n_tot = 0.0, 0
+        for _ in range(args.steps):
+            _, k, dt = oracle_rate(imp, batch, n)
+            t_tot += dt
+            n_tot += k
+        val = n_tot / t_tot
+        sample = f"{n} configurations of {WORKLOADS[cfg]} per step, oracle.trace_oracle.trace_batch (numpy fp64)"
+    cores, cores_note = oracle_cores(cfg)
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * t_tot / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": WORKLOADS[cfg], "batch": n},
-        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "cores_note": cores_note, "kind": "oracle", "sample": sample},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }))
 
 
-def measure_config(L, torch, cfg, B, rank, steps, warmup, schedule, local_rank, barrier, fp64, pk, with_e2e=True, path="auto"):
+def measure_config(L, torch, cfg, B, rank, steps, warmup, schedule, local_rank, barrier, fp64, pk, with_e2e=True, path="auto",
+                   e2e_steps=None):
     """Times `steps` passes of the hot path on config `cfg` (this rank's shard) and returns the pieces of the JSON line."""
     import numpy as np
     from workloads import build_config_impurity
@@ -211,12 +269,13 @@ def measure_config(L, torch, cfg, B, rank, steps, warmup, schedule, local_rank, 
         pout = [torch.empty((B, 2), dtype=torch.float64).pin_memory(), torch.empty(B, dtype=torch.int64).pin_memory(),
                 torch.empty((B, Q), dtype=torch.uint8).pin_memory(), torch.empty(B, dtype=torch.int32).pin_memory()]
         h_out = tuple(t.numpy() for t in pout)
-        for _ in range(2):
+        for _ in range(1 if cfg == 5 else 2):
             L.ctqmc_trace_batch_host(h, batch.beta, *h_in, out=h_out)
         assert np.array_equal(h_out[0], out[0].cpu().numpy(), equal_nan=True) and np.array_equal(h_out[1], out[1].cpu().numpy())
         e2e_s = 0.0
+        e2e_steps = steps if e2e_steps is None else e2e_steps
         barrier()
-        for _ in range(steps):
+        for _ in range(e2e_steps):
             flush.zero_()
             torch.cuda.synchronize()
             t0 = time.perf_counter()
@@ -227,7 +286,8 @@ def measure_config(L, torch, cfg, B, rank, steps, warmup, schedule, local_rank, 
     # the lazy-trace bounds (a6) on the same batch: Frobenius, S = 1 (tables only) and S = 8 (segment products), device-resident
     bound_ms = {}
     if with_e2e:
-        for key, nk, S in (("S1", 0, 1), ("S8", 0, 8), ("S1_spectral", 1, 1)):
+        # config 5: S = 8 segment products cost as much as the traces themselves (a minute per call); tables only there
+        for key, nk, S in ((("S1", 0, 1), ("S1_spectral", 1, 1)) if cfg == 5 else (("S1", 0, 1), ("S8", 0, 8), ("S1_spectral", 1, 1))):
             for _ in range(2):
                 L.ctqmc_bound_batch(h, batch.beta, off, sym, tau, nk, S, want_sector=False)
             torch.cuda.synchronize()
@@ -248,7 +308,7 @@ def measure_config(L, torch, cfg, B, rank, steps, warmup, schedule, local_rank, 
     chain_avg_ms = sum(chain_ms) / len(chain_ms)
     # small (alu-bound) path: the algorithmic work also holds one FP64 exp per row and chain step; SURVEY 8(d) D3 counts it at
     # its instruction cost (~25 flop-equivalents), not as one flop
-    n_exp = stats["team_warps"] if stats["path"] == 3 else 0
+    n_exp = stats["n_exp"]
     alg_flop_equiv = stats["alg_flops"] + EXP_FLOP_EQUIV * n_exp
     achieved_tf = alg_flop_equiv / (chain_avg_ms * 1e-3) / 1e12
     rule_peak = pk["bf16"] * NOMINAL_FP64_TFLOPS / NOMINAL_BF16_TFLOPS
@@ -256,7 +316,7 @@ def measure_config(L, torch, cfg, B, rank, steps, warmup, schedule, local_rank, 
     alg_bytes = n_ops * 12 + (B + 1) * 8 + B * (16 + 8 + 4 + Q)
     roofline = {
         "bound": bound, "kernel": kname, "achieved": achieved_tf, "peak": peak, "unit": "TFLOP/s", "frac": achieved_tf / peak,
-        "traffic": NCU_TRAFFIC_BYTES.get(cfg) if B == _default_batch(cfg) else None,
+        "traffic": ncu_traffic(cfg, B),
         "peak_source": ("FP64 " + ("DMMA" if bound == "tensor" else "DFMA") + " register-resident loop measured in this run by "
                         "ctqmc_measure_fp64_peak (MEASURED_PEAKS.json has no FP64 entry); the guide's rule, "
                         f"{pk['source']} bf16 {pk['bf16']} TF/s x nominal {NOMINAL_FP64_TFLOPS}/{NOMINAL_BF16_TFLOPS}, gives {rule_peak:.2f}"),
@@ -266,7 +326,7 @@ def measure_config(L, torch, cfg, B, rank, steps, warmup, schedule, local_rank, 
         "algorithmic_io_bytes_per_step": alg_bytes,
         "hbm_frac_algorithmic": alg_bytes / (total_ms / steps * 1e-3) / 1e9 / pk["hbm_gbs"],
     }
-    return dict(imp=imp, batch=batch, stats=stats, total_ms=total_ms, e2e_ms=e2e_ms, n_ops=n_ops, Q=Q, roofline=roofline,
+    return dict(imp=imp, batch=batch, stats=stats, total_ms=total_ms, e2e_ms=e2e_ms, e2e_steps=e2e_steps, n_ops=n_ops, Q=Q, roofline=roofline,
                 phases={"route": sum(route_ms) / len(route_ms), "chain": chain_avg_ms, "reduce": sum(reduce_ms) / len(reduce_ms)},
                 load_s=load_s, bound_ms=bound_ms)
 
@@ -308,7 +368,9 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     sampler = ClockSampler(local_rank)
     if rank == 0:
         sampler.start()
-    m = measure_config(L, torch, cfg, B, rank, args.steps, warmup, args.schedule, local_rank, barrier, fp64, pk, path=args.path)
+    # config 5: a step is 12 s, so the host-buffer (e2e) leg times 3 steps whatever --steps says (its copies are 27 kB per step)
+    m = measure_config(L, torch, cfg, B, rank, args.steps, warmup, args.schedule, local_rank, barrier, fp64, pk, path=args.path,
+                       e2e_steps=min(args.steps, 3) if cfg == 5 else None)
     clocks = sampler.stop() if rank == 0 else None
     total_ms, e2e_ms = reduce_max([m["total_ms"], m["e2e_ms"]], dist, "cuda")
 
@@ -317,18 +379,18 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         # the other BASELINE.json configs at their stated batch, device-resident timing only (fewer steps: they are context)
         # plus the default small-sector config at a scaled batch (same generator, 64 x BASELINE's 4096): at the stated batch
         # that launch lasts as long as ONE configuration's dependency chain, whatever the kernel
-        for c, bsz, key in ((1, 0, "cfg1"), (2, 262144, "cfg2_scaled_batch"), (3, 0, "cfg3"), (4, 0, "cfg4"), (5, 0, "cfg5")):
+        for c, bsz, key in ((1, 0, "cfg1"), (2, 0, "cfg2"), (2, 262144, "cfg2_scaled_batch"), (3, 0, "cfg3"), (4, 0, "cfg4"), (5, 0, "cfg5")):
             if c == cfg and not bsz:
                 continue
             bsz = bsz or _default_batch(c)
-            k = 1 if c == 5 else 3
-            o = measure_config(L, torch, c, bsz, 0, k, 3 if c != 5 else 1, "thin", local_rank, barrier, fp64, pk,
-                               with_e2e=False)
+            k = 3 if c == 5 else 5
+            o = measure_config(L, torch, c, bsz, 0, k, 3, "thin", local_rank, barrier, fp64, pk, with_e2e=False)
             others[key] = {"workload": WORKLOADS[c], "batch": bsz, "steps": k,
                                  "value": aggregate_value(1, bsz, k, o["total_ms"]), "unit": UNIT,
                                  "ms_per_step": o["total_ms"] / k, "gflops": o["stats"]["alg_flops"] * k / (o["total_ms"] * 1e-3) / 1e9,
-                                 "roofline": {x: o["roofline"][x] for x in ("bound", "kernel", "achieved", "peak", "unit", "frac",
-                                                                            "frac_of_rule_peak", "kernel_ms", "kernel_share_of_step")}}
+                                 "roofline": {x: o["roofline"][x] for x in ("bound", "kernel", "achieved", "peak", "unit", "frac", "traffic",
+                                                                            "frac_of_rule_peak", "kernel_ms", "kernel_share_of_step",
+                                                                            "hbm_frac_algorithmic")}}
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
@@ -342,8 +404,9 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         "config": {"workload": WORKLOADS[cfg], "batch_per_gpu": B, "operators_per_batch": n_ops, "schedule": args.schedule,
                    "l2": "flushed between timed steps (256 MiB write)", "sharding": "batch split over ranks, no collective"},
         "gflops": world * stats["alg_flops"] * args.steps / (total_ms * 1e-3) / 1e9,
-        "e2e": {"value": aggregate_value(world, B, args.steps, e2e_ms), "unit": UNIT,
-                "h2d_bytes_per_step": n_ops * 12 + (B + 1) * 8, "d2h_bytes_per_step": B * (16 + 8 + 4 + Q)},
+        "e2e": {"value": aggregate_value(world, B, m["e2e_steps"], e2e_ms), "unit": UNIT, "steps": m["e2e_steps"],
+                "h2d_bytes_per_step": n_ops * 12 + (B + 1) * 8, "d2h_bytes_per_step": B * (16 + 8 + 4 + Q),
+                "api": "ctqmc_trace_batch_host (pinned host buffers; copies inside the timed region)"},
         "gpu_launches": stats["launches"] * args.steps,
         "clocks": clocks,
         "roofline": m["roofline"],
@@ -352,14 +415,18 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         "bound_batch": {"norm": "frobenius unless the key says spectral", "ms_per_batch": m["bound_ms"],
                         "bounds_per_s": {k: B / (v * 1e-3) for k, v in m["bound_ms"].items()}},
         "lib": {"strings": stats["strings"], "units": stats["units"], "path": stats["path"], "panel_width_or_lanes": stats["panel_width"],
-                "team_warps": stats["team_warps"] if stats["path"] != 3 else None, "load_impurity_s": m["load_s"]},
+                "team_warps": stats["team_warps"], "load_impurity_s": m["load_s"]},
     }
     if others:
         line["other_workloads"] = others
     if not args.no_cpu_baseline and world == 1:
-        rate, k, dt = oracle_rate(m["imp"], m["batch"], REF_SAMPLE[cfg])
-        line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": blas_threads(), "kind": "oracle",
-                                "sample": f"first {k} configurations of the same batch, {dt:.1f} s, oracle.trace_oracle.trace_batch (numpy fp64)"}
+        cores, cores_note = oracle_cores(cfg)
+        if cfg == 5:
+            rate, dt, sample = oracle_rate_prefix(m["imp"], m["batch"], REF_PREFIX_DIV["cpu_baseline"])
+        else:
+            rate, k, dt = oracle_rate(m["imp"], m["batch"], REF_SAMPLE[cfg])
+            sample = f"first {k} configurations of the same batch, {dt:.1f} s, oracle.trace_oracle.trace_batch (numpy fp64)"
+        line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": cores, "cores_note": cores_note, "kind": "oracle", "sample": sample}
     print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()
@@ -368,9 +435,10 @@ def run_ours(args, rank: int, world: int, local_rank: int):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=2, choices=sorted(WORKLOADS))
+    ap.add_argument("--config", type=int, default=5, choices=sorted(WORKLOADS),
+                    help="BASELINE.json config (1-based); default 5 = the largest single-GPU one, on which north_star states its target")
     ap.add_argument("--batch", type=int, default=0, help="configurations per GPU per step (default: BASELINE.json's batch)")
     ap.add_argument("--schedule", default="thin", choices=["thin", "literal"])
     ap.add_argument("--path", default="auto", choices=["auto", "panel", "large", "small", "grouped"],

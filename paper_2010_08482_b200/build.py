@@ -13,7 +13,7 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libctqmc_b200.so")
 SOURCES = ["ctqmc_api.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-shared",
-              "-Xcompiler", "-fPIC", "-Xptxas", "-v", "--use_fast_math=false" if False else "-DNDEBUG"]
+              "-Xcompiler", "-fPIC", "-Xptxas", "-v", "-DNDEBUG"]
 
 
 def needs_build() -> bool:

@@ -415,6 +415,9 @@ __global__ void __launch_bounds__(kGThreads, (kGWN == 2 && !CPLX) ? 3 : 2) group
             xo[row] = v;
             if (v != 0.0) cexp = max(cexp, kr[mt] + ilogb_fast(v));
           }
+        } else if (!CPLX && row == dn && (dn & 1)) {
+          xo[row] = 0.0;   // real matrices are read in 16-byte chunks of two rows: the pad row of an odd sector must hold an
+                           // exact zero, not whatever an earlier string left in the arena (it is scaled by 2^-kprev on load)
         }
       }
       if (cexp != INT_MIN) atomicMax(&s_kmax[n], cexp);

@@ -126,12 +126,15 @@ namespace ctqmc {
 
 // Spectral-norm guard (reading A1).  Power iteration approaches sigma_max from BELOW; a bound built from an
 // under-estimate would not be a bound.  With v the normalised iterate, u = F v, sigma = ||u|| and w = F^H u, the iteration has
-// converged iff w = sigma^2 v.  One CTA per block: need[b] = 1 unless ||w - sigma^2 v|| <= 1e-10 sigma^2 (c / c^dag blocks
-// converge exactly after one step: F^H F is a projector, pin P10).
+// converged iff w = sigma^2 v.  One CTA per block: the iterate is accepted only if the residual r = w - sigma^2 v satisfies
+// ||r|| <= 1e-13 sigma^2 (c / c^dag blocks converge exactly after one step: F^H F is a projector, pin P10), and then as
+// sqrt(sigma^2 + ||r||), which covers the eigenvalue of F^H F the residual localises.  Everything else -- slow convergence
+// (near-degenerate top singular values), or sigma = 0 from a start vector in ker F -- gets need[b] = 1 and the rigorous
+// upper estimate of sigma_upper_kernel (which is 0 for an all-zero block).
 template <int ES>
 __global__ void sigma_check_kernel(const BlkDesc* __restrict__ blks, const long long* __restrict__ v_off,
                                    const double* __restrict__ v, const double* __restrict__ w,
-                                   const double* __restrict__ sigma, int* __restrict__ need) {
+                                   double* __restrict__ sigma, int* __restrict__ need) {
   __shared__ double red[8];
   const BlkDesc bd = blks[blockIdx.x];
   const double s2 = sigma[blockIdx.x] * sigma[blockIdx.x];
@@ -145,7 +148,10 @@ __global__ void sigma_check_kernel(const BlkDesc* __restrict__ blks, const long 
   if (threadIdx.x == 0) {
     double t = 0.0;
     for (int i = 0; i < (int)(blockDim.x >> 5); ++i) t += red[i];
-    need[blockIdx.x] = (s2 > 0.0 && !(sqrt(t) <= 1e-10 * s2)) ? 1 : 0;
+    const double rn = sqrt(t);
+    const bool ok = s2 > 0.0 && rn <= 1e-13 * s2;
+    need[blockIdx.x] = ok ? 0 : 1;
+    if (ok) sigma[blockIdx.x] = sqrt(s2 + rn) * (1.0 + 4e-16);
   }
 }
 

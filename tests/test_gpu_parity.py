@@ -3,14 +3,14 @@
 Bars (BASELINE.json north_star):
   * routing (`survive`) and the vanishing pattern (`status`): bit-exact;
   * trace: |w_gpu - w_cpu| <= 1e-9 |w_cpu| at a common exponent (checks sign / phase too; reading A5), loosened only
-    by the conditioning rule A8: (i) final cancellation, tolerance 1e-9 * max(1, kappa * 1e-5); (ii) a configuration the
-    ORACLE cannot evaluate to 1e-10 itself -- its value changes by more than that under the cyclic time shifts of pin
-    P2, which are exact identities of Eq. 65 -- is compared at 10x the oracle's own spread.  At most 1 % of a batch (and
-    never more than one configuration of a small batch) may need it -- except on BASELINE config 3, whose N-only sectors
-    hide the S_z / L_z symmetries: there 6 % of the configurations (measured on the first 150; up to 20 % of a batch of 40)
-    are not determined by fp64 in that basis (the same oracle in (N, S_z, L_z) sectors has a spread of 1e-12 on them), so up
-    to 25 % may be flagged, each one by the oracle's own spread, never by the GPU result;
-  * bound: relative 1e-9 against the oracle's bound, and bound >= |trace|.
+    by the conditioning rule A8: (i) final cancellation, tolerance 1e-9 * max(1, kappa * 1e-5), at most 1 % of a batch;
+    (ii) BASELINE config 3 only: its N-only sectors hide the S_z / L_z symmetries and fp64 does not determine a few per cent
+    of its configurations in that basis -- on EITHER side.  There a true value exists: the same oracle on the same Hamiltonian
+    labelled by (N, 2S_z, L_z) (equal by pin P4 (iii), stable to 1e-10 under the cyclic shifts of pin P2).  A configuration
+    that misses 1e-9 against the coarse oracle is judged against that truth: |gpu - truth| <= max(1e-9, 10 |coarse - truth|),
+    i.e. the GPU must be no worse than the fp64 oracle fed the same blocks.  Nothing is exempt;
+  * bound: relative 1e-9 against the oracle's bound (plus, for segment products, the rounding floor 2^-40 x the product of
+    the factor norms), bound >= |trace| per configuration AND per start sector.
 """
 import math
 
@@ -58,27 +58,30 @@ def _dev(torch, batch):
     return (torch.from_numpy(batch.offset).cuda(), torch.from_numpy(batch.symbol).cuda(), torch.from_numpy(batch.tau).cuda())
 
 
-def _oracle_self_spread(imp, beta, s, t, r):
-    """Largest relative change of the oracle's own value under cyclic time shifts (pin P2: exact identities of
-    Eq. 63/65).  Measures how well fp64 determines this configuration's trace at all (reading A8 (ii))."""
-    from oracle import trace_oracle as O
-    spread = 0.0
-    for frac in (0.23, 0.52, 0.77):
-        t2 = (t + frac * beta) % beta
-        o = np.argsort(t2, kind="stable")
-        r2 = O.trace_config(imp, beta, s[o], t2[o])
-        spread = max(spread, rel_diff(r2["mant"], r2["exp2"], r["mant"], r["exp2"]))
-    return spread
+_TRUTH = {}
+
+
+def _truth_for(imp):
+    """Config 3's Hamiltonian labelled by all its Abelian quantum numbers (N, 2S_z, L_z) (rule A8 (ii) above); None for
+    every other impurity (they use all their quantum numbers already, or have none left to hide)."""
+    if getattr(imp, "name", "") != "cfg3-dshell-N":
+        return None
+    if "cfg3" not in _TRUTH:
+        from golden.make_golden import _fine_cfg3
+        _TRUTH["cfg3"] = _fine_cfg3()
+    return _TRUTH["cfg3"]
 
 
 def _check_trace(lib, torch, imp, handle, batch, label, sample=None):
+    """GPU against the oracle on every (sampled) configuration."""
     from oracle import trace_oracle as O
+    truth_imp = _truth_for(imp)
     off, sym, tau = _dev(torch, batch)
     mant, exp2, surv, status = lib.ctqmc_trace_batch(handle, batch.beta, off, sym, tau)
     torch.cuda.synchronize()
     mant, exp2, surv, status = mant.cpu().numpy(), exp2.cpu().numpy(), surv.cpu().numpy(), status.cpu().numpy()
     worst = 0.0
-    loosened = 0
+    loosened = explained = 0
     checked = range(batch.n_configs) if sample is None else sample   # the GPU ran the whole batch; the oracle checks these
     for b in checked:
         s, t = batch.config(b)
@@ -96,19 +99,65 @@ def _check_trace(lib, torch, imp, handle, batch, label, sample=None):
         assert 1.0 <= mx < 2.0, f"{label} config {b}: mantissa {w} not normalised"
         d = rel_diff(w, int(exp2[b]), r["mant"], r["exp2"])
         tol = TOL * max(1.0, r["kappa"] * 1e-5)
-        if d > tol and len(s) > 0:
-            spread = _oracle_self_spread(imp, batch.beta, s, t, r)
-            if spread > 1e-10:
-                print(f"{label} config {b}: oracle's own spread under cyclic shifts {spread:.2e} (ill-conditioned in fp64), gpu-oracle {d:.2e}")
-                tol = max(tol, 10.0 * spread)
         if tol > TOL:
             loosened += 1
+        if d > tol and truth_imp is not None and len(s) > 0:
+            rt = O.trace_config(truth_imp, batch.beta, s, t)
+            d_coarse = rel_diff(r["mant"], r["exp2"], rt["mant"], rt["exp2"])
+            d_gpu = rel_diff(w, int(exp2[b]), rt["mant"], rt["exp2"])
+            print(f"{label} config {b}: coarse oracle is {d_coarse:.2e} from the (N,Sz,Lz) truth, gpu {d_gpu:.2e}, gpu-coarse {d:.2e}")
+            assert d_gpu <= max(TOL, 10.0 * d_coarse), f"{label} config {b}: gpu {d_gpu:.3e} from the truth, coarse oracle {d_coarse:.3e}"
+            explained += 1
+            continue
         assert d <= tol, f"{label} config {b}: rel diff {d:.3e} > {tol:.1e} (kappa {r['kappa']:.2e})"
         if tol == TOL:
             worst = max(worst, d)          # worst difference among the configurations held to 1e-9
     n_checked = len(checked)
-    allowed = max(1, n_checked // 4) if label.startswith("cfg3") else max(1, n_checked // 100)
-    assert loosened <= allowed, f"{label}: {loosened} configurations needed the A8 loosening"
+    assert loosened <= max(1, n_checked // 100), f"{label}: {loosened} configurations needed the kappa loosening"
+    if explained:
+        print(f"{label}: {explained} of {n_checked} configurations judged against the (N,Sz,Lz) truth")
+    return worst
+
+
+def _load_golden(cfg):
+    import json
+    import os
+    from workloads import BASELINE_CONFIGS
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", f"cfg{cfg}_batch{BASELINE_CONFIGS[cfg]['batch']}.json")
+    with open(path) as fh:
+        return json.load(fh)
+
+
+def _check_trace_golden(lib, torch, handle, batch, doc, label, records=None):
+    """GPU against the stored oracle values (tests/golden/make_golden.py wrote them from oracle/ alone): EVERY record."""
+    off, sym, tau = _dev(torch, batch)
+    mant, exp2, surv, status = lib.ctqmc_trace_batch(handle, batch.beta, off, sym, tau)
+    torch.cuda.synchronize()
+    mant, exp2, surv, status = mant.cpu().numpy(), exp2.cpu().numpy(), surv.cpu().numpy(), status.cpu().numpy()
+    recs = doc["records"] if records is None else records
+    worst, judged_by_truth, loosened = 0.0, 0, 0
+    for rec in recs:
+        b = rec["b"]
+        assert b < batch.n_configs and rec["n_ops"] == len(batch.config(b)[0]), f"{label}: golden record {b} is not this batch's configuration"
+        assert status[b] == rec["status"], f"{label} config {b}: status"
+        assert "".join(str(int(x)) for x in surv[b]) == rec["survive"], f"{label} config {b}: survive mask differs"
+        w = complex(mant[b, 0], mant[b, 1])
+        om, oe = complex(*rec["mant"]), rec["exp2"]
+        assert om != 0 and 1.0 <= max(abs(w.real), abs(w.imag)) < 2.0
+        d = rel_diff(w, int(exp2[b]), om, oe)
+        tol = TOL * max(1.0, rec["kappa"] * 1e-5)
+        loosened += tol > TOL
+        if "fine" in rec and d > tol:
+            tm, te = complex(*rec["fine"]["mant"]), rec["fine"]["exp2"]
+            d_coarse, d_gpu = rel_diff(om, oe, tm, te), rel_diff(w, int(exp2[b]), tm, te)
+            assert d_gpu <= max(TOL, 10.0 * d_coarse), f"{label} config {b}: gpu {d_gpu:.3e} from the truth, coarse oracle {d_coarse:.3e}"
+            judged_by_truth += 1
+            continue
+        assert d <= tol, f"{label} config {b}: rel diff {d:.3e} > {tol:.1e} (kappa {rec['kappa']:.2e})"
+        worst = max(worst, d)
+    assert loosened <= max(1, len(recs) // 100), f"{label}: {loosened} configurations needed the kappa loosening"
+    print(f"{label}: {len(recs)} outputs against the golden file, worst relative difference {worst:.3e}, "
+          f"{judged_by_truth} judged against the (N,Sz,Lz) truth")
     return worst
 
 
@@ -121,16 +170,25 @@ def test_trace_parity_baseline_configs(cfg, n, lib, torch_cuda, impurities, hand
     print(f"cfg{cfg}: worst relative difference {worst:.3e}")
 
 
-@pytest.mark.parametrize("cfg,n_sample", [(1, 1024), (2, 4096), (3, 48), (4, 12)])
-def test_trace_parity_full_baseline_batch_sampled(cfg, n_sample, lib, torch_cuda, impurities, handles):
-    """BASELINE.json's full batch in the launch configuration bench.py times (configs 1-2: every output; 3-4: evenly spaced
-    samples the oracle can afford; config 5: see test_trace_parity_cfg5_crystal_field)."""
+@pytest.mark.parametrize("cfg", [1, 2])
+def test_trace_parity_full_baseline_batch(cfg, lib, torch_cuda, impurities, handles):
+    """BASELINE.json's full batch in the launch configuration bench.py times, EVERY output against the oracle run here
+    (configs 1-2); configs 3-5: test_trace_parity_full_baseline_batch_golden."""
     from workloads import BASELINE_CONFIGS, make_batch
     B = BASELINE_CONFIGS[cfg]["batch"]
-    batch = make_batch(cfg, B)
-    sample = list(range(B)) if n_sample >= B else [int(i * B / n_sample) for i in range(n_sample)]
-    worst = _check_trace(lib, torch_cuda, impurities(cfg), handles(cfg), batch, f"cfg{cfg}-full", sample=sample)
-    print(f"cfg{cfg} full batch {B}, {len(sample)} outputs checked: worst relative difference {worst:.3e}")
+    worst = _check_trace(lib, torch_cuda, impurities(cfg), handles(cfg), make_batch(cfg, B), f"cfg{cfg}-full")
+    print(f"cfg{cfg} full batch {B}, every output checked: worst relative difference {worst:.3e}")
+
+
+@pytest.mark.parametrize("cfg", [3, 4])
+def test_trace_parity_full_baseline_batch_golden(cfg, lib, torch_cuda, impurities, handles):
+    """BASELINE.json's full batches of configs 3 (1024) and 4 (256) in the launch configuration bench.py times: EVERY output
+    against the oracle values stored by tests/golden/make_golden.py; config 5: test_trace_parity_cfg5_*."""
+    from workloads import BASELINE_CONFIGS, make_batch
+    doc = _load_golden(cfg)
+    B = BASELINE_CONFIGS[cfg]["batch"]
+    assert doc["batch"] == B and len(doc["records"]) == B
+    _check_trace_golden(lib, torch_cuda, handles(cfg), make_batch(cfg, B), doc, f"cfg{cfg}-full")
 
 
 @pytest.mark.parametrize("cfg,n", [(1, 64), (2, 64), (3, 6), (4, 2)])
@@ -417,16 +475,22 @@ def test_large_path_edge_cases(lib, torch_cuda, impurities, handles):
 
 
 def test_trace_parity_cfg5_crystal_field(lib, torch_cuda, impurities):
-    """BASELINE config 5 (sectors 1001 / 2002 / 3003, complex): one full configuration against the oracle (about 1e13 flop
-    of numpy matmul on the host), thin schedule, at the launch configuration bench.py times."""
+    """BASELINE config 5 (sectors 1001 / 2002 / 3003, complex), the config north_star's tensor-pipe target is stated on: the
+    full batch of 64 at the launch configuration bench.py times (thin schedule), EVERY output against the stored oracle
+    values (tests/golden/cfg5_batch64.json: 1.1e13 flop of numpy each, computed once by tests/golden/make_golden.py); then
+    the literal schedule of Eq. 65 on the first 6, which must agree with the same file; then the S = 1 Frobenius bound."""
     from workloads import make_batch
+    doc = _load_golden(5)
+    assert doc["batch"] == 64 and len(doc["records"]) == 64
     imp = impurities(5)
     h = lib.ctqmc_load_impurity(imp, 0)
     try:
         assert lib.ctqmc_last_stats(h)["path"] == lib.CTQMC_PATH_LARGE
-        worst = _check_trace(lib, torch_cuda, imp, h, make_batch(5, 64), "cfg5", sample=[0])   # full BASELINE batch on the GPU
-        print(f"cfg5: worst relative difference {worst:.3e}")
-        _check_bound(lib, torch_cuda, imp, h, make_batch(5, 1), 0, 1, "cfg5-frobenius-S1")
+        _check_trace_golden(lib, torch_cuda, h, make_batch(5, 64), doc, "cfg5-thin")
+        lib.ctqmc_set_option(h, lib.CTQMC_OPT_SCHEDULE, lib.CTQMC_SCHEDULE_LITERAL)
+        _check_trace_golden(lib, torch_cuda, h, make_batch(5, 6), doc, "cfg5-literal", records=doc["records"][:6])
+        lib.ctqmc_set_option(h, lib.CTQMC_OPT_SCHEDULE, lib.CTQMC_SCHEDULE_THIN)
+        _check_bound(lib, torch_cuda, imp, h, make_batch(5, 1), 0, 1, "cfg5-frobenius-S1", golden=doc)
     finally:
         h.free()
 
@@ -593,7 +657,13 @@ def test_repeatable_and_stream_ordered(lib, torch_cuda, impurities, handles):
 
 
 # --------------------------------------------------------------------------- bounds
-def _check_bound(lib, torch, imp, handle, batch, norm_kind, S, label):
+def _check_bound(lib, torch, imp, handle, batch, norm_kind, S, label, golden=None):
+    """Bounds against the oracle's (1e-9), and against the traces they bound: per configuration (GPU trace) and per start
+    sector (the oracle's t(q0): the lazy trace consumes per-sector bounds).  Segment products (S != 1): where a
+    start sector's product vanishes by a symmetry the sector labels do not resolve, fl(G) is rounding noise on both sides and
+    its norm has no digits; such a sector's bound is 2^-45 ... 2^-53 of the configuration's.  So a per-sector bound must match
+    to 1e-9 relative OR to 2^-40 of the configuration's bound in absolute terms; the configuration's
+    bound itself always to 1e-9.  `golden`: stored oracle traces (config 5: the oracle takes a minute per configuration)."""
     from oracle import trace_oracle as O
     off, sym, tau = _dev(torch, batch)
     bm, be, sm, se, status = lib.ctqmc_bound_batch(handle, batch.beta, off, sym, tau, norm_kind, S)
@@ -610,16 +680,22 @@ def _check_bound(lib, torch, imp, handle, batch, norm_kind, S, label):
             continue
         d = rel_diff(bm[b], int(be[b]), r["mant"], r["exp2"])
         assert d <= TOL, f"{label} config {b}: bound rel diff {d:.3e}"
+        if golden is not None:
+            tsec = {q0: (complex(re, im), e) for q0, re, im, e in golden["records"][b]["sector"]}
+        else:
+            tsec = {q0: se_ for q0, se_ in enumerate(O.trace_config(imp, batch.beta, s, t)["sector"]) if se_ is not None}
         for q0, sec in enumerate(r["sector"]):
             if sec is None:
                 assert sm[b, q0] == 0.0 and se[b, q0] == 0
+                continue
+            if sec[0] == 0:
+                assert sm[b, q0] == 0.0
             else:
+                floor_q = 0.0 if S == 1 else r["mant"] * 2.0 ** max(-300, min(300, r["exp2"] - sec[1] - 40)) / sec[0]
                 dq = rel_diff(sm[b, q0], int(se[b, q0]), sec[0], sec[1])
-                # DESIGN.md reading A8 for bounds: a start sector whose bound is more than 2^-40 below the
-                # configuration's bound may be rounding-noise limited (segment products lose Delta (E - Emin) >> 36
-                # decades against the factor norms); it is checked to a factor 2 there, to 1e-9 otherwise.
-                negligible = sec[0] == 0 or (sec[1] - r["exp2"]) < -40
-                assert dq <= (1.0 if negligible else TOL), f"{label} config {b} sector {q0}: rel diff {dq:.3e}"
+                assert dq <= TOL + floor_q, f"{label} config {b} sector {q0}: rel diff {dq:.3e} (rounding floor {floor_q:.1e})"
+            zs, es = tsec[q0]
+            assert scaled_ge(sm[b, q0], int(se[b, q0]), abs(zs), es), f"{label} config {b} sector {q0}: B(q0) < |t(q0)|"
         w = abs(complex(mant[b, 0], mant[b, 1]))
         assert scaled_ge(bm[b], int(be[b]), w, int(exp2[b])), f"{label} config {b}: bound < |trace|"
 
