@@ -47,15 +47,22 @@ extern "C" {
 #define CTQMC_OPT_PANEL_WIDTH  2   /* columns carried per work unit: 8, 16, 32 (0 = automatic) */
 #define CTQMC_OPT_TIMING       3   /* 1: record CUDA events around the phases of every batch call (see ctqmc_last_timing) */
 #define CTQMC_OPT_PATH         4   /* which chain kernel family runs (CTQMC_PATH_*); results agree up to rounding */
-#define CTQMC_OPT_SCRATCH_LIMIT 5  /* bytes the grouped path may allocate for its schedule and carried matrices (0 = no limit).
-                                      Above it, or when the allocation fails, AUTO falls back to the panel kernel and an explicit
-                                      CTQMC_PATH_GROUPED request returns CTQMC_ERR_OOM */
+#define CTQMC_OPT_SCRATCH_LIMIT 5  /* upper limit in bytes for the AUTOMATIC growth of the scratch arena (0 = 80 % of the free device
+                                      memory).  A batch whose scratch exceeds the arena is evaluated in rounds of configurations;
+                                      if not even one configuration fits, AUTO falls back from the grouped to the panel kernel and
+                                      an explicit CTQMC_PATH_GROUPED request returns CTQMC_ERR_OOM */
+#define CTQMC_OPT_ARENA_BYTES  6   /* allocate the scratch arena NOW with exactly this many bytes and never grow it (0 = back to
+                                      automatic growth).  PAPER.md:574: "we pre-allocate ... and develop our own memory allocator
+                                      which can work asynchronously with that block": after this call no batch call allocates,
+                                      frees or synchronises; a batch that does not fit is cut into rounds, and CTQMC_ERR_OOM is
+                                      returned BEFORE anything is enqueued if one configuration alone does not fit */
 
 /* Kernel families for CTQMC_OPT_PATH.  AUTO: the small-sector kernel (whole path in one launch, operator store in shared
  * memory) when every sector has at most 16 states; else, when a panel of the largest sector fits in shared memory, the
  * step-synchronous grouped GEMM kernel for batches of 64 configurations or more and the persistent shared-memory panel
- * kernel for smaller ones; else the large-sector tiled GEMM kernel (one launch per chain position).  The grouped and the large path read the
- * routing counters back from the device before enqueueing their step loop, so those calls are not fully asynchronous.
+ * kernel for smaller ones; else the large-sector tiled GEMM kernel (one launch per chain position).  Every path only enqueues:
+ * scratch and launch shapes are sized on the host from upper bounds it knows (n_configs, n_ops, max_len, the sector dimensions),
+ * the actual counts stay on the device.
  * ctqmc_bound_batch: segment_len 1 uses tables only (one fused launch for small real impurities); other segment lengths run
  * the panel kernel family, or the large-sector one when the sectors do not fit in shared memory. */
 #define CTQMC_PATH_AUTO        0
@@ -99,8 +106,15 @@ typedef struct {
 typedef struct {
   int64_t        n_configs;    /* B >= 0 */
   const int64_t* offset;       /* [B+1], offset[0] = 0, non-decreasing */
-  const int32_t* symbol;       /* [offset[B]] */
-  const double*  tau;          /* [offset[B]] */
+  const int32_t* symbol;       /* [n_ops] */
+  const double*  tau;          /* [n_ops] */
+  int64_t        n_ops;        /* HOST value: length of symbol / tau (= offset[B]).  The device forms cannot read offset[B] without
+                                  waiting for the device, so the caller states it; a configuration whose offsets leave [0, n_ops]
+                                  gets status 2 instead of an out-of-bounds read.  Host forms: 0 = take offset[B] */
+  int32_t        max_len;      /* HOST value: no configuration has more than this many operators (sizes the per-chain-position
+                                  launch loops and the scratch); longer configurations get status 2.  0 = unknown: the library
+                                  falls back to n_ops, which is correct but enqueues one step per operator of the WHOLE batch --
+                                  state it.  Host forms compute it from the offsets */
 } ctqmc_batch;
 
 /* Load an impurity onto CUDA device `device`: copies dims / energies, builds the routing table s_alpha(q), the padded
@@ -117,8 +131,9 @@ int ctqmc_set_option(ctqmc_impurity* imp, int option, int64_t value);
 /*
  * Evaluate w_loc (Eq. 65) for every configuration of the batch.  `batch` fields and all outputs are DEVICE pointers.
  * The call only enqueues work on `cuda_stream` (a cudaStream_t, NULL = default stream) and returns; outputs are valid
- * once the stream reaches that point.  The scratch arena is (re)allocated before enqueueing if the batch needs more
- * than any previous call did (allocation synchronises the device, hence it never happens mid-call).
+ * once the stream reaches that point; it never waits for the device and never reads anything back.  The scratch arena is one
+ * device block: with CTQMC_OPT_ARENA_BYTES it is fixed and no call ever allocates; otherwise it grows -- before anything is
+ * enqueued, and only when a call needs more than every earlier one (allocation synchronises the device).
  *
  *   mant    [B][2]  (re, im) mantissa; im = 0 for real impurities; max(|re|,|im|) in [1,2), or (0,0) for an exact zero,
  *                   or (NaN, NaN) for status 2
@@ -166,14 +181,15 @@ int ctqmc_bound_batch_host(ctqmc_impurity* imp, double beta, const ctqmc_batch* 
                            double* bound_mant, int64_t* bound_exp2, double* sector_bound_mant, int64_t* sector_bound_exp2,
                            int32_t* status, void* cuda_stream);
 
-/* Counters of the most recent batch call on this handle (HOST outputs; synchronises the stream it ran on):
+/* Counters of the most recent batch call on this handle, summed over its rounds and (host form) chunks (HOST outputs;
+ * synchronises the stream it ran on):
  * stats[0] = surviving strings, stats[1] = work units, stats[2] = kernels launched by the call,
  * stats[3] = real multiply-adds executed by the chain kernel (padded tiles included),
  * stats[4] = algorithmic real flops of the schedule executed (2 per real MAC, 8 per complex MAC, unpadded dims),
- * stats[5] = panel width (panel path) or lanes per configuration (small path), stats[6] = warps per team (panel path) or the
- * number of propagator exponentials evaluated (small path: sum over chain steps of the sector dimension),
- * stats[7] = kernel family that ran (CTQMC_PATH_PANEL / _LARGE / _SMALL). */
-int ctqmc_last_stats(ctqmc_impurity* imp, int64_t stats[8]);
+ * stats[5] = panel width (panel path) or lanes per configuration (small path), stats[6] = warps per team (panel path),
+ * stats[7] = kernel family that ran (CTQMC_PATH_*), stats[8] = propagator exponentials evaluated (small path: sum over chain
+ * steps of the sector dimension), stats[9] = bytes of the scratch arena. */
+int ctqmc_last_stats(ctqmc_impurity* imp, int64_t stats[10]);
 
 /* With CTQMC_OPT_TIMING = 1: device time in milliseconds of the phases of the most recent batch call on this handle,
  * from CUDA events recorded on the call's stream (HOST output; synchronises that stream):

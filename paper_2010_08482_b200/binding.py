@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(HERE, "libctqmc_b200.so")
 CTQMC_OK, CTQMC_ERR_ARG, CTQMC_ERR_OOM, CTQMC_ERR_CUDA, CTQMC_ERR_UNSUPPORTED = 0, -1, -2, -3, -4
 CTQMC_STATUS_OK, CTQMC_STATUS_VANISHING, CTQMC_STATUS_INVALID = 0, 1, 2
 CTQMC_SCHEDULE_THIN, CTQMC_SCHEDULE_LITERAL = 0, 1
-CTQMC_OPT_SCHEDULE, CTQMC_OPT_PANEL_WIDTH, CTQMC_OPT_TIMING, CTQMC_OPT_PATH, CTQMC_OPT_SCRATCH_LIMIT = 1, 2, 3, 4, 5
+CTQMC_OPT_SCHEDULE, CTQMC_OPT_PANEL_WIDTH, CTQMC_OPT_TIMING, CTQMC_OPT_PATH, CTQMC_OPT_SCRATCH_LIMIT, CTQMC_OPT_ARENA_BYTES = 1, 2, 3, 4, 5, 6
 CTQMC_PATH_AUTO, CTQMC_PATH_PANEL, CTQMC_PATH_LARGE, CTQMC_PATH_SMALL, CTQMC_PATH_GROUPED = 0, 1, 2, 3, 4
 
 EXPORTS = ["ctqmc_load_impurity", "ctqmc_free_impurity", "ctqmc_set_option", "ctqmc_trace_batch", "ctqmc_bound_batch",
@@ -38,7 +38,8 @@ class _Desc(C.Structure):
 
 
 class _Batch(C.Structure):
-    _fields_ = [("n_configs", C.c_int64), ("offset", C.c_void_p), ("symbol", C.c_void_p), ("tau", C.c_void_p)]
+    _fields_ = [("n_configs", C.c_int64), ("offset", C.c_void_p), ("symbol", C.c_void_p), ("tau", C.c_void_p),
+                ("n_ops", C.c_int64), ("max_len", C.c_int32)]
 
 
 _lib = None
@@ -67,7 +68,7 @@ def library() -> C.CDLL:
             fn = getattr(lib, name)
             fn.argtypes = [vp, dbl, C.POINTER(_Batch), C.c_int, C.c_int, vp, vp, vp, vp, vp, vp]
             fn.restype = C.c_int
-        lib.ctqmc_last_stats.argtypes = [vp, C.POINTER(i64 * 8)]
+        lib.ctqmc_last_stats.argtypes = [vp, C.POINTER(i64 * 10)]
         lib.ctqmc_last_stats.restype = C.c_int
         lib.ctqmc_last_timing.argtypes = [vp, C.POINTER(dbl * 4)]
         lib.ctqmc_last_timing.restype = C.c_int
@@ -144,10 +145,9 @@ def ctqmc_set_option(imp: ImpurityHandle, option: int, value: int):
 
 
 def ctqmc_last_stats(imp: ImpurityHandle) -> dict:
-    buf = (C.c_int64 * 8)()
+    buf = (C.c_int64 * 10)()
     _check(library().ctqmc_last_stats(imp.ptr, C.byref(buf)))
-    # "team_warps" is the number of propagator exponentials evaluated when path == CTQMC_PATH_SMALL (include/ctqmc.h)
-    keys = ["strings", "units", "launches", "macs", "alg_flops", "panel_width", "team_warps", "path"]
+    keys = ["strings", "units", "launches", "macs", "alg_flops", "panel_width", "team_warps", "path", "n_exp", "arena_bytes"]
     return dict(zip(keys, [int(x) for x in buf]))
 
 
@@ -172,16 +172,21 @@ def _stream_ptr(stream, host: bool = False):
     return C.c_void_p(int(stream.cuda_stream))
 
 
-def _dev_batch(offset, symbol, tau):
+def _dev_batch(offset, symbol, tau, max_len):
+    """n_ops is the length of the symbol tensor (host-known).  max_len: the caller's bound on the longest configuration; a
+    caller that does not state it pays one device read here, in the binding (the C call itself never waits for the device)."""
     import torch
     assert offset.is_cuda and offset.dtype == torch.int64 and offset.is_contiguous()
     assert symbol.is_cuda and symbol.dtype == torch.int32 and symbol.is_contiguous()
-    assert tau.is_cuda and tau.dtype == torch.float64 and tau.is_contiguous()
-    return _Batch(offset.numel() - 1, offset.data_ptr(), symbol.data_ptr(), tau.data_ptr())
+    assert tau.is_cuda and tau.dtype == torch.float64 and tau.is_contiguous() and tau.numel() == symbol.numel()
+    if max_len is None:
+        max_len = int((offset[1:] - offset[:-1]).max().item()) if offset.numel() > 1 else 0
+        max_len = max(max_len, 1)
+    return _Batch(offset.numel() - 1, offset.data_ptr(), symbol.data_ptr(), tau.data_ptr(), symbol.numel(), int(max_len))
 
 
 def ctqmc_trace_batch(imp: ImpurityHandle, beta: float, offset, symbol, tau, want_survive: bool = True, stream=None,
-                      out=None):
+                      out=None, max_len=None):
     """Device form.  offset int64[B+1], symbol int32[n], tau float64[n]: torch CUDA tensors.  Returns torch CUDA
     tensors (mant[B,2], exp2[B], survive[B,Q] or None, status[B]); asynchronous on `stream` (default: current)."""
     import torch
@@ -194,7 +199,7 @@ def ctqmc_trace_batch(imp: ImpurityHandle, beta: float, offset, symbol, tau, wan
         status = torch.empty(B, dtype=torch.int32, device=dev)
     else:
         mant, exp2, surv, status = out
-    b = _dev_batch(offset, symbol, tau)
+    b = _dev_batch(offset, symbol, tau, max_len)
     _check(library().ctqmc_trace_batch(imp.ptr, float(beta), C.byref(b), mant.data_ptr(), exp2.data_ptr(),
                                        surv.data_ptr() if surv is not None else None, status.data_ptr(),
                                        _stream_ptr(stream)))
@@ -202,7 +207,7 @@ def ctqmc_trace_batch(imp: ImpurityHandle, beta: float, offset, symbol, tau, wan
 
 
 def ctqmc_bound_batch(imp: ImpurityHandle, beta: float, offset, symbol, tau, norm_kind: int = 0, segment_len: int = 1,
-                      want_sector: bool = True, stream=None):
+                      want_sector: bool = True, stream=None, max_len=None):
     """Device form.  Returns (bound_mant[B], bound_exp2[B], sector_mant[B,Q] | None, sector_exp2[B,Q] | None, status[B])."""
     import torch
     B = offset.numel() - 1
@@ -212,7 +217,7 @@ def ctqmc_bound_batch(imp: ImpurityHandle, beta: float, offset, symbol, tau, nor
     sm = torch.empty((B, imp.n_sectors), dtype=torch.float64, device=dev) if want_sector else None
     se = torch.empty((B, imp.n_sectors), dtype=torch.int64, device=dev) if want_sector else None
     status = torch.empty(B, dtype=torch.int32, device=dev)
-    b = _dev_batch(offset, symbol, tau)
+    b = _dev_batch(offset, symbol, tau, max_len)
     _check(library().ctqmc_bound_batch(imp.ptr, float(beta), C.byref(b), int(norm_kind), int(segment_len),
                                        bm.data_ptr(), be.data_ptr(), sm.data_ptr() if want_sector else None,
                                        se.data_ptr() if want_sector else None, status.data_ptr(), _stream_ptr(stream)))
@@ -223,7 +228,7 @@ def _host_batch(offset, symbol, tau):
     offset, symbol, tau = _np(offset, np.int64), _np(symbol, np.int32), _np(tau, np.float64)
     keep = (offset, symbol, tau)
     return _Batch(len(offset) - 1, offset.ctypes.data, symbol.ctypes.data if len(symbol) else None,
-                  tau.ctypes.data if len(tau) else None), keep
+                  tau.ctypes.data if len(tau) else None, len(symbol), 0), keep
 
 
 def ctqmc_trace_batch_host(imp: ImpurityHandle, beta: float, offset, symbol, tau, want_survive: bool = True,

@@ -41,7 +41,8 @@ struct GroupedParams {
   BatchView bv;
   const StringRec* strings;
   const int2* units;
-  int n_units, Lmax, ldx, nb;
+  const Counters* cnt;       // cnt->n_slots = number of units (device-side; the host sizes everything by upper bounds)
+  int Lmax, ldx, nb;
   long long xtot;            // elements per parity buffer
   double* X;                 // [2][xtot] elements
   long long* xoff;           // [n_units] element offset of the unit's carried matrix
@@ -55,6 +56,7 @@ struct GroupedParams {
   int* colbase;              // [Lmax][nb]
   int4* tiles;               // [Lmax][tile_cap] {block, first column, columns, -}
   int* ntiles;               // [Lmax]
+  int* tilecur;              // [Lmax] next (tile, row slab) of the step: the persistent step kernel's work counter
   int2* colmap;              // [Lmax][col_cap] (unit, column of the unit)
   int tile_cap;
   long long col_cap;
@@ -64,7 +66,7 @@ struct GroupedParams {
 // One thread per unit: sector walk in multiplication order, per-unit sizes.
 __global__ void grouped_plan_kernel(GroupedParams P) {
   const int u = blockIdx.x * blockDim.x + threadIdx.x;
-  if (u >= P.n_units) return;
+  if (u >= (int)P.cnt->n_slots) return;
   const int2 un = P.units[u];
   const StringRec sr = P.strings[un.x];
   const int Q = P.imp.Q;
@@ -91,11 +93,12 @@ __global__ void grouped_plan_kernel(GroupedParams P) {
 __global__ void grouped_xoff_kernel(GroupedParams P) {
   __shared__ long long s_part[1024];
   __shared__ long long s_run;
+  const int n_units = (int)P.cnt->n_slots;
   if (threadIdx.x == 0) s_run = 0;
   __syncthreads();
-  for (int base = 0; base < P.n_units; base += 1024) {
+  for (int base = 0; base < n_units; base += 1024) {
     const int u = base + threadIdx.x;
-    const long long v = (u < P.n_units) ? (long long)P.ucols[u] * P.ldx : 0;
+    const long long v = (u < n_units) ? (long long)P.ucols[u] * P.ldx : 0;
     s_part[threadIdx.x] = v;
     __syncthreads();
     for (int o = 1; o < 1024; o <<= 1) {
@@ -104,7 +107,7 @@ __global__ void grouped_xoff_kernel(GroupedParams P) {
       s_part[threadIdx.x] += add;
       __syncthreads();
     }
-    if (u < P.n_units) P.xoff[u] = s_run + s_part[threadIdx.x] - v;
+    if (u < n_units) P.xoff[u] = s_run + s_part[threadIdx.x] - v;
     __syncthreads();
     if (threadIdx.x == 0) s_run += s_part[1023];
     __syncthreads();
@@ -114,7 +117,7 @@ __global__ void grouped_xoff_kernel(GroupedParams P) {
 // Schedule, pass 1: columns per (chain position, block); each unit reserves its column range inside the group.
 __global__ void grouped_count_kernel(GroupedParams P) {
   const long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-  if (idx >= (long long)P.n_units * P.Lmax) return;
+  if (idx >= (long long)P.cnt->n_slots * P.Lmax) return;
   const int u = (int)(idx / P.Lmax), j = (int)(idx - (long long)u * P.Lmax);
   if (j >= P.ulen[u]) return;
   const int blk = P.plan_blk[idx];
@@ -142,7 +145,7 @@ __global__ void grouped_tiles_kernel(GroupedParams P) {
 // Schedule, pass 3: column -> (unit, column of the unit).
 __global__ void grouped_fill_kernel(GroupedParams P) {
   const long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-  if (idx >= (long long)P.n_units * P.Lmax) return;
+  if (idx >= (long long)P.cnt->n_slots * P.Lmax) return;
   const int u = (int)(idx / P.Lmax), j = (int)(idx - (long long)u * P.Lmax);
   if (j >= P.ulen[u]) return;
   const int blk = P.plan_blk[idx];
@@ -155,19 +158,30 @@ __global__ void grouped_fill_kernel(GroupedParams P) {
 template <bool CPLX>
 __global__ void grouped_init_kernel(GroupedParams P) {
   constexpr int ES = CPLX ? 2 : 1;
-  const int u = blockIdx.x;
-  const int c = P.ucols[u];
-  double* X = P.X + P.xoff[u] * ES;
-  const int dpad = round_up(c, 2);
-  for (int idx = threadIdx.x; idx < c * dpad; idx += blockDim.x) {
-    const int col = idx / dpad, k = idx - col * dpad;
-    const double v = (k == col) ? 1.0 : 0.0;
-    if constexpr (CPLX) *reinterpret_cast<double2*>(X + ((size_t)col * P.ldx + k) * 2) = make_double2(v, 0.0);
-    else X[(size_t)col * P.ldx + k] = v;
+  const int n_units = (int)P.cnt->n_slots;
+  // whole columns (ldx rows) of BOTH parity buffers: rows beyond the current sector's dimension are read (and multiplied by
+  // an exact 0 or by zero padding of F) by later steps, so they must be finite whatever the shared arena held before
+  for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
+    const int c = P.ucols[u];
+    double* X0 = P.X + P.xoff[u] * ES;
+    double* X1 = X0 + P.xtot * ES;
+    for (int idx = threadIdx.x; idx < c * P.ldx; idx += blockDim.x) {
+      const int col = idx / P.ldx, k = idx - col * P.ldx;
+      const double v = (k == col) ? 1.0 : 0.0;
+      if constexpr (CPLX) {
+        *reinterpret_cast<double2*>(X0 + ((size_t)col * P.ldx + k) * 2) = make_double2(v, 0.0);
+        *reinterpret_cast<double2*>(X1 + ((size_t)col * P.ldx + k) * 2) = make_double2(0.0, 0.0);
+      } else {
+        X0[(size_t)col * P.ldx + k] = v;
+        X1[(size_t)col * P.ldx + k] = 0.0;
+      }
+    }
   }
 }
 
-// One chain position for every string: blockIdx.x = (tile of the step's tile list, 64-row slab of F).
+// One chain position for every string.  Work item = (tile of the step's tile list, 64-row slab of F); the number of items is
+// known on the device only (the host sizes the launch by an upper bound and never reads a counter back), so the grid is
+// persistent: a few CTAs per SM pull items from an atomic counter, heaviest tiles first.
 template <bool CPLX>
 __global__ void __launch_bounds__(kGThreads, (kGWN == 2 && !CPLX) ? 3 : 2) grouped_step_kernel(GroupedParams P, int j, int MTmax) {
   constexpr int ES = CPLX ? 2 : 1;
@@ -178,23 +192,36 @@ __global__ void __launch_bounds__(kGThreads, (kGWN == 2 && !CPLX) ? 3 : 2) group
   __shared__ double s_dprev[kGBN], s_delta[kGBN];
   __shared__ int s_kprev[kGBN], s_u[kGBN], s_kmax[kGBN];
   __shared__ __align__(8) unsigned long long g_full[kGStages], g_empty[kGStages];
+  __shared__ int s_item;
   double* sde = reinterpret_cast<double*>(gsm + kGStages * kGStageBytes);   // E[k] - Emin of the source sector
 
   // Programmatic dependent launch: the next chain position's grid may start as soon as every CTA of this one is resident, so
   // its CTAs fill the SM slots this launch's tail leaves empty and run their prologue (tile list, column map, barrier
   // set-up: nothing a previous step writes) there; they wait (griddepcontrol.wait, below) before touching the carried matrices.
   asm volatile("griddepcontrol.launch_dependents;");
-  const int tile_id = blockIdx.x / MTmax, slab = blockIdx.x - tile_id * MTmax;   // slabs of a tile are neighbours in launch order
-  if (tile_id >= P.ntiles[j]) return;
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int g = lane >> 2, t = lane & 3;
+  const int wm = warp / kGWN, wn = warp % kGWN;
+  if (tid == 0) {
+#pragma unroll
+    for (int st = 0; st < kGStages; ++st) { mbar_init(&g_full[st], kGThreads); mbar_init(&g_empty[st], kGThreads / 32); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  const int n_items = P.ntiles[j] * MTmax;
+  unsigned gk = 0;          // k-tiles this CTA has pushed through the ring so far: slot = gk % stages, phase = (gk / stages) & 1
+  bool waited = false;
+  for (;;) {
+  __syncthreads();          // everybody is done with the previous item's shared arrays
+  if (tid == 0) s_item = atomicAdd(&P.tilecur[j], 1);
+  __syncthreads();
+  const int item = s_item;
+  if (item >= n_items) break;
+  const int tile_id = item / MTmax, slab = item - tile_id * MTmax;   // slabs of a tile are neighbours: F rows stay in L2
   const int4 tl = P.tiles[(size_t)j * P.tile_cap + tile_id];
   const BlkDesc bd = P.imp.blks[tl.x];
   const int dn = bd.rows, d = bd.cols, ncols = tl.z;
   const int m0 = slab * kGBM;
-  if (m0 >= dn) return;
-
-  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int g = lane >> 2, t = lane & 3;
-  const int wm = warp / kGWN, wn = warp % kGWN;
+  if (m0 >= dn) continue;
   const int nkt = (d + BKE - 1) / BKE;
   // 8-row / 8-column blocks are dealt to the warps round-robin, and blocks that are all padding are skipped: the tensor
   // work is quantised to 8 x 8 although the CTA stages 64 x 64 tiles
@@ -202,17 +229,12 @@ __global__ void __launch_bounds__(kGThreads, (kGWN == 2 && !CPLX) ? 3 : 2) group
   const int ntu = ((ncols + 7) / 8 - wn + kGWN - 1) / kGWN;
   const size_t par_in = (size_t)(j & 1) * P.xtot, par_out = (size_t)((j + 1) & 1) * P.xtot;
 
-  if (tid == 0) {
-#pragma unroll
-    for (int st = 0; st < kGStages; ++st) { mbar_init(&g_full[st], kGThreads); mbar_init(&g_empty[st], kGThreads / 32); }
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-  }
   {   // source-sector energies: static data, still before the wait
     const double* Eq = P.imp.energy + P.imp.e_off[bd.src];
     const double emin = P.imp.e_min[bd.src];
     for (int k = tid; k < nkt * BKE; k += kGThreads) sde[k] = (k < d) ? __dsub_rn(Eq[k], emin) : 0.0;
   }
-  asm volatile("griddepcontrol.wait;" ::: "memory");   // the previous chain position is complete and its writes are visible
+  if (!waited) { asm volatile("griddepcontrol.wait;" ::: "memory"); waited = true; }   // the previous chain position is complete and its writes are visible
   if (tid < kGBN) {
     const int n = tid;
     if (n < ncols) {
@@ -285,19 +307,26 @@ __global__ void __launch_bounds__(kGThreads, (kGWN == 2 && !CPLX) ? 3 : 2) group
     constexpr int kAhead = kGStages - 2;
   #pragma unroll
     for (int st = 0; st < kAhead; ++st)
-      if (st < nkt) { load_stage(st, st); cp_async_arrive(&g_full[st]); }
+      if (st < nkt) {
+        const unsigned n = gk + st;
+        if (n >= kGStages) mbar_wait(&g_empty[n % kGStages], ((n / kGStages) - 1) & 1);
+        load_stage(st, n % kGStages);
+        cp_async_arrive(&g_full[n % kGStages]);
+      }
     const int swz = (g & 1) << 2;
     for (int kt = 0; kt < nkt; ++kt) {
       {
         const int nx = kt + kAhead;
         if (nx < nkt) {
-          if (nx >= kGStages) mbar_wait(&g_empty[nx % kGStages], ((nx / kGStages) - 1) & 1);
-          load_stage(nx, nx % kGStages);
-          cp_async_arrive(&g_full[nx % kGStages]);
+          const unsigned n = gk + nx;
+          if (n >= kGStages) mbar_wait(&g_empty[n % kGStages], ((n / kGStages) - 1) & 1);
+          load_stage(nx, n % kGStages);
+          cp_async_arrive(&g_full[n % kGStages]);
         }
       }
-      mbar_wait(&g_full[kt % kGStages], (kt / kGStages) & 1);
-      const unsigned char* As = gsm + (kt % kGStages) * kGStageBytes;
+      const unsigned nc = gk + kt;
+      mbar_wait(&g_full[nc % kGStages], (nc / kGStages) & 1);
+      const unsigned char* As = gsm + (nc % kGStages) * kGStageBytes;
       const unsigned char* Bs = As + kGBM * 128;
   #pragma unroll
       for (int sub = 0; sub < 2; ++sub) {
@@ -353,7 +382,7 @@ __global__ void __launch_bounds__(kGThreads, (kGWN == 2 && !CPLX) ? 3 : 2) group
         }
       }
       __syncwarp();
-      if (lane == 0) mbar_arrive(&g_empty[kt % kGStages]);
+      if (lane == 0) mbar_arrive(&g_empty[nc % kGStages]);
     }
   };
 #define CTQMC_GD(M, N) case (M) * 8 + (N): mainloop(std::integral_constant<int, M>{}, std::integral_constant<int, N>{}); break;
@@ -368,6 +397,7 @@ __global__ void __launch_bounds__(kGThreads, (kGWN == 2 && !CPLX) ? 3 : 2) group
     default: mainloop(std::integral_constant<int, 0>{}, std::integral_constant<int, 0>{}); break;
   }
 #undef CTQMC_GD
+  gk += nkt;
 
   // ---- epilogue: per (row, string) propagator mantissa, scatter to the strings' matrices, largest exponent per column
   const double* E = P.imp.energy + P.imp.e_off[bd.dst];
@@ -432,6 +462,7 @@ __global__ void __launch_bounds__(kGThreads, (kGWN == 2 && !CPLX) ? 3 : 2) group
       if (k != INT_MIN) atomicMax(&P.kmax[(size_t)u * P.Lmax + j], k);
     }
   }
+  }   // item loop
 }
 
 // Trace of each string's final matrix (a5); one CTA per unit.
@@ -440,6 +471,7 @@ __global__ void grouped_finish_kernel(GroupedParams P) {
   constexpr int ES = CPLX ? 2 : 1;
   __shared__ double red[2][8];
   const int u = blockIdx.x;
+  if (u >= (int)P.cnt->n_slots) return;
   const int2 un = P.units[u];
   const StringRec sr = P.strings[un.x];
   const int L = P.ulen[u], c = sr.c, q = sr.q_start;

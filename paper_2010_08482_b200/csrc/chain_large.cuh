@@ -30,12 +30,15 @@ struct LargeParams {
   BatchView bv;
   const StringRec* strings;
   const int2* units;      // unit u -> (string index, 0)
+  const Counters* cnt;    // cnt->n_slots = units that exist (device-side: the host only knows an upper bound)
   long long u0;           // first unit of this group
-  int n_group;            // units in this group
+  int n_group;            // unit slots in this group (host-side upper bound; slots beyond cnt->n_slots stay idle)
   int Lmax;               // plan stride
   int ldx;                // leading dimension (elements) of an X column
-  long long xslab;        // elements per X buffer (one string, one parity)
-  double* X;              // [n_group][2][xslab] elements
+  long long sum_d;        // sum of all sector dimensions (mode 0: column slab of one configuration, per parity)
+  double* X;              // carried matrices: columns of ldx elements; unit s owns columns [u_x[s], u_x[s] + 2 u_w[s])
+  long long* u_x;         // [n_group] first column of the unit's two parity buffers
+  int* u_w;               // [n_group] columns per parity buffer
   int* plan_blk;          // [n_group][Lmax]
   double* plan_delta;     // [n_group][Lmax]
   int* kmax;              // [n_group][Lmax]
@@ -45,7 +48,6 @@ struct LargeParams {
   int mode;               // 0 trace of the whole (rotated) chain, 1 Frobenius norm^2 of one segment per unit
   int segment_len;        // mode 1
   const CUtensorMap* amaps;   // [n_blocks] tensor maps of the operator blocks (TMA variant)
-  const CUtensorMap* xmaps;   // [n_group][2] tensor maps of the carried matrices
   Slot* slots;
 };
 
@@ -53,6 +55,10 @@ struct LargeParams {
 __global__ void large_plan_kernel(LargeParams P) {
   const int s = blockIdx.x * blockDim.x + threadIdx.x;
   if (s >= P.n_group) return;
+  if ((unsigned long long)(P.u0 + s) >= P.cnt->n_slots) {   // idle slot: every later kernel skips it
+    P.u_q[s] = 0; P.u_n[s] = -1; P.u_c[s] = 0; P.u_x[s] = 0; P.u_w[s] = 0;
+    return;
+  }
   const int2 un = P.units[P.u0 + s];
   const StringRec sr = P.strings[un.x];
   const int Q = P.imp.Q;
@@ -69,6 +75,12 @@ __global__ void large_plan_kernel(LargeParams P) {
     c = P.imp.dim[q];
   }
   P.u_q[s] = q; P.u_n[s] = n; P.u_c[s] = c;
+  if (P.mode == 1) { P.u_w[s] = P.imp.dmax; P.u_x[s] = (long long)s * 2 * P.imp.dmax; }
+  else {   // string (b, q0) of the round owns dim(q0) >= c columns per parity at a position the host can compute
+    const int q0 = un.x - (int)(b * Q);
+    P.u_w[s] = P.imp.dim[q0];
+    P.u_x[s] = 2 * (b * P.sum_d + P.imp.e_off[q0]);
+  }
   for (int j = 0; j < n; ++j) {
     int i = i0 + j;
     if (i >= L) i -= L;
@@ -80,19 +92,27 @@ __global__ void large_plan_kernel(LargeParams P) {
   }
 }
 
-// X_0 = identity (c x c, c = dim of the start sector); grid (column blocks, strings).
+// X_0 = identity (c x c, c = dim of the start sector); grid (column blocks, strings).  Whole columns (ldx rows) of BOTH parity
+// buffers are written: rows beyond the current sector's dimension are read by later steps (multiplied by an exact 0), so they
+// must hold finite numbers, and the arena they live in is shared with integer tables of earlier calls.
 template <bool CPLX>
 __global__ void large_init_kernel(LargeParams P) {
   const int s = blockIdx.y;
   const int c = P.u_c[s];
+  if (P.u_n[s] < 0) return;
   constexpr int ES = CPLX ? 2 : 1;
-  double* X = P.X + (size_t)s * 2 * P.xslab * ES;
-  const int dpad = round_up(c, 2);
+  double* X0 = P.X + (size_t)P.u_x[s] * P.ldx * ES;
+  double* X1 = X0 + (size_t)P.u_w[s] * P.ldx * ES;
   for (int col = blockIdx.x; col < c; col += gridDim.x)
-    for (int k = threadIdx.x; k < dpad; k += blockDim.x) {
+    for (int k = threadIdx.x; k < P.ldx; k += blockDim.x) {
       const double v = (k == col) ? 1.0 : 0.0;
-      if constexpr (CPLX) *reinterpret_cast<double2*>(X + ((size_t)col * P.ldx + k) * 2) = make_double2(v, 0.0);
-      else X[(size_t)col * P.ldx + k] = v;
+      if constexpr (CPLX) {
+        *reinterpret_cast<double2*>(X0 + ((size_t)col * P.ldx + k) * 2) = make_double2(v, 0.0);
+        *reinterpret_cast<double2*>(X1 + ((size_t)col * P.ldx + k) * 2) = make_double2(0.0, 0.0);
+      } else {
+        X0[(size_t)col * P.ldx + k] = v;
+        X1[(size_t)col * P.ldx + k] = 0.0;
+      }
     }
 }
 
@@ -134,8 +154,10 @@ __device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* map, u
 
 // One chain position for every string of the group.  blockIdx.x = mt * NTmax + nt (nt fastest: CTAs that share rows of
 // F run together and hit L2), blockIdx.y = string.
+// `xmap`: ONE tensor map over the whole carried-matrix region (2-D: ldx elements x all columns), passed by value; a unit
+// addresses its matrix by its global column index, so no per-string maps have to be built or copied.
 template <bool CPLX, bool TMA>
-__global__ void __launch_bounds__(256, 1) large_step_kernel(LargeParams P, int j, int NTmax) {
+__global__ void __launch_bounds__(256, 1) large_step_kernel(const __grid_constant__ CUtensorMap xmap_all, LargeParams P, int j, int NTmax) {
   constexpr int ES = CPLX ? 2 : 1;
   constexpr int BKE = CPLX ? 8 : 16;       // contraction indices per stage (128-byte rows)
   extern __shared__ __align__(128) unsigned char lsm[];
@@ -154,8 +176,9 @@ __global__ void __launch_bounds__(256, 1) large_step_kernel(LargeParams P, int j
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int g = lane >> 2, t = lane & 3;
   const int wm = warp >> 1, wn = warp & 1;
-  const double* Xin = P.X + ((size_t)s * 2 + (j & 1)) * P.xslab * ES;
-  double* Xout = P.X + ((size_t)s * 2 + ((j + 1) & 1)) * P.xslab * ES;
+  const long long xcol_in = P.u_x[s] + (long long)(j & 1) * P.u_w[s], xcol_out = P.u_x[s] + (long long)((j + 1) & 1) * P.u_w[s];
+  const double* Xin = P.X + (size_t)xcol_in * P.ldx * ES;
+  double* Xout = P.X + (size_t)xcol_out * P.ldx * ES;
   const int nkt = (d + BKE - 1) / BKE;
 
   // exact power-of-two factor per contraction index: row exponent of the previous step minus its largest (a4)
@@ -186,7 +209,8 @@ __global__ void __launch_bounds__(256, 1) large_step_kernel(LargeParams P, int j
   const int ld_chunks = bd.ld * ES / 2;          // 16-byte chunks per row of F (padded with zeros)
   const int x_chunks = CPLX ? d : (d + 1) / 2;   // 16-byte chunks of an X column that hold data
   const CUtensorMap* amap = P.amaps + blk;
-  const CUtensorMap* xmap = P.xmaps + (size_t)s * 2 + (j & 1);
+  const CUtensorMap* xmap = &xmap_all;
+  const int xcol0 = (int)xcol_in + n0;
 
   // cp.async variant: 128-byte rows, 16-byte chunks XOR-swizzled by the row parity.
   // TMA variant: per k-half a dense box of 64-byte rows (two adjacent rows = one 128-byte line, so the 128-bit fragment loads
@@ -199,7 +223,7 @@ __global__ void __launch_bounds__(256, 1) large_step_kernel(LargeParams P, int j
 #pragma unroll
         for (int sub = 0; sub < 2; ++sub) {
           tma_load_2d(As + sub * (kLBM * 64), amap, &full_bar[stage], kt * 16 + sub * 8, m0);
-          tma_load_2d(As + 2 * (kLBM * 64) + sub * (kLBN * 64), xmap, &full_bar[stage], kt * 16 + sub * 8, n0);
+          tma_load_2d(As + 2 * (kLBM * 64) + sub * (kLBN * 64), xmap, &full_bar[stage], kt * 16 + sub * 8, xcol0);
         }
       }
     } else {
@@ -375,6 +399,7 @@ __global__ void large_finish_kernel(LargeParams P) {
   constexpr int ES = CPLX ? 2 : 1;
   __shared__ double red[2][8];
   const int s = blockIdx.x;
+  if (P.u_n[s] < 0) return;   // idle slot
   const int2 un = P.units[P.u0 + s];
   const StringRec sr = P.strings[un.x];
   const int n_steps = P.u_n[s], c = P.u_c[s];
@@ -398,7 +423,7 @@ __global__ void large_finish_kernel(LargeParams P) {
       const double emin = P.imp.e_min[bl.dst];
       const int klast = P.kmax[(size_t)s * P.Lmax + n_steps - 1];
       const double dlast = P.plan_delta[(size_t)s * P.Lmax + n_steps - 1];
-      const double* X = P.X + ((size_t)s * 2 + (n_steps & 1)) * P.xslab * ES;
+      const double* X = P.X + (size_t)(P.u_x[s] + (long long)(n_steps & 1) * P.u_w[s]) * P.ldx * ES;
       if (P.mode == 0) {
         for (int n = threadIdx.x; n < c; n += blockDim.x) {
           const long long sh = (long long)row_exp(prop_x(dlast, E[n], emin)) - (long long)klast;

@@ -89,13 +89,15 @@ __global__ void __launch_bounds__(256) small_trace_kernel(SmallParams P) {
   unsigned long long st_strings = 0, st_flops = 0, st_exp = 0;
   for (long long b = (long long)blockIdx.x * (blockDim.x / G) + grp_in_cta; b < P.bv.B; b += n_groups) {
     const long long lo = P.bv.offset[b];
-    const int L = (int)(P.bv.offset[b + 1] - lo);
+    const long long hi_off = P.bv.offset[b + 1];
+    const bool off_ok = lo >= 0 && hi_off >= lo && hi_off <= P.bv.n_ops && hi_off - lo <= (long long)P.bv.max_len;
+    const int L = off_ok ? (int)(hi_off - lo) : 0;   // corrupt offsets: status 2, and no read through them
     const int* sym = P.bv.symbol + lo;
     const double* tau = P.bv.tau + lo;
     const double beta = P.bv.beta;
 
     // ---- validation (reading A7): symbols in range, tau non-decreasing in [0, beta)
-    bool ok = L >= 0;
+    bool ok = off_ok;
     for (int i = lg; i < L; i += G) {
       const int a = sym[i];
       const double t = tau[i];

@@ -44,6 +44,8 @@ struct BatchView {
   const int* symbol;
   const double* tau;
   double beta;
+  long long n_ops;   // length of symbol / tau as stated by the caller: every offset is checked against it
+  int max_len;       // longest configuration the caller vouches for (sizes the step loops); longer ones are invalid
 };
 
 // One surviving (configuration, start sector) string, written by the routing kernel.

@@ -57,31 +57,42 @@ int upload(T** dst, const std::vector<T>& v) {
   return 0;
 }
 
-struct DevBuf {   // grow-only device buffer
-  void* p = nullptr;
-  size_t cap = 0;
-  bool grew = false;
-};
-
 struct Arena {
-  long long cap_strings = 0, cap_units = 0, cap_configs = 0;
-  int* status = nullptr;
-  uint8_t* survive = nullptr;
-  StringRec* strings = nullptr;
-  int2* units = nullptr;
-  Slot* slots = nullptr;
-  Scaled* sector = nullptr;
-  Counters* cnt = nullptr;
-  // large-sector path: carried matrices (two per string), step plan, per-step largest exponents
-  double* lx = nullptr; size_t lx_bytes = 0;
-  int* plan_blk = nullptr; double* plan_delta = nullptr; int* lkmax = nullptr; size_t plan_cap = 0;
-  DevBuf lunit;   // u_q, u_n, u_c
-  DevBuf xmaps; const void* xmaps_base = nullptr; long long xmaps_g = 0, xmaps_slab = 0; int xmaps_cmax = 0;
-  // grouped path
-  DevBuf gx, gxoff, gplan_blk, gplan_delta, gkmax, gcoff, gulen, gucols, gcolcnt, gcolbase, gtiles, gntiles, gcolmap;
+  // ONE device block, allocated between calls (at the first call that needs it, when a later call needs more and growth is
+  // allowed, or by ctqmc_set_option(CTQMC_OPT_ARENA_BYTES)) and carved up on the host from upper bounds the host knows (B, Q,
+  // n_ops, max_len, sector dimensions): nothing is sized from a device counter, so a batch call never waits for the device
+  // ("only asynchronous CUDA functions ... pre-allocate ... our own memory allocator").
+  char* base = nullptr;
+  size_t cap = 0;
+  size_t fixed_bytes = 0;            // > 0: size set by the caller, never grown
+  Counters* cnt = nullptr;           // counters of the current round
+  Counters* cnt_total = nullptr;     // summed over the rounds of the last call (ctqmc_last_stats)
   // host-variant staging
   void* h_stage = nullptr; size_t h_stage_bytes = 0;
   void* d_stage = nullptr; size_t d_stage_bytes = 0;
+};
+
+enum RoundKind { K_PANEL = 0, K_GROUPED = 1, K_LARGE = 2, K_TABLES = 3 };
+
+// Pointers of one round's scratch inside the arena block.
+struct RoundBuf {
+  int* status; uint8_t* survive; StringRec* strings; Scaled* sector; int2* units; Slot* slots;
+  long long n_units_cap;
+  // large-sector path
+  double* lx; long long lx_cols; int* plan_blk; double* plan_delta; int* lkmax; int* lunit; long long* lux; long long G; int lstride;
+  // grouped path
+  double* gx; long long sum_c_cap; long long* gxoff; int* gplan_blk; double* gplan_delta; int* gkmax; int* gcoff; int* gulen; int* gucols;
+  int* gcolcnt; int* gcolbase; int4* gtiles; int* gntiles; int* gtilecur; int2* gcolmap; int tile_cap;
+};
+
+struct Bump {
+  char* base; size_t off = 0;
+  template <class T> T* take(size_t n) {
+    off = (off + 255) / 256 * 256;
+    T* p = base ? reinterpret_cast<T*>(base + off) : nullptr;
+    off += (n ? n : 1) * sizeof(T);
+    return p;
+  }
 };
 
 }  // namespace
@@ -113,11 +124,13 @@ struct ctqmc_impurity {
   long long scratch_limit = 0;   // bytes the grouped path may use for its schedule and carried matrices (0 = no limit)
   int nt = 0, team_warps = 8, ldx = 0, large = 0, grouped = 0, grouped_ok = 0, grouped_now = 0, last_path = 0;
   size_t grouped_smem = 0;
+  int grouped_ctas_per_sm = 2;
   size_t smem_bytes = 0;
   int grid = 0;
   Arena arena;
   cudaStream_t last_stream = nullptr;
   long long last_launches = 0;
+  int keep_totals = 0;                         // host form, chunked: later chunks add to the first chunk's counters
   int timing = 0, timing_valid = 0;
   cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
   cudaStream_t copy_stream = nullptr;          // host form, pinned inputs: H2D of chunk k+1 overlaps the kernel of chunk k
@@ -259,6 +272,10 @@ int configure(ctqmc_impurity* h, int want_w) {
     if (h->grouped_smem <= smem_max) {
       if (cplx) CU(cudaFuncSetAttribute(grouped_step_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->grouped_smem));
       else      CU(cudaFuncSetAttribute(grouped_step_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->grouped_smem));
+      int occ = 0;
+      if (cplx) CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, grouped_step_kernel<true>, kGThreads, h->grouped_smem));
+      else      CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, grouped_step_kernel<false>, kGThreads, h->grouped_smem));
+      h->grouped_ctas_per_sm = occ > 0 ? occ : 1;
       h->grouped_ok = 1;
     }
     if (h->path == CTQMC_PATH_GROUPED) {
@@ -303,33 +320,117 @@ int configure(ctqmc_impurity* h, int want_w) {
   return 0;
 }
 
-int ensure_arena(ctqmc_impurity* h, long long B, long long units_per_string) {
+long long unit_bound(const ctqmc_impurity* h, int kind, int mode, long long Bs, int Lmax, int S) {
+  const long long nS = Bs * h->dev.Q;
+  if (mode == 2 || kind == K_TABLES) return nS;
+  const long long panels = kind == K_PANEL ? (h->dev.dmax + 8 * h->nt - 1) / (8 * h->nt) : 1;
+  if (mode == 0) return nS * panels;
+  const long long segs = (S >= Lmax) ? 1 : (long long)Lmax / S + 1;   // ceil(L / S) <= Lmax / S + 1 for every L <= Lmax
+  return nS * panels * segs;
+}
+
+// Carves one round's scratch out of `base` (nullptr: size computation only) and returns the bytes used.  Every size is an
+// upper bound computed from host-known numbers; the kernels learn the actual counts from the device-side counters.
+size_t layout_round(const ctqmc_impurity* h, int kind, int mode, long long Bs, int Lmax, int S, long long G, char* base, RoundBuf* rb) {
+  Bump bp{base};
+  RoundBuf r{};
+  const long long Q = h->dev.Q, nS = Bs * Q, nU = unit_bound(h, kind, mode, Bs, Lmax, S);
+  const int es = h->dev.cplx ? 2 : 1;
+  r.status = bp.take<int>(Bs);
+  r.survive = bp.take<uint8_t>(nS);
+  r.strings = bp.take<StringRec>(nS);
+  r.sector = bp.take<Scaled>(nS);
+  r.units = bp.take<int2>(nU);
+  r.slots = bp.take<Slot>(nU);
+  r.n_units_cap = nU;
+  if (kind == K_LARGE) {
+    r.G = mode == 1 ? G : nU;
+    r.lstride = mode == 1 ? (S < Lmax ? S : Lmax) : Lmax;
+    if (r.lstride < 1) r.lstride = 1;
+    r.lx_cols = mode == 1 ? 2 * r.G * h->dev.dmax : 2 * Bs * (long long)h->n_energy;
+    r.lx = bp.take<double>((size_t)r.lx_cols * h->ldx * es);
+    r.plan_blk = bp.take<int>((size_t)r.G * r.lstride);
+    r.plan_delta = bp.take<double>((size_t)r.G * r.lstride);
+    r.lkmax = bp.take<int>((size_t)r.G * r.lstride);
+    r.lunit = bp.take<int>((size_t)4 * r.G);
+    r.lux = bp.take<long long>((size_t)r.G);
+  } else if (kind == K_GROUPED) {
+    const int ldx = (h->dev.dmax + 7) / 8 * 8, nb = h->n_blocks;
+    const size_t L = (size_t)(Lmax > 0 ? Lmax : 1), nul = (size_t)nU * L;
+    r.sum_c_cap = Bs * (long long)h->n_energy;          // every start sector q0 carries at most dim(q0) columns
+    r.tile_cap = (int)(r.sum_c_cap / kGBN + (nU < nb ? nU : nb) + 1);
+    r.gx = bp.take<double>((size_t)2 * r.sum_c_cap * ldx * es);
+    r.gxoff = bp.take<long long>(nU);
+    r.gplan_blk = bp.take<int>(nul); r.gplan_delta = bp.take<double>(nul); r.gkmax = bp.take<int>(nul); r.gcoff = bp.take<int>(nul);
+    r.gulen = bp.take<int>(nU); r.gucols = bp.take<int>(nU);
+    r.gcolcnt = bp.take<int>(L * nb); r.gcolbase = bp.take<int>(L * nb);
+    r.gtiles = bp.take<int4>(L * r.tile_cap);
+    r.gntiles = bp.take<int>(L); r.gtilecur = bp.take<int>(L);
+    r.gcolmap = bp.take<int2>(L * (size_t)r.sum_c_cap);
+  }
+  if (rb) *rb = r;
+  return bp.off + 256;
+}
+
+bool round_ok(const ctqmc_impurity* h, int kind, int mode, long long Bs, int Lmax, int S) {
+  // int indexing inside the kernels
+  const long long nU = unit_bound(h, kind, mode, Bs, Lmax, S);
+  if (nU > 2000000000LL) return false;
+  if (kind == K_GROUPED && (nU * (long long)(Lmax > 0 ? Lmax : 1) > 2000000000LL || Bs * (long long)h->n_energy > 1000000000LL)) return false;
+  if (kind == K_LARGE && mode == 0 && (2 * Bs * (long long)h->n_energy > 2000000000LL || nU > 65535)) return false;   // grid.y
+  return true;
+}
+
+// Decides how the batch is cut into rounds of `*Bs` configurations (and, large-sector bounds, groups of `*G` units) so that
+// one round's scratch fits the arena; grows the arena first when that is allowed.  Everything here is host arithmetic plus,
+// at most, one cudaFree / cudaMalloc BEFORE anything of this call is enqueued.  CTQMC_ERR_OOM: not even one configuration fits.
+int plan_rounds(ctqmc_impurity* h, int kind, int mode, long long B, int Lmax, int S, long long* Bs_out, long long* G_out) {
   Arena& a = h->arena;
-  const long long n_strings = B * h->dev.Q;
-  const long long n_units = n_strings * units_per_string;
-  if (!a.cnt) CU(cudaMalloc((void**)&a.cnt, sizeof(Counters)));
-  if (B > a.cap_configs) {
-    cudaFree(a.status);
-    CU(cudaMalloc((void**)&a.status, (size_t)(B ? B : 1) * sizeof(int)));
-    a.cap_configs = B;
+  long long Bs = B;
+  while (Bs > 1 && !round_ok(h, kind, mode, Bs, Lmax, S)) Bs = (Bs + 1) / 2;
+  if (!round_ok(h, kind, mode, Bs, Lmax, S)) return fail(CTQMC_ERR_ARG, "one configuration exceeds the library's index range (max_len %d)", Lmax);
+  const bool var_g = (kind == K_LARGE && mode == 1);
+  auto need = [&](long long bs, long long g) { return layout_round(h, kind, mode, bs, Lmax, S, g, nullptr, nullptr); };
+  const size_t want = need(Bs, var_g ? unit_bound(h, kind, mode, Bs, Lmax, S) : 0);
+  if (want > a.cap && a.fixed_bytes == 0) {
+    size_t free_b = 0, total_b = 0;
+    CU(cudaMemGetInfo(&free_b, &total_b));
+    size_t limit = (size_t)(0.8 * (double)(free_b + a.cap));
+    if (h->scratch_limit > 0 && (size_t)h->scratch_limit < limit) limit = (size_t)h->scratch_limit;
+    size_t target = want < limit ? want : limit;
+    if (target > a.cap) {
+      // growing synchronises the device (cudaFree): it happens before this call enqueues anything, and only when a call is
+      // larger than every earlier one; a caller that must never stall fixes the size once with CTQMC_OPT_ARENA_BYTES
+      target += target / 16;
+      if (target > limit) target = limit;
+      CU(cudaDeviceSynchronize());
+      cudaFree(a.base); a.base = nullptr; a.cap = 0;
+      cudaError_t e = cudaMalloc((void**)&a.base, target);
+      if (e != cudaSuccess) { cudaGetLastError(); return fail(CTQMC_ERR_OOM, "cannot allocate a scratch arena of %zu bytes", target); }
+      a.cap = target;
+      CU(cudaMemset(a.base, 0, a.cap));
+    }
   }
-  if (n_strings > a.cap_strings) {
-    cudaFree(a.survive); cudaFree(a.strings); cudaFree(a.sector);
-    a.survive = nullptr; a.strings = nullptr; a.sector = nullptr; a.cap_strings = 0;
-    size_t n = (size_t)(n_strings ? n_strings : 1);
-    CU(cudaMalloc((void**)&a.survive, n));
-    CU(cudaMalloc((void**)&a.strings, n * sizeof(StringRec)));
-    CU(cudaMalloc((void**)&a.sector, n * sizeof(Scaled)));
-    a.cap_strings = n_strings;
+  if (need(Bs, var_g ? 1 : 0) > a.cap) {   // rounds: largest Bs whose round fits
+    long long lo = 0, hi = Bs;             // need(lo) fits (lo = 0: nothing), need(hi) does not
+    while (hi - lo > 1) {
+      const long long mid = (lo + hi) / 2;
+      if (need(mid, var_g ? 1 : 0) <= a.cap) lo = mid; else hi = mid;
+    }
+    if (lo < 1) return fail(CTQMC_ERR_OOM, "the scratch arena (%zu bytes) cannot hold one configuration of this batch (%zu bytes needed)%s",
+                            a.cap, need(1, var_g ? 1 : 0), a.fixed_bytes ? "; raise CTQMC_OPT_ARENA_BYTES" : "");
+    Bs = lo;
   }
-  if (n_units > a.cap_units) {
-    cudaFree(a.units); cudaFree(a.slots);
-    a.units = nullptr; a.slots = nullptr; a.cap_units = 0;
-    size_t n = (size_t)(n_units ? n_units : 1);
-    CU(cudaMalloc((void**)&a.units, n * sizeof(int2)));
-    CU(cudaMalloc((void**)&a.slots, n * sizeof(Slot)));
-    a.cap_units = n_units;
+  long long G = 0;
+  if (var_g) {
+    const long long nU = unit_bound(h, kind, mode, Bs, Lmax, S);
+    const size_t base_need = need(Bs, 1), per = need(Bs, 2) - base_need;
+    G = 1 + (long long)((a.cap - base_need) / (per ? per : 1));
+    if (G > nU) G = nU;
+    if (G > 65535) G = 65535;
+    while (G > 1 && need(Bs, G) > a.cap) --G;
   }
+  *Bs_out = Bs; *G_out = G;
   return 0;
 }
 
@@ -342,205 +443,151 @@ int check_batch_args(const ctqmc_impurity* h, double beta, const ctqmc_batch* ba
   if (!(beta > 0.0) || !std::isfinite(beta)) return fail(CTQMC_ERR_ARG, "beta must be positive and finite");
   if (batch->n_configs < 0) return fail(CTQMC_ERR_ARG, "n_configs < 0");
   if (batch->n_configs > 0 && (!batch->offset)) return fail(CTQMC_ERR_ARG, "batch.offset is null");
+  if (batch->n_ops < 0) return fail(CTQMC_ERR_ARG, "batch.n_ops < 0");
+  if (batch->n_ops > 0 && (!batch->symbol || !batch->tau)) return fail(CTQMC_ERR_ARG, "batch.symbol / batch.tau is null");
+  if (batch->max_len < 0) return fail(CTQMC_ERR_ARG, "batch.max_len < 0");
   if (batch->n_configs * (long long)h->dev.Q > 2000000000LL) return fail(CTQMC_ERR_ARG, "n_configs * n_sectors exceeds 2^31");
   return 0;
 }
 
-// validate -> route -> class scan -> unit scatter; leaves strings / units / counters ready.
-int enqueue_routing(ctqmc_impurity* h, const BatchView& bv, uint8_t* survive_out, int mode, int segment_len, cudaStream_t st) {
+// Longest configuration the step loops are sized for: the caller's max_len, or -- when the caller does not know it -- the
+// only bound the host has, n_ops (correct, but one launch per operator of the whole batch: callers should state max_len).
+int effective_max_len(const ctqmc_batch* batch) {
+  long long m = batch->max_len > 0 ? (long long)batch->max_len : batch->n_ops;
+  if (m > batch->n_ops) m = batch->n_ops;
+  if (m > 0x3fffffff) m = 0x3fffffff;
+  return (int)m;
+}
+
+BatchView make_view(const ctqmc_batch* batch, double beta, long long b0, long long Bs, int Lmax) {
+  BatchView bv;
+  bv.B = Bs; bv.offset = (const long long*)batch->offset + b0; bv.symbol = batch->symbol; bv.tau = batch->tau; bv.beta = beta;
+  bv.n_ops = batch->n_ops; bv.max_len = Lmax;
+  return bv;
+}
+
+// validate -> route -> class scan -> unit scatter; leaves strings / units / counters of the round ready.
+int enqueue_routing(ctqmc_impurity* h, const BatchView& bv, const RoundBuf& rb, uint8_t* survive_out, int mode, int segment_len,
+                    bool whole_matrix_units, cudaStream_t st) {
   Arena& a = h->arena;
   const long long B = bv.B, nS = B * h->dev.Q;
   CU(cudaMemsetAsync(a.cnt, 0, sizeof(Counters), st));
-  validate_kernel<<<(unsigned)((B + 255) / 256), 256, 0, st>>>(bv, h->dev.A, a.status);
+  validate_kernel<<<(unsigned)((B + 255) / 256), 256, 0, st>>>(bv, h->dev.A, rb.status);
   RouteParams rp;
-  rp.imp = h->dev; rp.bv = bv; rp.status = a.status; rp.survive = a.survive; rp.survive_out = survive_out;
-  rp.strings = a.strings; rp.cnt = a.cnt; rp.W = (h->large || (h->grouped_now && mode == 0)) ? (1 << 20) : 8 * h->nt; rp.kstep = h->dev.cplx ? 4 : 8;
+  rp.imp = h->dev; rp.bv = bv; rp.status = rb.status; rp.survive = rb.survive; rp.survive_out = survive_out;
+  rp.strings = rb.strings; rp.cnt = a.cnt; rp.W = whole_matrix_units ? (1 << 20) : 8 * h->nt; rp.kstep = h->dev.cplx ? 4 : 8;
   rp.literal = (h->schedule == CTQMC_SCHEDULE_LITERAL); rp.flops_per_mac = h->dev.cplx ? 8 : 2;
   rp.mode = mode; rp.segment_len = segment_len;
   route_kernel<<<(unsigned)((nS + 255) / 256), 256, 0, st>>>(rp);
   h->last_launches += 2;
   if (mode != 2) {
     class_scan_kernel<<<1, 32, 0, st>>>(a.cnt);
-    unit_scatter_kernel<<<(unsigned)((nS + 255) / 256), 256, 0, st>>>(a.strings, nS, a.cnt, a.units);
+    unit_scatter_kernel<<<(unsigned)((nS + 255) / 256), 256, 0, st>>>(rb.strings, nS, a.cnt, rb.units);
     h->last_launches += 2;
   }
   CU(cudaGetLastError());
   return 0;
 }
 
-int enqueue_chain(ctqmc_impurity* h, const BatchView& bv, int mode, int segment_len, cudaStream_t st) {
-  Arena& a = h->arena;
+int enqueue_chain(ctqmc_impurity* h, const BatchView& bv, const RoundBuf& rb, int mode, int segment_len, cudaStream_t st) {
   ChainParams cp;
-  cp.imp = h->dev; cp.bv = bv; cp.strings = a.strings; cp.units = a.units; cp.cnt = a.cnt; cp.slots = a.slots;
+  cp.imp = h->dev; cp.bv = bv; cp.strings = rb.strings; cp.units = rb.units; cp.cnt = h->arena.cnt; cp.slots = rb.slots;
   cp.ldx = h->ldx; cp.mode = mode; cp.segment_len = segment_len;
-  if (h->large) {
-    return fail(CTQMC_ERR_UNSUPPORTED, "internal: large-sector path is driven by enqueue_large");
-  } else {
-    KernelFn fn = pick_kernel(h->dev.cplx, h->nt, h->team_warps);
-    fn<<<h->grid, kCtaThreads, h->smem_bytes, st>>>(cp);
-  }
+  KernelFn fn = pick_kernel(h->dev.cplx, h->nt, h->team_warps);
+  fn<<<h->grid, kCtaThreads, h->smem_bytes, st>>>(cp);
   h->last_launches += 1;
   CU(cudaGetLastError());
   return 0;
 }
 
-
-int grow(DevBuf& b, size_t bytes) {
-  b.grew = false;
-  if (bytes <= b.cap) return 0;
-  cudaFree(b.p); b.p = nullptr; b.cap = 0;
-  const size_t want = bytes + bytes / 8;
-  CU(cudaMalloc(&b.p, want));
-  b.cap = want; b.grew = true;
-  return 0;
-}
-
-// Grouped path (chain_grouped.cuh): schedule for all chain positions, then one GEMM launch per position.  Like the
-// large path it reads the routing counters back once to size its buffers and the step loop.
-int enqueue_grouped(ctqmc_impurity* h, const BatchView& bv, cudaStream_t st) {
-  Arena& a = h->arena;
-  Counters c;
-  CU(cudaMemcpyAsync(&c, a.cnt, sizeof c, cudaMemcpyDeviceToHost, st));
-  CU(cudaStreamSynchronize(st));
-  const long long n_units = (long long)c.n_slots;
-  if (n_units == 0) return 0;
-  if (n_units > 2000000000LL / ((long long)c.max_len + 1)) return fail(CTQMC_ERR_OOM, "batch too large for the grouped path's per-position schedule");   // AUTO falls back to the panel kernel
-  const int Lmax = (int)c.max_len > 0 ? (int)c.max_len : 1;
-  const long long sum_c = (long long)c.sum_c > 0 ? (long long)c.sum_c : 1;
-  const int es = h->dev.cplx ? 2 : 1, nb = h->n_blocks;
+// Grouped path (chain_grouped.cuh): schedule for all chain positions, then one persistent GEMM launch per position.  The
+// number of units, columns and tiles is known on the device only; buffers and the step loop are sized by host-known bounds
+// (configurations x sectors, sum of sector dimensions, max_len), so nothing is read back.
+int enqueue_grouped(ctqmc_impurity* h, const BatchView& bv, const RoundBuf& rb, int Lmax, cudaStream_t st) {
+  if (Lmax < 1) Lmax = 1;
+  const int nb = h->n_blocks;
   const int ldx = (h->dev.dmax + 7) / 8 * 8;
-  const long long xtot = sum_c * ldx;
-  const int tile_cap = (int)(sum_c / kGBN + (n_units < nb ? n_units : nb) + 1);
-  const size_t nul = (size_t)n_units * Lmax;
-  int rc;
-  {
-    const double need = 2.0 * (double)xtot * es * 8.0 + (double)Lmax * (double)sum_c * 8.0 + (double)nul * 20.0;
-    if (h->scratch_limit > 0 && need > (double)h->scratch_limit)
-      return fail(CTQMC_ERR_OOM, "grouped path needs %.0f bytes of scratch, limit is %lld", need, h->scratch_limit);
-  }
-  if ((rc = grow(a.gx, (size_t)2 * xtot * es * sizeof(double)))) return rc;
-  if (a.gx.grew) CU(cudaMemsetAsync(a.gx.p, 0, a.gx.cap, st));
-  if ((rc = grow(a.gxoff, n_units * sizeof(long long))) || (rc = grow(a.gplan_blk, nul * sizeof(int))) ||
-      (rc = grow(a.gplan_delta, nul * sizeof(double))) || (rc = grow(a.gkmax, nul * sizeof(int))) ||
-      (rc = grow(a.gcoff, nul * sizeof(int))) || (rc = grow(a.gulen, n_units * sizeof(int))) ||
-      (rc = grow(a.gucols, n_units * sizeof(int))) || (rc = grow(a.gcolcnt, (size_t)Lmax * nb * sizeof(int))) ||
-      (rc = grow(a.gcolbase, (size_t)Lmax * nb * sizeof(int))) || (rc = grow(a.gtiles, (size_t)Lmax * tile_cap * sizeof(int4))) ||
-      (rc = grow(a.gntiles, (size_t)Lmax * sizeof(int))) || (rc = grow(a.gcolmap, (size_t)Lmax * sum_c * sizeof(int2))))
-    return rc;
+  const long long nU = rb.n_units_cap;
+  const size_t nul = (size_t)nU * Lmax;
   GroupedParams gp;
-  gp.imp = h->dev; gp.bv = bv; gp.strings = a.strings; gp.units = a.units; gp.n_units = (int)n_units; gp.Lmax = Lmax; gp.ldx = ldx;
-  gp.nb = nb; gp.xtot = xtot; gp.X = (double*)a.gx.p; gp.xoff = (long long*)a.gxoff.p; gp.plan_blk = (int*)a.gplan_blk.p;
-  gp.plan_delta = (double*)a.gplan_delta.p; gp.kmax = (int*)a.gkmax.p; gp.coff = (int*)a.gcoff.p; gp.ulen = (int*)a.gulen.p;
-  gp.ucols = (int*)a.gucols.p; gp.colcnt = (int*)a.gcolcnt.p; gp.colbase = (int*)a.gcolbase.p; gp.tiles = (int4*)a.gtiles.p;
-  gp.ntiles = (int*)a.gntiles.p; gp.colmap = (int2*)a.gcolmap.p; gp.tile_cap = tile_cap; gp.col_cap = sum_c; gp.slots = a.slots;
+  gp.imp = h->dev; gp.bv = bv; gp.strings = rb.strings; gp.units = rb.units; gp.cnt = h->arena.cnt; gp.Lmax = Lmax; gp.ldx = ldx;
+  gp.nb = nb; gp.xtot = rb.sum_c_cap * ldx; gp.X = rb.gx; gp.xoff = rb.gxoff; gp.plan_blk = rb.gplan_blk;
+  gp.plan_delta = rb.gplan_delta; gp.kmax = rb.gkmax; gp.coff = rb.gcoff; gp.ulen = rb.gulen;
+  gp.ucols = rb.gucols; gp.colcnt = rb.gcolcnt; gp.colbase = rb.gcolbase; gp.tiles = rb.gtiles;
+  gp.ntiles = rb.gntiles; gp.tilecur = rb.gtilecur; gp.colmap = rb.gcolmap; gp.tile_cap = rb.tile_cap; gp.col_cap = rb.sum_c_cap; gp.slots = rb.slots;
   CU(cudaMemsetAsync(gp.colcnt, 0, (size_t)Lmax * nb * sizeof(int), st));
+  CU(cudaMemsetAsync(gp.tilecur, 0, (size_t)Lmax * sizeof(int), st));
   const unsigned g_ul = (unsigned)((nul + 255) / 256);
-  grouped_plan_kernel<<<(unsigned)((n_units + 127) / 128), 128, 0, st>>>(gp);
+  const unsigned g_units = (unsigned)(nU < 4LL * h->sm_count * 8 ? nU : 4LL * h->sm_count * 8);
+  grouped_plan_kernel<<<(unsigned)((nU + 127) / 128), 128, 0, st>>>(gp);
   grouped_xoff_kernel<<<1, 1024, 0, st>>>(gp);
   grouped_count_kernel<<<g_ul, 256, 0, st>>>(gp);
   grouped_tiles_kernel<<<Lmax, 32, 0, st>>>(gp);
   grouped_fill_kernel<<<g_ul, 256, 0, st>>>(gp);
   const int MTmax = (h->dev.dmax + kGBM - 1) / kGBM;
-  const unsigned sg = (unsigned)tile_cap * (unsigned)MTmax;
-  // step launches use programmatic stream serialization (see the kernel): launch gaps and tails overlap the next step's prologue
+  // persistent step grid: as many CTAs as the SMs hold (never more than the item bound); the next position's CTAs start
+  // under programmatic stream serialization as this one's run out of items
+  long long sg = (long long)h->grouped_ctas_per_sm * h->sm_count;
+  const long long item_bound = (long long)rb.tile_cap * MTmax;
+  if (sg > item_bound) sg = item_bound;
   cudaLaunchConfig_t lc = {};
-  lc.gridDim = dim3(sg); lc.blockDim = dim3(kGThreads); lc.dynamicSmemBytes = h->grouped_smem; lc.stream = st;
+  lc.gridDim = dim3((unsigned)sg); lc.blockDim = dim3(kGThreads); lc.dynamicSmemBytes = h->grouped_smem; lc.stream = st;
   cudaLaunchAttribute lattr[1];
   lattr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   lattr[0].val.programmaticStreamSerializationAllowed = 1;
   lc.attrs = lattr; lc.numAttrs = 1;
   if (h->dev.cplx) {
-    grouped_init_kernel<true><<<(unsigned)n_units, 128, 0, st>>>(gp);
+    grouped_init_kernel<true><<<g_units ? g_units : 1, 128, 0, st>>>(gp);
     for (int j = 0; j < Lmax; ++j) CU(cudaLaunchKernelEx(&lc, grouped_step_kernel<true>, gp, j, MTmax));
-    grouped_finish_kernel<true><<<(unsigned)n_units, 256, 0, st>>>(gp);
+    grouped_finish_kernel<true><<<(unsigned)(nU ? nU : 1), 256, 0, st>>>(gp);
   } else {
-    grouped_init_kernel<false><<<(unsigned)n_units, 128, 0, st>>>(gp);
+    grouped_init_kernel<false><<<g_units ? g_units : 1, 128, 0, st>>>(gp);
     for (int j = 0; j < Lmax; ++j) CU(cudaLaunchKernelEx(&lc, grouped_step_kernel<false>, gp, j, MTmax));
-    grouped_finish_kernel<false><<<(unsigned)n_units, 256, 0, st>>>(gp);
+    grouped_finish_kernel<false><<<(unsigned)(nU ? nU : 1), 256, 0, st>>>(gp);
   }
   h->last_launches += 7 + Lmax;
   CU(cudaGetLastError());
   return 0;
 }
 
-// Large-sector path: one launch per chain position over all strings of a group (chain_large.cuh).  Reads back three
-// integers (strings with work, longest chain, widest carried matrix) to size the step loop and the carried matrices:
-// the one host synchronisation of this path.
-int enqueue_large(ctqmc_impurity* h, const BatchView& bv, int mode, int segment_len, cudaStream_t st) {
-  Arena& a = h->arena;
-  Counters c;
-  CU(cudaMemcpyAsync(&c, a.cnt, sizeof c, cudaMemcpyDeviceToHost, st));
-  CU(cudaStreamSynchronize(st));
-  const long long n_units = (long long)c.n_slots;
-  if (n_units == 0) return 0;
-  const int Lmax = (int)c.max_len > 0 ? (int)c.max_len : 1;
-  const int cmax = mode == 1 ? h->dev.dmax : ((int)c.max_c > 0 ? (int)c.max_c : 1);   // segments start from full identities
-  const int n_launch = mode == 1 ? (segment_len < Lmax ? segment_len : Lmax) : Lmax;
+// Large-sector path (chain_large.cuh): one launch per chain position over all unit slots of a group.  Unit slots, the step
+// loop and the carried matrices are sized by host-known bounds; idle slots and steps beyond a string's length exit at once.
+int enqueue_large(ctqmc_impurity* h, const BatchView& bv, const RoundBuf& rb, int mode, int segment_len, int Lmax, cudaStream_t st) {
+  const long long nU = rb.n_units_cap, G = rb.G;
+  if (G < 1) return 0;
+  const int n_launch = mode == 1 ? rb.lstride : (Lmax > 0 ? Lmax : 0);
   const int es = h->dev.cplx ? 2 : 1;
-  const long long xslab = (long long)cmax * h->ldx;
-  const size_t per_string = (size_t)2 * xslab * es * sizeof(double);
-  size_t free_b = 0, total_b = 0;
-  CU(cudaMemGetInfo(&free_b, &total_b));
-  const size_t budget = a.lx_bytes + (size_t)(0.7 * (double)free_b);
-  long long G = (long long)(budget / per_string);
-  if (G < 1) return fail(CTQMC_ERR_OOM, "not enough device memory for one carried matrix pair (%zu bytes)", per_string);
-  if (G > n_units) G = n_units;
-  if (G > 65535) G = 65535;
-  if ((size_t)G * per_string > a.lx_bytes) {
-    cudaFree(a.lx); a.lx = nullptr; a.lx_bytes = 0;
-    CU(cudaMalloc((void**)&a.lx, (size_t)G * per_string));
-    a.lx_bytes = (size_t)G * per_string;
-    CU(cudaMemsetAsync(a.lx, 0, a.lx_bytes, st));
-  }
-  if ((size_t)G * Lmax > a.plan_cap) {
-    cudaFree(a.plan_blk); cudaFree(a.plan_delta); cudaFree(a.lkmax);
-    a.plan_blk = nullptr; a.plan_delta = nullptr; a.lkmax = nullptr; a.plan_cap = 0;
-    const size_t n = (size_t)G * Lmax;
-    CU(cudaMalloc((void**)&a.plan_blk, n * sizeof(int)));
-    CU(cudaMalloc((void**)&a.plan_delta, n * sizeof(double)));
-    CU(cudaMalloc((void**)&a.lkmax, n * sizeof(int)));
-    a.plan_cap = n;
-  }
-  { int rc = grow(a.lunit, (size_t)3 * G * sizeof(int)); if (rc) return rc; }
   LargeParams lp;
-  lp.u_q = (int*)a.lunit.p; lp.u_n = lp.u_q + G; lp.u_c = lp.u_n + G; lp.mode = mode; lp.segment_len = segment_len;
-  lp.imp = h->dev; lp.bv = bv; lp.strings = a.strings; lp.units = a.units; lp.Lmax = Lmax; lp.ldx = h->ldx;
-  lp.xslab = xslab; lp.X = a.lx; lp.plan_blk = a.plan_blk; lp.plan_delta = a.plan_delta; lp.kmax = a.lkmax; lp.slots = a.slots;
-  lp.amaps = h->d_amaps; lp.xmaps = nullptr;
+  lp.u_q = rb.lunit; lp.u_n = lp.u_q + G; lp.u_c = lp.u_n + G; lp.u_w = lp.u_c + G; lp.u_x = rb.lux; lp.mode = mode; lp.segment_len = segment_len;
+  lp.imp = h->dev; lp.bv = bv; lp.strings = rb.strings; lp.units = rb.units; lp.cnt = h->arena.cnt; lp.Lmax = rb.lstride; lp.ldx = h->ldx;
+  lp.sum_d = h->n_energy; lp.X = rb.lx; lp.plan_blk = rb.plan_blk; lp.plan_delta = rb.plan_delta; lp.kmax = rb.lkmax; lp.slots = rb.slots;
+  lp.amaps = h->d_amaps;
   const bool tma = h->use_tma && h->d_amaps;
-  if (tma) {   // tensor maps of the carried matrices (two per string slot); rebuilt only when the arena changed
-    if (a.xmaps_base != a.lx || a.xmaps_g < G || a.xmaps_slab != xslab || a.xmaps_cmax != cmax) {
-      std::vector<CUtensorMap> maps((size_t)2 * G);
-      for (long long i = 0; i < 2 * G; ++i) {
-        int rc = encode_2d(&maps[i], a.lx + (size_t)i * xslab * es, (unsigned long long)h->ldx * es, (unsigned long long)cmax,
-                           (unsigned long long)h->ldx * es * 8, kLBN);
-        if (rc) return rc;
-      }
-      { int rc = grow(a.xmaps, maps.size() * sizeof(CUtensorMap)); if (rc) return rc; }
-      CU(cudaMemcpyAsync(a.xmaps.p, maps.data(), maps.size() * sizeof(CUtensorMap), cudaMemcpyHostToDevice, st));
-      CU(cudaStreamSynchronize(st));   // `maps` is a pageable host vector
-      a.xmaps_base = a.lx; a.xmaps_g = G; a.xmaps_slab = xslab; a.xmaps_cmax = cmax;
-    }
-    lp.xmaps = (const CUtensorMap*)a.xmaps.p;
+  CUtensorMap xmap;
+  memset(&xmap, 0, sizeof xmap);
+  if (tma) {   // one map over the whole carried-matrix region, passed to the kernel by value: no per-string maps, no copy
+    int rc = encode_2d(&xmap, rb.lx, (unsigned long long)h->ldx * es, (unsigned long long)rb.lx_cols, (unsigned long long)h->ldx * es * 8, kLBN);
+    if (rc) return rc;
   }
-  const int MTmax = (h->dev.dmax + kLBM - 1) / kLBM, NTmax = (cmax + kLBN - 1) / kLBN;
-  for (long long u0 = 0; u0 < n_units; u0 += G) {
-    lp.u0 = u0; lp.n_group = (int)((n_units - u0 < G) ? (n_units - u0) : G);
+  const int cw = h->dev.dmax;   // widest carried matrix the host can promise
+  const int MTmax = (h->dev.dmax + kLBM - 1) / kLBM, NTmax = (cw + kLBN - 1) / kLBN;
+  for (long long u0 = 0; u0 < nU; u0 += G) {
+    lp.u0 = u0; lp.n_group = (int)((nU - u0 < G) ? (nU - u0) : G);
     large_plan_kernel<<<(lp.n_group + 127) / 128, 128, 0, st>>>(lp);
-    dim3 ig((unsigned)((cmax < 1024) ? cmax : 1024), (unsigned)lp.n_group);
+    dim3 ig((unsigned)((cw < 256) ? cw : 256), (unsigned)lp.n_group);
     dim3 sg((unsigned)(MTmax * NTmax), (unsigned)lp.n_group);
     if (h->dev.cplx) {
       large_init_kernel<true><<<ig, 256, 0, st>>>(lp);
       for (int j = 0; j < n_launch; ++j) {
-        if (tma) large_step_kernel<true, true><<<sg, 256, h->smem_bytes, st>>>(lp, j, NTmax);
-        else     large_step_kernel<true, false><<<sg, 256, h->smem_bytes, st>>>(lp, j, NTmax);
+        if (tma) large_step_kernel<true, true><<<sg, 256, h->smem_bytes, st>>>(xmap, lp, j, NTmax);
+        else     large_step_kernel<true, false><<<sg, 256, h->smem_bytes, st>>>(xmap, lp, j, NTmax);
       }
       large_finish_kernel<true><<<lp.n_group, 256, 0, st>>>(lp);
     } else {
       large_init_kernel<false><<<ig, 256, 0, st>>>(lp);
       for (int j = 0; j < n_launch; ++j) {
-        if (tma) large_step_kernel<false, true><<<sg, 256, h->smem_bytes, st>>>(lp, j, NTmax);
-        else     large_step_kernel<false, false><<<sg, 256, h->smem_bytes, st>>>(lp, j, NTmax);
+        if (tma) large_step_kernel<false, true><<<sg, 256, h->smem_bytes, st>>>(xmap, lp, j, NTmax);
+        else     large_step_kernel<false, false><<<sg, 256, h->smem_bytes, st>>>(xmap, lp, j, NTmax);
       }
       large_finish_kernel<false><<<lp.n_group, 256, 0, st>>>(lp);
     }
@@ -736,6 +783,10 @@ extern "C" int ctqmc_load_impurity(const ctqmc_impurity_desc* desc, int device, 
   cleanup_tmp();
   d_raw = nullptr; d_rawoff = nullptr; d_voff = nullptr; d_v = nullptr; d_u = nullptr; d_w = nullptr; d_need = nullptr;
 
+  TRYCU(cudaMalloc((void**)&h->arena.cnt, sizeof(Counters)));
+  TRYCU(cudaMalloc((void**)&h->arena.cnt_total, sizeof(Counters)));
+  TRYCU(cudaMemset(h->arena.cnt, 0, sizeof(Counters)));
+  TRYCU(cudaMemset(h->arena.cnt_total, 0, sizeof(Counters)));
   h->dev.Q = Q; h->dev.A = A; h->dev.cplx = cplx; h->dev.dmax = dmax;
   h->dev.dim = h->d_dim; h->dev.e_off = h->d_eoff; h->dev.energy = h->d_energy; h->dev.e_min = h->d_emin;
   h->dev.blk_of = h->d_blkof; h->dev.blks = h->d_blks; h->dev.store = h->d_store; h->dev.rownorm2 = h->d_rownorm2;
@@ -755,10 +806,7 @@ extern "C" void ctqmc_free_impurity(ctqmc_impurity* h) {
   cudaFree(h->d_pack); cudaFree(h->d_pblk); cudaFree(h->d_blkorder);
   cudaFree(h->d_blks); cudaFree(h->d_store); cudaFree(h->d_rownorm2); cudaFree(h->d_sigma);
   Arena& a = h->arena;
-  cudaFree(a.status); cudaFree(a.survive); cudaFree(a.strings); cudaFree(a.units); cudaFree(a.slots); cudaFree(a.sector);
-  for (DevBuf* b : {&a.gx, &a.gxoff, &a.gplan_blk, &a.gplan_delta, &a.gkmax, &a.gcoff, &a.gulen, &a.gucols, &a.gcolcnt, &a.gcolbase,
-                     &a.gtiles, &a.gntiles, &a.gcolmap}) cudaFree(b->p);
-  cudaFree(a.lunit.p); cudaFree(a.xmaps.p); cudaFree(h->d_amaps); cudaFree(a.cnt); cudaFree(a.lx); cudaFree(a.plan_blk); cudaFree(a.plan_delta); cudaFree(a.lkmax); cudaFree(a.d_stage);
+  cudaFree(a.base); cudaFree(a.cnt); cudaFree(a.cnt_total); cudaFree(h->d_amaps); cudaFree(a.d_stage);
   if (a.h_stage) cudaFreeHost(a.h_stage);
   for (int i = 0; i < 4; ++i) if (h->ev[i]) cudaEventDestroy(h->ev[i]);
   for (int i = 0; i < 9; ++i) if (h->ev_chunk[i]) cudaEventDestroy(h->ev_chunk[i]);
@@ -777,10 +825,13 @@ extern "C" int ctqmc_set_option(ctqmc_impurity* h, int option, int64_t value) {
   if (option == CTQMC_OPT_PANEL_WIDTH) {
     if (value != 0 && value != 8 && value != 16 && value != 32) return fail(CTQMC_ERR_ARG, "panel width must be 0, 8, 16 or 32");
     if (h->large) return 0;
-    int nt = h->nt, tw = h->team_warps, ldx = h->ldx, grid = h->grid; size_t sm = h->smem_bytes;
     int rc = configure(h, (int)value);
-    if (rc || h->large) { h->nt = nt; h->team_warps = tw; h->ldx = ldx; h->grid = grid; h->smem_bytes = sm; h->large = 0;
-                          return rc ? rc : fail(CTQMC_ERR_UNSUPPORTED, "panel width %lld does not fit in shared memory for this impurity", (long long)value); }
+    if (rc || h->large) {   // restore the whole schedule state (configure() touches the small / grouped flags as well)
+      std::string msg = g_err;
+      configure(h, 0);
+      g_err = msg;
+      return rc ? rc : fail(CTQMC_ERR_UNSUPPORTED, "panel width %lld does not fit in shared memory for this impurity", (long long)value);
+    }
     return 0;
   }
   if (option == CTQMC_OPT_PATH) {
@@ -796,6 +847,20 @@ extern "C" int ctqmc_set_option(ctqmc_impurity* h, int option, int64_t value) {
     h->scratch_limit = (long long)value;
     return 0;
   }
+  if (option == CTQMC_OPT_ARENA_BYTES) {
+    // pre-allocate the whole scratch arena now; from here on no batch call allocates or frees device memory
+    if (value < 0) return fail(CTQMC_ERR_ARG, "arena size must be >= 0");
+    Arena& a = h->arena;
+    CU(cudaDeviceSynchronize());
+    cudaFree(a.base); a.base = nullptr; a.cap = 0; a.fixed_bytes = 0;
+    if (value > 0) {
+      cudaError_t e = cudaMalloc((void**)&a.base, (size_t)value);
+      if (e != cudaSuccess) { cudaGetLastError(); return fail(CTQMC_ERR_OOM, "cannot allocate a scratch arena of %lld bytes", (long long)value); }
+      a.cap = (size_t)value; a.fixed_bytes = (size_t)value;
+      CU(cudaMemset(a.base, 0, a.cap));
+    }
+    return 0;
+  }
   if (option == CTQMC_OPT_TIMING) {
     if (value && !h->ev[0])
       for (int i = 0; i < 4; ++i) CU(cudaEventCreate(&h->ev[i]));
@@ -805,6 +870,32 @@ extern "C" int ctqmc_set_option(ctqmc_impurity* h, int option, int64_t value) {
   }
   return fail(CTQMC_ERR_ARG, "unknown option %d", option);
 }
+
+namespace {
+
+// One round of ctqmc_trace_batch on a sub-batch (panel / grouped / large kernel families).
+int trace_round(ctqmc_impurity* h, int kind, const BatchView& bv, const RoundBuf& rb, int Lmax, double* mant, int64_t* exp2,
+                uint8_t* survive, int32_t* status, cudaStream_t st) {
+  mark(h, 0, st);
+  int rc = enqueue_routing(h, bv, rb, survive, 0, 0, kind != K_PANEL, st);
+  if (rc) return rc;
+  mark(h, 1, st);
+  rc = kind == K_GROUPED ? enqueue_grouped(h, bv, rb, Lmax, st) : kind == K_LARGE ? enqueue_large(h, bv, rb, 0, 0, Lmax, st)
+                                                                                 : enqueue_chain(h, bv, rb, 0, 0, st);
+  if (rc) return rc;
+  mark(h, 2, st);
+  TraceReduceParams tp;
+  tp.B = bv.B; tp.Q = h->dev.Q; tp.status_in = rb.status; tp.survive = rb.survive; tp.strings = rb.strings;
+  tp.slots = rb.slots; tp.mant = mant; tp.exp2 = (long long*)exp2; tp.status = status;
+  trace_reduce_kernel<<<(unsigned)((bv.B + 127) / 128), 128, 0, st>>>(tp);
+  accumulate_counters_kernel<<<1, 1, 0, st>>>(h->arena.cnt, h->arena.cnt_total);
+  h->last_launches += 2;
+  mark(h, 3, st);
+  CU(cudaGetLastError());
+  return 0;
+}
+
+}  // namespace
 
 // ------------------------------------------------------------------------------------------------ batch calls
 extern "C" int ctqmc_trace_batch(ctqmc_impurity* h, double beta, const ctqmc_batch* batch, double* mant, int64_t* exp2,
@@ -816,19 +907,18 @@ extern "C" int ctqmc_trace_batch(ctqmc_impurity* h, double beta, const ctqmc_bat
   if (!mant || !exp2 || !status) return fail(CTQMC_ERR_ARG, "null output (mant, exp2 and status are required)");
   CU(cudaSetDevice(h->device));
   cudaStream_t st = (cudaStream_t)cuda_stream;
+  const int Lmax = effective_max_len(batch);
   // AUTO: batches of at least kGroupedMinBatch configurations take the step-synchronous grouped path (one launch per chain
   // position pays off once many strings share blocks); smaller ones the persistent panel kernel
   h->grouped_now = h->grouped || (h->path == CTQMC_PATH_AUTO && h->grouped_ok && !h->small && !h->large && B >= kGroupedMinBatch);
   h->last_path = h->small ? CTQMC_PATH_SMALL : h->grouped_now ? CTQMC_PATH_GROUPED : h->large ? CTQMC_PATH_LARGE : CTQMC_PATH_PANEL;
-  const int W = (h->large || h->grouped_now) ? (1 << 20) : 8 * h->nt;
-  if (h->small) { if (!h->arena.cnt) CU(cudaMalloc((void**)&h->arena.cnt, sizeof(Counters))); }
-  else { rc = ensure_arena(h, B, (h->dev.dmax + W - 1) / W); if (rc) return rc; }
-  h->last_stream = st; h->last_launches = 0;
-  BatchView bv; bv.B = B; bv.offset = (const long long*)batch->offset; bv.symbol = batch->symbol; bv.tau = batch->tau; bv.beta = beta;
+  h->last_stream = st;
+  if (!h->keep_totals) { h->last_launches = 0; CU(cudaMemsetAsync(h->arena.cnt_total, 0, sizeof(Counters), st)); }
   h->timing_valid = 0;
   if (h->small) {
     // everything (validation, routing, chain, trace, sector sum) in one launch: chain_small.cuh
     Arena& a = h->arena;
+    const BatchView bv = make_view(batch, beta, 0, B, Lmax);
     mark(h, 0, st);
     CU(cudaMemsetAsync(a.cnt, 0, sizeof(Counters), st));
     mark(h, 1, st);
@@ -865,40 +955,33 @@ extern "C" int ctqmc_trace_batch(ctqmc_impurity* h, double beta, const ctqmc_bat
       if (grid > h->small_grid_max) grid = h->small_grid_max;
       pick_small(h->dev.cplx, h->small_g)<<<(unsigned)grid, kCtaThreads, h->small_smem, st>>>(sp);
     }
-    h->last_launches += 1;
+    accumulate_counters_kernel<<<1, 1, 0, st>>>(a.cnt, a.cnt_total);
+    h->last_launches += 2;
     mark(h, 2, st);
     mark(h, 3, st);
     h->timing_valid = h->timing;
     CU(cudaGetLastError());
     return 0;
   }
-  mark(h, 0, st);
-  rc = enqueue_routing(h, bv, survive, 0, 0, st);
-  if (rc) return rc;
-  mark(h, 1, st);
-  rc = h->grouped_now ? enqueue_grouped(h, bv, st) : h->large ? enqueue_large(h, bv, 0, 0, st) : enqueue_chain(h, bv, 0, 0, st);
-  if (rc == CTQMC_ERR_OOM && h->grouped_now && h->path == CTQMC_PATH_AUTO && !h->large) {
-    // the grouped path's schedule (one column map per chain position) did not fit: AUTO falls back to the persistent
-    // panel kernel, which needs no per-position scratch.  Routing is redone with panel-sized work units.
-    cudaGetLastError();
-    h->grouped_now = 0; h->last_path = CTQMC_PATH_PANEL; h->last_launches = 0;
-    const int Wp = 8 * h->nt;
-    rc = ensure_arena(h, B, (h->dev.dmax + Wp - 1) / Wp);
-    if (rc) return rc;
-    rc = enqueue_routing(h, bv, survive, 0, 0, st);
-    if (rc) return rc;
-    rc = enqueue_chain(h, bv, 0, 0, st);
+  int kind = h->grouped_now ? K_GROUPED : h->large ? K_LARGE : K_PANEL;
+  long long Bs = 0, G = 0;
+  rc = plan_rounds(h, kind, 0, B, Lmax, 0, &Bs, &G);
+  if (rc == CTQMC_ERR_OOM && kind == K_GROUPED && h->path == CTQMC_PATH_AUTO) {
+    // the grouped path's schedule (one column map per chain position) does not fit: AUTO falls back to the persistent panel
+    // kernel, which needs no per-position scratch
+    h->grouped_now = 0; h->last_path = CTQMC_PATH_PANEL; kind = K_PANEL;
+    rc = plan_rounds(h, kind, 0, B, Lmax, 0, &Bs, &G);
   }
   if (rc) return rc;
-  mark(h, 2, st);
-  TraceReduceParams tp;
-  tp.B = B; tp.Q = h->dev.Q; tp.status_in = h->arena.status; tp.survive = h->arena.survive; tp.strings = h->arena.strings;
-  tp.slots = h->arena.slots; tp.mant = mant; tp.exp2 = (long long*)exp2; tp.status = status;
-  trace_reduce_kernel<<<(unsigned)((B + 127) / 128), 128, 0, st>>>(tp);
-  h->last_launches += 1;
-  mark(h, 3, st);
+  for (long long b0 = 0; b0 < B; b0 += Bs) {
+    const long long bs = (B - b0 < Bs) ? (B - b0) : Bs;
+    RoundBuf rb;
+    layout_round(h, kind, 0, bs, Lmax, 0, G, h->arena.base, &rb);
+    const BatchView bv = make_view(batch, beta, b0, bs, Lmax);
+    rc = trace_round(h, kind, bv, rb, Lmax, mant + 2 * b0, exp2 + b0, survive ? survive + b0 * h->dev.Q : nullptr, status + b0, st);
+    if (rc) return rc;
+  }
   h->timing_valid = h->timing;
-  CU(cudaGetLastError());
   return 0;
 }
 
@@ -917,15 +1000,16 @@ extern "C" int ctqmc_bound_batch(ctqmc_impurity* h, double beta, const ctqmc_bat
   if (!bound_mant || !bound_exp2 || !status) return fail(CTQMC_ERR_ARG, "null output");
   CU(cudaSetDevice(h->device));
   cudaStream_t st = (cudaStream_t)cuda_stream;
+  const int Lmax = effective_max_len(batch);
   const int W = h->large ? (1 << 20) : 8 * h->nt;
-  const long long nS = B * h->dev.Q;
-  BatchView bv; bv.B = B; bv.offset = (const long long*)batch->offset; bv.symbol = batch->symbol; bv.tau = batch->tau; bv.beta = beta;
+  const long long Q = h->dev.Q;
   h->last_stream = st; h->last_launches = 0;
+  CU(cudaMemsetAsync(h->arena.cnt_total, 0, sizeof(Counters), st));
   h->timing_valid = 0;
   h->grouped_now = 0; h->last_path = h->large ? CTQMC_PATH_LARGE : CTQMC_PATH_PANEL;
-  BoundParams bp;
   if (segment_len == 1 && h->small2) {
     // small real impurities: validation, routing, norm products and the sector sum in one launch (bound_small2.cuh)
+    const BatchView bv = make_view(batch, beta, 0, B, Lmax);
     const int dp = h->small2_dp, gpw = 32 / dp;
     long long per_sm = (B + h->sm_count - 1) / h->sm_count;
     int warps = (int)((per_sm + gpw - 1) / gpw);
@@ -951,63 +1035,48 @@ extern "C" int ctqmc_bound_batch(ctqmc_impurity* h, double beta, const ctqmc_bat
       return 0;
     }
   }
-  if (segment_len == 1) {
-    rc = ensure_arena(h, B, 1);
-    if (rc) return rc;
+  // segment_len 1: norms come from the load-time tables; otherwise the chain kernels multiply every segment.  The number of
+  // segments per string is bounded on the host by max_len / S + 1, so nothing is read back from the device.
+  const int mode = segment_len == 1 ? 2 : 1;
+  const int S = segment_len == 0 ? (1 << 30) : segment_len;
+  const int kind = mode == 2 ? K_TABLES : h->large ? K_LARGE : K_PANEL;
+  long long Bs = 0, G = 0;
+  rc = plan_rounds(h, kind, mode, B, Lmax, S, &Bs, &G);
+  if (rc) return rc;
+  for (long long b0 = 0; b0 < B; b0 += Bs) {
+    const long long bs = (B - b0 < Bs) ? (B - b0) : Bs, nS = bs * Q;
+    RoundBuf rb;
+    layout_round(h, kind, mode, bs, Lmax, S, G, h->arena.base, &rb);
+    const BatchView bv = make_view(batch, beta, b0, bs, Lmax);
+    BoundParams bp;
     mark(h, 0, st);
-    rc = enqueue_routing(h, bv, nullptr, 2, 1, st);
+    rc = enqueue_routing(h, bv, rb, nullptr, mode, mode == 2 ? 1 : S, h->large, st);
     if (rc) return rc;
     mark(h, 1, st);
-    bp.imp = h->dev; bp.bv = bv; bp.survive = h->arena.survive; bp.strings = h->arena.strings; bp.slots = h->arena.slots;
-    bp.sector = h->arena.sector; bp.norm_kind = norm_kind; bp.segment_len = 1; bp.W = W;
-    bound_s1_kernel<<<(unsigned)((nS * 32 + 255) / 256), 256, 0, st>>>(bp);
-    h->last_launches += 1;
-  } else {
-    // units per string depend on the chain lengths, which live on the device: one small read-back of the total
-    // operator count sizes the arena (the only host synchronisation in the library's device-pointer API).
-    long long n_ops = 0;
-    CU(cudaMemcpyAsync(&n_ops, batch->offset + B, sizeof(long long), cudaMemcpyDeviceToHost, st));
-    CU(cudaStreamSynchronize(st));
-    const int S = segment_len == 0 ? 1 << 30 : segment_len;
-    const long long panels = (h->dev.dmax + W - 1) / W;
-    long long max_units_per_string = (segment_len == 0) ? panels : ((n_ops / S) / (B ? 1 : 1) + 1) * panels;
-    // worst case: one configuration holds every operator
-    rc = ensure_arena(h, B, 1);
-    if (rc) return rc;
-    {
-      // exact sizing would need the per-configuration lengths; bound it by sum over configurations instead:
-      // sum_b Q * (L_b / S + 1) * panels <= Q * panels * (n_ops / S + B)
-      long long need = (long long)h->dev.Q * panels * ((segment_len == 0 ? 0 : n_ops / S) + B);
-      Arena& a = h->arena;
-      if (need > a.cap_units) {
-        cudaFree(a.units); cudaFree(a.slots); a.units = nullptr; a.slots = nullptr; a.cap_units = 0;
-        CU(cudaMalloc((void**)&a.units, (size_t)need * sizeof(int2)));
-        CU(cudaMalloc((void**)&a.slots, (size_t)need * sizeof(Slot)));
-        a.cap_units = need;
-      }
-      (void)max_units_per_string;
+    bp.imp = h->dev; bp.bv = bv; bp.survive = rb.survive; bp.strings = rb.strings; bp.slots = rb.slots;
+    bp.sector = rb.sector; bp.W = W;
+    if (mode == 2) {
+      bp.norm_kind = norm_kind; bp.segment_len = 1;
+      bound_s1_kernel<<<(unsigned)((nS * 32 + 255) / 256), 256, 0, st>>>(bp);
+    } else {
+      rc = h->large ? enqueue_large(h, bv, rb, 1, S, Lmax, st) : enqueue_chain(h, bv, rb, 1, S, st);
+      if (rc) return rc;
+      bp.norm_kind = 0; bp.segment_len = S;
+      bound_segments_kernel<<<(unsigned)((nS + 127) / 128), 128, 0, st>>>(bp);
     }
-    mark(h, 0, st);
-    rc = enqueue_routing(h, bv, nullptr, 1, S, st);
-    if (rc) return rc;
-    mark(h, 1, st);
-    rc = h->large ? enqueue_large(h, bv, 1, S, st) : enqueue_chain(h, bv, 1, S, st);
-    if (rc) return rc;
-    bp.imp = h->dev; bp.bv = bv; bp.survive = h->arena.survive; bp.strings = h->arena.strings; bp.slots = h->arena.slots;
-    bp.sector = h->arena.sector; bp.norm_kind = 0; bp.segment_len = S; bp.W = W;
-    bound_segments_kernel<<<(unsigned)((nS + 127) / 128), 128, 0, st>>>(bp);
-    h->last_launches += 1;
+    mark(h, 2, st);
+    BoundReduceParams rp;
+    rp.B = bs; rp.Q = h->dev.Q; rp.status_in = rb.status; rp.survive = rb.survive; rp.sector = rb.sector;
+    rp.bound_mant = bound_mant + b0; rp.bound_exp2 = (long long*)bound_exp2 + b0;
+    rp.sector_mant = sector_bound_mant ? sector_bound_mant + b0 * Q : nullptr;
+    rp.sector_exp2 = sector_bound_exp2 ? (long long*)sector_bound_exp2 + b0 * Q : nullptr; rp.status = status + b0;
+    bound_reduce_kernel<<<(unsigned)((bs + 127) / 128), 128, 0, st>>>(rp);
+    accumulate_counters_kernel<<<1, 1, 0, st>>>(h->arena.cnt, h->arena.cnt_total);
+    h->last_launches += 3;
+    mark(h, 3, st);
+    CU(cudaGetLastError());
   }
-  mark(h, 2, st);
-  BoundReduceParams rp;
-  rp.B = B; rp.Q = h->dev.Q; rp.status_in = h->arena.status; rp.survive = h->arena.survive; rp.sector = h->arena.sector;
-  rp.bound_mant = bound_mant; rp.bound_exp2 = (long long*)bound_exp2; rp.sector_mant = sector_bound_mant;
-  rp.sector_exp2 = (long long*)sector_bound_exp2; rp.status = status;
-  bound_reduce_kernel<<<(unsigned)((B + 127) / 128), 128, 0, st>>>(rp);
-  h->last_launches += 1;
-  mark(h, 3, st);
   h->timing_valid = h->timing;
-  CU(cudaGetLastError());
   return 0;
 }
 
@@ -1022,12 +1091,29 @@ struct Staged {
 
 size_t align_up(size_t x) { return (x + 255) / 256 * 256; }
 
-int stage_in(ctqmc_impurity* h, const ctqmc_batch* hb, size_t out_bytes, Staged* sg, cudaStream_t st) {
+// Host forms: the offsets are host memory, so the library derives n_ops and max_len itself (and rejects offsets that would
+// make it read outside the caller's symbol / tau arrays before anything is copied).
+int host_batch_shape(const ctqmc_batch* hb, long long* n_ops, int* max_len) {
   const long long B = hb->n_configs;
   if (!hb->offset) return fail(CTQMC_ERR_ARG, "batch.offset is null");
-  const long long n_ops = hb->offset[B];
-  if (n_ops < 0) return fail(CTQMC_ERR_ARG, "negative operator count");
-  if (n_ops > 0 && (!hb->symbol || !hb->tau)) return fail(CTQMC_ERR_ARG, "null symbol / tau");
+  if (hb->offset[0] != 0) return fail(CTQMC_ERR_ARG, "batch.offset[0] must be 0");
+  long long mx = 0;
+  for (long long b = 0; b < B; ++b) {
+    const long long l = hb->offset[b + 1] - hb->offset[b];
+    if (l < 0) return fail(CTQMC_ERR_ARG, "batch.offset is decreasing at configuration %lld", b);
+    if (l > mx) mx = l;
+  }
+  if (mx > 0x3fffffff) return fail(CTQMC_ERR_ARG, "configuration longer than 2^30 operators");
+  *n_ops = hb->offset[B]; *max_len = (int)mx;
+  if (hb->n_ops != 0 && hb->n_ops < *n_ops) return fail(CTQMC_ERR_ARG, "batch.n_ops (%lld) < offset[B] (%lld)", (long long)hb->n_ops, *n_ops);
+  if (*n_ops > 0 && (!hb->symbol || !hb->tau)) return fail(CTQMC_ERR_ARG, "null symbol / tau");
+  return 0;
+}
+
+int stage_in(ctqmc_impurity* h, const ctqmc_batch* hb, size_t out_bytes, Staged* sg, cudaStream_t st) {
+  const long long B = hb->n_configs;
+  long long n_ops = 0; int max_len = 0;
+  { int rc = host_batch_shape(hb, &n_ops, &max_len); if (rc) return rc; }
   const size_t b_off = align_up((size_t)(B + 1) * 8), b_sym = align_up((size_t)n_ops * 4), b_tau = align_up((size_t)n_ops * 8);
   const size_t total = b_off + b_sym + b_tau + align_up(out_bytes);
   Arena& a = h->arena;
@@ -1044,6 +1130,7 @@ int stage_in(ctqmc_impurity* h, const ctqmc_batch* hb, size_t out_bytes, Staged*
   if (n_ops) { memcpy(hs + b_off, hb->symbol, (size_t)n_ops * 4); memcpy(hs + b_off + b_sym, hb->tau, (size_t)n_ops * 8); }
   CU(cudaMemcpyAsync(ds, hs, b_off + b_sym + b_tau, cudaMemcpyHostToDevice, st));
   sg->dev_batch.n_configs = B;
+  sg->dev_batch.n_ops = n_ops; sg->dev_batch.max_len = max_len;
   sg->dev_batch.offset = (const int64_t*)ds;
   sg->dev_batch.symbol = (const int32_t*)(ds + b_off);
   sg->dev_batch.tau = (const double*)(ds + b_off + b_sym);
@@ -1065,7 +1152,8 @@ bool is_pinned(const void* p) {
 int trace_host_pinned(ctqmc_impurity* h, double beta, const ctqmc_batch* hb, double* mant, int64_t* exp2, uint8_t* survive,
                       int32_t* status, cudaStream_t st) {
   const long long B = hb->n_configs;
-  const long long n_ops = hb->offset[B];
+  long long n_ops = 0; int max_len = 0;
+  { int rc = host_batch_shape(hb, &n_ops, &max_len); if (rc) return rc; }
   const size_t Q = h->dev.Q;
   const size_t b_off = align_up((size_t)(B + 1) * 8), b_sym = align_up((size_t)n_ops * 4), b_tau = align_up((size_t)n_ops * 8);
   const size_t o_mant = 0, o_exp = align_up(B * 16), o_stat = o_exp + align_up(B * 8), o_surv = o_stat + align_up(B * 4);
@@ -1111,8 +1199,11 @@ int trace_host_pinned(ctqmc_impurity* h, double beta, const ctqmc_batch* hb, dou
     }
     ctqmc_batch sub;
     sub.n_configs = b1 - b0; sub.offset = (const int64_t*)(d_off + b0); sub.symbol = d_sym; sub.tau = d_tau;
+    sub.n_ops = n_ops; sub.max_len = max_len;
+    h->keep_totals = k > 0;   // ctqmc_last_stats reports the whole batch, not the last chunk
     int rc = ctqmc_trace_batch(h, beta, &sub, (double*)(d_out + o_mant) + 2 * b0, (int64_t*)(d_out + o_exp) + b0,
                                survive ? (uint8_t*)(d_out + o_surv) + b0 * Q : nullptr, (int32_t*)(d_out + o_stat) + b0, st);
+    h->keep_totals = 0;
     if (rc) return rc;
   }
   CU(cudaMemcpyAsync(mant, d_out + o_mant, B * 16, cudaMemcpyDeviceToHost, st));
@@ -1135,8 +1226,7 @@ extern "C" int ctqmc_trace_batch_host(ctqmc_impurity* h, double beta, const ctqm
   CU(cudaSetDevice(h->device));
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const size_t Q = h->dev.Q;
-  if (batch->offset && batch->offset[B] >= 0 && (batch->offset[B] == 0 || (batch->symbol && batch->tau)) &&
-      is_pinned(batch->offset) && (batch->offset[B] == 0 || (is_pinned(batch->symbol) && is_pinned(batch->tau))) &&
+  if (batch->offset && is_pinned(batch->offset) && (batch->offset[B] == 0 || (is_pinned(batch->symbol) && is_pinned(batch->tau))) &&
       is_pinned(mant) && is_pinned(exp2) && is_pinned(status) && (!survive || is_pinned(survive)))
     return trace_host_pinned(h, beta, batch, mant, exp2, survive, status, st);
   const size_t o_mant = 0, o_exp = align_up(B * 16), o_stat = o_exp + align_up(B * 8), o_surv = o_stat + align_up(B * 4);
@@ -1188,18 +1278,18 @@ extern "C" int ctqmc_bound_batch_host(ctqmc_impurity* h, double beta, const ctqm
   return 0;
 }
 
-extern "C" int ctqmc_last_stats(ctqmc_impurity* h, int64_t stats[8]) {
+extern "C" int ctqmc_last_stats(ctqmc_impurity* h, int64_t stats[10]) {
   if (!h || !stats) return fail(CTQMC_ERR_ARG, "null argument");
-  for (int i = 0; i < 8; ++i) stats[i] = 0;
+  for (int i = 0; i < 10; ++i) stats[i] = 0;
   stats[5] = h->small ? (h->small2 ? h->small2_dp : h->small_g) : h->nt * 8; stats[6] = h->team_warps; stats[7] = h->last_path ? h->last_path : (h->small ? 3 : h->grouped ? 4 : h->large ? 2 : 1);
-  if (!h->arena.cnt) return 0;
+  stats[9] = (int64_t)h->arena.cap;
+  if (!h->arena.cnt_total) return 0;
   CU(cudaSetDevice(h->device));
   Counters c;
   CU(cudaStreamSynchronize(h->last_stream));
-  CU(cudaMemcpy(&c, h->arena.cnt, sizeof c, cudaMemcpyDeviceToHost));
+  CU(cudaMemcpy(&c, h->arena.cnt_total, sizeof c, cudaMemcpyDeviceToHost));
   stats[0] = (int64_t)c.n_strings; stats[1] = (int64_t)c.n_slots; stats[2] = h->last_launches;
-  stats[3] = (int64_t)c.macs; stats[4] = (int64_t)c.alg_flops;
-  if (h->last_path == CTQMC_PATH_SMALL) stats[6] = (int64_t)c.n_exp;
+  stats[3] = (int64_t)c.macs; stats[4] = (int64_t)c.alg_flops; stats[8] = (int64_t)c.n_exp;
   return 0;
 }
 

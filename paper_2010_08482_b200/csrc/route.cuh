@@ -10,7 +10,8 @@ __global__ void validate_kernel(BatchView bv, int A, int* __restrict__ status) {
   long long b = blockIdx.x * (long long)blockDim.x + threadIdx.x;
   if (b >= bv.B) return;
   long long lo = bv.offset[b], hi = bv.offset[b + 1];
-  bool ok = hi >= lo;
+  // a corrupt offset array must give status 2, not an out-of-bounds read
+  bool ok = lo >= 0 && hi >= lo && hi <= bv.n_ops && hi - lo <= (long long)bv.max_len;
   double prev = 0.0;
   for (long long i = lo; ok && i < hi; ++i) {
     int a = bv.symbol[i];
@@ -111,6 +112,15 @@ __global__ void route_kernel(RouteParams P) {
   P.survive[s] = alive;
   if (P.survive_out) P.survive_out[s] = alive;
   P.strings[s] = rec;
+}
+
+// Adds one round's counters to the call's totals (a call is cut into rounds of configurations when its scratch would not
+// fit the arena; ctqmc_last_stats reports the totals).
+__global__ void accumulate_counters_kernel(const Counters* __restrict__ c, Counters* __restrict__ tot) {
+  if (threadIdx.x != 0 || blockIdx.x != 0) return;
+  tot->n_strings += c->n_strings; tot->n_slots += c->n_slots; tot->macs += c->macs; tot->alg_flops += c->alg_flops;
+  tot->sum_c += c->sum_c; tot->n_exp += c->n_exp;
+  tot->max_len = max(tot->max_len, c->max_len); tot->max_c = max(tot->max_c, c->max_c);
 }
 
 // Heaviest cost class first (longest-processing-time order for the persistent chain kernel).

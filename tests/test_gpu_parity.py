@@ -8,7 +8,8 @@ Bars (BASELINE.json north_star):
     of its configurations in that basis -- on EITHER side.  There a true value exists: the same oracle on the same Hamiltonian
     labelled by (N, 2S_z, L_z) (equal by pin P4 (iii), stable to 1e-10 under the cyclic shifts of pin P2).  A configuration
     that misses 1e-9 against the coarse oracle is judged against that truth: |gpu - truth| <= max(1e-9, 10 |coarse - truth|),
-    i.e. the GPU must be no worse than the fp64 oracle fed the same blocks.  Nothing is exempt;
+    |coarse - truth| being the largest of four samples of the coarse oracle's own noise (the configuration as given and after
+    three exact cyclic shifts), i.e. the GPU must be no worse than the fp64 oracle fed the same blocks.  Nothing is exempt;
   * bound: relative 1e-9 against the oracle's bound (plus, for segment products, the rounding floor 2^-40 x the product of
     the factor norms), bound >= |trace| per configuration AND per start sector.
 """
@@ -98,14 +99,22 @@ def _check_trace(lib, torch, imp, handle, batch, label, sample=None):
         mx = max(abs(w.real), abs(w.imag))
         assert 1.0 <= mx < 2.0, f"{label} config {b}: mantissa {w} not normalised"
         d = rel_diff(w, int(exp2[b]), r["mant"], r["exp2"])
-        tol = TOL * max(1.0, r["kappa"] * 1e-5)
+        # kappa (final cancellation) loosens the bar only where no truth is available; with one, a miss is judged against it
+        tol = TOL * max(1.0, r["kappa"] * 1e-5) if truth_imp is None else TOL
         if tol > TOL:
             loosened += 1
         if d > tol and truth_imp is not None and len(s) > 0:
             rt = O.trace_config(truth_imp, batch.beta, s, t)
-            d_coarse = rel_diff(r["mant"], r["exp2"], rt["mant"], rt["exp2"])
             d_gpu = rel_diff(w, int(exp2[b]), rt["mant"], rt["exp2"])
-            print(f"{label} config {b}: coarse oracle is {d_coarse:.2e} from the (N,Sz,Lz) truth, gpu {d_gpu:.2e}, gpu-coarse {d:.2e}")
+            # the coarse oracle's own noise: its distance from the truth as computed, and after three exact cyclic shifts
+            noise = [rel_diff(r["mant"], r["exp2"], rt["mant"], rt["exp2"])]
+            for frac in (0.23, 0.52, 0.77):
+                t2 = (t + frac * batch.beta) % batch.beta
+                o = np.argsort(t2, kind="stable")
+                r2 = O.trace_config(imp, batch.beta, s[o], t2[o])
+                noise.append(rel_diff(r2["mant"], r2["exp2"], rt["mant"], rt["exp2"]))
+            d_coarse = max(noise)
+            print(f"{label} config {b}: coarse oracle is up to {d_coarse:.2e} from the (N,Sz,Lz) truth, gpu {d_gpu:.2e}, gpu-coarse {d:.2e}")
             assert d_gpu <= max(TOL, 10.0 * d_coarse), f"{label} config {b}: gpu {d_gpu:.3e} from the truth, coarse oracle {d_coarse:.3e}"
             explained += 1
             continue
@@ -146,10 +155,11 @@ def _check_trace_golden(lib, torch, handle, batch, doc, label, records=None):
         assert om != 0 and 1.0 <= max(abs(w.real), abs(w.imag)) < 2.0
         d = rel_diff(w, int(exp2[b]), om, oe)
         tol = TOL * max(1.0, rec["kappa"] * 1e-5)
-        loosened += tol > TOL
+        loosened += tol > TOL and "coarse_shifts" not in rec     # kappa of a configuration fp64 does not determine means nothing
         if "fine" in rec and d > tol:
             tm, te = complex(*rec["fine"]["mant"]), rec["fine"]["exp2"]
-            d_coarse, d_gpu = rel_diff(om, oe, tm, te), rel_diff(w, int(exp2[b]), tm, te)
+            d_gpu = rel_diff(w, int(exp2[b]), tm, te)
+            d_coarse = max([rel_diff(om, oe, tm, te)] + [rel_diff(complex(*x["mant"]), x["exp2"], tm, te) for x in rec.get("coarse_shifts", [])])
             assert d_gpu <= max(TOL, 10.0 * d_coarse), f"{label} config {b}: gpu {d_gpu:.3e} from the truth, coarse oracle {d_coarse:.3e}"
             judged_by_truth += 1
             continue
@@ -830,3 +840,246 @@ def test_coarse_sectors_do_not_underflow(lib, torch_cuda):
             _check_bound(lib, torch_cuda, imp, h, batch, nk, S, f"ising-coarse-nk{nk}-S{S}")
     finally:
         h.free()
+
+
+# --------------------------------------------------------------------------- asynchrony contract and the scratch arena
+def _spin(torch, stream, ms):
+    """Occupy `stream` for about `ms` milliseconds (torch's spin kernel; 1.9 GHz SM clock)."""
+    with torch.cuda.stream(stream):
+        torch.cuda._sleep(int(ms * 1.9e6))
+
+
+@pytest.mark.parametrize("cfg,n", [(2, 256), (3, 16), (3, 72), (4, 4), (4, 64)])
+def test_batch_calls_only_enqueue(cfg, n, lib, torch_cuda, impurities, handles):
+    """SURVEY 8(b) / PAPER.md:574 ("only asynchronous CUDA functions"): with the arena in place, ctqmc_trace_batch and
+    ctqmc_bound_batch return while the stream is still busy with work enqueued BEFORE them -- small, panel, grouped (72 / 64
+    configurations) and, forced, large-sector paths; the results are those of a quiet stream."""
+    import time
+    from workloads import make_batch
+    torch = torch_cuda
+    h = handles(cfg)
+    batch = make_batch(cfg, n, start=21000)
+    off, sym, tau = _dev(torch, batch)
+    L = int(np.diff(batch.offset).max())
+    paths = [lib.CTQMC_PATH_AUTO] + ([lib.CTQMC_PATH_LARGE] if cfg in (3, 4) and n <= 16 else [])
+    st = torch.cuda.Stream()
+    for path in paths:
+        lib.ctqmc_set_option(h, lib.CTQMC_OPT_PATH, path)
+        try:
+            ref = lib.ctqmc_trace_batch(h, batch.beta, off, sym, tau, max_len=L)        # also brings the arena to size
+            refb = lib.ctqmc_bound_batch(h, batch.beta, off, sym, tau, 0, 4, max_len=L)
+            torch.cuda.synchronize()
+            for which in ("trace", "bound"):
+                done = torch.cuda.Event()
+                _spin(torch, st, 400.0)
+                t0 = time.perf_counter()
+                with torch.cuda.stream(st):
+                    if which == "trace":
+                        got = lib.ctqmc_trace_batch(h, batch.beta, off, sym, tau, stream=st, max_len=L)
+                    else:
+                        got = lib.ctqmc_bound_batch(h, batch.beta, off, sym, tau, 0, 4, stream=st, max_len=L)
+                    done.record(st)
+                dt = time.perf_counter() - t0
+                busy = not done.query()
+                st.synchronize()
+                assert busy, f"cfg{cfg} path {path} {which}: the call returned only after the stream had drained ({dt * 1e3:.0f} ms)"
+                assert dt < 0.3, f"cfg{cfg} path {path} {which}: the call took {dt * 1e3:.0f} ms of host time behind a 400 ms spin"
+                for x, y in zip(ref if which == "trace" else refb, got):
+                    assert torch.equal(x, y)
+        finally:
+            lib.ctqmc_set_option(h, lib.CTQMC_OPT_PATH, lib.CTQMC_PATH_AUTO)
+
+
+@pytest.mark.parametrize("cfg,n,path", [(3, 40, "panel"), (3, 96, "grouped"), (3, 12, "large"), (4, 6, "large")])
+def test_fixed_arena_runs_in_rounds_and_reports_oom_before_enqueueing(cfg, n, path, lib, torch_cuda, impurities):
+    """CTQMC_OPT_ARENA_BYTES: the arena is allocated once and never grown.  A batch that does not fit is evaluated in rounds
+    of configurations with identical results and summed counters; an arena too small for one configuration gives
+    CTQMC_ERR_OOM and leaves the outputs untouched."""
+    from workloads import make_batch
+    torch = torch_cuda
+    imp = impurities(cfg)
+    batch = make_batch(cfg, n, start=23000)
+    off, sym, tau = _dev(torch, batch)
+    L = int(np.diff(batch.offset).max())
+    h = lib.ctqmc_load_impurity(imp, 0)
+    try:
+        lib.ctqmc_set_option(h, lib.CTQMC_OPT_PATH, {"panel": lib.CTQMC_PATH_PANEL, "grouped": lib.CTQMC_PATH_GROUPED,
+                                                     "large": lib.CTQMC_PATH_LARGE}[path])
+        ref = lib.ctqmc_trace_batch(h, batch.beta, off, sym, tau, max_len=L)
+        refb = lib.ctqmc_bound_batch(h, batch.beta, off, sym, tau, 0, 8, max_len=L)
+        torch.cuda.synchronize()
+        lb_full = lib.ctqmc_last_stats(h)
+        lib.ctqmc_trace_batch(h, batch.beta, off, sym, tau, max_len=L)
+        lt_full = lib.ctqmc_last_stats(h)
+        full = lt_full["arena_bytes"]          # the larger of the two calls' needs
+        assert full > 0 and lt_full["strings"] > 0
+        small = max(full // 5, 1 << 16)
+        lib.ctqmc_set_option(h, lib.CTQMC_OPT_ARENA_BYTES, small)
+        gotb = lib.ctqmc_bound_batch(h, batch.beta, off, sym, tau, 0, 8, max_len=L)
+        lb_r = lib.ctqmc_last_stats(h)
+        got = lib.ctqmc_trace_batch(h, batch.beta, off, sym, tau, max_len=L)
+        lt_r = lib.ctqmc_last_stats(h)
+        torch.cuda.synchronize()
+        for x, y in zip(ref + refb, got + gotb):
+            assert torch.equal(x, y)
+        assert lt_r["arena_bytes"] == small
+        assert lt_r["launches"] > lt_full["launches"] or lb_r["launches"] > lb_full["launches"]      # the larger call ran in rounds
+        assert (lt_r["strings"], lt_r["alg_flops"]) == (lt_full["strings"], lt_full["alg_flops"])
+        lib.ctqmc_set_option(h, lib.CTQMC_OPT_ARENA_BYTES, 4096)
+        out = (torch.full((n, 2), -7.0, dtype=torch.float64, device="cuda"), torch.zeros(n, dtype=torch.int64, device="cuda"),
+               torch.zeros((n, imp.n_sectors), dtype=torch.uint8, device="cuda"), torch.full((n,), -1, dtype=torch.int32, device="cuda"))
+        with pytest.raises(lib.CtqmcError) as ei:
+            lib.ctqmc_trace_batch(h, batch.beta, off, sym, tau, out=out, max_len=L)
+        assert ei.value.code == lib.binding.CTQMC_ERR_OOM
+        torch.cuda.synchronize()
+        assert (out[0] == -7.0).all().item() and (out[3] == -1).all().item()
+        lib.ctqmc_set_option(h, lib.CTQMC_OPT_ARENA_BYTES, 0)     # back to automatic growth
+        got = lib.ctqmc_trace_batch(h, batch.beta, off, sym, tau, max_len=L)
+        torch.cuda.synchronize()
+        for x, y in zip(ref, got):
+            assert torch.equal(x, y)
+    finally:
+        h.free()
+
+
+def test_corrupt_offsets_and_understated_max_len_give_status_2(lib, torch_cuda, impurities, handles):
+    """A corrupt offset array (negative, beyond n_ops, decreasing) or a configuration longer than the stated max_len must
+    give status 2 / NaN for that configuration, never an out-of-bounds read, and leave the neighbours alone -- on the
+    single-launch small path and on the routed paths."""
+    from workloads import make_batch
+    torch = torch_cuda
+    for cfg, n, paths in ((2, 12, [0, 1, 4, 2]), (3, 6, [1, 4, 2])):
+        h = handles(cfg)
+        batch = make_batch(cfg, n, start=24000)
+        L = int(np.diff(batch.offset).max())
+        off, sym, tau = _dev(torch, batch)
+        for path in paths:
+            lib.ctqmc_set_option(h, lib.CTQMC_OPT_PATH, path)
+            try:
+                good = lib.ctqmc_trace_batch(h, batch.beta, off, sym, tau, max_len=L)
+                torch.cuda.synchronize()
+                # (i) configuration 2 starts at a negative offset, configuration 4 ends beyond n_ops
+                bad = batch.offset.copy()
+                bad[2] = -5
+                bad[5] = len(batch.symbol) + 1000
+                boff = torch.from_numpy(bad).cuda()
+                got = lib.ctqmc_trace_batch(h, batch.beta, boff, sym, tau, max_len=L)
+                torch.cuda.synchronize()
+                st = got[3].cpu().numpy()
+                for b in range(n):
+                    if b in (1, 2, 4, 5):      # each corrupt offset spoils the configuration before and after it
+                        assert st[b] == 2 and torch.isnan(got[0][b]).all(), (cfg, path, b, st)
+                    else:
+                        assert st[b] == good[3][b].item() and torch.equal(got[0][b], good[0][b]) and got[1][b] == good[1][b]
+                # (ii) max_len understated: longer configurations are invalid, the others unchanged
+                lens = np.diff(batch.offset)
+                cut = int(np.sort(lens)[n // 2])
+                got = lib.ctqmc_trace_batch(h, batch.beta, off, sym, tau, max_len=cut)
+                torch.cuda.synchronize()
+                for b in range(n):
+                    if lens[b] > cut:
+                        assert got[3][b].item() == 2 and torch.isnan(got[0][b]).all()
+                    else:
+                        assert torch.equal(got[0][b], good[0][b]) and got[1][b] == good[1][b]
+                bm = lib.ctqmc_bound_batch(h, batch.beta, boff, sym, tau, 0, 1, max_len=L)
+                torch.cuda.synchronize()
+                assert bm[4][2].item() == 2 and bm[4][0].item() == 0
+            finally:
+                lib.ctqmc_set_option(h, lib.CTQMC_OPT_PATH, lib.CTQMC_PATH_AUTO)
+
+
+def test_spectral_bound_with_near_degenerate_singular_values(lib, torch_cuda):
+    """sigma_max comes from a power iteration, which converges from below and stalls when the two largest singular values
+    are 1 and 1 - 1e-9: the library must then fall back to its rigorous upper estimate, so that the spectral S = 1 bound still
+    dominates the exact one (oracle: SVD) and the trace."""
+    import types
+    from oracle import trace_oracle as O
+    from workloads import Batch
+    from workloads.rng import Stream
+    rng = Stream(515)
+    d = 6
+
+    def orth():
+        m = np.array([[rng.normal() for _ in range(d)] for _ in range(d)])
+        return np.linalg.qr(m)[0]
+
+    sv = np.array([1.0, 1.0 - 1e-9, 0.7, 0.4, 0.2, 0.1])
+    blocks = [orth() @ np.diag(sv) @ orth().T, orth() @ np.diag(sv[::-1].copy()) @ orth().T]
+    data = np.concatenate([b.reshape(-1, order="F") for b in blocks])
+    imp = types.SimpleNamespace(dims=np.array([d, d], np.int32), energy=np.array([0.1 * i for i in range(2 * d)]), n_symbols=2,
+                                is_complex=False, n_sectors=2, beta=2.0, blk_symbol=np.array([0, 1], np.int32),
+                                blk_src=np.array([0, 1], np.int32), blk_dst=np.array([1, 0], np.int32),
+                                blk_offset=np.array([0, d * d], np.int64), blk_data=data)
+    batch = Batch.from_lists(2.0, [([0, 1], [0.3, 1.1]), ([0, 1, 0, 1], [0.1, 0.5, 0.9, 1.7]), ([1, 0], [0.2, 0.4])])
+    h = lib.ctqmc_load_impurity(imp, 0)
+    try:
+        off, sym, tau = _dev(torch_cuda, batch)
+        bm, be, sm, se, st = lib.ctqmc_bound_batch(h, 2.0, off, sym, tau, 1, 1)
+        mant, exp2, _, _ = lib.ctqmc_trace_batch(h, 2.0, off, sym, tau)
+        torch_cuda.cuda.synchronize()
+        for b in range(batch.n_configs):
+            s, t = batch.config(b)
+            r = O.bound_config(imp, 2.0, s, t, 1, 1)
+            assert scaled_ge(bm[b].item() * (1 + 1e-12), int(be[b].item()), r["mant"], r["exp2"]), f"config {b}: spectral bound below the exact one"
+            assert scaled_ge(bm[b].item(), int(be[b].item()), abs(complex(mant[b, 0].item(), mant[b, 1].item())), int(exp2[b].item()))
+        _check_trace(lib, torch_cuda, imp, h, batch, "near-degenerate")
+    finally:
+        h.free()
+
+
+def test_odd_sector_dimension_with_a_dirty_arena_and_large_exponents(lib, torch_cuda):
+    """Grouped real kernel, odd sector dimensions: its 16-byte loads read one row beyond an odd-dimensional column.  With
+    Delta (E - Emin) > 800 on every populated row that row is scaled by 2^(+large); whatever an earlier call left in the arena
+    there must not reach the result (stale * 2^k -> inf, inf * 0 -> NaN).  A first call with 7-dimensional sectors
+    dirties the arena, the second runs 5- and 3-dimensional ones over the same memory."""
+    import types
+    from workloads import Batch
+    from workloads.rng import Stream
+    rng = Stream(9091)
+    torch = torch_cuda
+
+    def make(d0, d1, spread):
+        blocks = [(0, 0, 1), (1, 1, 0), (2, 0, 0)]
+        dims = (d0, d1)
+        data, off, pos = [], [], 0
+        for _, s_, d_ in blocks:
+            m, n = dims[d_], dims[s_]
+            data.append(np.array([rng.normal() for _ in range(m * n)]) * (0.9 / np.sqrt(max(m, n))))
+            off.append(pos); pos += m * n
+        energy = np.concatenate([[0.0] + [spread * (1.0 + 0.01 * i) for i in range(1, d0)], [0.0] + [spread * (1.0 + 0.013 * i) for i in range(1, d1)]])
+        return types.SimpleNamespace(dims=np.array(dims, np.int32), energy=energy, n_symbols=3, is_complex=False, n_sectors=2, name="odd",
+                                     blk_symbol=np.array([b[0] for b in blocks], np.int32), blk_src=np.array([b[1] for b in blocks], np.int32),
+                                     blk_dst=np.array([b[2] for b in blocks], np.int32), blk_offset=np.array(off, np.int64),
+                                     blk_data=np.concatenate(data))
+
+    beta = 10.0
+
+    def walks(count):
+        cfgs = []
+        for _ in range(count):
+            q, syms = 0, []
+            for _ in range(4 + rng.integer(12)):
+                a = (rng.integer(2) * 2) if q == 0 else 1
+                syms.append(a)
+                q = 1 if a == 0 else 0
+            if q == 1:
+                syms.append(1)
+            cfgs.append((syms, np.sort(beta * rng.uniforms(len(syms)))))
+        return Batch.from_lists(beta, cfgs)
+
+    big = make(7, 7, 0.3)
+    h = lib.ctqmc_load_impurity(big, 0)
+    try:
+        lib.ctqmc_set_option(h, lib.CTQMC_OPT_PATH, lib.CTQMC_PATH_GROUPED)
+        _check_trace(lib, torch, big, h, walks(70), "odd-dirty-7")
+    finally:
+        h.free()
+    for dims in ((5, 3), (3, 5), (7, 1)):
+        imp = make(dims[0], dims[1], 900.0)          # Delta (E - Emin) ~ 900 per time unit on every row but the lowest
+        h = lib.ctqmc_load_impurity(imp, 0)
+        try:
+            for path in (lib.CTQMC_PATH_GROUPED, lib.CTQMC_PATH_LARGE, lib.CTQMC_PATH_PANEL):
+                lib.ctqmc_set_option(h, lib.CTQMC_OPT_PATH, path)
+                _check_trace(lib, torch, imp, h, walks(70), f"odd-{dims}-path{path}")
+        finally:
+            h.free()
