@@ -845,6 +845,11 @@ extern "C" int ctqmc_set_option(ctqmc_impurity* h, int option, int64_t value) {
   if (option == CTQMC_OPT_SCRATCH_LIMIT) {
     if (value < 0) return fail(CTQMC_ERR_ARG, "scratch limit must be >= 0");
     h->scratch_limit = (long long)value;
+    Arena& a = h->arena;
+    if (value > 0 && a.fixed_bytes == 0 && a.cap > (size_t)value) {   // an arena already larger than the new limit is released
+      CU(cudaDeviceSynchronize());
+      cudaFree(a.base); a.base = nullptr; a.cap = 0;
+    }
     return 0;
   }
   if (option == CTQMC_OPT_ARENA_BYTES) {
@@ -920,16 +925,15 @@ extern "C" int ctqmc_trace_batch(ctqmc_impurity* h, double beta, const ctqmc_bat
     Arena& a = h->arena;
     const BatchView bv = make_view(batch, beta, 0, B, Lmax);
     mark(h, 0, st);
-    CU(cudaMemsetAsync(a.cnt, 0, sizeof(Counters), st));
     mark(h, 1, st);
-    SmallParams sp;
+    SmallParams sp;   // the one launch adds its counters straight into the call's totals (zeroed above)
     sp.imp = h->dev; sp.bv = bv; sp.pack = h->d_pack; sp.pblk = h->d_pblk; sp.n_blocks = h->n_blocks; sp.pack_len = h->pack_len;
     sp.n_energy = h->n_energy; sp.literal = (h->schedule == CTQMC_SCHEDULE_LITERAL); sp.mant = mant; sp.exp2 = (long long*)exp2;
-    sp.survive = survive; sp.status = status; sp.cnt = a.cnt; sp.dmax = h->dev.dmax;
+    sp.survive = survive; sp.status = status; sp.cnt = a.cnt_total; sp.dmax = h->dev.dmax;
     if (h->small2) {
       Small2Params s2;
       s2.imp = h->dev; s2.bv = bv; s2.ftpad = h->d_ftpad; s2.binfo = h->d_binfo; s2.n_blocks = h->n_blocks; s2.literal = sp.literal;
-      s2.mant = mant; s2.exp2 = (long long*)exp2; s2.survive = survive; s2.status = status; s2.cnt = a.cnt;
+      s2.mant = mant; s2.exp2 = (long long*)exp2; s2.survive = survive; s2.status = status; s2.cnt = a.cnt_total;
       // CTA size: small batches are latency-bound, so they are spread over all SMs in ONE wave: warps per CTA =
       // ceil(configurations per SM / configurations per warp), at most the configured maximum
       const int gpw = 32 / h->small2_dp, max_warps = h->small2_threads / 32;
@@ -955,8 +959,7 @@ extern "C" int ctqmc_trace_batch(ctqmc_impurity* h, double beta, const ctqmc_bat
       if (grid > h->small_grid_max) grid = h->small_grid_max;
       pick_small(h->dev.cplx, h->small_g)<<<(unsigned)grid, kCtaThreads, h->small_smem, st>>>(sp);
     }
-    accumulate_counters_kernel<<<1, 1, 0, st>>>(a.cnt, a.cnt_total);
-    h->last_launches += 2;
+    h->last_launches += 1;
     mark(h, 2, st);
     mark(h, 3, st);
     h->timing_valid = h->timing;

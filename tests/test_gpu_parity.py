@@ -705,7 +705,11 @@ def _check_bound(lib, torch, imp, handle, batch, norm_kind, S, label, golden=Non
                 dq = rel_diff(sm[b, q0], int(se[b, q0]), sec[0], sec[1])
                 assert dq <= TOL + floor_q, f"{label} config {b} sector {q0}: rel diff {dq:.3e} (rounding floor {floor_q:.1e})"
             zs, es = tsec[q0]
-            assert scaled_ge(sm[b, q0], int(se[b, q0]), abs(zs), es), f"{label} config {b} sector {q0}: B(q0) < |t(q0)|"
+            if S == 1:      # tables: strict
+                assert scaled_ge(sm[b, q0], int(se[b, q0]), abs(zs), es), f"{label} config {b} sector {q0}: B(q0) < |t(q0)|"
+            else:           # segment products: B(q0) + 2^-40 B(configuration) >= |t(q0)| (floor of fl(G))
+                ok = scaled_ge(sm[b, q0], int(se[b, q0]), abs(zs), es) or scaled_ge(r["mant"], r["exp2"] - 40, abs(zs), es)
+                assert ok, f"{label} config {b} sector {q0}: B(q0) + 2^-40 B < |t(q0)|"
         w = abs(complex(mant[b, 0], mant[b, 1]))
         assert scaled_ge(bm[b], int(be[b]), w, int(exp2[b])), f"{label} config {b}: bound < |trace|"
 
