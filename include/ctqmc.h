@@ -203,6 +203,87 @@ int ctqmc_last_timing(ctqmc_impurity* imp, double ms[4]);
  * MEASURED_PEAKS.json holds HBM and bf16 peaks only.  HOST outputs; synchronises. */
 int ctqmc_measure_fp64_peak(int device, double* tflops_dmma, double* tflops_dfma);
 
+/* ------------------------------------------------------------------------------------------------------------------------
+ * Chain sets: the incremental, lazy local trace for many Markov chains at once.
+ *
+ * "we can store these subproducts in a data structure, e.g., a balanced binary tree or a skip-list ... requiring
+ * O[log(k)] matrix multiplications rather than O(k)".  PAPER.md:542-548 (lazy trace): the random number of the Metropolis
+ * test is drawn first; bounds from submultiplicative norms of the stored sub-products decide the move as early as possible,
+ * start sectors being evaluated one at a time.  PAPER.md:560-574: many chains share one device, device memory is one
+ * pre-allocated block, only asynchronous calls.  The paper defers the data structure to its Ref. [9]; readings F1-F4 of
+ * DESIGN.md fix it:
+ *
+ *   F1  every chain owns a complete binary tree over a FIXED dyadic partition of [0, beta) into 2^depth leaves; node (l, i)
+ *       stores, for every sector q that survives it, the evolution operator across its interval (propagators to both ends
+ *       included) as a dense matrix with an integer and a real exponent, its target sector and its Frobenius norm;
+ *   F2  a proposal dirties the leaves containing its times and their ancestors: at most max_edits * (depth + 1) nodes;
+ *   F3  bound of a proposal without multiplying the dirty ancestors: B(q0) = sqrt(r) * prod ||U_node||_F over the cover of the
+ *       time axis by the recomputed dirty leaves and the maximal clean subtrees, r = smallest sector dimension at its seams,
+ *       rounded outward by (1 + 2^-40);
+ *   F4  decision against the caller's threshold T on |w_new| (log2 T per chain): sum_q0 B(q0) <= T rejects at once; else the
+ *       start sectors are evaluated exactly in order of decreasing bound, and with S the sum so far and R the sum of the
+ *       remaining bounds, |S| - R > T accepts and |S| + R <= T rejects.  An accepted proposal is completed (all sectors), so
+ *       its trace is returned.
+ *
+ * All chains advance in lock-step through the same launches; which chains still need work is decided on the device.  Every
+ * call only enqueues on `cuda_stream`; nothing is read back and nothing is allocated after ctqmc_chains_create.
+ * Sector dimensions up to 512 (dense nodes per chain: "the simulation drops the Markov chain if the memory
+ * request is denied" -- here ctqmc_chains_create returns CTQMC_ERR_OOM with the size needed). */
+typedef struct ctqmc_chains ctqmc_chains;
+
+typedef struct {
+  int64_t n_chains;        /* C >= 1 */
+  int32_t depth;           /* the time axis is cut into 2^depth leaves (choose 2^depth ~ expansion order) */
+  int32_t leaf_capacity;   /* operators one leaf can hold (1 .. 64); a proposal that overflows a leaf gets status 4 */
+  int32_t max_edits;       /* inserted + removed operators per chain per proposal (1 .. 16); 4 covers a pair move */
+  int32_t lazy_rounds;     /* start sectors evaluated one at a time (one round of launches each) before the remaining
+                              sectors of still-undecided chains are evaluated together; 0 = all at once */
+} ctqmc_chains_desc;
+
+/* Proposed edits in CSR form, DEVICE pointers: chain c proposes edits [offset[c], offset[c+1]): operator (symbol, tau) is
+ * inserted (kind = +1) or removed (kind = -1; it must be present with exactly this tau).  n_edits is a HOST value. */
+typedef struct {
+  const int64_t* offset;   /* [C+1] */
+  const double*  tau;      /* [n_edits] */
+  const int32_t* symbol;   /* [n_edits] */
+  const int32_t* kind;     /* [n_edits] */
+  int64_t        n_edits;
+} ctqmc_edit_batch;
+
+/* Per-chain status of a proposal */
+#define CTQMC_CHAIN_OK          0
+#define CTQMC_CHAIN_BAD_EDIT    2   /* tau outside [0, beta), symbol out of range, kind not +-1, too many edits, corrupt offsets */
+#define CTQMC_CHAIN_NOT_FOUND   3   /* removal of an operator the chain does not hold */
+#define CTQMC_CHAIN_LEAF_FULL   4   /* a leaf would hold more than leaf_capacity operators */
+
+/* Allocates the chain set in ONE device block and builds the trees of the empty configuration (w_loc = Z). */
+int ctqmc_chains_create(ctqmc_impurity* imp, double beta, const ctqmc_chains_desc* desc, void* cuda_stream, ctqmc_chains** out);
+void ctqmc_chains_destroy(ctqmc_chains* chains);
+
+/* Lazy evaluation of one proposal per chain (readings F3, F4); the chains are not modified.  DEVICE pointers:
+ *   log2_threshold [C]  log2 of T (-inf accepts every non-vanishing proposal); NULL = -inf for every chain
+ *   accept [C]          1 / 0;   decided_by [C]  0 = by the bound alone, 1 = after part of the sectors, 2 = after all
+ *   n_sectors_evaluated [C]  start sectors whose exact term entered the decision (all of them when accepted)
+ *   bound_mant / bound_exp2 [C]  sum_q0 B(q0) of the proposed configuration (NaN for a non-zero status)
+ *   trace_mant [C][2] / trace_exp2 [C]  w_loc of the proposed configuration when accepted, else 0
+ *   status [C]          CTQMC_CHAIN_*; a chain with non-zero status is not accepted */
+int ctqmc_chains_propose(ctqmc_chains* chains, const ctqmc_edit_batch* edits, const double* log2_threshold, int32_t* accept,
+                         int32_t* decided_by, int32_t* n_sectors_evaluated, double* bound_mant, int64_t* bound_exp2,
+                         double* trace_mant, int64_t* trace_exp2, int32_t* status, void* cuda_stream);
+
+/* Applies the most recent proposal of every chain c with mask[c] != 0 (DEVICE [C]; NULL = its accept flags): the proposed
+ * operators become the configuration, the shadow nodes the stored sub-products (entries the lazy evaluation never needed
+ * are multiplied now).  Committing swaps slot indices; nothing is copied. */
+int ctqmc_chains_commit(ctqmc_chains* chains, const int32_t* mask, void* cuda_stream);
+
+/* w_loc of every chain's current configuration from its stored root: mant [C][2], exp2 [C] (DEVICE). */
+int ctqmc_chains_trace(ctqmc_chains* chains, double* mant, int64_t* exp2, void* cuda_stream);
+
+/* HOST outputs; synchronises the stream of the most recent call: stats[0] = matrix products performed since creation,
+ * stats[1] = bytes of the chain set's device block, stats[2] = kernels enqueued by the most recent call,
+ * stats[3] = node slots per chain (stored + shadow + scratch). */
+int ctqmc_chains_stats(ctqmc_chains* chains, int64_t stats[4]);
+
 /* Thread-local description of the last error on this thread ("" if none). */
 const char* ctqmc_last_error(void);
 

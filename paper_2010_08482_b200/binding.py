@@ -21,8 +21,12 @@ CTQMC_SCHEDULE_THIN, CTQMC_SCHEDULE_LITERAL = 0, 1
 CTQMC_OPT_SCHEDULE, CTQMC_OPT_PANEL_WIDTH, CTQMC_OPT_TIMING, CTQMC_OPT_PATH, CTQMC_OPT_SCRATCH_LIMIT, CTQMC_OPT_ARENA_BYTES = 1, 2, 3, 4, 5, 6
 CTQMC_PATH_AUTO, CTQMC_PATH_PANEL, CTQMC_PATH_LARGE, CTQMC_PATH_SMALL, CTQMC_PATH_GROUPED = 0, 1, 2, 3, 4
 
+CTQMC_CHAIN_OK, CTQMC_CHAIN_BAD_EDIT, CTQMC_CHAIN_NOT_FOUND, CTQMC_CHAIN_LEAF_FULL = 0, 2, 3, 4
+
 EXPORTS = ["ctqmc_load_impurity", "ctqmc_free_impurity", "ctqmc_set_option", "ctqmc_trace_batch", "ctqmc_bound_batch",
-           "ctqmc_trace_batch_host", "ctqmc_bound_batch_host", "ctqmc_last_stats", "ctqmc_last_timing", "ctqmc_measure_fp64_peak", "ctqmc_last_error"]
+           "ctqmc_trace_batch_host", "ctqmc_bound_batch_host", "ctqmc_last_stats", "ctqmc_last_timing", "ctqmc_measure_fp64_peak", "ctqmc_last_error",
+           "ctqmc_chains_create", "ctqmc_chains_destroy", "ctqmc_chains_propose", "ctqmc_chains_commit", "ctqmc_chains_trace",
+           "ctqmc_chains_stats"]
 
 
 class CtqmcError(RuntimeError):
@@ -40,6 +44,15 @@ class _Desc(C.Structure):
 class _Batch(C.Structure):
     _fields_ = [("n_configs", C.c_int64), ("offset", C.c_void_p), ("symbol", C.c_void_p), ("tau", C.c_void_p),
                 ("n_ops", C.c_int64), ("max_len", C.c_int32)]
+
+
+class _ChainsDesc(C.Structure):
+    _fields_ = [("n_chains", C.c_int64), ("depth", C.c_int32), ("leaf_capacity", C.c_int32), ("max_edits", C.c_int32),
+                ("lazy_rounds", C.c_int32)]
+
+
+class _EditBatch(C.Structure):
+    _fields_ = [("offset", C.c_void_p), ("tau", C.c_void_p), ("symbol", C.c_void_p), ("kind", C.c_void_p), ("n_edits", C.c_int64)]
 
 
 _lib = None
@@ -76,6 +89,18 @@ def library() -> C.CDLL:
         lib.ctqmc_measure_fp64_peak.restype = C.c_int
         lib.ctqmc_last_error.argtypes = []
         lib.ctqmc_last_error.restype = C.c_char_p
+        lib.ctqmc_chains_create.argtypes = [vp, dbl, C.POINTER(_ChainsDesc), vp, C.POINTER(vp)]
+        lib.ctqmc_chains_create.restype = C.c_int
+        lib.ctqmc_chains_destroy.argtypes = [vp]
+        lib.ctqmc_chains_destroy.restype = None
+        lib.ctqmc_chains_propose.argtypes = [vp, C.POINTER(_EditBatch)] + [vp] * 10
+        lib.ctqmc_chains_propose.restype = C.c_int
+        lib.ctqmc_chains_commit.argtypes = [vp, vp, vp]
+        lib.ctqmc_chains_commit.restype = C.c_int
+        lib.ctqmc_chains_trace.argtypes = [vp, vp, vp, vp]
+        lib.ctqmc_chains_trace.restype = C.c_int
+        lib.ctqmc_chains_stats.argtypes = [vp, C.POINTER(i64 * 4)]
+        lib.ctqmc_chains_stats.restype = C.c_int
         _lib = lib
     return _lib
 
@@ -267,3 +292,92 @@ def ctqmc_bound_batch_host(imp: ImpurityHandle, beta: float, offset, symbol, tau
                                             se.ctypes.data if want_sector else None, status.ctypes.data,
                                             _stream_ptr(stream, host=True)))
     return bm, be, sm, se, status
+
+
+# ----------------------------------------------------------------------------------------------- chain sets (lazy trace)
+class ChainsHandle:
+    """Owns a `ctqmc_chains*` (and keeps its impurity alive).  Created by `ctqmc_chains_create`."""
+
+    def __init__(self, ptr: int, imp: ImpurityHandle, n_chains: int):
+        self._ptr = C.c_void_p(ptr)
+        self.imp = imp
+        self.n_chains = n_chains
+
+    @property
+    def ptr(self):
+        if not self._ptr:
+            raise CtqmcError(CTQMC_ERR_ARG, "chain set already destroyed")
+        return self._ptr
+
+    def destroy(self):
+        if self._ptr:
+            library().ctqmc_chains_destroy(self._ptr)
+            self._ptr = C.c_void_p(None)
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+def ctqmc_chains_create(imp: ImpurityHandle, beta: float, n_chains: int, depth: int, leaf_capacity: int = 8, max_edits: int = 4,
+                        lazy_rounds: int = 1, stream=None) -> ChainsHandle:
+    d = _ChainsDesc(int(n_chains), int(depth), int(leaf_capacity), int(max_edits), int(lazy_rounds))
+    out = C.c_void_p(None)
+    _check(library().ctqmc_chains_create(imp.ptr, float(beta), C.byref(d), _stream_ptr(stream), C.byref(out)))
+    return ChainsHandle(out.value, imp, int(n_chains))
+
+
+def ctqmc_chains_destroy(chains: ChainsHandle):
+    chains.destroy()
+
+
+def ctqmc_chains_propose(chains: ChainsHandle, edit_offset, edit_tau, edit_symbol, edit_kind, log2_threshold=None, stream=None):
+    """edit_offset int64[C+1], edit_tau float64[n], edit_symbol int32[n], edit_kind int32[n] (+1 insert, -1 remove),
+    log2_threshold float64[C] or None: torch CUDA tensors.  Returns a dict of torch CUDA tensors (accept, decided_by,
+    n_sectors_evaluated, bound_mant, bound_exp2, trace_mant[C,2], trace_exp2, status); asynchronous on `stream`."""
+    import torch
+    nC = chains.n_chains
+    dev = edit_offset.device
+    assert edit_offset.is_cuda and edit_offset.dtype == torch.int64 and edit_offset.numel() == nC + 1
+    assert edit_tau.dtype == torch.float64 and edit_symbol.dtype == torch.int32 and edit_kind.dtype == torch.int32
+    assert edit_tau.numel() == edit_symbol.numel() == edit_kind.numel()
+    if log2_threshold is not None:
+        assert log2_threshold.is_cuda and log2_threshold.dtype == torch.float64 and log2_threshold.numel() == nC
+    i32 = dict(dtype=torch.int32, device=dev)
+    out = dict(accept=torch.empty(nC, **i32), decided_by=torch.empty(nC, **i32), n_sectors_evaluated=torch.empty(nC, **i32),
+               bound_mant=torch.empty(nC, dtype=torch.float64, device=dev), bound_exp2=torch.empty(nC, dtype=torch.int64, device=dev),
+               trace_mant=torch.empty((nC, 2), dtype=torch.float64, device=dev), trace_exp2=torch.empty(nC, dtype=torch.int64, device=dev),
+               status=torch.empty(nC, **i32))
+    n = edit_tau.numel()
+    eb = _EditBatch(edit_offset.data_ptr(), edit_tau.data_ptr() if n else None, edit_symbol.data_ptr() if n else None,
+                    edit_kind.data_ptr() if n else None, n)
+    _check(library().ctqmc_chains_propose(chains.ptr, C.byref(eb), log2_threshold.data_ptr() if log2_threshold is not None else None,
+                                          out["accept"].data_ptr(), out["decided_by"].data_ptr(), out["n_sectors_evaluated"].data_ptr(),
+                                          out["bound_mant"].data_ptr(), out["bound_exp2"].data_ptr(), out["trace_mant"].data_ptr(),
+                                          out["trace_exp2"].data_ptr(), out["status"].data_ptr(), _stream_ptr(stream)))
+    return out
+
+
+def ctqmc_chains_commit(chains: ChainsHandle, mask=None, stream=None):
+    """mask: int32[C] torch CUDA tensor, or None = the accept flags of the most recent proposal."""
+    import torch
+    if mask is not None:
+        assert mask.is_cuda and mask.dtype == torch.int32 and mask.numel() == chains.n_chains
+    _check(library().ctqmc_chains_commit(chains.ptr, mask.data_ptr() if mask is not None else None, _stream_ptr(stream)))
+
+
+def ctqmc_chains_trace(chains: ChainsHandle, stream=None):
+    import torch
+    nC = chains.n_chains
+    mant = torch.empty((nC, 2), dtype=torch.float64, device="cuda")
+    exp2 = torch.empty(nC, dtype=torch.int64, device="cuda")
+    _check(library().ctqmc_chains_trace(chains.ptr, mant.data_ptr(), exp2.data_ptr(), _stream_ptr(stream)))
+    return mant, exp2
+
+
+def ctqmc_chains_stats(chains: ChainsHandle) -> dict:
+    buf = (C.c_int64 * 4)()
+    _check(library().ctqmc_chains_stats(chains.ptr, C.byref(buf)))
+    return dict(zip(["products", "bytes", "launches", "slots_per_chain"], [int(x) for x in buf]))

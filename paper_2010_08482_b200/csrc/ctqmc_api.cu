@@ -1343,3 +1343,5 @@ extern "C" int ctqmc_measure_fp64_peak(int device, double* tflops_dmma, double* 
 }
 
 extern "C" const char* ctqmc_last_error(void) { return g_err.c_str(); }
+
+#include "lazy_api.cuh"
