@@ -68,7 +68,7 @@ def _check_traces(lib, torch, ch, oracles, imp, beta, label):
 
 
 @pytest.mark.parametrize("cfg,depth,n_chains,n_steps,lazy_rounds", [(1, 3, 6, 10, 1), (2, 5, 5, 8, 2), (2, 4, 3, 5, 0), (3, 4, 2, 4, 1),
-                                                                      (4, 3, 2, 4, 2)])
+                                                                      (4, 3, 2, 7, 2)])
 def test_chains_follow_the_lazy_oracle(lib, torch_cuda, impurities, cfg, depth, n_chains, n_steps, lazy_rounds):
     from oracle import lazy_oracle as LZ
     from workloads import make_batch
@@ -86,7 +86,7 @@ def test_chains_follow_the_lazy_oracle(lib, torch_cuda, impurities, cfg, depth, 
         #      configurations are arbitrary, most of them vanish)
         starts = [_ops_of(make_batch(cfg, 1, start=40 + c), 0) for c in range(n_chains)]
         if cfg == 4:
-            starts = [s[:48] for s in starts]      # keeps the oracle's share of the test short
+            starts = [[] for _ in starts]          # grown from the empty configuration by the pair moves below (keeps the oracle's share short)
         nchunk = max((len(s) + 7) // 8 for s in starts)
         ones = torch.ones(n_chains, dtype=torch.int32, device="cuda")
         for k in range(nchunk):
