@@ -73,7 +73,7 @@ __global__ void __launch_bounds__(512) small2_trace_kernel(Small2Params P) {
   int* s_sv = s_qs + Q;   // [Q + 1]: start sectors with a chain to multiply, then their count
 
   const long long n_groups = (long long)gridDim.x * groups_per_cta;
-  unsigned long long st_strings = 0, st_flops = 0, st_exp = 0;
+  unsigned long long st_strings = 0, st_flops = 0, st_exp = 0, st_pmacs = 0;
   for (long long b = (long long)blockIdx.x * groups_per_cta + grp_in_cta; b < P.bv.B; b += n_groups) {
     const long long lo = P.bv.offset[b];
     const long long hi_off = P.bv.offset[b + 1];
@@ -220,6 +220,7 @@ __global__ void __launch_bounds__(512) small2_trace_kernel(Small2Params P) {
         if (lg == 0) {
           if (!dead) for (int n = 0; n < c; ++n) tr += X[n * DP + n];
           st_strings += 1; st_flops += macs * (unsigned long long)c * 2ull; st_exp += nexp;
+          st_pmacs += (unsigned long long)L * (unsigned long long)(DP * DP * c);   // executed: every step multiplies the padded DP x DP block
         }
         __syncwarp(mask);
       }
@@ -267,7 +268,7 @@ __global__ void __launch_bounds__(512) small2_trace_kernel(Small2Params P) {
     atomicAdd(&P.cnt->n_strings, st_strings);
     atomicAdd(&P.cnt->n_slots, st_strings);
     atomicAdd(&P.cnt->alg_flops, st_flops);
-    atomicAdd(&P.cnt->macs, st_flops / 2);
+    atomicAdd(&P.cnt->macs, st_pmacs);
     atomicAdd(&P.cnt->n_exp, st_exp);
   }
 }
