@@ -32,7 +32,7 @@ extern "C" {
 #define CTQMC_ERR_ARG         -1   /* null pointer, bad size, inconsistent description */
 #define CTQMC_ERR_OOM         -2   /* device or host allocation failed */
 #define CTQMC_ERR_CUDA        -3   /* a CUDA call or kernel launch failed */
-#define CTQMC_ERR_UNSUPPORTED -4   /* valid request the library does not implement (e.g. spectral norm with segment_len != 1) */
+#define CTQMC_ERR_UNSUPPORTED -4   /* valid request the library does not implement (e.g. a device that is not sm_100) */
 
 /* Per-configuration status values written to `status[b]`. */
 #define CTQMC_STATUS_OK        0
@@ -150,7 +150,10 @@ int ctqmc_trace_batch(ctqmc_impurity* imp, double beta, const ctqmc_batch* batch
  * G_j of `segment_len` consecutive factors (0 = the whole chain, i.e. one segment):
  *
  *   norm_kind 0 (Frobenius):  B(q0) = sqrt(d_min) * prod_j ||G_j||_F
- *   norm_kind 1 (spectral):   B(q0) = d_min * prod_i exp(-Delta_i Emin(q_i)) sigma_max(F_{alpha_i}(q_{i-1}))   (segment_len 1 only)
+ *   norm_kind 1 (spectral):   B(q0) = d_min * prod_j u_j, u_j a rigorous upper estimate of ||G_j||_2:
+ *                             segment_len 1:  u_i = exp(-Delta_i Emin(q_i)) sigma_max(F_{alpha_i}(q_{i-1}));
+ *                             otherwise:      u_j = min(||G_j||_F, prod_{i in segment j} u_i)  (||XY||_2 <= ||X||_2 ||Y||_2 and
+ *                             ||G||_2 <= ||G||_F; an iterative estimate of ||G_j||_2 approaches it from below and is not used).
  *                             sigma_max comes from a power iteration at load time, which approaches it from below: where the
  *                             iteration has not converged to 1e-10 (it converges exactly for c / c^dag blocks, whose F^H F is a
  *                             projector) the rigorous upper estimate min(||F||_F, sqrt(||F||_1 ||F||_inf)) is used instead, so the

@@ -242,6 +242,8 @@ def _string_bound(imp: _Imp, beta: float, symbols, taus, visited, norm_kind: int
     L = len(symbols)
     dmin = min(int(imp.dims[q]) for q in visited)
     pref = math.sqrt(dmin) if norm_kind == 0 else float(dmin)
+    if norm_kind == 2 and segment_len == 1:
+        norm_kind = 1          # one factor per segment: the estimate IS the factorised closed form
     if L == 0:
         q0 = visited[0]
         p = np.exp(-float(beta) * (imp.E[q0] - imp.Emin[q0]))
@@ -260,16 +262,29 @@ def _string_bound(imp: _Imp, beta: float, symbols, taus, visited, norm_kind: int
             lg += -deltas[start] * imp.Emin[q] * LOG2E
             continue
         M = np.eye(int(imp.dims[visited[start]]), dtype=np.complex128 if imp.is_complex else np.float64)
+        ex_seg = 0
         for i in range(start, stop):
             q_prev, q = visited[i], visited[i + 1]
             M = imp.F[(int(symbols[i]), q_prev)] @ M
             M, ex = _propagate(M, deltas[i], imp.E[q], imp.Emin[q])
             lg += -deltas[i] * imp.Emin[q] * LOG2E
             e2 += ex
+            ex_seg += ex
         if norm_kind == 0:
             nrm = math.sqrt(math.fsum((np.abs(M) ** 2).ravel()))
-        else:
+        elif norm_kind == 1:
             nrm = float(np.linalg.svd(M, compute_uv=False)[0])
+        else:
+            # norm_kind 2, the certified estimate of ||G_j||_2 the CUDA path returns for spectral bounds with S != 1 (DESIGN.md
+            # reading A1): min(||G_j||_F, prod_i sigma_max(F_i)); M is scaled by 2**-ex_seg, the sigma product is not
+            fro = math.sqrt(math.fsum((np.abs(M) ** 2).ravel()))
+            sprod = 1.0
+            for i in range(start, stop):
+                sprod *= float(np.linalg.svd(imp.F[(int(symbols[i]), visited[i])], compute_uv=False)[0])
+            if fro == 0.0 or math.log2(fro) + ex_seg <= math.log2(sprod):
+                nrm = fro
+            else:
+                nrm, e2 = sprod, e2 - ex_seg
         val *= nrm
         if val != 0.0:
             m, ex = math.frexp(val)
@@ -278,7 +293,8 @@ def _string_bound(imp: _Imp, beta: float, symbols, taus, visited, norm_kind: int
 
 
 def bound_config(desc, beta: float, symbols, taus, norm_kind: int = 0, segment_len: int = 1) -> dict:
-    """Upper bound on |w_loc| (and per start sector).  norm_kind 0 Frobenius / 1 spectral; segment_len S >= 1, 0 = whole
+    """Upper bound on |w_loc| (and per start sector).  norm_kind 0 Frobenius / 1 spectral (exact SVD of every segment
+    product) / 2 certified spectral estimate min(||G_j||_F, prod sigma_max(F_i)) >= ||G_j||_2; segment_len S >= 1, 0 = whole
     chain.  B(q0) = prefactor(d_min) * prod_j ||G_j||, G_j = product of S consecutive cyclic factors A_i;
     prefactor sqrt(d_min) (Frobenius) or d_min (spectral), d_min = min_i dim(q_i)  (|Tr M| <= sqrt(rank)||M||_F <= rank||M||_2).
     Returned values are multiplied by BOUND_INFLATION.  Keys: mant, exp2, sector (per q0 (mant, exp2) or None), status."""

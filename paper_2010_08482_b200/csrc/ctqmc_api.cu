@@ -995,8 +995,6 @@ extern "C" int ctqmc_bound_batch(ctqmc_impurity* h, double beta, const ctqmc_bat
   if (rc) return rc;
   if (norm_kind != 0 && norm_kind != 1) return fail(CTQMC_ERR_ARG, "norm_kind must be 0 (Frobenius) or 1 (spectral)");
   if (segment_len < 0) return fail(CTQMC_ERR_ARG, "segment_len < 0");
-  if (norm_kind == 1 && segment_len != 1)
-    return fail(CTQMC_ERR_UNSUPPORTED, "spectral norm is implemented for segment_len = 1 only");
   if ((sector_bound_mant == nullptr) != (sector_bound_exp2 == nullptr)) return fail(CTQMC_ERR_ARG, "sector_bound_mant / _exp2 must both be given or both be null");
   const long long B = batch->n_configs;
   if (B == 0) return 0;
@@ -1064,7 +1062,7 @@ extern "C" int ctqmc_bound_batch(ctqmc_impurity* h, double beta, const ctqmc_bat
     } else {
       rc = h->large ? enqueue_large(h, bv, rb, 1, S, Lmax, st) : enqueue_chain(h, bv, rb, 1, S, st);
       if (rc) return rc;
-      bp.norm_kind = 0; bp.segment_len = S;
+      bp.norm_kind = norm_kind; bp.segment_len = S;
       bound_segments_kernel<<<(unsigned)((nS + 127) / 128), 128, 0, st>>>(bp);
     }
     mark(h, 2, st);

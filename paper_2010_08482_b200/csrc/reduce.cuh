@@ -172,8 +172,12 @@ __global__ void bound_s1_kernel(BoundParams P) {
   if (lane == 0) P.sector[s] = finish_sector_bound(val, e, rec.lg + lgx);
 }
 
-// segment_len != 1, Frobenius: the chain kernel (mode 1) left sum |X|^2 per (segment, panel) in the slots; combine
-// panels of a segment at a common exponent, take the root, multiply the segments.  One thread per string.
+// segment_len != 1: the chain kernel (mode 1) left sum |X|^2 per (segment, panel) in the slots; combine panels of a segment
+// at a common exponent, take the root, multiply the segments.  One thread per string.
+// norm_kind 0: B = sqrt(d_min) prod_j ||G_j||_F.   norm_kind 1 ("spectral norm"): B = d_min prod_j u_j with
+// u_j = min(||G_j||_F, prod_{i in segment j} sigma_max(F_i)), both rigorous upper estimates of ||G_j||_2 (the propagator
+// part exp(-Delta (E - Emin)) <= 1 never increases a spectral norm; exp(-Delta Emin) is in lg): an iterative estimate of
+// ||G_j||_2 itself approaches it from below and cannot be certified, so it is not used (reading A1).
 __global__ void bound_segments_kernel(BoundParams P) {
   const int Q = P.imp.Q;
   long long s = blockIdx.x * (long long)blockDim.x + threadIdx.x;
@@ -184,9 +188,9 @@ __global__ void bound_segments_kernel(BoundParams P) {
   const StringRec rec = P.strings[s];
   const long long lo = P.bv.offset[b];
   const int L = (int)(P.bv.offset[b + 1] - lo);
-  double val = sqrt((double)rec.dmin);
+  double val = P.norm_kind == 0 ? sqrt((double)rec.dmin) : (double)rec.dmin;
   long long e = 0;
-  if (L == 0) {
+  if (L == 0 && P.norm_kind == 0) {
     const double* E = P.imp.energy + P.imp.e_off[q0];
     const double emin = P.imp.e_min[q0];
     double ss = 0.0;
@@ -209,12 +213,14 @@ __global__ void bound_segments_kernel(BoundParams P) {
         ss += shift_clamped(sl.re, 2 * sl.e2 - emax);
       }
     }
-    val *= sqrt(ss);
-    e += emax / 2;
+    const double fro = sqrt(ss);
+    const int stop = min(L, i + P.segment_len);
+    double sprod = 1.0;
+    for (; i < stop; ++i) { const int blk = P.imp.blk_of[P.bv.symbol[lo + i] * Q + q]; sprod *= P.imp.sigma[blk]; q = P.imp.blks[blk].dst; }
+    if (P.norm_kind == 0 || fro == 0.0 || log2(fro) + (double)(emax / 2) <= log2(sprod)) { val *= fro; e += emax / 2; }
+    else val *= sprod;
     if (val != 0.0) { int k = ilogb(val); val = scalbn(val, -k); e += k; } else { e = 0; }
     slot += np;
-    const int stop = min(L, i + P.segment_len);
-    for (; i < stop; ++i) q = P.imp.blks[P.imp.blk_of[P.bv.symbol[lo + i] * Q + q]].dst;
   }
   P.sector[s] = finish_sector_bound(val, e, rec.lg);
 }

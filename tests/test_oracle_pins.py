@@ -404,3 +404,32 @@ def test_A8_config3_coarse_sectors_are_ill_conditioned_in_fp64(impurities):
     s, t = b.config(1)
     rc, rf = O.trace_config(coarse, coarse.beta, s, t), O.trace_config(fine, fine.beta, s, t)
     assert rel_diff(rc["mant"], rc["exp2"], rf["mant"], rf["exp2"]) < 1e-10
+
+
+@pytest.mark.parametrize("cfg,S", [(1, 2), (2, 3), (2, 0)])
+def test_PB5_certified_spectral_estimate_lies_between_the_exact_spectral_and_the_frobenius_bound(impurities, cfg, S):
+    """norm_kind 2 (reading A1: min(||G_j||_F, prod sigma_max(F_i)) per segment) is pinned by the two inequalities that make it
+    a bound -- it dominates the exact spectral-norm product (SVD) and, the prefactor aside, never exceeds the Frobenius
+    product -- by bound >= |trace| per sector, and by the case where it must coincide with the exact value: c / c^dag blocks have
+    sigma_max = 1 (pin P10), so with segment length 1 it equals the factorised closed form P-B3."""
+    imp = impurities(cfg)
+    batch = make_batch(cfg, 6, start=900)
+    for b in range(batch.n_configs):
+        s, t = batch.config(b)
+        est = O.bound_config(imp, batch.beta, s, t, 2, S)
+        exact = O.bound_config(imp, batch.beta, s, t, 1, S)
+        fro = O.bound_config(imp, batch.beta, s, t, 0, S)
+        tr = O.trace_config(imp, batch.beta, s, t)
+        dmin_max = math.sqrt(max(int(d) for d in imp.dims))
+        for q0, se in enumerate(est["sector"]):
+            if se is None:
+                assert exact["sector"][q0] is None
+                continue
+            ex, fr = exact["sector"][q0], fro["sector"][q0]
+            assert scaled_ge(se[0] * (1 + 1e-12), se[1], ex[0], ex[1])
+            assert scaled_ge(fr[0] * dmin_max * (1 + 1e-12), fr[1], se[0], se[1])
+            z, e = tr["sector"][q0]
+            assert scaled_ge(se[0], se[1], abs(z), e)
+        one = O.bound_config(imp, batch.beta, s, t, 2, 1)
+        closed = O.bound_config(imp, batch.beta, s, t, 1, 1)
+        assert rel_diff(one["mant"], one["exp2"], closed["mant"], closed["exp2"]) < 1e-14
