@@ -287,6 +287,26 @@ int ctqmc_chains_trace(ctqmc_chains* chains, double* mant, int64_t* exp2, void* 
  * stats[3] = node slots per chain (stored + shadow + scratch). */
 int ctqmc_chains_stats(ctqmc_chains* chains, int64_t stats[4]);
 
+/* ------------------------------------------------------------------------------------------------------------------------
+ * Reduced density matrix of the impurity.  PAPER.md:254, Eq. 27:
+ *     rho_uv = (1 / beta) < int_0^beta w_loc(C, P_vu(tau)) / w_loc(C) dtau >,   P_vu = |v><u|,  u, v eigenstates of one sector,
+ * "this integration is done analytically".  The call ADDS, for every configuration b with status[b] == 0 and
+ * w_loc != 0, weight[b] times the configuration's estimator to `rho` ("matrix addition" kernel): per surviving
+ * closed string one forward sweep that keeps every prefix product and one backward sweep that forms (G_i Y_i)_uv for every
+ * interval between two operators.  Each configuration's contribution has unit trace.
+ *
+ *   batch                    as for ctqmc_trace_batch (DEVICE; max_len must be stated: it sizes the per-string scratch)
+ *   w_mant [B][2], w_exp2 [B], status [B]   DEVICE: the outputs of ctqmc_trace_batch for the SAME batch
+ *   weight [B] or NULL       DEVICE: e.g. the sign of the configuration (NULL = 1)
+ *   rho                      DEVICE, ctqmc_density_size(imp) elements (doubles, or (re, im) pairs for complex impurities):
+ *                            sector q at offset sum_{q' < q} dim[q']^2, column-major, element rho_uv at u + v * dim[q].
+ *                            The caller zeroes it before the first call and divides by the number of samples afterwards.
+ * Only enqueues on `cuda_stream`.  Sector dimensions up to 512; scratch (max_len * d_max^2 elements per string in flight) comes
+ * from the handle's arena under the rules of ctqmc_trace_batch. */
+int64_t ctqmc_density_size(const ctqmc_impurity* imp);
+int ctqmc_density_batch(ctqmc_impurity* imp, double beta, const ctqmc_batch* batch, const double* w_mant, const int64_t* w_exp2,
+                        const int32_t* status, const double* weight, double* rho, void* cuda_stream);
+
 /* Thread-local description of the last error on this thread ("" if none). */
 const char* ctqmc_last_error(void);
 

@@ -26,7 +26,7 @@ CTQMC_CHAIN_OK, CTQMC_CHAIN_BAD_EDIT, CTQMC_CHAIN_NOT_FOUND, CTQMC_CHAIN_LEAF_FU
 EXPORTS = ["ctqmc_load_impurity", "ctqmc_free_impurity", "ctqmc_set_option", "ctqmc_trace_batch", "ctqmc_bound_batch",
            "ctqmc_trace_batch_host", "ctqmc_bound_batch_host", "ctqmc_last_stats", "ctqmc_last_timing", "ctqmc_measure_fp64_peak", "ctqmc_last_error",
            "ctqmc_chains_create", "ctqmc_chains_destroy", "ctqmc_chains_propose", "ctqmc_chains_commit", "ctqmc_chains_trace",
-           "ctqmc_chains_stats"]
+           "ctqmc_chains_stats", "ctqmc_density_size", "ctqmc_density_batch"]
 
 
 class CtqmcError(RuntimeError):
@@ -101,6 +101,10 @@ def library() -> C.CDLL:
         lib.ctqmc_chains_trace.restype = C.c_int
         lib.ctqmc_chains_stats.argtypes = [vp, C.POINTER(i64 * 4)]
         lib.ctqmc_chains_stats.restype = C.c_int
+        lib.ctqmc_density_size.argtypes = [vp]
+        lib.ctqmc_density_size.restype = i64
+        lib.ctqmc_density_batch.argtypes = [vp, dbl, C.POINTER(_Batch), vp, vp, vp, vp, vp, vp]
+        lib.ctqmc_density_batch.restype = C.c_int
         _lib = lib
     return _lib
 
@@ -381,3 +385,27 @@ def ctqmc_chains_stats(chains: ChainsHandle) -> dict:
     buf = (C.c_int64 * 4)()
     _check(library().ctqmc_chains_stats(chains.ptr, C.byref(buf)))
     return dict(zip(["products", "bytes", "launches", "slots_per_chain"], [int(x) for x in buf]))
+
+
+# ----------------------------------------------------------------------------------------------- reduced density matrix
+def ctqmc_density_size(imp: ImpurityHandle) -> int:
+    return int(library().ctqmc_density_size(imp.ptr))
+
+
+def ctqmc_density_batch(imp: ImpurityHandle, beta: float, offset, symbol, tau, w_mant, w_exp2, status, weight=None, rho=None,
+                        stream=None, max_len=None):
+    """Adds the batch's estimator of the reduced density matrix (Eq. 27) to `rho` (torch CUDA float64 tensor of
+    ctqmc_density_size elements, x2 for complex impurities; created zeroed if None) and returns it.  w_mant, w_exp2, status:
+    the outputs of ctqmc_trace_batch for the same batch."""
+    import torch
+    n = ctqmc_density_size(imp) * (2 if imp.is_complex else 1)
+    if rho is None:
+        rho = torch.zeros(n, dtype=torch.float64, device=offset.device)
+    assert rho.is_cuda and rho.dtype == torch.float64 and rho.numel() == n and rho.is_contiguous()
+    assert w_mant.dtype == torch.float64 and w_exp2.dtype == torch.int64 and status.dtype == torch.int32
+    if weight is not None:
+        assert weight.is_cuda and weight.dtype == torch.float64 and weight.numel() == offset.numel() - 1
+    b = _dev_batch(offset, symbol, tau, max_len)
+    _check(library().ctqmc_density_batch(imp.ptr, float(beta), C.byref(b), w_mant.data_ptr(), w_exp2.data_ptr(), status.data_ptr(),
+                                         weight.data_ptr() if weight is not None else None, rho.data_ptr(), _stream_ptr(stream)))
+    return rho

@@ -107,6 +107,8 @@ struct ctqmc_impurity {
   int* d_blkof = nullptr; BlkDesc* d_blks = nullptr; double* d_store = nullptr; double* d_rownorm2 = nullptr;
   double* d_sigma = nullptr;
   int* d_blkorder = nullptr;
+  long long* d_rho_off = nullptr;     // [Q] offset of sector q's block in the reduced density matrix (sum of dim^2)
+  long long rho_len = 0;
   std::vector<BlkDesc> h_blks;        // host copy (tensor-map construction)
   CUtensorMap* d_amaps = nullptr;     // large path, TMA variant: one tensor map per operator block
   int use_tma = 1;
@@ -729,6 +731,13 @@ extern "C" int ctqmc_load_impurity(const ctqmc_impurity_desc* desc, int device, 
     h->small2_dp = dp2;
   }
   h->n_energy = (int)ne;
+  {
+    std::vector<long long> roff(Q);
+    long long acc = 0;
+    for (int q = 0; q < Q; ++q) { roff[q] = acc; acc += (long long)dim[q] * dim[q]; }
+    h->rho_len = acc;
+    TRY(upload(&h->d_rho_off, roff));
+  }
   TRY(upload(&d_voff, v_off));
   TRYCU(cudaMalloc((void**)&h->d_store, (size_t)(store_len ? store_len : 1) * sizeof(double)));
   TRYCU(cudaMemset(h->d_store, 0, (size_t)(store_len ? store_len : 1) * sizeof(double)));
@@ -803,7 +812,7 @@ extern "C" void ctqmc_free_impurity(ctqmc_impurity* h) {
   cudaSetDevice(h->device);
   cudaFree(h->d_dim); cudaFree(h->d_eoff); cudaFree(h->d_energy); cudaFree(h->d_emin); cudaFree(h->d_blkof);
   cudaFree(h->d_ftpad); cudaFree(h->d_binfo);
-  cudaFree(h->d_pack); cudaFree(h->d_pblk); cudaFree(h->d_blkorder);
+  cudaFree(h->d_pack); cudaFree(h->d_pblk); cudaFree(h->d_blkorder); cudaFree(h->d_rho_off);
   cudaFree(h->d_blks); cudaFree(h->d_store); cudaFree(h->d_rownorm2); cudaFree(h->d_sigma);
   Arena& a = h->arena;
   cudaFree(a.base); cudaFree(a.cnt); cudaFree(a.cnt_total); cudaFree(h->d_amaps); cudaFree(a.d_stage);
@@ -1343,3 +1352,4 @@ extern "C" int ctqmc_measure_fp64_peak(int device, double* tflops_dmma, double* 
 extern "C" const char* ctqmc_last_error(void) { return g_err.c_str(); }
 
 #include "lazy_api.cuh"
+#include "density_api.cuh"

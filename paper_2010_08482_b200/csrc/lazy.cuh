@@ -138,7 +138,7 @@ __device__ inline int lz_block_max(int v, int* red) {
 
 // ------------------------------------------------------------------------------------------------ node product tile
 // C (M x N, column-major ldc) = [diag(2^x mantissas)] A (M x K, element (r, k) at A[(r a_rs + k a_cs) ES]) B (K x N, column-
-// major ldb, or -- B == nullptr -- the diagonal propagator P_delta of a sector).  64 x 64 tile per CTA, 8 warps of 16 x 32,
+// major ldb with contraction stride b_ks, or -- B == nullptr -- the diagonal propagator P_delta of a sector).  64 x 64 tile per CTA, 8 warps of 16 x 32,
 // FP64 tensor-core mma (DMMA m8n8k4), operands staged in shared memory with bounds guards (sector dimensions are arbitrary).
 // The largest binary exponent of the tile's non-zero results (plus the row exponent of the propagator) goes to *kmax_out.
 template <bool CPLX>
@@ -161,7 +161,7 @@ __device__ __forceinline__ double lz_diag_value(const LzDiag& d, int n) {
 template <bool CPLX>
 __device__ void lz_gemm_tile(LzSmem<CPLX>& S, int m0, int n0, int M, int N, int K, const double* __restrict__ A, long long a_rs,
                              long long a_cs, const double* __restrict__ B, int ldb, LzDiag dg, double* __restrict__ Cm, int ldc,
-                             LzRowScale rs, int* kmax_out) {
+                             LzRowScale rs, int* kmax_out, int b_ks = 1) {
   constexpr int ES = CPLX ? 2 : 1;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int wm = warp & 3, wn = warp >> 2, g = lane >> 2, t = lane & 3;
@@ -197,7 +197,7 @@ __device__ void lz_gemm_tile(LzSmem<CPLX>& S, int m0, int n0, int M, int N, int 
       const int kk = idx % kLzKC, nn = idx / kLzKC;
       double vr = 0.0, vi = 0.0;
       if (n0 + nn < N && k0 + kk < K) {
-        if (B) { const double* p = B + ((long long)(n0 + nn) * ldb + (k0 + kk)) * ES; vr = p[0]; if (CPLX) vi = p[1]; }
+        if (B) { const double* p = B + ((long long)(n0 + nn) * ldb + (long long)(k0 + kk) * b_ks) * ES; vr = p[0]; if (CPLX) vi = p[1]; }
         else if (n0 + nn == k0 + kk) vr = lz_diag_value(dg, n0 + nn);
       }
       S.B[0][nn][kk] = vr; if (CPLX) S.B[CPLX ? 1 : 0][nn][kk] = vi;
