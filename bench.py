@@ -332,6 +332,114 @@ def measure_config(L, torch, cfg, B, rank, steps, warmup, schedule, local_rank, 
                 load_s=load_s, bound_ms=bound_ms)
 
 
+def _edit_tensors(torch, per_chain):
+    off, tau, sym, kind = [0], [], [], []
+    for ins, rem in per_chain:
+        for t, a in rem:
+            tau.append(t); sym.append(a); kind.append(-1)
+        for t, a in ins:
+            tau.append(t); sym.append(a); kind.append(1)
+        off.append(len(tau))
+    return (torch.tensor(off, dtype=torch.int64, device="cuda"), torch.tensor(tau, dtype=torch.float64, device="cuda"),
+            torch.tensor(sym, dtype=torch.int32, device="cuda"), torch.tensor(kind, dtype=torch.int32, device="cuda"))
+
+
+def measure_chains(L, torch, cfg, n_chains, depth, rounds, local_rank, leaf_capacity=32, lazy_rounds=2):
+    """Incremental lazy trace: `n_chains` Markov chains in lock-step, each loaded with a
+    BASELINE configuration, then `rounds` Metropolis rounds of pair moves (insert / remove, workloads.moves).  The threshold of
+    chain c is |w_old| u with a pre-drawn u, computed on the device from ctqmc_chains_trace.  Timed with CUDA
+    events around propose + commit; the host reads the accept flags back between rounds (outside the timed pair) to keep its
+    mirror of the configurations, as the CPU side of the paper's solver does."""
+    import math as _m
+    from workloads import apply_move, build_config_impurity, make_batch, random_pair_move
+    from workloads.rng import Stream
+    imp = build_config_impurity(cfg, keep_eigvecs=False)
+    h = L.ctqmc_load_impurity(imp, local_rank)
+    ch = L.ctqmc_chains_create(h, imp.beta, n_chains, depth, leaf_capacity=leaf_capacity, max_edits=8, lazy_rounds=lazy_rounds)
+    try:
+        nf = imp.n_symbols // 2
+        starts = []
+        for c in range(n_chains):
+            s, t = make_batch(cfg, 1, start=c % 64).config(0)
+            starts.append([(float(tt), int(a)) for a, tt in zip(s, t)])
+        ones = torch.ones(n_chains, dtype=torch.int32, device="cuda")
+        for k in range(max((len(s) + 7) // 8 for s in starts)):
+            L.ctqmc_chains_propose(ch, *_edit_tensors(torch, [(s[8 * k:8 * k + 8], []) for s in starts]))
+            L.ctqmc_chains_commit(ch, ones)
+        torch.cuda.synchronize()
+        st0 = L.ctqmc_chains_stats(ch)
+        ops = [list(s) for s in starts]
+        rngs = [Stream(770000 + 1000 * cfg + c) for c in range(n_chains)]
+        stream = torch.cuda.current_stream()
+        ms, n_acc, n_ok, by = 0.0, 0, 0, [0, 0, 0]
+        for r in range(rounds + 1):
+            moves = [random_pair_move(rngs[c], nf, imp.beta, ops[c]) for c in range(n_chains)]
+            ed = _edit_tensors(torch, moves)
+            u = torch.tensor([max(rngs[c].uniform(), 1e-300) for c in range(n_chains)], dtype=torch.float64, device="cuda")
+            mant, exp2 = L.ctqmc_chains_trace(ch)
+            thr = torch.log2(torch.hypot(mant[:, 0], mant[:, 1])) + exp2.to(torch.float64) + torch.log2(u)
+            torch.cuda.synchronize()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            out = L.ctqmc_chains_propose(ch, *ed, thr, stream=stream)
+            L.ctqmc_chains_commit(ch, stream=stream)
+            b.record(stream)
+            torch.cuda.synchronize()
+            acc = out["accept"].cpu().numpy()
+            okc = out["status"].cpu().numpy() == 0
+            dby = out["decided_by"].cpu().numpy()
+            for c in range(n_chains):
+                if acc[c]:
+                    ops[c] = apply_move(ops[c], *moves[c])
+            if r == 0:
+                continue                      # warm-up round
+            ms += a.elapsed_time(b)
+            n_acc += int(acc.sum()); n_ok += int(okc.sum())
+            for v in dby[okc]:
+                by[int(v)] += 1
+        st1 = L.ctqmc_chains_stats(ch)
+        n_moves = n_chains * rounds
+        return {"workload": WORKLOADS[cfg], "chains": n_chains, "depth": depth, "leaf_capacity": leaf_capacity, "lazy_rounds": lazy_rounds,
+                "rounds": rounds, "moves_per_s": n_moves / (ms * 1e-3), "ms_per_round": ms / rounds, "accept_rate": n_acc / max(n_moves, 1),
+                "invalid_proposals": n_moves - n_ok, "decided_by": {"bound": by[0], "partial": by[1], "full": by[2]},
+                "mean_operators": sum(len(o) for o in ops) / n_chains,
+                "device_bytes": st1["bytes"], "unit": "moves/s (propose + commit, device time)",
+                "api": "ctqmc_chains_propose + ctqmc_chains_commit"}
+    finally:
+        ch.destroy()
+        h.free()
+        torch.cuda.empty_cache()
+
+
+def measure_density(L, torch, cfg, B, steps, local_rank):
+    """ctqmc_density_batch (Eq. 27) on a BASELINE batch: configurations per second, device time."""
+    import numpy as np
+    from workloads import build_config_impurity, make_batch
+    imp = build_config_impurity(cfg, keep_eigvecs=False)
+    h = L.ctqmc_load_impurity(imp, local_rank)
+    try:
+        batch = make_batch(cfg, B)
+        off, sym, tau = (torch.from_numpy(x).cuda() for x in (batch.offset, batch.symbol, batch.tau))
+        Lmax = int(np.diff(batch.offset).max())
+        mant, exp2, _, status = L.ctqmc_trace_batch(h, batch.beta, off, sym, tau, max_len=Lmax)
+        rho = L.ctqmc_density_batch(h, batch.beta, off, sym, tau, mant, exp2, status, max_len=Lmax)
+        torch.cuda.synchronize()
+        stream = torch.cuda.current_stream()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        for _ in range(steps):
+            L.ctqmc_density_batch(h, batch.beta, off, sym, tau, mant, exp2, status, rho=rho, stream=stream, max_len=Lmax)
+        b.record(stream)
+        torch.cuda.synchronize()
+        ms = a.elapsed_time(b) / steps
+        return {"workload": WORKLOADS[cfg], "batch": B, "steps": steps, "ms_per_batch": ms, "configurations_per_s": B / (ms * 1e-3),
+                "api": "ctqmc_density_batch (after ctqmc_trace_batch of the same batch)"}
+    finally:
+        h.free()
+        torch.cuda.empty_cache()
+
+
+
 def _default_batch(cfg: int) -> int:
     from workloads import BASELINE_CONFIGS
     return BASELINE_CONFIGS[cfg]["batch"]
@@ -392,6 +500,14 @@ def run_ours(args, rank: int, world: int, local_rank: int):
                                  "roofline": {x: o["roofline"][x] for x in ("bound", "kernel", "achieved", "peak", "unit", "frac", "traffic",
                                                                             "frac_of_rule_peak", "kernel_ms", "kernel_share_of_step",
                                                                             "hbm_frac_algorithmic")}}
+    next_rows = {}
+    if args.others and world == 1:
+        # SURVEY 8(f) rows built beyond the stateless batch path: the incremental lazy trace over many chains (f1, f2) and the
+        # density-matrix accumulation (f3), each on a small-sector and a mid-size complex config
+        next_rows["lazy_chains"] = {"cfg2": measure_chains(L, torch, 2, 1024, 6, 8, local_rank),
+                                    "cfg4": measure_chains(L, torch, 4, 4, 5, 4, local_rank, leaf_capacity=48)}
+        next_rows["density"] = {"cfg2": measure_density(L, torch, 2, 4096, 3, local_rank),
+                                "cfg4": measure_density(L, torch, 4, 16, 2, local_rank)}
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
@@ -420,6 +536,8 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     }
     if others:
         line["other_workloads"] = others
+    if next_rows:
+        line["next_rows"] = next_rows
     if not args.no_cpu_baseline and world == 1:
         cores, cores_note = oracle_cores(cfg)
         if cfg == 5:

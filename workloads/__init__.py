@@ -10,3 +10,4 @@ Recipe and readings: DESIGN.md §4 (inputs), SURVEY.md §8(d) D1–D2.
 """
 from .impurity import Impurity, build_config_impurity, build_impurity  # noqa: F401
 from .configs import Batch, make_batch, BASELINE_CONFIGS  # noqa: F401
+from .moves import apply_move, random_pair_move  # noqa: F401
