@@ -315,6 +315,7 @@ def measure_config(L, torch, cfg, B, rank, steps, warmup, schedule, local_rank, 
     rule_peak = pk["bf16"] * NOMINAL_FP64_TFLOPS / NOMINAL_BF16_TFLOPS
     peak = fp64["dmma_tflops"] if bound == "tensor" else fp64["dfma_tflops"]
     alg_bytes = n_ops * 12 + (B + 1) * 8 + B * (16 + 8 + 4 + Q)
+    k_launches = max(max_len, 1) if stats["path"] in (2, 4) else 1
     roofline = {
         "bound": bound, "kernel": kname, "achieved": achieved_tf, "peak": peak, "unit": "TFLOP/s", "frac": achieved_tf / peak,
         "traffic": ncu_traffic(cfg, B),
@@ -323,6 +324,11 @@ def measure_config(L, torch, cfg, B, rank, steps, warmup, schedule, local_rank, 
                         f"{pk['source']} bf16 {pk['bf16']} TF/s x nominal {NOMINAL_FP64_TFLOPS}/{NOMINAL_BF16_TFLOPS}, gives {rule_peak:.2f}"),
         "frac_of_rule_peak": achieved_tf / rule_peak,
         "kernel_ms": chain_avg_ms, "kernel_share_of_step": chain_avg_ms * steps / total_ms,
+        # the step kernels of the grouped and large paths are launched once per chain position (max_len launches per step): the
+        # same ratio per kernel launch, which is what `traffic` (one ncu capture of one launch) refers to
+        "kernel_launches_per_step": k_launches, "kernel_launch_ms_avg": chain_avg_ms / k_launches,
+        "flops_per_kernel_launch_algorithmic": stats["alg_flops"] / k_launches,
+        "traffic_per": "kernel launch (dram__bytes_read.sum + dram__bytes_write.sum, profiles/traffic.json)",
         "flops_per_launch_algorithmic": stats["alg_flops"], "exp_per_launch": n_exp, "flop_equivalents_per_launch": alg_flop_equiv, "executed_real_macs_padded": stats["macs"],
         "algorithmic_io_bytes_per_step": alg_bytes,
         "hbm_frac_algorithmic": alg_bytes / (total_ms / steps * 1e-3) / 1e9 / pk["hbm_gbs"],
