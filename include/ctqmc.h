@@ -51,6 +51,7 @@ extern "C" {
                                       memory).  A batch whose scratch exceeds the arena is evaluated in rounds of configurations;
                                       if not even one configuration fits, AUTO falls back from the grouped to the panel kernel and
                                       an explicit CTQMC_PATH_GROUPED request returns CTQMC_ERR_OOM */
+#define CTQMC_OPT_SPLIT_SLICES 7   /* int8 slices per operand of CTQMC_PATH_SPLIT: 5 .. 8 (default 7); set before selecting the path */
 #define CTQMC_OPT_ARENA_BYTES  6   /* allocate the scratch arena NOW with exactly this many bytes and never grow it (0 = back to
                                       automatic growth).  PAPER.md:574: "we pre-allocate ... and develop our own memory allocator
                                       which can work asynchronously with that block": after this call no batch call allocates,
@@ -70,6 +71,9 @@ extern "C" {
 #define CTQMC_PATH_LARGE       2
 #define CTQMC_PATH_SMALL       3
 #define CTQMC_PATH_GROUPED     4   /* step-synchronous grouped GEMM: strings that apply the same block share one GEMM per chain position */
+#define CTQMC_PATH_SPLIT       5   /* large-sector path with every chain step evaluated by split-precision (Ozaki-type) int8 tensor-core
+                                      products, exact up to 7 * slices - 1 bits below the largest entry of each operand row / column
+                                      ("mixed-precision matrix-multiplication kernel"); complex impurities; never chosen by AUTO */
 
 /* Diagnostic environment variables, read when an impurity is loaded or a path is selected (results do not depend on them
  * beyond rounding): CTQMC_LARGE_TMA=0 stages the large-sector kernel's tiles with cp.async instead of TMA; CTQMC_SMALL_V1=1

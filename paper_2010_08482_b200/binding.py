@@ -18,8 +18,8 @@ LIB_PATH = os.path.join(HERE, "libctqmc_b200.so")
 CTQMC_OK, CTQMC_ERR_ARG, CTQMC_ERR_OOM, CTQMC_ERR_CUDA, CTQMC_ERR_UNSUPPORTED = 0, -1, -2, -3, -4
 CTQMC_STATUS_OK, CTQMC_STATUS_VANISHING, CTQMC_STATUS_INVALID = 0, 1, 2
 CTQMC_SCHEDULE_THIN, CTQMC_SCHEDULE_LITERAL = 0, 1
-CTQMC_OPT_SCHEDULE, CTQMC_OPT_PANEL_WIDTH, CTQMC_OPT_TIMING, CTQMC_OPT_PATH, CTQMC_OPT_SCRATCH_LIMIT, CTQMC_OPT_ARENA_BYTES = 1, 2, 3, 4, 5, 6
-CTQMC_PATH_AUTO, CTQMC_PATH_PANEL, CTQMC_PATH_LARGE, CTQMC_PATH_SMALL, CTQMC_PATH_GROUPED = 0, 1, 2, 3, 4
+CTQMC_OPT_SCHEDULE, CTQMC_OPT_PANEL_WIDTH, CTQMC_OPT_TIMING, CTQMC_OPT_PATH, CTQMC_OPT_SCRATCH_LIMIT, CTQMC_OPT_ARENA_BYTES, CTQMC_OPT_SPLIT_SLICES = 1, 2, 3, 4, 5, 6, 7
+CTQMC_PATH_AUTO, CTQMC_PATH_PANEL, CTQMC_PATH_LARGE, CTQMC_PATH_SMALL, CTQMC_PATH_GROUPED, CTQMC_PATH_SPLIT = 0, 1, 2, 3, 4, 5
 
 CTQMC_CHAIN_OK, CTQMC_CHAIN_BAD_EDIT, CTQMC_CHAIN_NOT_FOUND, CTQMC_CHAIN_LEAF_FULL = 0, 2, 3, 4
 

@@ -23,6 +23,7 @@
 #include "reduce.cuh"
 #include "route.cuh"
 #include "store.cuh"
+#include "split_gemm.cuh"
 
 using namespace ctqmc;
 
@@ -79,6 +80,7 @@ struct RoundBuf {
   int* status; uint8_t* survive; StringRec* strings; Scaled* sector; int2* units; Slot* slots;
   long long n_units_cap;
   // large-sector path
+  signed char* sp_b; int* sp_eb; int sp_npad, sp_kpad;
   double* lx; long long lx_cols; int* plan_blk; double* plan_delta; int* lkmax; int* lunit; long long* lux; long long G; int lstride;
   // grouped path
   double* gx; long long sum_c_cap; long long* gxoff; int* gplan_blk; double* gplan_delta; int* gkmax; int* gcoff; int* gulen; int* gucols;
@@ -107,6 +109,10 @@ struct ctqmc_impurity {
   int* d_blkof = nullptr; BlkDesc* d_blks = nullptr; double* d_store = nullptr; double* d_rownorm2 = nullptr;
   double* d_sigma = nullptr;
   int* d_blkorder = nullptr;
+  // split-precision large-sector path (split_gemm.cuh): int8 slice planes of the operator store, their tensor maps
+  int split = 0, split_slices = 7;
+  signed char* d_sp_planes = nullptr; long long* d_sp_aoff = nullptr; int* d_sp_ea = nullptr; long long* d_sp_eaoff = nullptr;
+  CUtensorMap* d_amaps8 = nullptr;
   long long* d_rho_off = nullptr;     // [Q] offset of sector q's block in the reduced density matrix (sum of dim^2)
   long long rho_len = 0;
   std::vector<BlkDesc> h_blks;        // host copy (tensor-map construction)
@@ -180,6 +186,55 @@ int encode_2d(CUtensorMap* m, const void* base, unsigned long long inner, unsign
   CUresult r = fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<void*>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
                   CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) return fail(CTQMC_ERR_CUDA, "cuTensorMapEncodeTiled failed (%d): inner %llu outer %llu stride %llu", (int)r, inner, outer, stride_bytes);
+  return 0;
+}
+
+// 2-D uint8 tensor map of K-major int8 slice planes: `inner` bytes contiguous, `outer` rows; box = 128 bytes x 128 rows with
+// the 128-byte swizzle the tcgen05 shared-memory descriptors expect.
+int encode_2d_u8(CUtensorMap* m, const void* base, unsigned long long inner, unsigned long long outer) {
+  EncodeTiledFn fn = encode_tiled_fn();
+  if (!fn) return fail(CTQMC_ERR_CUDA, "cuTensorMapEncodeTiled is not available from this driver");
+  const cuuint64_t dims[2] = {inner, outer}, strides[1] = {inner};
+  const cuuint32_t box[2] = {128, 128}, estr[2] = {1, 1};
+  CUresult r = fn(m, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<void*>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                  CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return fail(CTQMC_ERR_CUDA, "cuTensorMapEncodeTiled (uint8) failed (%d): inner %llu outer %llu", (int)r, inner, outer);
+  return 0;
+}
+
+// Builds (once) the int8 slice planes of the operator store and their tensor maps for the split-precision path.
+int split_prepare(ctqmc_impurity* h) {
+  if (h->d_sp_planes) return 0;
+  const int nb = h->n_blocks, S = h->split_slices;
+  std::vector<long long> aoff(nb), eaoff(nb);
+  long long bytes = 0, rows = 0;
+  int mpmax = 0;
+  for (int b = 0; b < nb; ++b) {
+    const BlkDesc& bd = h->h_blks[b];
+    const long long Mp = sp_pad(bd.rows), Kp = sp_pad(bd.cols);
+    aoff[b] = bytes; eaoff[b] = rows;
+    bytes += 2LL * S * Mp * Kp; rows += Mp;
+    if (Mp > mpmax) mpmax = (int)Mp;
+  }
+  CU(cudaMalloc((void**)&h->d_sp_planes, (size_t)(bytes ? bytes : 1)));
+  CU(cudaMemset(h->d_sp_planes, 0, (size_t)(bytes ? bytes : 1)));
+  CU(cudaMalloc((void**)&h->d_sp_ea, (size_t)(rows ? rows : 1) * sizeof(int)));
+  CU(cudaMemset(h->d_sp_ea, 0, (size_t)(rows ? rows : 1) * sizeof(int)));
+  int rc = upload(&h->d_sp_aoff, aoff); if (rc) return rc;
+  rc = upload(&h->d_sp_eaoff, eaoff); if (rc) return rc;
+  SplitStore st; st.planes = h->d_sp_planes; st.a_off = h->d_sp_aoff; st.ea = h->d_sp_ea; st.ea_off = h->d_sp_eaoff; st.S = S;
+  if (nb > 0) split_slice_store_kernel<<<dim3((unsigned)mpmax, (unsigned)nb), 128>>>(h->dev, st);
+  CU(cudaGetLastError());
+  std::vector<CUtensorMap> maps(nb > 0 ? nb : 1);
+  for (int b = 0; b < nb; ++b) {
+    const BlkDesc& bd = h->h_blks[b];
+    rc = encode_2d_u8(&maps[b], h->d_sp_planes + aoff[b], (unsigned long long)sp_pad(bd.cols), 2ULL * S * sp_pad(bd.rows));
+    if (rc) return rc;
+  }
+  CU(cudaMalloc((void**)&h->d_amaps8, maps.size() * sizeof(CUtensorMap)));
+  CU(cudaMemcpy(h->d_amaps8, maps.data(), maps.size() * sizeof(CUtensorMap), cudaMemcpyHostToDevice));
+  CU(cudaFuncSetAttribute(split_step_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSpSmemBytes));
+  CU(cudaDeviceSynchronize());
   return 0;
 }
 
@@ -259,7 +314,7 @@ int configure(ctqmc_impurity* h, int want_w) {
   int nt_try[3] = {4, 2, 1};
   h->nt = 0;
   h->large = 0;
-  for (int i = 0; i < 3 && h->path != CTQMC_PATH_LARGE; ++i) {
+  for (int i = 0; i < 3 && h->path != CTQMC_PATH_LARGE && h->path != CTQMC_PATH_SPLIT; ++i) {
     int nt = nt_try[i];
     if (want_w && nt * 8 != want_w) continue;
     if (!pick_kernel(cplx, nt, h->team_warps)) continue;
@@ -285,7 +340,9 @@ int configure(ctqmc_impurity* h, int want_w) {
       h->grouped = 1;
     }
   }
-  h->large = (h->nt == 0 || h->path == CTQMC_PATH_LARGE);
+  h->split = (h->path == CTQMC_PATH_SPLIT);
+  if (h->split && !cplx) return fail(CTQMC_ERR_UNSUPPORTED, "the split-precision path is built for complex impurities");
+  h->large = (h->nt == 0 || h->path == CTQMC_PATH_LARGE || h->split);
   if (h->large) {
     h->nt = 0;
     h->ldx = (h->dev.dmax + 7) / 8 * 8;
@@ -311,6 +368,7 @@ int configure(ctqmc_impurity* h, int want_w) {
       CU(cudaMemcpy(h->d_amaps, maps.data(), maps.size() * sizeof(CUtensorMap), cudaMemcpyHostToDevice));
     }
     h->grid = 0;
+    if (h->split) { int rc = split_prepare(h); if (rc) return rc; }
     return 0;
   }
   KernelFn fn = pick_kernel(cplx, h->nt, h->team_warps);
@@ -356,6 +414,11 @@ size_t layout_round(const ctqmc_impurity* h, int kind, int mode, long long Bs, i
     r.lkmax = bp.take<int>((size_t)r.G * r.lstride);
     r.lunit = bp.take<int>((size_t)4 * r.G);
     r.lux = bp.take<long long>((size_t)r.G);
+    if (h->split && mode == 0) {   // int8 slice planes of every unit's carried matrix (split_gemm.cuh)
+      r.sp_npad = sp_pad(h->dev.dmax); r.sp_kpad = sp_pad(h->dev.dmax);
+      r.sp_eb = bp.take<int>((size_t)r.G * r.sp_npad);
+      r.sp_b = bp.take<signed char>((size_t)r.G * 3 * h->split_slices * r.sp_npad * r.sp_kpad);
+    }
   } else if (kind == K_GROUPED) {
     const int ldx = (h->dev.dmax + 7) / 8 * 8, nb = h->n_blocks;
     const size_t L = (size_t)(Lmax > 0 ? Lmax : 1), nul = (size_t)nU * L;
@@ -578,7 +641,25 @@ int enqueue_large(ctqmc_impurity* h, const BatchView& bv, const RoundBuf& rb, in
     large_plan_kernel<<<(lp.n_group + 127) / 128, 128, 0, st>>>(lp);
     dim3 ig((unsigned)((cw < 256) ? cw : 256), (unsigned)lp.n_group);
     dim3 sg((unsigned)(MTmax * NTmax), (unsigned)lp.n_group);
-    if (h->dev.cplx) {
+    if (h->split && mode == 0) {
+      // split-precision step (split_gemm.cuh): slice the carried matrices, then the int8 tensor-core product
+      SplitStepParams sq;
+      sq.st.planes = h->d_sp_planes; sq.st.a_off = h->d_sp_aoff; sq.st.ea = h->d_sp_ea; sq.st.ea_off = h->d_sp_eaoff; sq.st.S = h->split_slices;
+      sq.bplanes = rb.sp_b; sq.eb = rb.sp_eb; sq.Npad = rb.sp_npad; sq.Kpad = rb.sp_kpad; sq.amaps8 = h->d_amaps8;
+      CUtensorMap bmap;
+      int rc = encode_2d_u8(&bmap, rb.sp_b, (unsigned long long)rb.sp_kpad, (unsigned long long)G * 3 * h->split_slices * rb.sp_npad);
+      if (rc) return rc;
+      CU(cudaMemsetAsync(rb.sp_b, 0, (size_t)G * 3 * h->split_slices * rb.sp_npad * rb.sp_kpad, st));
+      const int MT8 = (h->dev.dmax + kSpM - 1) / kSpM, NT8 = (cw + kSpN - 1) / kSpN;
+      dim3 xg((unsigned)cw, (unsigned)lp.n_group), gg((unsigned)(MT8 * NT8 * 2), (unsigned)lp.n_group);
+      large_init_kernel<true><<<ig, 256, 0, st>>>(lp);
+      for (int j = 0; j < n_launch; ++j) {
+        split_slice_x_kernel<<<xg, 128, 0, st>>>(lp, sq, j);
+        split_step_kernel<<<gg, kSpThreads, kSpSmemBytes, st>>>(bmap, lp, sq, j, NT8);
+      }
+      large_finish_kernel<true><<<lp.n_group, 256, 0, st>>>(lp);
+      h->last_launches += n_launch;
+    } else if (h->dev.cplx) {
       large_init_kernel<true><<<ig, 256, 0, st>>>(lp);
       for (int j = 0; j < n_launch; ++j) {
         if (tma) large_step_kernel<true, true><<<sg, 256, h->smem_bytes, st>>>(xmap, lp, j, NTmax);
@@ -813,6 +894,7 @@ extern "C" void ctqmc_free_impurity(ctqmc_impurity* h) {
   cudaFree(h->d_dim); cudaFree(h->d_eoff); cudaFree(h->d_energy); cudaFree(h->d_emin); cudaFree(h->d_blkof);
   cudaFree(h->d_ftpad); cudaFree(h->d_binfo);
   cudaFree(h->d_pack); cudaFree(h->d_pblk); cudaFree(h->d_blkorder); cudaFree(h->d_rho_off);
+  cudaFree(h->d_sp_planes); cudaFree(h->d_sp_aoff); cudaFree(h->d_sp_ea); cudaFree(h->d_sp_eaoff); cudaFree(h->d_amaps8);
   cudaFree(h->d_blks); cudaFree(h->d_store); cudaFree(h->d_rownorm2); cudaFree(h->d_sigma);
   Arena& a = h->arena;
   cudaFree(a.base); cudaFree(a.cnt); cudaFree(a.cnt_total); cudaFree(h->d_amaps); cudaFree(a.d_stage);
@@ -844,7 +926,7 @@ extern "C" int ctqmc_set_option(ctqmc_impurity* h, int option, int64_t value) {
     return 0;
   }
   if (option == CTQMC_OPT_PATH) {
-    if (value != CTQMC_PATH_AUTO && value != CTQMC_PATH_PANEL && value != CTQMC_PATH_LARGE && value != CTQMC_PATH_SMALL && value != CTQMC_PATH_GROUPED) return fail(CTQMC_ERR_ARG, "unknown path %lld", (long long)value);
+    if (value != CTQMC_PATH_AUTO && value != CTQMC_PATH_PANEL && value != CTQMC_PATH_LARGE && value != CTQMC_PATH_SMALL && value != CTQMC_PATH_GROUPED && value != CTQMC_PATH_SPLIT) return fail(CTQMC_ERR_ARG, "unknown path %lld", (long long)value);
     const int old = h->path;
     h->path = (int)value;
     int rc = configure(h, 0);
@@ -859,6 +941,12 @@ extern "C" int ctqmc_set_option(ctqmc_impurity* h, int option, int64_t value) {
       CU(cudaDeviceSynchronize());
       cudaFree(a.base); a.base = nullptr; a.cap = 0;
     }
+    return 0;
+  }
+  if (option == CTQMC_OPT_SPLIT_SLICES) {
+    if (value < 5 || value > kSpMaxSlices) return fail(CTQMC_ERR_ARG, "split slices must be 5 .. %d", kSpMaxSlices);
+    if (h->d_sp_planes && value != h->split_slices) return fail(CTQMC_ERR_ARG, "the slice planes are already built with %d slices", h->split_slices);
+    h->split_slices = (int)value;
     return 0;
   }
   if (option == CTQMC_OPT_ARENA_BYTES) {
@@ -925,7 +1013,7 @@ extern "C" int ctqmc_trace_batch(ctqmc_impurity* h, double beta, const ctqmc_bat
   // AUTO: batches of at least kGroupedMinBatch configurations take the step-synchronous grouped path (one launch per chain
   // position pays off once many strings share blocks); smaller ones the persistent panel kernel
   h->grouped_now = h->grouped || (h->path == CTQMC_PATH_AUTO && h->grouped_ok && !h->small && !h->large && B >= kGroupedMinBatch);
-  h->last_path = h->small ? CTQMC_PATH_SMALL : h->grouped_now ? CTQMC_PATH_GROUPED : h->large ? CTQMC_PATH_LARGE : CTQMC_PATH_PANEL;
+  h->last_path = h->small ? CTQMC_PATH_SMALL : h->grouped_now ? CTQMC_PATH_GROUPED : h->split ? CTQMC_PATH_SPLIT : h->large ? CTQMC_PATH_LARGE : CTQMC_PATH_PANEL;
   h->last_stream = st;
   if (!h->keep_totals) { h->last_launches = 0; CU(cudaMemsetAsync(h->arena.cnt_total, 0, sizeof(Counters), st)); }
   h->timing_valid = 0;
