@@ -189,15 +189,15 @@ int encode_2d(CUtensorMap* m, const void* base, unsigned long long inner, unsign
   return 0;
 }
 
-// 2-D uint8 tensor map of K-major int8 slice planes: `inner` bytes contiguous, `outer` rows; box = 128 bytes x 128 rows with
-// the 128-byte swizzle the tcgen05 shared-memory descriptors expect.
+// 2-D uint8 tensor map of K-major int8 slice planes: `inner` bytes contiguous, `outer` rows; box = 64 bytes x 128 rows with
+// the 64-byte swizzle the tcgen05 shared-memory descriptors of split_gemm.cuh expect.
 int encode_2d_u8(CUtensorMap* m, const void* base, unsigned long long inner, unsigned long long outer) {
   EncodeTiledFn fn = encode_tiled_fn();
   if (!fn) return fail(CTQMC_ERR_CUDA, "cuTensorMapEncodeTiled is not available from this driver");
   const cuuint64_t dims[2] = {inner, outer}, strides[1] = {inner};
-  const cuuint32_t box[2] = {128, 128}, estr[2] = {1, 1};
+  const cuuint32_t box[2] = {kSpKC, 128}, estr[2] = {1, 1};
   CUresult r = fn(m, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<void*>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                  CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+                  CU_TENSOR_MAP_SWIZZLE_64B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) return fail(CTQMC_ERR_CUDA, "cuTensorMapEncodeTiled (uint8) failed (%d): inner %llu outer %llu", (int)r, inner, outer);
   return 0;
 }
@@ -233,7 +233,7 @@ int split_prepare(ctqmc_impurity* h) {
   }
   CU(cudaMalloc((void**)&h->d_amaps8, maps.size() * sizeof(CUtensorMap)));
   CU(cudaMemcpy(h->d_amaps8, maps.data(), maps.size() * sizeof(CUtensorMap), cudaMemcpyHostToDevice));
-  CU(cudaFuncSetAttribute(split_step_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSpSmemBytes));
+  CU(cudaFuncSetAttribute(split_step_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSpSmem2));
   CU(cudaDeviceSynchronize());
   return 0;
 }
@@ -651,11 +651,12 @@ int enqueue_large(ctqmc_impurity* h, const BatchView& bv, const RoundBuf& rb, in
       if (rc) return rc;
       CU(cudaMemsetAsync(rb.sp_b, 0, (size_t)G * 3 * h->split_slices * rb.sp_npad * rb.sp_kpad, st));
       const int MT8 = (h->dev.dmax + kSpM - 1) / kSpM, NT8 = (cw + kSpN - 1) / kSpN;
-      dim3 xg((unsigned)cw, (unsigned)lp.n_group), gg((unsigned)(MT8 * NT8 * 2), (unsigned)lp.n_group);
+      const int tiles_per_unit = MT8 * NT8 * 2;
+      dim3 xg((unsigned)cw, (unsigned)lp.n_group), gg((unsigned)tiles_per_unit, (unsigned)lp.n_group);
       large_init_kernel<true><<<ig, 256, 0, st>>>(lp);
       for (int j = 0; j < n_launch; ++j) {
         split_slice_x_kernel<<<xg, 128, 0, st>>>(lp, sq, j);
-        split_step_kernel<<<gg, kSpThreads, kSpSmemBytes, st>>>(bmap, lp, sq, j, NT8);
+        split_step_kernel<<<gg, kSpThreads, kSpSmem2, st>>>(bmap, lp, sq, j, NT8, tiles_per_unit);
       }
       large_finish_kernel<true><<<lp.n_group, 256, 0, st>>>(lp);
       h->last_launches += n_launch;

@@ -67,6 +67,7 @@ __device__ __forceinline__ unsigned long long sp_smem_desc(unsigned saddr) {
 }
 // instruction descriptor: S32 accumulate, signed 8-bit A and B, both K-major, N = 128, M = 128
 constexpr unsigned kSpIdesc = (2u << 4) | (1u << 7) | (1u << 10) | ((unsigned)(kSpN >> 3) << 17) | ((unsigned)(kSpM >> 4) << 24);
+constexpr unsigned kSpIdesc256 = (2u << 4) | (1u << 7) | (1u << 10) | ((unsigned)(256 >> 3) << 17) | ((unsigned)(kSpM >> 4) << 24);   // N = 256
 
 // ---- slicing: one vector (a row of F, or a column of X with the deferred row scaling of the previous step) per CTA.
 // v_k = 2^e sum_t q_t[k] 2^(-7 (t + 1)), e = exponent of the largest |re| / |im| of the vector + 2, |q_t| <= 64.
@@ -165,109 +166,182 @@ __global__ void split_slice_x_kernel(LargeParams P, SplitStepParams Q, int j) {
   sp_slice_vector(col, 2, d, scale, Q.st.S, o, Q.eb + (size_t)s * Q.Npad + n, redi);
 }
 
-// One chain position of every unit on the int8 tensor pipe.  blockIdx.x = (mt * NTmax + nt) * 2 + part (0: real, 1: imaginary
-// part of the result tile), blockIdx.y = unit.
-__global__ void __launch_bounds__(kSpThreads, 1) split_step_kernel(const __grid_constant__ CUtensorMap bmap, LargeParams P, SplitStepParams Q, int j, int NTmax) {
+// One chain position of every unit on the int8 tensor pipe; a work item is (unit, 128 x 128 tile, real | imaginary part).
+//
+// Operand traffic decides this kernel: with one (A slice, B slice) pair fetched per product the ring pulls 17 TB/s out of L2 and
+// the tensor pipe waits (57 % busy, profiles/r02_split_step.md).  So the diagonals are evaluated in GROUPS of up to four that are
+// accumulated side by side in TMEM (4 x 128 columns): per 64-byte K chunk every B slice the group needs is loaded ONCE (double-
+// buffered set of up to 8 tiles) and every A slice ONCE (ring), and all their pairs t + u in the group's range are issued from
+// shared memory -- 22 tile loads per chunk instead of 56.  The accumulators of a group are drained by the epilogue warps before the
+// next group starts.
+constexpr int kSpKC = 64;                                  // bytes of K per chunk (2 MMAs of K = 32), 64-byte swizzle
+constexpr int kSpTile = kSpM * kSpKC;                      // 8 KB: one operand tile of one slice
+constexpr int kSpTilesTotal = 28;                         // operand tiles that fit in shared memory: kSpBBuf S for the B sets, the rest is the A ring
+constexpr int kSpBBuf = 3;                                 // B sets in flight: a set must be requested two chunks ahead to cover the TMA round trip
+constexpr int kSpARingMax = kSpTilesTotal - kSpBBuf * 5;
+constexpr size_t kSpSmem2 = (size_t)kSpTilesTotal * kSpTile + 1024;
+// the epilogue warps wait for a whole group of diagonals: back off instead of spinning on the issue slots
+__device__ __forceinline__ void mbar_wait_sleep(unsigned long long* bar, unsigned parity) {
+  unsigned ok = 0;
+  while (!ok) {
+    asm volatile("{\n.reg .pred P1;\nmbarrier.try_wait.parity.shared::cta.b64 P1, [%1], %2;\nselp.u32 %0, 1, 0, P1;\n}" : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+    if (!ok) __nanosleep(500);
+  }
+}
+// shared-memory matrix descriptor: K-major, 64-byte swizzle, rows of 64 bytes, 8-row groups 512 bytes apart
+__device__ __forceinline__ unsigned long long sp_smem_desc64(unsigned saddr) {
+  return (unsigned long long)((saddr & 0x3FFFFu) >> 4) | (1ull << 16) | ((unsigned long long)(512 >> 4) << 32) | (1ull << 46) | (4ull << 61);
+}
+
+struct SpTile { int ok, s, blk, dn, d, c, m0, n0, part, Mp, nch; };
+__device__ __forceinline__ SpTile sp_decode(const LargeParams& P, long long w, int tiles_per_unit, int NTmax, int j) {
+  SpTile T; T.ok = 0;
+  T.s = (int)(w / tiles_per_unit);
+  const int r = (int)(w - (long long)T.s * tiles_per_unit);
+  if (j >= P.u_n[T.s]) return T;
+  T.blk = P.plan_blk[(size_t)T.s * P.Lmax + j];
+  const BlkDesc bd = P.imp.blks[T.blk];
+  T.dn = bd.rows; T.d = bd.cols; T.c = P.u_c[T.s];
+  T.part = r & 1;
+  const int tile = r >> 1, mt0 = tile / NTmax, nt0 = tile - mt0 * NTmax;
+  T.m0 = mt0 * kSpM; T.n0 = nt0 * kSpN;
+  if (T.m0 >= T.dn || T.n0 >= T.c) return T;
+  T.Mp = sp_pad(T.dn); T.nch = 2 * (sp_pad(T.d) / kSpKC);            // chunks: both sub-products, one after the other
+  T.ok = 1;
+  return T;
+}
+
+__global__ void __launch_bounds__(kSpThreads, 1) split_step_kernel(const __grid_constant__ CUtensorMap bmap, LargeParams P, SplitStepParams Q, int j, int NTmax,
+                                                                   int tiles_per_unit) {
   extern __shared__ unsigned char sp_raw[];
-  __shared__ __align__(8) unsigned long long full_bar[kSpStages], empty_bar[kSpStages], tfull_bar[2], tempty_bar[2];
+  __shared__ __align__(8) unsigned long long afull[kSpARingMax], aempty[kSpARingMax], bfull[kSpBBuf], bempty[kSpBBuf], tfull_bar, tempty_bar;
   __shared__ unsigned s_tmem;
-  const int s = blockIdx.y;
-  if (j >= P.u_n[s]) return;
-  const int blk = P.plan_blk[(size_t)s * P.Lmax + j];
-  const BlkDesc bd = P.imp.blks[blk];
-  const int dn = bd.rows, d = bd.cols, c = P.u_c[s];
-  const int part = blockIdx.x & 1, tile = blockIdx.x >> 1;
-  const int mt0 = tile / NTmax, nt0 = tile - mt0 * NTmax;
-  const int m0 = mt0 * kSpM, n0 = nt0 * kSpN;
-  if (m0 >= dn || n0 >= c) return;
-  unsigned char* smem = reinterpret_cast<unsigned char*>(((uintptr_t)sp_raw + 1023) & ~(uintptr_t)1023);   // 128-byte swizzle atoms are 1024-byte aligned
+  // one CTA per work item (the hardware scheduler balances items of very different size better than a static stride did:
+  // a persistent variant measured 17 % slower); items that do not exist exit before touching barriers or TMEM
+  const long long w = (long long)blockIdx.y * tiles_per_unit + blockIdx.x;
+  const SpTile T = sp_decode(P, w, tiles_per_unit, NTmax, j);
+  if (!T.ok) return;
+  unsigned char* smem = reinterpret_cast<unsigned char*>(((uintptr_t)sp_raw + 1023) & ~(uintptr_t)1023);
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int S = Q.st.S;
-  const int Mp = sp_pad(dn), nkc = sp_pad(d) / kSpKB;
+  const int nA = kSpTilesTotal - kSpBBuf * S;                      // depth of the A ring: what the B sets leave
+  unsigned char* sB = smem;                                        // [kSpBBuf][S] tiles
+  unsigned char* sA = smem + kSpBBuf * S * kSpTile;                // [nA] tiles
+  const int n_groups = (S + 3) / 4;
 
   if (tid == 0) {
-    for (int i = 0; i < kSpStages; ++i) { mbar_init(&full_bar[i], 1); mbar_init(&empty_bar[i], 1); }
-    for (int i = 0; i < 2; ++i) { mbar_init(&tfull_bar[i], 1); mbar_init(&tempty_bar[i], 8); }
+    for (int i = 0; i < nA; ++i) { mbar_init(&afull[i], 1); mbar_init(&aempty[i], 1); }
+    for (int i = 0; i < kSpBBuf; ++i) { mbar_init(&bfull[i], 1); mbar_init(&bempty[i], 1); }
+    mbar_init(&tfull_bar, 1); mbar_init(&tempty_bar, 8);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  if (warp == 1) tmem_alloc(&s_tmem, 256);
+  if (warp == 1) tmem_alloc(&s_tmem, 512);
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
   const unsigned tmem = s_tmem;
 
-  // sub-products of this part: real = Fr Xr + Fi (-Xi), imaginary = Fi Xr + Fr Xi   (A planes: 0 re, 1 im; B planes: 0 Xr, 1 Xi, 2 -Xi)
-  const int pa[2] = {part == 0 ? 0 : 1, part == 0 ? 1 : 0};
-  const int pb[2] = {0, part == 0 ? 2 : 1};
-
   if (warp == 0) {
     if (lane == 0) {            // ===== TMA producer
-      const CUtensorMap* amap = Q.amaps8 + blk;
-      int stage = 0, phase = 0;
-      for (int dg = 0; dg < S; ++dg)
-        for (int t = 0; t <= dg; ++t)
-          for (int sub = 0; sub < 2; ++sub) {
-            const int arow = (pa[sub] * S + t) * Mp + m0;
-            const int brow = ((s * 3 + pb[sub]) * S + (dg - t)) * Q.Npad + n0;
-            for (int kc = 0; kc < nkc; ++kc) {
-              mbar_wait(&empty_bar[stage], phase ^ 1);
-              unsigned char* As = smem + stage * kSpStageBytes;
-              mbar_expect_tx(&full_bar[stage], kSpStageBytes);
-              tma_load_2d(As, amap, &full_bar[stage], kc * kSpKB, arow);
-              tma_load_2d(As + kSpM * kSpKB, &bmap, &full_bar[stage], kc * kSpKB, brow);
-              if (++stage == kSpStages) { stage = 0; phase ^= 1; }
-            }
+      int aslot = 0, aphase = 0, bcount = 0;
+      {
+      const int s = T.s, m0 = T.m0, n0 = T.n0, Mp = T.Mp, nch = T.nch, half_ch = T.nch >> 1;
+      // sub-products of this part: real = Fr Xr + Fi (-Xi), imaginary = Fi Xr + Fr Xi   (A planes: 0 re, 1 im; B planes: 0 Xr, 1 Xi, 2 -Xi)
+      const int pa[2] = {T.part == 0 ? 0 : 1, T.part == 0 ? 1 : 0};
+      const int pb[2] = {0, T.part == 0 ? 2 : 1};
+      const CUtensorMap* amap = Q.amaps8 + T.blk;
+      for (int g = 0; g < n_groups; ++g) {
+        const int dg0 = 4 * g, dg1 = min(S, dg0 + 4) - 1;          // diagonals of this group; slices 0 .. dg1 of both operands
+        for (int ch = 0; ch < nch; ++ch, ++bcount) {
+          const int sub = ch >= half_ch, kc = (sub ? ch - half_ch : ch) * kSpKC;
+          const int buf = bcount % kSpBBuf;
+          mbar_wait(&bempty[buf], ((bcount / kSpBBuf) & 1) ^ 1);
+          mbar_expect_tx(&bfull[buf], (unsigned)((dg1 + 1) * kSpTile));
+          for (int u = 0; u <= dg1; ++u)
+            tma_load_2d(sB + (buf * S + u) * kSpTile, &bmap, &bfull[buf], kc, ((s * 3 + pb[sub]) * S + u) * Q.Npad + n0);
+          for (int t = 0; t <= dg1; ++t) {
+            mbar_wait(&aempty[aslot], aphase ^ 1);
+            mbar_expect_tx(&afull[aslot], kSpTile);
+            tma_load_2d(sA + aslot * kSpTile, amap, &afull[aslot], kc, (pa[sub] * S + t) * Mp + m0);
+            if (++aslot == nA) { aslot = 0; aphase ^= 1; }
           }
+        }
+      }
+      }
     }
   } else if (warp == 1) {
     if (lane == 0) {            // ===== MMA issuer
-      int stage = 0, phase = 0;
-      for (int dg = 0; dg < S; ++dg) {
-        const int buf = dg & 1;
-        mbar_wait(&tempty_bar[buf], ((dg >> 1) & 1) ^ 1);      // the epilogue has drained this accumulator
+      int aslot = 0, aphase = 0, bcount = 0, gcount = 0;
+      {
+      const int nch = T.nch;
+      for (int g = 0; g < n_groups; ++g, ++gcount) {
+        const int dg0 = 4 * g, dg1 = min(S, dg0 + 4) - 1;
+        mbar_wait(&tempty_bar, (gcount & 1) ^ 1);                  // the epilogue has drained the previous group's accumulators
         tc_fence_after();
-        unsigned acc = 0;
-        for (int t = 0; t <= dg; ++t)
-          for (int sub = 0; sub < 2; ++sub)
-            for (int kc = 0; kc < nkc; ++kc) {
-              mbar_wait(&full_bar[stage], phase);
-              tc_fence_after();
-              const unsigned sa = smem_u32(smem + stage * kSpStageBytes);
-              const unsigned long long ad = sp_smem_desc(sa), bdsc = sp_smem_desc(sa + kSpM * kSpKB);
-#pragma unroll
-              for (int k = 0; k < kSpKB / 32; ++k) {
-                tc_mma_i8(tmem + buf * kSpN, ad + (unsigned long long)(k * 2), bdsc + (unsigned long long)(k * 2), kSpIdesc, acc);
-                acc = 1;
-              }
-              tc_commit(&empty_bar[stage]);                   // the slot is free once these MMAs have read it
-              if (++stage == kSpStages) { stage = 0; phase ^= 1; }
+        // descriptors are plain offsets from two bases (tiles are 8 KB = 512 descriptor units apart)
+        const unsigned long long a_base = sp_smem_desc64(smem_u32(sA)), b_base = sp_smem_desc64(smem_u32(sB));
+        for (int ch = 0; ch < nch; ++ch, ++bcount) {
+          const int buf = bcount % kSpBBuf;
+          mbar_wait(&bfull[buf], (bcount / kSpBBuf) & 1);
+          tc_fence_after();
+          for (int t = 0; t <= dg1; ++t) {
+            mbar_wait(&afull[aslot], aphase);
+            tc_fence_after();
+            const unsigned long long ad = a_base + (unsigned long long)(aslot * (kSpTile >> 4));
+            const unsigned accum = (ch > 0 || t > 0) ? 1u : 0u;     // t = 0 of the first chunk touches every accumulator of the group
+            int u = max(0, dg0 - t);
+            const int uhi = dg1 - t;
+            // two neighbouring B slices are one 256-row operand and their diagonals neighbouring accumulators: N = 256
+            for (; u + 1 <= uhi; u += 2) {
+              const unsigned long long bdsc = b_base + (unsigned long long)((buf * S + u) * (kSpTile >> 4));
+              const unsigned dst = tmem + (unsigned)((t + u - dg0) * kSpN);
+              tc_mma_i8(dst, ad, bdsc, kSpIdesc256, accum);
+              tc_mma_i8(dst, ad + 2, bdsc + 2, kSpIdesc256, 1u);
             }
-        tc_commit(&tfull_bar[buf]);                           // diagonal dg is complete in TMEM
+            if (u <= uhi) {
+              const unsigned long long bdsc = b_base + (unsigned long long)((buf * S + u) * (kSpTile >> 4));
+              const unsigned dst = tmem + (unsigned)((t + u - dg0) * kSpN);
+              tc_mma_i8(dst, ad, bdsc, kSpIdesc, accum);
+              tc_mma_i8(dst, ad + 2, bdsc + 2, kSpIdesc, 1u);
+            }
+            tc_commit(&aempty[aslot]);
+            if (++aslot == nA) { aslot = 0; aphase ^= 1; }
+          }
+          tc_commit(&bempty[buf]);
+        }
+        tc_commit(&tfull_bar);                                     // the group's diagonals are complete in TMEM
+      }
       }
     }
   } else {
     // ===== epilogue warps: TMEM lane quarter = warp % 4, column half = (warp - 2) / 4
     const int quarter = warp & 3, half = (warp - 2) >> 2;
+    int gcount = 0;
+    {
+    const int s = T.s, blk = T.blk, dn = T.dn, c = T.c, m0 = T.m0, n0 = T.n0, part = T.part;
+    const BlkDesc bd = P.imp.blks[blk];
     const int row = m0 + quarter * 32 + lane;
     double accd[64];
 #pragma unroll
     for (int i = 0; i < 64; ++i) accd[i] = 0.0;
-    double w = 1.0;
-    for (int dg = 0; dg < S; ++dg) {
-      const int buf = dg & 1;
-      mbar_wait(&tfull_bar[buf], (dg >> 1) & 1);
+    double wgt = 1.0;
+    for (int g = 0; g < n_groups; ++g, ++gcount) {
+      const int dg0 = 4 * g, dg1 = min(S, dg0 + 4) - 1;
+      mbar_wait_sleep(&tfull_bar, gcount & 1);
       tc_fence_after();
+      for (int a = 0; a <= dg1 - dg0; ++a) {
 #pragma unroll
-      for (int h = 0; h < 2; ++h) {
-        int v[32];
-        tmem_ld32(tmem + ((unsigned)(quarter * 32) << 16) + (unsigned)(buf * kSpN + half * 64 + h * 32), v);
+        for (int h = 0; h < 2; ++h) {
+          int v[32];
+          tmem_ld32(tmem + ((unsigned)(quarter * 32) << 16) + (unsigned)(a * kSpN + half * 64 + h * 32), v);
 #pragma unroll
-        for (int i = 0; i < 32; ++i) accd[h * 32 + i] = fma((double)v[i], w, accd[h * 32 + i]);
+          for (int i = 0; i < 32; ++i) accd[h * 32 + i] = fma((double)v[i], wgt, accd[h * 32 + i]);
+        }
+        wgt *= 0.0078125;                                            // 2^-7 per diagonal
       }
       tc_fence_before();
       __syncwarp();
-      if (lane == 0) mbar_arrive(&tempty_bar[buf]);
-      w *= 0.0078125;                                         // 2^-7 per diagonal
+      if (lane == 0) mbar_arrive(&tempty_bar);
     }
     // finish as large_step_kernel: exponents of the slices, propagator mantissa of the row, store, largest row exponent
     const double delta = P.plan_delta[(size_t)s * P.Lmax + j];
@@ -287,7 +361,8 @@ __global__ void __launch_bounds__(kSpThreads, 1) split_step_kernel(const __grid_
       for (int i = 0; i < 64; ++i) {
         const int col = n0 + half * 64 + i;
         if (col < c) {
-          const double v = scalbn(accd[i], ea + eb[i] - 14) * mr;
+          const int sh = ea + eb[i] - 14;
+          const double v = ((sh >= -1000 && sh <= 1000) ? accd[i] * pow2i(sh) : scalbn(accd[i], sh)) * mr;
           Xout[((size_t)col * P.ldx + row) * 2 + part] = v;
           rmax = fmax(rmax, fabs(v));
         }
@@ -296,10 +371,11 @@ __global__ void __launch_bounds__(kSpThreads, 1) split_step_kernel(const __grid_
     }
     wexp = __reduce_max_sync(0xffffffffu, wexp);
     if (lane == 0 && wexp != INT_MIN) atomicMax(&P.kmax[(size_t)s * P.Lmax + j], wexp);
+    }
   }
   tc_fence_before();
   __syncthreads();
-  if (warp == 1) tmem_dealloc(tmem, 256);
+  if (warp == 1) tmem_dealloc(tmem, 512);
 }
 
 }  // namespace ctqmc
