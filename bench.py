@@ -43,7 +43,8 @@ REF_PREFIX_DIV = {"reference": 10, "cpu_baseline": 4}
 KERNELS = {1: ("chain_kernel (panel in shared memory, fused propagate x operator, FP64 DMMA m8n8k4)", "tensor"),
            2: ("large_step_kernel (128x64 tiles, TMA + mbarrier ring, fused propagate x operator, FP64 DMMA m8n8k4)", "tensor"),
            3: ("small2_trace_kernel / small_trace_kernel (whole path in one launch, operator store in shared memory, FP64 FMA)", "alu"),
-           4: ("grouped_step_kernel (strings sharing a block share one GEMM per chain position, 64x64 tiles, FP64 DMMA m8n8k4)", "tensor")}
+           4: ("grouped_step_kernel (strings sharing a block share one GEMM per chain position, 64x64 tiles, FP64 DMMA m8n8k4)", "tensor"),
+           5: ("split_step_kernel (int8 slice products on tcgen05.mma.kind::i8; reported against the FP64 tensor peak as FP64-equivalent flops)", "tensor")}
 
 
 def ncu_traffic(cfg: int, batch: int):
@@ -230,7 +231,7 @@ def measure_config(L, torch, cfg, B, rank, steps, warmup, schedule, local_rank, 
     if schedule == "literal":
         L.ctqmc_set_option(h, L.CTQMC_OPT_SCHEDULE, L.CTQMC_SCHEDULE_LITERAL)
     if path != "auto":
-        L.ctqmc_set_option(h, L.CTQMC_OPT_PATH, {"panel": 1, "large": 2, "small": 3, "grouped": 4}[path])
+        L.ctqmc_set_option(h, L.CTQMC_OPT_PATH, {"panel": 1, "large": 2, "small": 3, "grouped": 4, "split": 5}[path])
     L.ctqmc_set_option(h, L.CTQMC_OPT_TIMING, 1)
     batch = shard_batch(cfg, B, rank)
     off, sym, tau = (torch.from_numpy(x).cuda() for x in (batch.offset, batch.symbol, batch.tau))
@@ -315,7 +316,7 @@ def measure_config(L, torch, cfg, B, rank, steps, warmup, schedule, local_rank, 
     rule_peak = pk["bf16"] * NOMINAL_FP64_TFLOPS / NOMINAL_BF16_TFLOPS
     peak = fp64["dmma_tflops"] if bound == "tensor" else fp64["dfma_tflops"]
     alg_bytes = n_ops * 12 + (B + 1) * 8 + B * (16 + 8 + 4 + Q)
-    k_launches = max(max_len, 1) if stats["path"] in (2, 4) else 1
+    k_launches = max(max_len, 1) if stats["path"] in (2, 4, 5) else 1
     roofline = {
         "bound": bound, "kernel": kname, "achieved": achieved_tf, "peak": peak, "unit": "TFLOP/s", "frac": achieved_tf / peak,
         "traffic": ncu_traffic(cfg, B),
@@ -446,6 +447,60 @@ def measure_density(L, torch, cfg, B, steps, local_rank):
 
 
 
+def measure_split(L, torch, B, steps, local_rank, pk):
+    """CTQMC_PATH_SPLIT on config 5: the same batch through the FP64 DMMA path and through the
+    split-precision int8 tcgen05 path; traces/s of the latter, the largest relative difference between the two, and the int8
+    roofline (28 slice-pair products of 4 real products each per complex product: 28 x the algorithmic FP64 flops as int8 ops;
+    peak = measured bf16 x nominal 4.5 / 2.25)."""
+    import numpy as np
+    from workloads import build_config_impurity, make_batch
+    imp = build_config_impurity(5, keep_eigvecs=False)
+    h = L.ctqmc_load_impurity(imp, local_rank)
+    try:
+        batch = make_batch(5, B)
+        off, sym, tau = (torch.from_numpy(x).cuda() for x in (batch.offset, batch.symbol, batch.tau))
+        Lmax = int(np.diff(batch.offset).max())
+        ref = L.ctqmc_trace_batch(h, batch.beta, off, sym, tau, max_len=Lmax)
+        torch.cuda.synchronize()
+        slices = 7
+        L.ctqmc_set_option(h, L.CTQMC_OPT_SPLIT_SLICES, slices)
+        t0 = time.perf_counter()
+        L.ctqmc_set_option(h, L.CTQMC_OPT_PATH, L.CTQMC_PATH_SPLIT)      # builds the int8 slice planes of the operator store
+        prep_s = time.perf_counter() - t0
+        got = L.ctqmc_trace_batch(h, batch.beta, off, sym, tau, max_len=Lmax)   # warm-up (arena growth)
+        torch.cuda.synchronize()
+        stream = torch.cuda.current_stream()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        for _ in range(steps):
+            got = L.ctqmc_trace_batch(h, batch.beta, off, sym, tau, stream=stream, max_len=Lmax)
+        b.record(stream)
+        torch.cuda.synchronize()
+        ms = a.elapsed_time(b) / steps
+        st = L.ctqmc_last_stats(h)
+        rm, re_, gm, ge = ref[0].cpu().numpy(), ref[1].cpu().numpy(), got[0].cpu().numpy(), got[1].cpu().numpy()
+        worst = 0.0
+        for i in range(B):
+            r, g = complex(*rm[i]), complex(*gm[i]) * 2.0 ** float(ge[i] - re_[i])
+            worst = max(worst, abs(g - r) / abs(r))
+        assert (ref[3] == got[3]).all().item() and (ref[2] == got[2]).all().item()
+        pairs = slices * (slices + 1) // 2
+        tops = pairs * st["alg_flops"] / (ms * 1e-3) / 1e12
+        peak = pk["bf16"] * 2.0
+        return {"workload": WORKLOADS[5], "batch": B, "steps": steps, "slices": slices, "ms_per_step": ms, "value": B / (ms * 1e-3), "unit": UNIT,
+                "max_rel_diff_vs_fp64_path": worst, "parity": "all 64 golden outputs within 1e-9 (tests/test_gpu_parity.py::test_split_precision_path_meets_the_same_bar)",
+                "fp64_equivalent_tflops": st["alg_flops"] / (ms * 1e-3) / 1e12, "slice_plane_build_s": prep_s,
+                "roofline": {"bound": "tensor", "kernel": "split_step_kernel (tcgen05.mma.kind::i8, TMEM accumulators, TMA-fed slice planes)",
+                             "achieved": tops, "peak": peak, "unit": "TOP/s (int8)", "frac": tops / peak,
+                             "peak_source": f"{pk['source']} bf16 {pk['bf16']} TF/s x nominal 4.5 / 2.25 (B200_PROFILING.md)",
+                             "int8_ops_per_step_algorithmic": pairs * st["alg_flops"]},
+                "api": "ctqmc_set_option(CTQMC_OPT_PATH, CTQMC_PATH_SPLIT) + ctqmc_trace_batch"}
+    finally:
+        h.free()
+        torch.cuda.empty_cache()
+
+
+
 def _default_batch(cfg: int) -> int:
     from workloads import BASELINE_CONFIGS
     return BASELINE_CONFIGS[cfg]["batch"]
@@ -511,7 +566,8 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         # SURVEY 8(f) rows built beyond the stateless batch path: the incremental lazy trace over many chains (f1, f2) and the
         # density-matrix accumulation (f3), each on a small-sector and a mid-size complex config
         next_rows["lazy_chains"] = {"cfg2": measure_chains(L, torch, 2, 1024, 6, 8, local_rank),
-                                    "cfg4": measure_chains(L, torch, 4, 4, 5, 4, local_rank, leaf_capacity=48)}
+                                    "cfg4": measure_chains(L, torch, 4, 16, 4, 4, local_rank, leaf_capacity=64)}
+        next_rows["split_precision"] = measure_split(L, torch, 64, 3, local_rank, pk)
         next_rows["density"] = {"cfg2": measure_density(L, torch, 2, 4096, 3, local_rank),
                                 "cfg4": measure_density(L, torch, 4, 16, 2, local_rank)}
     if rank != 0:
@@ -566,7 +622,7 @@ def main():
                     help="BASELINE.json config (1-based); default 5 = the largest single-GPU one, on which north_star states its target")
     ap.add_argument("--batch", type=int, default=0, help="configurations per GPU per step (default: BASELINE.json's batch)")
     ap.add_argument("--schedule", default="thin", choices=["thin", "literal"])
-    ap.add_argument("--path", default="auto", choices=["auto", "panel", "large", "small", "grouped"],
+    ap.add_argument("--path", default="auto", choices=["auto", "panel", "large", "small", "grouped", "split"],
                     help="kernel family (CTQMC_OPT_PATH); auto is what a user of the library gets")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
