@@ -80,7 +80,7 @@ struct RoundBuf {
   int* status; uint8_t* survive; StringRec* strings; Scaled* sector; int2* units; Slot* slots;
   long long n_units_cap;
   // large-sector path
-  signed char* sp_b; int* sp_eb; int sp_npad, sp_kpad;
+  signed char* sp_b; int* sp_eb; int sp_npad, sp_kpad; int* sp_items; int* sp_ctr;
   double* lx; long long lx_cols; int* plan_blk; double* plan_delta; int* lkmax; int* lunit; long long* lux; long long G; int lstride;
   // grouped path
   double* gx; long long sum_c_cap; long long* gxoff; int* gplan_blk; double* gplan_delta; int* gkmax; int* gcoff; int* gulen; int* gucols;
@@ -417,6 +417,8 @@ size_t layout_round(const ctqmc_impurity* h, int kind, int mode, long long Bs, i
     if (h->split && mode == 0) {   // int8 slice planes of every unit's carried matrix (split_gemm.cuh)
       r.sp_npad = sp_pad(h->dev.dmax); r.sp_kpad = sp_pad(h->dev.dmax);
       r.sp_eb = bp.take<int>((size_t)r.G * r.sp_npad);
+      r.sp_ctr = bp.take<int>(4);
+      r.sp_items = bp.take<int>((size_t)r.G * 2 * ((h->dev.dmax + kSpM - 1) / kSpM) * ((h->dev.dmax + kSpN - 1) / kSpN));
       r.sp_b = bp.take<signed char>((size_t)r.G * 3 * h->split_slices * r.sp_npad * r.sp_kpad);
     }
   } else if (kind == K_GROUPED) {
@@ -652,14 +654,17 @@ int enqueue_large(ctqmc_impurity* h, const BatchView& bv, const RoundBuf& rb, in
       CU(cudaMemsetAsync(rb.sp_b, 0, (size_t)G * 3 * h->split_slices * rb.sp_npad * rb.sp_kpad, st));
       const int MT8 = (h->dev.dmax + kSpM - 1) / kSpM, NT8 = (cw + kSpN - 1) / kSpN;
       const int tiles_per_unit = MT8 * NT8 * 2;
-      dim3 xg((unsigned)cw, (unsigned)lp.n_group), gg((unsigned)tiles_per_unit, (unsigned)lp.n_group);
+      const long long total8 = (long long)tiles_per_unit * lp.n_group;
+      dim3 xg((unsigned)cw, (unsigned)lp.n_group), gg((unsigned)(total8 < h->sm_count ? total8 : h->sm_count));
+      SplitList wl; wl.items = rb.sp_items; wl.ctr = rb.sp_ctr;
       large_init_kernel<true><<<ig, 256, 0, st>>>(lp);
       for (int j = 0; j < n_launch; ++j) {
         split_slice_x_kernel<<<xg, 128, 0, st>>>(lp, sq, j);
-        split_step_kernel<<<gg, kSpThreads, kSpSmem2, st>>>(bmap, lp, sq, j, NT8, tiles_per_unit);
+        split_list_kernel<<<1, 1024, 0, st>>>(lp, wl, j, tiles_per_unit, NT8, total8);
+        split_step_kernel<<<gg, kSpThreads, kSpSmem2, st>>>(bmap, lp, sq, j, NT8, tiles_per_unit, wl);
       }
       large_finish_kernel<true><<<lp.n_group, 256, 0, st>>>(lp);
-      h->last_launches += n_launch;
+      h->last_launches += 2 * n_launch;
     } else if (h->dev.cplx) {
       large_init_kernel<true><<<ig, 256, 0, st>>>(lp);
       for (int j = 0; j < n_launch; ++j) {

@@ -24,7 +24,7 @@ namespace ctqmc {
 constexpr int kSpM = 128, kSpN = 128, kSpKB = 128;        // tile, bytes of K per stage row (= 128 int8 = 4 MMAs of K = 32)
 constexpr int kSpStages = 5;
 constexpr int kSpStageBytes = (kSpM + kSpN) * kSpKB;      // 32 KB
-constexpr int kSpThreads = 320;                           // producer warp, MMA warp, 8 epilogue warps
+constexpr int kSpThreads = 352;                           // B-producer warp, MMA warp, 8 epilogue warps, A-producer warp
 constexpr int kSpMaxSlices = 8;
 constexpr size_t kSpSmemBytes = (size_t)kSpStages * kSpStageBytes + 1024;   // + alignment slack
 
@@ -177,7 +177,7 @@ __global__ void split_slice_x_kernel(LargeParams P, SplitStepParams Q, int j) {
 constexpr int kSpKC = 64;                                  // bytes of K per chunk (2 MMAs of K = 32), 64-byte swizzle
 constexpr int kSpTile = kSpM * kSpKC;                      // 8 KB: one operand tile of one slice
 constexpr int kSpTilesTotal = 28;                         // operand tiles that fit in shared memory: kSpBBuf S for the B sets, the rest is the A ring
-constexpr int kSpBBuf = 3;                                 // B sets in flight: a set must be requested two chunks ahead to cover the TMA round trip
+constexpr int kSpBBuf = 2;                                 // B sets in flight; the A ring takes the rest (two chunks deep at 7 slices)
 constexpr int kSpARingMax = kSpTilesTotal - kSpBBuf * 5;
 constexpr size_t kSpSmem2 = (size_t)kSpTilesTotal * kSpTile + 1024;
 // the epilogue warps wait for a whole group of diagonals: back off instead of spinning on the issue slots
@@ -211,16 +211,41 @@ __device__ __forceinline__ SpTile sp_decode(const LargeParams& P, long long w, i
   return T;
 }
 
+// Work list of one chain position: the (unit, tile, part) items that exist, heaviest (longest contraction) first.  The host only
+// knows upper bounds, and launching one CTA per CANDIDATE cost more than the products themselves (a CTA that needs all of an SM's
+// shared memory occupies the SM's only slot even if it exits at once: 1.6 ms of a 3.4 ms launch).  One CTA, three passes.
+struct SplitList { int* items; int* ctr; };     // items[n], ctr[0] = n, ctr[1] = next item to hand out
+__global__ void split_list_kernel(LargeParams P, SplitList W, int j, int tiles_per_unit, int NTmax, long long total) {
+  __shared__ int cnt[4], base[4];
+  if (threadIdx.x < 4) cnt[threadIdx.x] = 0;
+  __syncthreads();
+  for (long long w = threadIdx.x; w < total; w += blockDim.x) {
+    const SpTile T = sp_decode(P, w, tiles_per_unit, NTmax, j);
+    if (T.ok) atomicAdd(&cnt[min(3, (T.nch - 1) / 32)], 1);          // contraction length class (chunks of both sub-products): <= 32, <= 64, <= 96, more
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    int b = 0;
+    for (int k = 3; k >= 0; --k) { base[k] = b; b += cnt[k]; cnt[k] = 0; }
+    W.ctr[0] = b; W.ctr[1] = 0;
+  }
+  __syncthreads();
+  for (long long w = threadIdx.x; w < total; w += blockDim.x) {
+    const SpTile T = sp_decode(P, w, tiles_per_unit, NTmax, j);
+    if (T.ok) { const int k = min(3, (T.nch - 1) / 32); W.items[base[k] + atomicAdd(&cnt[k], 1)] = (int)w; }
+  }
+}
+
 __global__ void __launch_bounds__(kSpThreads, 1) split_step_kernel(const __grid_constant__ CUtensorMap bmap, LargeParams P, SplitStepParams Q, int j, int NTmax,
-                                                                   int tiles_per_unit) {
+                                                                   int tiles_per_unit, SplitList W) {
   extern __shared__ unsigned char sp_raw[];
   __shared__ __align__(8) unsigned long long afull[kSpARingMax], aempty[kSpARingMax], bfull[kSpBBuf], bempty[kSpBBuf], tfull_bar, tempty_bar;
+  __shared__ __align__(8) unsigned long long qfull[4], qempty[4];
+  __shared__ int q_item[4];
   __shared__ unsigned s_tmem;
-  // one CTA per work item (the hardware scheduler balances items of very different size better than a static stride did:
-  // a persistent variant measured 17 % slower); items that do not exist exit before touching barriers or TMEM
-  const long long w = (long long)blockIdx.y * tiles_per_unit + blockIdx.x;
-  const SpTile T = sp_decode(P, w, tiles_per_unit, NTmax, j);
-  if (!T.ok) return;
+  // Persistent: one CTA per SM takes items off the work list (atomic counter); the producer thread fetches them and hands them to
+  // the MMA thread and the epilogue warps through a four-deep queue, so barriers, the TMEM allocation and the ring / phase counters
+  // live across items and the epilogue's final store of one item overlaps the next item's first products.
   unsigned char* smem = reinterpret_cast<unsigned char*>(((uintptr_t)sp_raw + 1023) & ~(uintptr_t)1023);
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int S = Q.st.S;
@@ -233,6 +258,7 @@ __global__ void __launch_bounds__(kSpThreads, 1) split_step_kernel(const __grid_
     for (int i = 0; i < nA; ++i) { mbar_init(&afull[i], 1); mbar_init(&aempty[i], 1); }
     for (int i = 0; i < kSpBBuf; ++i) { mbar_init(&bfull[i], 1); mbar_init(&bempty[i], 1); }
     mbar_init(&tfull_bar, 1); mbar_init(&tempty_bar, 8);
+    for (int i = 0; i < 4; ++i) { mbar_init(&qfull[i], 1); mbar_init(&qempty[i], 10); }    // consumers: A producer, MMA thread, 8 epilogue warps
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == 1) tmem_alloc(&s_tmem, 512);
@@ -243,15 +269,21 @@ __global__ void __launch_bounds__(kSpThreads, 1) split_step_kernel(const __grid_
 
   if (warp == 0) {
     if (lane == 0) {            // ===== TMA producer
-      int aslot = 0, aphase = 0, bcount = 0;
-      {
-      const int s = T.s, m0 = T.m0, n0 = T.n0, Mp = T.Mp, nch = T.nch, half_ch = T.nch >> 1;
+      int bcount = 0;
+      const int n_items = W.ctr[0];
+      for (int qn = 0;; ++qn) {
+      mbar_wait(&qempty[qn & 3], ((qn >> 2) & 1) ^ 1);
+      const int it = atomicAdd(&W.ctr[1], 1);
+      const int wi = it < n_items ? W.items[it] : -1;
+      q_item[qn & 3] = wi;
+      mbar_arrive(&qfull[qn & 3]);
+      if (wi < 0) break;
+      const SpTile T = sp_decode(P, wi, tiles_per_unit, NTmax, j);
+      const int s = T.s, n0 = T.n0, nch = T.nch, half_ch = T.nch >> 1;
       // sub-products of this part: real = Fr Xr + Fi (-Xi), imaginary = Fi Xr + Fr Xi   (A planes: 0 re, 1 im; B planes: 0 Xr, 1 Xi, 2 -Xi)
-      const int pa[2] = {T.part == 0 ? 0 : 1, T.part == 0 ? 1 : 0};
       const int pb[2] = {0, T.part == 0 ? 2 : 1};
-      const CUtensorMap* amap = Q.amaps8 + T.blk;
       for (int g = 0; g < n_groups; ++g) {
-        const int dg0 = 4 * g, dg1 = min(S, dg0 + 4) - 1;          // diagonals of this group; slices 0 .. dg1 of both operands
+        const int dg1 = min(S, 4 * g + 4) - 1;                     // slices 0 .. dg1 of both operands feed this group's diagonals
         for (int ch = 0; ch < nch; ++ch, ++bcount) {
           const int sub = ch >= half_ch, kc = (sub ? ch - half_ch : ch) * kSpKC;
           const int buf = bcount % kSpBBuf;
@@ -259,6 +291,26 @@ __global__ void __launch_bounds__(kSpThreads, 1) split_step_kernel(const __grid_
           mbar_expect_tx(&bfull[buf], (unsigned)((dg1 + 1) * kSpTile));
           for (int u = 0; u <= dg1; ++u)
             tma_load_2d(sB + (buf * S + u) * kSpTile, &bmap, &bfull[buf], kc, ((s * 3 + pb[sub]) * S + u) * Q.Npad + n0);
+        }
+      }
+      }
+    }
+  } else if (warp == 10) {
+    if (lane == 0) {            // ===== TMA producer of the A slices (its own thread: the two operand streams never wait for each other)
+      int aslot = 0, aphase = 0;
+      for (int qn = 0;; ++qn) {
+      mbar_wait(&qfull[qn & 3], (qn >> 2) & 1);
+      const int wi = q_item[qn & 3];
+      mbar_arrive(&qempty[qn & 3]);
+      if (wi < 0) break;
+      const SpTile T = sp_decode(P, wi, tiles_per_unit, NTmax, j);
+      const int m0 = T.m0, Mp = T.Mp, nch = T.nch, half_ch = T.nch >> 1;
+      const int pa[2] = {T.part == 0 ? 0 : 1, T.part == 0 ? 1 : 0};
+      const CUtensorMap* amap = Q.amaps8 + T.blk;
+      for (int g = 0; g < n_groups; ++g) {
+        const int dg1 = min(S, 4 * g + 4) - 1;
+        for (int ch = 0; ch < nch; ++ch) {
+          const int sub = ch >= half_ch, kc = (sub ? ch - half_ch : ch) * kSpKC;
           for (int t = 0; t <= dg1; ++t) {
             mbar_wait(&aempty[aslot], aphase ^ 1);
             mbar_expect_tx(&afull[aslot], kSpTile);
@@ -272,7 +324,12 @@ __global__ void __launch_bounds__(kSpThreads, 1) split_step_kernel(const __grid_
   } else if (warp == 1) {
     if (lane == 0) {            // ===== MMA issuer
       int aslot = 0, aphase = 0, bcount = 0, gcount = 0;
-      {
+      for (int qn = 0;; ++qn) {
+      mbar_wait(&qfull[qn & 3], (qn >> 2) & 1);
+      const int wi = q_item[qn & 3];
+      mbar_arrive(&qempty[qn & 3]);
+      if (wi < 0) break;
+      const SpTile T = sp_decode(P, wi, tiles_per_unit, NTmax, j);
       const int nch = T.nch;
       for (int g = 0; g < n_groups; ++g, ++gcount) {
         const int dg0 = 4 * g, dg1 = min(S, dg0 + 4) - 1;
@@ -313,11 +370,17 @@ __global__ void __launch_bounds__(kSpThreads, 1) split_step_kernel(const __grid_
       }
       }
     }
-  } else {
+  } else if (warp >= 2) {
     // ===== epilogue warps: TMEM lane quarter = warp % 4, column half = (warp - 2) / 4
     const int quarter = warp & 3, half = (warp - 2) >> 2;
     int gcount = 0;
-    {
+    for (int qn = 0;; ++qn) {
+    mbar_wait_sleep(&qfull[qn & 3], (qn >> 2) & 1);
+    const int wi = q_item[qn & 3];
+    __syncwarp();
+    if (lane == 0) mbar_arrive(&qempty[qn & 3]);
+    if (wi < 0) break;
+    const SpTile T = sp_decode(P, wi, tiles_per_unit, NTmax, j);
     const int s = T.s, blk = T.blk, dn = T.dn, c = T.c, m0 = T.m0, n0 = T.n0, part = T.part;
     const BlkDesc bd = P.imp.blks[blk];
     const int row = m0 + quarter * 32 + lane;
