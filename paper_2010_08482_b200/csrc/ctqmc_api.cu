@@ -189,18 +189,25 @@ int encode_2d(CUtensorMap* m, const void* base, unsigned long long inner, unsign
   return 0;
 }
 
-// 2-D uint8 tensor map of K-major int8 slice planes: `inner` bytes contiguous, `outer` rows; box = 64 bytes x 128 rows with
-// the 64-byte swizzle the tcgen05 shared-memory descriptors of split_gemm.cuh expect.
-int encode_2d_u8(CUtensorMap* m, const void* base, unsigned long long inner, unsigned long long outer) {
+// 3-D uint8 tensor map of K-major int8 slice planes: `inner` bytes of K contiguous, `rows` rows per slice, `slices` slices; box =
+// 32 bytes x 128 rows x `depth` slices with the 32-byte swizzle the tcgen05 shared-memory descriptors of split_gemm.cuh expect.
+int encode_3d_u8(CUtensorMap* m, const void* base, unsigned long long inner, unsigned long long rows, unsigned long long slices, unsigned depth) {
   EncodeTiledFn fn = encode_tiled_fn();
   if (!fn) return fail(CTQMC_ERR_CUDA, "cuTensorMapEncodeTiled is not available from this driver");
-  const cuuint64_t dims[2] = {inner, outer}, strides[1] = {inner};
-  const cuuint32_t box[2] = {kSpKC, 128}, estr[2] = {1, 1};
-  CUresult r = fn(m, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<void*>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                  CU_TENSOR_MAP_SWIZZLE_64B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-  if (r != CUDA_SUCCESS) return fail(CTQMC_ERR_CUDA, "cuTensorMapEncodeTiled (uint8) failed (%d): inner %llu outer %llu", (int)r, inner, outer);
+  const cuuint64_t dims[3] = {inner, rows, slices}, strides[2] = {inner, inner * rows};
+  const cuuint32_t box[3] = {kSpKC, 128, depth}, estr[3] = {1, 1, 1};
+  CUresult r = fn(m, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<void*>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                  CU_TENSOR_MAP_SWIZZLE_32B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return fail(CTQMC_ERR_CUDA, "cuTensorMapEncodeTiled (uint8, 3-D) failed (%d): inner %llu rows %llu slices %llu", (int)r, inner, rows, slices);
   return 0;
 }
+
+using SplitStepFn = void (*)(const CUtensorMap, const CUtensorMap, LargeParams, SplitStepParams, int, int, int, SplitList);
+SplitStepFn pick_split(int S) {
+  switch (S) { case 5: return split_step_kernel<5>; case 6: return split_step_kernel<6>; case 7: return split_step_kernel<7>; case 8: return split_step_kernel<8>; }
+  return nullptr;
+}
+size_t split_smem(int S) { return (size_t)sp_stages(S) * 2 * S * kSpTile + 1024; }
 
 // Builds (once) the int8 slice planes of the operator store and their tensor maps for the split-precision path.
 int split_prepare(ctqmc_impurity* h) {
@@ -225,15 +232,18 @@ int split_prepare(ctqmc_impurity* h) {
   SplitStore st; st.planes = h->d_sp_planes; st.a_off = h->d_sp_aoff; st.ea = h->d_sp_ea; st.ea_off = h->d_sp_eaoff; st.S = S;
   if (nb > 0) split_slice_store_kernel<<<dim3((unsigned)mpmax, (unsigned)nb), 128>>>(h->dev, st);
   CU(cudaGetLastError());
-  std::vector<CUtensorMap> maps(nb > 0 ? nb : 1);
+  std::vector<CUtensorMap> maps(nb > 0 ? 2 * nb : 1);      // per block: box depth 4 (first group of diagonals) and depth S
   for (int b = 0; b < nb; ++b) {
     const BlkDesc& bd = h->h_blks[b];
-    rc = encode_2d_u8(&maps[b], h->d_sp_planes + aoff[b], (unsigned long long)sp_pad(bd.cols), 2ULL * S * sp_pad(bd.rows));
-    if (rc) return rc;
+    for (int k = 0; k < 2; ++k) {
+      rc = encode_3d_u8(&maps[2 * b + k], h->d_sp_planes + aoff[b], (unsigned long long)sp_pad(bd.cols), (unsigned long long)sp_pad(bd.rows), 2ULL * S,
+                        (unsigned)(k == 0 ? (S < 4 ? S : 4) : S));
+      if (rc) return rc;
+    }
   }
   CU(cudaMalloc((void**)&h->d_amaps8, maps.size() * sizeof(CUtensorMap)));
   CU(cudaMemcpy(h->d_amaps8, maps.data(), maps.size() * sizeof(CUtensorMap), cudaMemcpyHostToDevice));
-  CU(cudaFuncSetAttribute(split_step_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSpSmem2));
+  CU(cudaFuncSetAttribute(pick_split(S), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)split_smem(S)));
   CU(cudaDeviceSynchronize());
   return 0;
 }
@@ -648,8 +658,11 @@ int enqueue_large(ctqmc_impurity* h, const BatchView& bv, const RoundBuf& rb, in
       SplitStepParams sq;
       sq.st.planes = h->d_sp_planes; sq.st.a_off = h->d_sp_aoff; sq.st.ea = h->d_sp_ea; sq.st.ea_off = h->d_sp_eaoff; sq.st.S = h->split_slices;
       sq.bplanes = rb.sp_b; sq.eb = rb.sp_eb; sq.Npad = rb.sp_npad; sq.Kpad = rb.sp_kpad; sq.amaps8 = h->d_amaps8;
-      CUtensorMap bmap;
-      int rc = encode_2d_u8(&bmap, rb.sp_b, (unsigned long long)rb.sp_kpad, (unsigned long long)G * 3 * h->split_slices * rb.sp_npad);
+      CUtensorMap bmap4, bmapS;
+      const int Ssl = h->split_slices;
+      int rc = encode_3d_u8(&bmap4, rb.sp_b, (unsigned long long)rb.sp_kpad, (unsigned long long)rb.sp_npad, (unsigned long long)G * 3 * Ssl, (unsigned)(Ssl < 4 ? Ssl : 4));
+      if (rc) return rc;
+      rc = encode_3d_u8(&bmapS, rb.sp_b, (unsigned long long)rb.sp_kpad, (unsigned long long)rb.sp_npad, (unsigned long long)G * 3 * Ssl, (unsigned)Ssl);
       if (rc) return rc;
       CU(cudaMemsetAsync(rb.sp_b, 0, (size_t)G * 3 * h->split_slices * rb.sp_npad * rb.sp_kpad, st));
       const int MT8 = (h->dev.dmax + kSpM - 1) / kSpM, NT8 = (cw + kSpN - 1) / kSpN;
@@ -661,7 +674,7 @@ int enqueue_large(ctqmc_impurity* h, const BatchView& bv, const RoundBuf& rb, in
       for (int j = 0; j < n_launch; ++j) {
         split_slice_x_kernel<<<xg, 128, 0, st>>>(lp, sq, j);
         split_list_kernel<<<1, 1024, 0, st>>>(lp, wl, j, tiles_per_unit, NT8, total8);
-        split_step_kernel<<<gg, kSpThreads, kSpSmem2, st>>>(bmap, lp, sq, j, NT8, tiles_per_unit, wl);
+        pick_split(Ssl)<<<gg, kSpThreads, split_smem(Ssl), st>>>(bmap4, bmapS, lp, sq, j, NT8, tiles_per_unit, wl);
       }
       large_finish_kernel<true><<<lp.n_group, 256, 0, st>>>(lp);
       h->last_launches += 2 * n_launch;

@@ -174,12 +174,10 @@ __global__ void split_slice_x_kernel(LargeParams P, SplitStepParams Q, int j) {
 // buffered set of up to 8 tiles) and every A slice ONCE (ring), and all their pairs t + u in the group's range are issued from
 // shared memory -- 22 tile loads per chunk instead of 56.  The accumulators of a group are drained by the epilogue warps before the
 // next group starts.
-constexpr int kSpKC = 64;                                  // bytes of K per chunk (2 MMAs of K = 32), 64-byte swizzle
-constexpr int kSpTile = kSpM * kSpKC;                      // 8 KB: one operand tile of one slice
-constexpr int kSpTilesTotal = 28;                         // operand tiles that fit in shared memory: kSpBBuf S for the B sets, the rest is the A ring
-constexpr int kSpBBuf = 2;                                 // B sets in flight; the A ring takes the rest (two chunks deep at 7 slices)
-constexpr int kSpARingMax = kSpTilesTotal - kSpBBuf * 5;
-constexpr size_t kSpSmem2 = (size_t)kSpTilesTotal * kSpTile + 1024;
+constexpr int kSpKC = 32;                                  // bytes of K per chunk: one MMA K step, 32-byte swizzle
+constexpr int kSpTile = kSpM * kSpKC;                      // 4 KB: one operand tile of one slice
+constexpr size_t kSpSmemMax = 226 * 1024;
+__host__ __device__ constexpr int sp_stages(int S) { return (int)((kSpSmemMax - 1024) / ((size_t)2 * S * kSpTile)) < 6 ? (int)((kSpSmemMax - 1024) / ((size_t)2 * S * kSpTile)) : 6; }
 // the epilogue warps wait for a whole group of diagonals: back off instead of spinning on the issue slots
 __device__ __forceinline__ void mbar_wait_sleep(unsigned long long* bar, unsigned parity) {
   unsigned ok = 0;
@@ -188,9 +186,13 @@ __device__ __forceinline__ void mbar_wait_sleep(unsigned long long* bar, unsigne
     if (!ok) __nanosleep(500);
   }
 }
-// shared-memory matrix descriptor: K-major, 64-byte swizzle, rows of 64 bytes, 8-row groups 512 bytes apart
-__device__ __forceinline__ unsigned long long sp_smem_desc64(unsigned saddr) {
-  return (unsigned long long)((saddr & 0x3FFFFu) >> 4) | (1ull << 16) | ((unsigned long long)(512 >> 4) << 32) | (1ull << 46) | (4ull << 61);
+// shared-memory matrix descriptor: K-major, 32-byte swizzle, rows of 32 bytes, 8-row groups 256 bytes apart
+__device__ __forceinline__ unsigned long long sp_smem_desc32(unsigned saddr) {
+  return (unsigned long long)((saddr & 0x3FFFFu) >> 4) | (1ull << 16) | ((unsigned long long)(256 >> 4) << 32) | (1ull << 46) | (6ull << 61);
+}
+__device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, unsigned long long* bar, int c0, int c1, int c2) {
+  asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+               ::"r"(smem_u32(dst)), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar)) : "memory");
 }
 
 struct SpTile { int ok, s, blk, dn, d, c, m0, n0, part, Mp, nch; };
@@ -236,27 +238,48 @@ __global__ void split_list_kernel(LargeParams P, SplitList W, int j, int tiles_p
   }
 }
 
-__global__ void __launch_bounds__(kSpThreads, 1) split_step_kernel(const __grid_constant__ CUtensorMap bmap, LargeParams P, SplitStepParams Q, int j, int NTmax,
-                                                                   int tiles_per_unit, SplitList W) {
+// The MMAs of one K chunk of one group of diagonals: compile-time (t, u) pattern, two neighbouring B slices as one N = 256 operand
+// feeding two neighbouring accumulators wherever a slice has a neighbour left.  Straight-line code: the single issuing thread has
+// ~100 cycles per instruction (a microbenchmark of the same instruction with ~50 scalar instructions of bookkeeping per product
+// ran at a third of the pipe's rate).
+template <int S, int G>
+__device__ __forceinline__ void sp_issue_chunk(unsigned tmem, unsigned long long a_set, unsigned long long b_set, unsigned accum) {
+  constexpr int dg0 = 4 * G, dg1 = (S < dg0 + 4 ? S : dg0 + 4) - 1;
+#pragma unroll
+  for (int t = 0; t <= dg1; ++t) {
+    const unsigned long long ad = a_set + (unsigned long long)(t * (kSpTile >> 4));
+    const int ulo = dg0 - t > 0 ? dg0 - t : 0, uhi = dg1 - t;
+    const unsigned acc_t = (t == 0) ? accum : 1u;            // t = 0 touches every accumulator of the group first
+#pragma unroll
+    for (int u = ulo; u <= uhi; u += 2) {
+      const unsigned long long bdsc = b_set + (unsigned long long)(u * (kSpTile >> 4));
+      const unsigned dst = tmem + (unsigned)((t + u - dg0) * kSpN);
+      if (u + 1 <= uhi) tc_mma_i8(dst, ad, bdsc, kSpIdesc256, acc_t);
+      else              tc_mma_i8(dst, ad, bdsc, kSpIdesc, acc_t);
+    }
+  }
+}
+
+template <int S>
+__global__ void __launch_bounds__(kSpThreads, 1) split_step_kernel(const __grid_constant__ CUtensorMap bmap4, const __grid_constant__ CUtensorMap bmapS, LargeParams P,
+                                                                   SplitStepParams Q, int j, int NTmax, int tiles_per_unit, SplitList W) {
+  constexpr int NST = sp_stages(S);                            // stages: every stage holds all slices of both operands for one K chunk
+  constexpr int n_groups = (S + 3) / 4;
   extern __shared__ unsigned char sp_raw[];
-  __shared__ __align__(8) unsigned long long afull[kSpARingMax], aempty[kSpARingMax], bfull[kSpBBuf], bempty[kSpBBuf], tfull_bar, tempty_bar;
+  __shared__ __align__(8) unsigned long long full[NST], empty[NST], tfull_bar, tempty_bar;
   __shared__ __align__(8) unsigned long long qfull[4], qempty[4];
   __shared__ int q_item[4];
   __shared__ unsigned s_tmem;
-  // Persistent: one CTA per SM takes items off the work list (atomic counter); the producer thread fetches them and hands them to
-  // the MMA thread and the epilogue warps through a four-deep queue, so barriers, the TMEM allocation and the ring / phase counters
-  // live across items and the epilogue's final store of one item overlaps the next item's first products.
+  // Persistent: one CTA per SM takes items off the work list (atomic counter); the B producer fetches them and hands them to the A
+  // producer, the MMA thread and the epilogue warps through a four-deep queue, so barriers, the TMEM allocation and the ring / phase
+  // counters live across items and the epilogue's final store of one item overlaps the next item's first products.
   unsigned char* smem = reinterpret_cast<unsigned char*>(((uintptr_t)sp_raw + 1023) & ~(uintptr_t)1023);
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int S = Q.st.S;
-  const int nA = kSpTilesTotal - kSpBBuf * S;                      // depth of the A ring: what the B sets leave
-  unsigned char* sB = smem;                                        // [kSpBBuf][S] tiles
-  unsigned char* sA = smem + kSpBBuf * S * kSpTile;                // [nA] tiles
-  const int n_groups = (S + 3) / 4;
+  unsigned char* sA = smem;                                        // [NST][S] tiles
+  unsigned char* sB = smem + NST * S * kSpTile;                    // [NST][S] tiles
 
   if (tid == 0) {
-    for (int i = 0; i < nA; ++i) { mbar_init(&afull[i], 1); mbar_init(&aempty[i], 1); }
-    for (int i = 0; i < kSpBBuf; ++i) { mbar_init(&bfull[i], 1); mbar_init(&bempty[i], 1); }
+    for (int i = 0; i < NST; ++i) { mbar_init(&full[i], 2); mbar_init(&empty[i], 1); }      // both producers arm a stage; one commit frees it
     mbar_init(&tfull_bar, 1); mbar_init(&tempty_bar, 8);
     for (int i = 0; i < 4; ++i) { mbar_init(&qfull[i], 1); mbar_init(&qempty[i], 10); }    // consumers: A producer, MMA thread, 8 epilogue warps
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -268,106 +291,83 @@ __global__ void __launch_bounds__(kSpThreads, 1) split_step_kernel(const __grid_
   const unsigned tmem = s_tmem;
 
   if (warp == 0) {
-    if (lane == 0) {            // ===== TMA producer
-      int bcount = 0;
+    if (lane == 0) {            // ===== work-item fetch + TMA producer of the B slices (one 3-D box per K chunk: all slices of the group)
+      int stage = 0, phase = 0;
       const int n_items = W.ctr[0];
       for (int qn = 0;; ++qn) {
-      mbar_wait(&qempty[qn & 3], ((qn >> 2) & 1) ^ 1);
-      const int it = atomicAdd(&W.ctr[1], 1);
-      const int wi = it < n_items ? W.items[it] : -1;
-      q_item[qn & 3] = wi;
-      mbar_arrive(&qfull[qn & 3]);
-      if (wi < 0) break;
-      const SpTile T = sp_decode(P, wi, tiles_per_unit, NTmax, j);
-      const int s = T.s, n0 = T.n0, nch = T.nch, half_ch = T.nch >> 1;
-      // sub-products of this part: real = Fr Xr + Fi (-Xi), imaginary = Fi Xr + Fr Xi   (A planes: 0 re, 1 im; B planes: 0 Xr, 1 Xi, 2 -Xi)
-      const int pb[2] = {0, T.part == 0 ? 2 : 1};
-      for (int g = 0; g < n_groups; ++g) {
-        const int dg1 = min(S, 4 * g + 4) - 1;                     // slices 0 .. dg1 of both operands feed this group's diagonals
-        for (int ch = 0; ch < nch; ++ch, ++bcount) {
-          const int sub = ch >= half_ch, kc = (sub ? ch - half_ch : ch) * kSpKC;
-          const int buf = bcount % kSpBBuf;
-          mbar_wait(&bempty[buf], ((bcount / kSpBBuf) & 1) ^ 1);
-          mbar_expect_tx(&bfull[buf], (unsigned)((dg1 + 1) * kSpTile));
-          for (int u = 0; u <= dg1; ++u)
-            tma_load_2d(sB + (buf * S + u) * kSpTile, &bmap, &bfull[buf], kc, ((s * 3 + pb[sub]) * S + u) * Q.Npad + n0);
+        mbar_wait(&qempty[qn & 3], ((qn >> 2) & 1) ^ 1);
+        const int it = atomicAdd(&W.ctr[1], 1);
+        const int wi = it < n_items ? W.items[it] : -1;
+        q_item[qn & 3] = wi;
+        mbar_arrive(&qfull[qn & 3]);
+        if (wi < 0) break;
+        const SpTile T = sp_decode(P, wi, tiles_per_unit, NTmax, j);
+        const int half_ch = T.nch >> 1;
+        // sub-products of this part: real = Fr Xr + Fi (-Xi), imaginary = Fi Xr + Fr Xi   (A planes: 0 re, 1 im; B planes: 0 Xr, 1 Xi, 2 -Xi)
+        const int pb[2] = {0, T.part == 0 ? 2 : 1};
+        for (int g = 0; g < n_groups; ++g) {
+          const int ns = g == 0 ? (S < 4 ? S : 4) : S;             // slices 0 .. ns-1 of both operands feed this group's diagonals
+          const CUtensorMap* bm = g == 0 ? &bmap4 : &bmapS;
+          for (int ch = 0; ch < T.nch; ++ch) {
+            const int sub = ch >= half_ch, kc = (sub ? ch - half_ch : ch) * kSpKC;
+            mbar_wait(&empty[stage], phase ^ 1);
+            mbar_expect_tx(&full[stage], (unsigned)(ns * kSpTile));
+            tma_load_3d(sB + stage * S * kSpTile, bm, &full[stage], kc, T.n0, (T.s * 3 + pb[sub]) * S);
+            if (++stage == NST) { stage = 0; phase ^= 1; }
+          }
         }
-      }
       }
     }
   } else if (warp == 10) {
     if (lane == 0) {            // ===== TMA producer of the A slices (its own thread: the two operand streams never wait for each other)
-      int aslot = 0, aphase = 0;
+      int stage = 0, phase = 0;
       for (int qn = 0;; ++qn) {
-      mbar_wait(&qfull[qn & 3], (qn >> 2) & 1);
-      const int wi = q_item[qn & 3];
-      mbar_arrive(&qempty[qn & 3]);
-      if (wi < 0) break;
-      const SpTile T = sp_decode(P, wi, tiles_per_unit, NTmax, j);
-      const int m0 = T.m0, Mp = T.Mp, nch = T.nch, half_ch = T.nch >> 1;
-      const int pa[2] = {T.part == 0 ? 0 : 1, T.part == 0 ? 1 : 0};
-      const CUtensorMap* amap = Q.amaps8 + T.blk;
-      for (int g = 0; g < n_groups; ++g) {
-        const int dg1 = min(S, 4 * g + 4) - 1;
-        for (int ch = 0; ch < nch; ++ch) {
-          const int sub = ch >= half_ch, kc = (sub ? ch - half_ch : ch) * kSpKC;
-          for (int t = 0; t <= dg1; ++t) {
-            mbar_wait(&aempty[aslot], aphase ^ 1);
-            mbar_expect_tx(&afull[aslot], kSpTile);
-            tma_load_2d(sA + aslot * kSpTile, amap, &afull[aslot], kc, (pa[sub] * S + t) * Mp + m0);
-            if (++aslot == nA) { aslot = 0; aphase ^= 1; }
+        mbar_wait(&qfull[qn & 3], (qn >> 2) & 1);
+        const int wi = q_item[qn & 3];
+        mbar_arrive(&qempty[qn & 3]);
+        if (wi < 0) break;
+        const SpTile T = sp_decode(P, wi, tiles_per_unit, NTmax, j);
+        const int half_ch = T.nch >> 1;
+        const int pa[2] = {T.part == 0 ? 0 : 1, T.part == 0 ? 1 : 0};
+        for (int g = 0; g < n_groups; ++g) {
+          const int ns = g == 0 ? (S < 4 ? S : 4) : S;
+          const CUtensorMap* am = Q.amaps8 + 2 * T.blk + (g == 0 ? 0 : 1);
+          for (int ch = 0; ch < T.nch; ++ch) {
+            const int sub = ch >= half_ch, kc = (sub ? ch - half_ch : ch) * kSpKC;
+            mbar_wait(&empty[stage], phase ^ 1);
+            mbar_expect_tx(&full[stage], (unsigned)(ns * kSpTile));
+            tma_load_3d(sA + stage * S * kSpTile, am, &full[stage], kc, T.m0, pa[sub] * S);
+            if (++stage == NST) { stage = 0; phase ^= 1; }
           }
         }
-      }
       }
     }
   } else if (warp == 1) {
     if (lane == 0) {            // ===== MMA issuer
-      int aslot = 0, aphase = 0, bcount = 0, gcount = 0;
+      int stage = 0, phase = 0, gcount = 0;
+      const unsigned long long a_base = sp_smem_desc32(smem_u32(sA)), b_base = sp_smem_desc32(smem_u32(sB));
       for (int qn = 0;; ++qn) {
-      mbar_wait(&qfull[qn & 3], (qn >> 2) & 1);
-      const int wi = q_item[qn & 3];
-      mbar_arrive(&qempty[qn & 3]);
-      if (wi < 0) break;
-      const SpTile T = sp_decode(P, wi, tiles_per_unit, NTmax, j);
-      const int nch = T.nch;
-      for (int g = 0; g < n_groups; ++g, ++gcount) {
-        const int dg0 = 4 * g, dg1 = min(S, dg0 + 4) - 1;
-        mbar_wait(&tempty_bar, (gcount & 1) ^ 1);                  // the epilogue has drained the previous group's accumulators
-        tc_fence_after();
-        // descriptors are plain offsets from two bases (tiles are 8 KB = 512 descriptor units apart)
-        const unsigned long long a_base = sp_smem_desc64(smem_u32(sA)), b_base = sp_smem_desc64(smem_u32(sB));
-        for (int ch = 0; ch < nch; ++ch, ++bcount) {
-          const int buf = bcount % kSpBBuf;
-          mbar_wait(&bfull[buf], (bcount / kSpBBuf) & 1);
+        mbar_wait(&qfull[qn & 3], (qn >> 2) & 1);
+        const int wi = q_item[qn & 3];
+        mbar_arrive(&qempty[qn & 3]);
+        if (wi < 0) break;
+        const SpTile T = sp_decode(P, wi, tiles_per_unit, NTmax, j);
+        const int nch = T.nch;
+#pragma unroll
+        for (int g = 0; g < n_groups; ++g, ++gcount) {
+          mbar_wait(&tempty_bar, (gcount & 1) ^ 1);                // the epilogue has drained the previous group's accumulators
           tc_fence_after();
-          for (int t = 0; t <= dg1; ++t) {
-            mbar_wait(&afull[aslot], aphase);
+          for (int ch = 0; ch < nch; ++ch) {
+            mbar_wait(&full[stage], phase);
             tc_fence_after();
-            const unsigned long long ad = a_base + (unsigned long long)(aslot * (kSpTile >> 4));
-            const unsigned accum = (ch > 0 || t > 0) ? 1u : 0u;     // t = 0 of the first chunk touches every accumulator of the group
-            int u = max(0, dg0 - t);
-            const int uhi = dg1 - t;
-            // two neighbouring B slices are one 256-row operand and their diagonals neighbouring accumulators: N = 256
-            for (; u + 1 <= uhi; u += 2) {
-              const unsigned long long bdsc = b_base + (unsigned long long)((buf * S + u) * (kSpTile >> 4));
-              const unsigned dst = tmem + (unsigned)((t + u - dg0) * kSpN);
-              tc_mma_i8(dst, ad, bdsc, kSpIdesc256, accum);
-              tc_mma_i8(dst, ad + 2, bdsc + 2, kSpIdesc256, 1u);
-            }
-            if (u <= uhi) {
-              const unsigned long long bdsc = b_base + (unsigned long long)((buf * S + u) * (kSpTile >> 4));
-              const unsigned dst = tmem + (unsigned)((t + u - dg0) * kSpN);
-              tc_mma_i8(dst, ad, bdsc, kSpIdesc, accum);
-              tc_mma_i8(dst, ad + 2, bdsc + 2, kSpIdesc, 1u);
-            }
-            tc_commit(&aempty[aslot]);
-            if (++aslot == nA) { aslot = 0; aphase ^= 1; }
+            const unsigned long long off = (unsigned long long)(stage * S * (kSpTile >> 4));
+            if (g == 0) sp_issue_chunk<S, 0>(tmem, a_base + off, b_base + off, ch > 0 ? 1u : 0u);
+            else        sp_issue_chunk<S, 1>(tmem, a_base + off, b_base + off, ch > 0 ? 1u : 0u);
+            tc_commit(&empty[stage]);                             // the stage is free once these MMAs have read it
+            if (++stage == NST) { stage = 0; phase ^= 1; }
           }
-          tc_commit(&bempty[buf]);
+          tc_commit(&tfull_bar);                                   // the group's diagonals are complete in TMEM
         }
-        tc_commit(&tfull_bar);                                     // the group's diagonals are complete in TMEM
-      }
       }
     }
   } else if (warp >= 2) {
