@@ -112,7 +112,6 @@ struct ctqmc_impurity {
   // split-precision large-sector path (split_gemm.cuh): int8 slice planes of the operator store, their tensor maps
   int split = 0, split_slices = 7;
   signed char* d_sp_planes = nullptr; long long* d_sp_aoff = nullptr; int* d_sp_ea = nullptr; long long* d_sp_eaoff = nullptr;
-  CUtensorMap* d_amaps8 = nullptr;
   long long* d_rho_off = nullptr;     // [Q] offset of sector q's block in the reduced density matrix (sum of dim^2)
   long long rho_len = 0;
   std::vector<BlkDesc> h_blks;        // host copy (tensor-map construction)
@@ -189,27 +188,14 @@ int encode_2d(CUtensorMap* m, const void* base, unsigned long long inner, unsign
   return 0;
 }
 
-// 3-D uint8 tensor map of K-major int8 slice planes: `inner` bytes of K contiguous, `rows` rows per slice, `slices` slices; box =
-// 32 bytes x 128 rows x `depth` slices with the 32-byte swizzle the tcgen05 shared-memory descriptors of split_gemm.cuh expect.
-int encode_3d_u8(CUtensorMap* m, const void* base, unsigned long long inner, unsigned long long rows, unsigned long long slices, unsigned depth) {
-  EncodeTiledFn fn = encode_tiled_fn();
-  if (!fn) return fail(CTQMC_ERR_CUDA, "cuTensorMapEncodeTiled is not available from this driver");
-  const cuuint64_t dims[3] = {inner, rows, slices}, strides[2] = {inner, inner * rows};
-  const cuuint32_t box[3] = {kSpKC, 128, depth}, estr[3] = {1, 1, 1};
-  CUresult r = fn(m, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<void*>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                  CU_TENSOR_MAP_SWIZZLE_32B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-  if (r != CUDA_SUCCESS) return fail(CTQMC_ERR_CUDA, "cuTensorMapEncodeTiled (uint8, 3-D) failed (%d): inner %llu rows %llu slices %llu", (int)r, inner, rows, slices);
-  return 0;
-}
-
-using SplitStepFn = void (*)(const CUtensorMap, const CUtensorMap, LargeParams, SplitStepParams, int, int, int, SplitList);
+using SplitStepFn = void (*)(LargeParams, SplitStepParams, int, int, int, SplitList);
 SplitStepFn pick_split(int S) {
   switch (S) { case 5: return split_step_kernel<5>; case 6: return split_step_kernel<6>; case 7: return split_step_kernel<7>; case 8: return split_step_kernel<8>; }
   return nullptr;
 }
 size_t split_smem(int S) { return (size_t)sp_stages(S) * 2 * S * kSpTile + 1024; }
 
-// Builds (once) the int8 slice planes of the operator store and their tensor maps for the split-precision path.
+// Builds (once) the int8 slice planes of the operator store for the split-precision path.
 int split_prepare(ctqmc_impurity* h) {
   if (h->d_sp_planes) return 0;
   const int nb = h->n_blocks, S = h->split_slices;
@@ -232,17 +218,6 @@ int split_prepare(ctqmc_impurity* h) {
   SplitStore st; st.planes = h->d_sp_planes; st.a_off = h->d_sp_aoff; st.ea = h->d_sp_ea; st.ea_off = h->d_sp_eaoff; st.S = S;
   if (nb > 0) split_slice_store_kernel<<<dim3((unsigned)mpmax, (unsigned)nb), 128>>>(h->dev, st);
   CU(cudaGetLastError());
-  std::vector<CUtensorMap> maps(nb > 0 ? 2 * nb : 1);      // per block: box depth 4 (first group of diagonals) and depth S
-  for (int b = 0; b < nb; ++b) {
-    const BlkDesc& bd = h->h_blks[b];
-    for (int k = 0; k < 2; ++k) {
-      rc = encode_3d_u8(&maps[2 * b + k], h->d_sp_planes + aoff[b], (unsigned long long)sp_pad(bd.cols), (unsigned long long)sp_pad(bd.rows), 2ULL * S,
-                        (unsigned)(k == 0 ? (S < 4 ? S : 4) : S));
-      if (rc) return rc;
-    }
-  }
-  CU(cudaMalloc((void**)&h->d_amaps8, maps.size() * sizeof(CUtensorMap)));
-  CU(cudaMemcpy(h->d_amaps8, maps.data(), maps.size() * sizeof(CUtensorMap), cudaMemcpyHostToDevice));
   CU(cudaFuncSetAttribute(pick_split(S), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)split_smem(S)));
   CU(cudaDeviceSynchronize());
   return 0;
@@ -657,13 +632,8 @@ int enqueue_large(ctqmc_impurity* h, const BatchView& bv, const RoundBuf& rb, in
       // split-precision step (split_gemm.cuh): slice the carried matrices, then the int8 tensor-core product
       SplitStepParams sq;
       sq.st.planes = h->d_sp_planes; sq.st.a_off = h->d_sp_aoff; sq.st.ea = h->d_sp_ea; sq.st.ea_off = h->d_sp_eaoff; sq.st.S = h->split_slices;
-      sq.bplanes = rb.sp_b; sq.eb = rb.sp_eb; sq.Npad = rb.sp_npad; sq.Kpad = rb.sp_kpad; sq.amaps8 = h->d_amaps8;
-      CUtensorMap bmap4, bmapS;
+      sq.bplanes = rb.sp_b; sq.eb = rb.sp_eb; sq.Npad = rb.sp_npad; sq.Kpad = rb.sp_kpad;
       const int Ssl = h->split_slices;
-      int rc = encode_3d_u8(&bmap4, rb.sp_b, (unsigned long long)rb.sp_kpad, (unsigned long long)rb.sp_npad, (unsigned long long)G * 3 * Ssl, (unsigned)(Ssl < 4 ? Ssl : 4));
-      if (rc) return rc;
-      rc = encode_3d_u8(&bmapS, rb.sp_b, (unsigned long long)rb.sp_kpad, (unsigned long long)rb.sp_npad, (unsigned long long)G * 3 * Ssl, (unsigned)Ssl);
-      if (rc) return rc;
       CU(cudaMemsetAsync(rb.sp_b, 0, (size_t)G * 3 * h->split_slices * rb.sp_npad * rb.sp_kpad, st));
       const int MT8 = (h->dev.dmax + kSpM - 1) / kSpM, NT8 = (cw + kSpN - 1) / kSpN;
       const int tiles_per_unit = MT8 * NT8 * 2;
@@ -674,7 +644,7 @@ int enqueue_large(ctqmc_impurity* h, const BatchView& bv, const RoundBuf& rb, in
       for (int j = 0; j < n_launch; ++j) {
         split_slice_x_kernel<<<xg, 128, 0, st>>>(lp, sq, j);
         split_list_kernel<<<1, 1024, 0, st>>>(lp, wl, j, tiles_per_unit, NT8, total8);
-        pick_split(Ssl)<<<gg, kSpThreads, split_smem(Ssl), st>>>(bmap4, bmapS, lp, sq, j, NT8, tiles_per_unit, wl);
+        pick_split(Ssl)<<<gg, kSpThreads, split_smem(Ssl), st>>>(lp, sq, j, NT8, tiles_per_unit, wl);
       }
       large_finish_kernel<true><<<lp.n_group, 256, 0, st>>>(lp);
       h->last_launches += 2 * n_launch;
@@ -913,7 +883,7 @@ extern "C" void ctqmc_free_impurity(ctqmc_impurity* h) {
   cudaFree(h->d_dim); cudaFree(h->d_eoff); cudaFree(h->d_energy); cudaFree(h->d_emin); cudaFree(h->d_blkof);
   cudaFree(h->d_ftpad); cudaFree(h->d_binfo);
   cudaFree(h->d_pack); cudaFree(h->d_pblk); cudaFree(h->d_blkorder); cudaFree(h->d_rho_off);
-  cudaFree(h->d_sp_planes); cudaFree(h->d_sp_aoff); cudaFree(h->d_sp_ea); cudaFree(h->d_sp_eaoff); cudaFree(h->d_amaps8);
+  cudaFree(h->d_sp_planes); cudaFree(h->d_sp_aoff); cudaFree(h->d_sp_ea); cudaFree(h->d_sp_eaoff);
   cudaFree(h->d_blks); cudaFree(h->d_store); cudaFree(h->d_rownorm2); cudaFree(h->d_sigma);
   Arena& a = h->arena;
   cudaFree(a.base); cudaFree(a.cnt); cudaFree(a.cnt_total); cudaFree(h->d_amaps); cudaFree(a.d_stage);

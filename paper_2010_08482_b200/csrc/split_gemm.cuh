@@ -9,10 +9,15 @@
 //     C_ij = 2^(eA_i + eB_j - 14) sum_{dg < S} 2^(-7 dg) D_dg,     D_dg = sum_{t + u = dg} sum_k q^A_t,ik q^B_u,kj   (int32, exact),
 // complex as [Cr; Ci] = [Fr Xr + Fi (-Xi); Fi Xr + Fr Xi] (the minus sign lives in a third set of X planes).  Every D_dg is one
 // accumulation chain of tcgen05.mma.kind::i8 (M = 128, N = 128, K = 32) into TMEM; |D_dg| <= 7 * 2 * 3003 * 64 * 64 < 2^31.
-// A CTA owns one 128 x 128 tile of Cr or Ci: warp 0 feeds a 5-stage shared-memory ring with TMA (128-byte swizzled boxes of
-// the K-major slice planes), one thread of warp 1 issues the MMAs and commits stages / accumulators to mbarriers, warps 2-9
-// drain the double-buffered TMEM accumulator with tcgen05.ld, weight the diagonals in FP64 registers, and finish the step exactly
-// like large_step_kernel (propagator mantissa per row, store, largest row exponent by atomicMax).
+// Work is cut into items of one 128-row tile x one group of up to four diagonals x one 128-column tile of [Cr; Ci]; the items of a
+// chain position are listed heaviest first (split_list_kernel) and persistent CTAs (one per SM) take them from an atomic counter
+// through a four-deep queue.  Per item and 32-byte K chunk ONE 1-D bulk copy per operand brings all slices the group needs into a
+// shared-memory stage (the planes are stored as the tensor core's shared-memory image, 32-byte swizzle pre-applied, so the copies
+// move whole 128-byte lines); warp 0 fetches items and copies X slices, warp 10 copies F slices, one thread of warp 1 issues the
+// MMAs as straight-line code (compile-time (t, u) pattern, neighbouring X slices paired into N = 256) and commits stages /
+// accumulators to mbarriers, warps 2-9 drain the TMEM accumulators (4 diagonals side by side = 512 columns) with tcgen05.ld,
+// weight the diagonals in FP64 registers, and finish the step exactly like large_step_kernel (propagator mantissa per row,
+// store, largest row exponent by atomicMax).  History and measurements: profiles/r02_split_step.md.
 #pragma once
 #include <cuda.h>
 
@@ -21,12 +26,9 @@
 
 namespace ctqmc {
 
-constexpr int kSpM = 128, kSpN = 128, kSpKB = 128;        // tile, bytes of K per stage row (= 128 int8 = 4 MMAs of K = 32)
-constexpr int kSpStages = 5;
-constexpr int kSpStageBytes = (kSpM + kSpN) * kSpKB;      // 32 KB
+constexpr int kSpM = 128, kSpN = 128;                     // output tile of one MMA accumulator
 constexpr int kSpThreads = 352;                           // B-producer warp, MMA warp, 8 epilogue warps, A-producer warp
 constexpr int kSpMaxSlices = 8;
-constexpr size_t kSpSmemBytes = (size_t)kSpStages * kSpStageBytes + 1024;   // + alignment slack
 
 // ---- tcgen05 / TMEM primitives (inline PTX; sm_100a)
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
@@ -61,21 +63,25 @@ __device__ __forceinline__ void tmem_ld32(unsigned taddr, int (&v)[32]) {
       : "r"(taddr) : "memory");
   asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 }
-// shared-memory matrix descriptor: K-major operand, 128-byte swizzle, rows of 128 bytes, 8-row groups 1024 bytes apart
-__device__ __forceinline__ unsigned long long sp_smem_desc(unsigned saddr) {
-  return (unsigned long long)((saddr & 0x3FFFFu) >> 4) | (1ull << 16) | ((unsigned long long)(1024 >> 4) << 32) | (1ull << 46) | (2ull << 61);
-}
 // instruction descriptor: S32 accumulate, signed 8-bit A and B, both K-major, N = 128, M = 128
 constexpr unsigned kSpIdesc = (2u << 4) | (1u << 7) | (1u << 10) | ((unsigned)(kSpN >> 3) << 17) | ((unsigned)(kSpM >> 4) << 24);
 constexpr unsigned kSpIdesc256 = (2u << 4) | (1u << 7) | (1u << 10) | ((unsigned)(256 >> 3) << 17) | ((unsigned)(kSpM >> 4) << 24);   // N = 256
 
 // ---- slicing: one vector (a row of F, or a column of X with the deferred row scaling of the previous step) per CTA.
 // v_k = 2^e sum_t q_t[k] 2^(-7 (t + 1)), e = exponent of the largest |re| / |im| of the vector + 2, |q_t| <= 64.
+// Plane layout = the shared-memory image the tensor core reads, tile by tile: [128-row tile][K chunk of 32 bytes][slice][4 KB], the
+// 4 KB being 128 rows x 32 bytes with the 32-byte swizzle applied (16-byte halves of a row exchanged when bit 2 of the row is set).
+// All slices of one (row tile, K chunk) are contiguous, so a stage is filled by ONE 1-D bulk copy per operand, in whole 128-byte lines.
 struct SliceOut {
-  signed char* re; signed char* im; signed char* nim;   // plane bases of THIS vector's row for slice 0 (nim may be null)
-  long long slice_stride;                               // bytes between consecutive slices of a plane
+  signed char* re; signed char* im; signed char* nim;   // plane bases (nim may be null)
+  int S, nkc;                                           // slices, K chunks per row of the plane
+  int row;                                              // this vector's row in the plane
   int kpad;                                             // bytes to fill (zero beyond the vector's length)
 };
+__device__ __forceinline__ long long sp_image_index(int k, int row, int t, int S, int nkc) {
+  const int r = row & 127;
+  return ((((long long)(row >> 7) * nkc + (k >> 5)) * S + t) << 12) + r * 32 + ((((k >> 4) & 1) ^ ((r >> 2) & 1)) << 4) + (k & 15);
+}
 template <class Scale>
 __device__ __forceinline__ void sp_slice_vector(const double* src, long long stride /*doubles between elements*/, int len, Scale kscale,
                                                 int S, const SliceOut& o, int* e_out, int* redi) {
@@ -98,15 +104,16 @@ __device__ __forceinline__ void sp_slice_vector(const double* src, long long str
       rr *= 128.0; ri *= 128.0;
       const double qr = rint(rr), qi = rint(ri);
       rr -= qr; ri -= qi;
-      o.re[t * o.slice_stride + k] = (signed char)(int)qr;
-      o.im[t * o.slice_stride + k] = (signed char)(int)qi;
-      if (o.nim) o.nim[t * o.slice_stride + k] = (signed char)(-(int)qi);
+      const long long at = sp_image_index(k, o.row, t, o.S, o.nkc);
+      o.re[at] = (signed char)(int)qr;
+      o.im[at] = (signed char)(int)qi;
+      if (o.nim) o.nim[at] = (signed char)(-(int)qi);
     }
   }
 }
 
 struct SplitStore {          // int8 slice planes of the operator store, built at load
-  signed char* planes;       // block b at a_off[b]: [2 (re, im)][S][Mpad_b][Kpad_b]
+  signed char* planes;       // block b at a_off[b]: [2 (re, im)] images of S * Mpad_b * Kpad_b bytes (sp_image_index)
   const long long* a_off;    // [n_blocks]
   int* ea;                   // row exponents, block b at ea_off[b] (Mpad_b entries)
   const long long* ea_off;
@@ -123,17 +130,15 @@ __global__ void split_slice_store_kernel(DevImp imp, SplitStore st) {
   const int Mp = sp_pad(bd.rows), Kp = sp_pad(bd.cols);
   signed char* base = st.planes + st.a_off[blockIdx.y];
   SliceOut o;
-  o.slice_stride = (long long)Mp * Kp;
-  o.re = base + (long long)i * Kp; o.im = base + (long long)st.S * o.slice_stride + (long long)i * Kp; o.nim = nullptr; o.kpad = Kp;
+  o.re = base; o.im = base + (long long)st.S * Mp * Kp; o.nim = nullptr; o.kpad = Kp; o.S = st.S; o.nkc = Kp / 32; o.row = i;
   sp_slice_vector(imp.store + bd.off + (long long)i * bd.ld * 2, 2, bd.cols, [](int) { return 1.0; }, st.S, o, st.ea + st.ea_off[blockIdx.y] + i, redi);
 }
 
 struct SplitStepParams {
   SplitStore st;
-  signed char* bplanes;      // per unit: [3 (Xr, Xi, -Xi)][S][Npad][Kpad]
+  signed char* bplanes;      // per unit: [3 (Xr, Xi, -Xi)] images of S * Npad * Kpad bytes (sp_image_index)
   int* eb;                   // [units][Npad] column exponents
   int Npad, Kpad;            // sp_pad(widest carried matrix), sp_pad(d_max)
-  const CUtensorMap* amaps8; // [n_blocks] uint8 maps of the slice planes (inner Kpad_b bytes, outer 2 S Mpad_b rows)
 };
 
 // columns of the carried matrix of every unit -> int8 slice planes, with the exact power-of-two row factor of the previous
@@ -159,10 +164,9 @@ __global__ void split_slice_x_kernel(LargeParams P, SplitStepParams Q, int j) {
     return (sh < -1022) ? 0.0 : pow2i((int)min(sh, 1022LL));
   };
   const long long row_bytes = Q.Kpad, plane = (long long)Q.st.S * Q.Npad * row_bytes;
-  signed char* base = Q.bplanes + (long long)s * 3 * plane + (long long)n * row_bytes;
+  signed char* base = Q.bplanes + (long long)s * 3 * plane;
   SliceOut o;
-  o.slice_stride = (long long)Q.Npad * row_bytes;
-  o.re = base; o.im = base + plane; o.nim = base + 2 * plane; o.kpad = sp_pad(d);
+  o.re = base; o.im = base + plane; o.nim = base + 2 * plane; o.kpad = sp_pad(d); o.S = Q.st.S; o.nkc = Q.Kpad / 32; o.row = n;
   sp_slice_vector(col, 2, d, scale, Q.st.S, o, Q.eb + (size_t)s * Q.Npad + n, redi);
 }
 
@@ -170,10 +174,9 @@ __global__ void split_slice_x_kernel(LargeParams P, SplitStepParams Q, int j) {
 //
 // Operand traffic decides this kernel: with one (A slice, B slice) pair fetched per product the ring pulls 17 TB/s out of L2 and
 // the tensor pipe waits (57 % busy, profiles/r02_split_step.md).  So the diagonals are evaluated in GROUPS of up to four that are
-// accumulated side by side in TMEM (4 x 128 columns): per 64-byte K chunk every B slice the group needs is loaded ONCE (double-
-// buffered set of up to 8 tiles) and every A slice ONCE (ring), and all their pairs t + u in the group's range are issued from
-// shared memory -- 22 tile loads per chunk instead of 56.  The accumulators of a group are drained by the epilogue warps before the
-// next group starts.
+// accumulated side by side in TMEM (4 x 128 columns): per 32-byte K chunk every slice of both operands the group needs is loaded
+// ONCE into one stage and all their pairs t + u in the group's range are issued from shared memory.  The accumulators of a group
+// are drained by the epilogue warps before the next group starts.
 constexpr int kSpKC = 32;                                  // bytes of K per chunk: one MMA K step, 32-byte swizzle
 constexpr int kSpTile = kSpM * kSpKC;                      // 4 KB: one operand tile of one slice
 constexpr size_t kSpSmemMax = 226 * 1024;
@@ -190,9 +193,9 @@ __device__ __forceinline__ void mbar_wait_sleep(unsigned long long* bar, unsigne
 __device__ __forceinline__ unsigned long long sp_smem_desc32(unsigned saddr) {
   return (unsigned long long)((saddr & 0x3FFFFu) >> 4) | (1ull << 16) | ((unsigned long long)(256 >> 4) << 32) | (1ull << 46) | (6ull << 61);
 }
-__device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, unsigned long long* bar, int c0, int c1, int c2) {
-  asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
-               ::"r"(smem_u32(dst)), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar)) : "memory");
+__device__ __forceinline__ void bulk_load(void* dst, const void* src, unsigned bytes, unsigned long long* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
 
 struct SpTile { int ok, s, blk, dn, d, c, m0, n0, part, Mp, nch; };
@@ -261,8 +264,7 @@ __device__ __forceinline__ void sp_issue_chunk(unsigned tmem, unsigned long long
 }
 
 template <int S>
-__global__ void __launch_bounds__(kSpThreads, 1) split_step_kernel(const __grid_constant__ CUtensorMap bmap4, const __grid_constant__ CUtensorMap bmapS, LargeParams P,
-                                                                   SplitStepParams Q, int j, int NTmax, int tiles_per_unit, SplitList W) {
+__global__ void __launch_bounds__(kSpThreads, 1) split_step_kernel(LargeParams P, SplitStepParams Q, int j, int NTmax, int tiles_per_unit, SplitList W) {
   constexpr int NST = sp_stages(S);                            // stages: every stage holds all slices of both operands for one K chunk
   constexpr int n_groups = (S + 3) / 4;
   extern __shared__ unsigned char sp_raw[];
@@ -291,7 +293,7 @@ __global__ void __launch_bounds__(kSpThreads, 1) split_step_kernel(const __grid_
   const unsigned tmem = s_tmem;
 
   if (warp == 0) {
-    if (lane == 0) {            // ===== work-item fetch + TMA producer of the B slices (one 3-D box per K chunk: all slices of the group)
+    if (lane == 0) {            // ===== work-item fetch + producer of the B slices (one bulk copy per K chunk: all slices of the group)
       int stage = 0, phase = 0;
       const int n_items = W.ctr[0];
       for (int qn = 0;; ++qn) {
@@ -307,19 +309,20 @@ __global__ void __launch_bounds__(kSpThreads, 1) split_step_kernel(const __grid_
         const int pb[2] = {0, T.part == 0 ? 2 : 1};
         for (int g = 0; g < n_groups; ++g) {
           const int ns = g == 0 ? (S < 4 ? S : 4) : S;             // slices 0 .. ns-1 of both operands feed this group's diagonals
-          const CUtensorMap* bm = g == 0 ? &bmap4 : &bmapS;
+          const int nkc = Q.Kpad / kSpKC;
           for (int ch = 0; ch < T.nch; ++ch) {
-            const int sub = ch >= half_ch, kc = (sub ? ch - half_ch : ch) * kSpKC;
+            const int sub = ch >= half_ch, kc = sub ? ch - half_ch : ch;
+            const signed char* src = Q.bplanes + ((long long)(T.s * 3 + pb[sub]) * Q.Npad * Q.Kpad) * S + ((((long long)(T.n0 >> 7) * nkc + kc) * S) << 12);
             mbar_wait(&empty[stage], phase ^ 1);
             mbar_expect_tx(&full[stage], (unsigned)(ns * kSpTile));
-            tma_load_3d(sB + stage * S * kSpTile, bm, &full[stage], kc, T.n0, (T.s * 3 + pb[sub]) * S);
+            bulk_load(sB + stage * S * kSpTile, src, (unsigned)(ns * kSpTile), &full[stage]);
             if (++stage == NST) { stage = 0; phase ^= 1; }
           }
         }
       }
     }
   } else if (warp == 10) {
-    if (lane == 0) {            // ===== TMA producer of the A slices (its own thread: the two operand streams never wait for each other)
+    if (lane == 0) {            // ===== producer of the A slices (its own thread: the two operand streams never wait for each other)
       int stage = 0, phase = 0;
       for (int qn = 0;; ++qn) {
         mbar_wait(&qfull[qn & 3], (qn >> 2) & 1);
@@ -331,12 +334,14 @@ __global__ void __launch_bounds__(kSpThreads, 1) split_step_kernel(const __grid_
         const int pa[2] = {T.part == 0 ? 0 : 1, T.part == 0 ? 1 : 0};
         for (int g = 0; g < n_groups; ++g) {
           const int ns = g == 0 ? (S < 4 ? S : 4) : S;
-          const CUtensorMap* am = Q.amaps8 + 2 * T.blk + (g == 0 ? 0 : 1);
+          const int nkc = sp_pad(T.d) / kSpKC;
+          const signed char* ablk = Q.st.planes + Q.st.a_off[T.blk];
           for (int ch = 0; ch < T.nch; ++ch) {
-            const int sub = ch >= half_ch, kc = (sub ? ch - half_ch : ch) * kSpKC;
+            const int sub = ch >= half_ch, kc = sub ? ch - half_ch : ch;
+            const signed char* src = ablk + (long long)pa[sub] * S * T.Mp * sp_pad(T.d) + ((((long long)(T.m0 >> 7) * nkc + kc) * S) << 12);
             mbar_wait(&empty[stage], phase ^ 1);
             mbar_expect_tx(&full[stage], (unsigned)(ns * kSpTile));
-            tma_load_3d(sA + stage * S * kSpTile, am, &full[stage], kc, T.m0, pa[sub] * S);
+            bulk_load(sA + stage * S * kSpTile, src, (unsigned)(ns * kSpTile), &full[stage]);
             if (++stage == NST) { stage = 0; phase ^= 1; }
           }
         }
