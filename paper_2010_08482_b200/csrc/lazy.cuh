@@ -50,11 +50,26 @@ struct LazyView {
   double* thr;
   int* p_accept;                                             // accept flags of the last proposal (commit's default mask)
   unsigned long long* n_products;
+  int* p_lvl_start; int* p_lvl_cnt;                          // [nC][D]: where the dirty ancestors of a level sit in p_node
+  // Work lists, built on the device (the host only knows bounds): what is launched per step is a fixed number of persistent
+  // CTAs that walk a compact list, so a step in which few chains (or none) have work costs a few microseconds instead of one
+  // CTA per candidate.  Leaf lists rotate over three buffers (step j reads j % 3, the fix of step j fills (j + 1) % 3, the
+  // step kernel clears (j + 2) % 3), node lists over two (parity of the host's launch sequence number).
+  int* w_cnt;                                                // [0..2] leaf tasks, [3..5] leaf tiles, [6..7] node tasks, [8..9] node tiles
+  int4* w_ltask; int4* w_ltile; int4* w_ntask; int4* w_ntile;
+  long long w_task_cap, w_tile_cap;                          // entries per buffer
 };
 
 struct LazyEdits {
   const long long* offset; const double* tau; const int* sym; const int* kind; long long n_edits;
 };
+
+// 64 x 64 tiles of an M x N result appended to a tile list (one thread)
+__device__ __forceinline__ void lz_push_tiles(int* cnt, int4* tiles, int task, int M, int N) {
+  const int tm = (M + kLzTile - 1) / kLzTile, tn = (N + kLzTile - 1) / kLzTile;
+  const int base = atomicAdd(cnt, tm * tn);
+  for (int i = 0; i < tm * tn; ++i) tiles[base + i] = make_int4(task, (i / tn) * kLzTile, (i % tn) * kLzTile, 0);
+}
 
 // ------------------------------------------------------------------------------------------------ small helpers
 __device__ __forceinline__ int lz_level(int node) { return 31 - __clz(node + 1); }
@@ -273,6 +288,10 @@ __global__ void lazy_reset_kernel(LazyView V) {
     V.free_slot[i] = V.nnode + (int)(i % (V.smax + V.emax));
   for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < (long long)V.nC * V.nleaf; i += (long long)gridDim.x * blockDim.x)
     V.leaf_n[i] = 0;
+  if (blockIdx.x == 0 && threadIdx.x < 16) V.w_cnt[threadIdx.x] = 0;
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < (long long)V.nC * V.D; i += (long long)gridDim.x * blockDim.x) {
+    V.p_lvl_start[i] = 0; V.p_lvl_cnt[i] = 0;
+  }
   for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < (long long)V.nC; i += (long long)gridDim.x * blockDim.x) {
     V.p_status[i] = 0; V.p_ndirty[i] = 0; V.p_nleaf[i] = 0; V.decided[i] = 2; V.decided_by[i] = 0; V.n_eval[i] = 0; V.n_alive[i] = 0;
   }
@@ -381,6 +400,7 @@ __global__ void lazy_prepare_kernel(LazyView V, LazyEdits E, const double* log2_
     V.sh_n[(size_t)c * V.emax + k] = cnt;
   }
   if (status != 0) nl = 0;
+  if (c == 0) for (int i = 0; i < 6; ++i) V.w_cnt[i] = 0;      // leaf work lists of this proposal start empty
   int total = nl;
   for (int i = 0; i < nl; ++i) pn[i] += V.nleaf - 1;
   {
@@ -388,6 +408,7 @@ __global__ void lazy_prepare_kernel(LazyView V, LazyEdits E, const double* log2_
     for (int level = V.D - 1; level >= 0; --level) {
       int prev = -1, nc = 0;
       for (int i = start; i < start + cnt; ++i) { const int p = (pn[i] - 1) >> 1; if (p != prev) { pn[total + nc++] = p; prev = p; } }
+      V.p_lvl_start[(size_t)c * V.D + level] = total; V.p_lvl_cnt[(size_t)c * V.D + level] = nc;
       start = total; total += nc; cnt = nc;
     }
   }
@@ -438,7 +459,8 @@ __device__ __forceinline__ LzLeafTask lz_leaf_task(const LazyView& V, int y, int
   return T;
 }
 
-// first propagation P_{t1 - a}(q0): exponent bookkeeping, and the whole entry when the shadow leaf holds no operator
+// first propagation P_{t1 - a}(q0): exponent bookkeeping, and the whole entry when the shadow leaf holds no operator;
+// a leaf with operators becomes a task of step 0 (grid: (chain, leaf) x start sector -- the one launch with a CTA per candidate)
 template <bool CPLX>
 __global__ void lazy_leaf_init_kernel(LazyView V) {
   __shared__ double red[32]; __shared__ int redi[32];
@@ -452,61 +474,88 @@ __global__ void lazy_leaf_init_kernel(LazyView V) {
   int km = INT_MIN;
   for (int r = threadIdx.x; r < d; r += blockDim.x) km = max(km, row_exp(prop_x(delta, E[r], emin)));
   km = lz_block_max(km, redi);
-  if (threadIdx.x == 0) { const size_t en = lz_ent(V, T.c, T.slot, T.q0); V.ent_e[en] = km; V.ent_lg[en] = -delta * emin * kLog2e; }
+  if (threadIdx.x == 0) {
+    const size_t en = lz_ent(V, T.c, T.slot, T.q0); V.ent_e[en] = km; V.ent_lg[en] = -delta * emin * kLog2e;
+    const int ti = atomicAdd(&V.w_cnt[0], 1);
+    V.w_ltask[ti] = make_int4((int)blockIdx.x, T.q0, T.q0, 0);
+    const int blk = V.imp.blk_of[V.sh_sym[((size_t)T.c * V.emax + T.k) * V.cap] * V.imp.Q + T.q0];
+    lz_push_tiles(&V.w_cnt[3], V.w_ltile, ti, V.imp.blks[blk].rows, d);
+  }
 }
 
-struct LzLeafStep { int blk, q, qn; double delta; double* in; double* out; };
-__device__ __forceinline__ LzLeafStep lz_leaf_step(const LazyView& V, const LzLeafTask& T, int j) {
+// operator j of the shadow leaf of a task {y = chain * emax + leaf index, start sector, sector the chain has reached}
+struct LzLeafStep { int c, k, q0, n, blk, qn; size_t en; double delta; double* in; double* out; };
+__device__ __forceinline__ LzLeafStep lz_leaf_step(const LazyView& V, int4 task, int j) {
   LzLeafStep S;
-  const int* ss = V.sh_sym + ((size_t)T.c * V.emax + T.k) * V.cap;
-  const double* st = V.sh_tau + ((size_t)T.c * V.emax + T.k) * V.cap;
-  int q = T.q0;
-  for (int i = 0; i < j; ++i) q = V.imp.blks[V.imp.blk_of[ss[i] * V.imp.Q + q]].dst;
-  S.q = q; S.blk = V.imp.blk_of[ss[j] * V.imp.Q + q]; S.qn = V.imp.blks[S.blk].dst;
-  S.delta = ((j + 1 < T.n) ? st[j + 1] : T.b) - st[j];
-  double* ent = lz_mat(V, T.c, T.slot, T.q0);
-  double* tmp = lz_mat(V, T.c, V.free_slot[(size_t)T.c * (V.smax + V.emax) + V.smax + T.k], T.q0);
-  S.out = ((T.n - 1 - j) & 1) ? tmp : ent;     // the last step lands in the entry
-  S.in = ((T.n - 1 - j) & 1) ? ent : tmp;
+  S.c = task.x / V.emax; S.k = task.x % V.emax; S.q0 = task.y;
+  const int* ss = V.sh_sym + (size_t)task.x * V.cap;
+  const double* st = V.sh_tau + (size_t)task.x * V.cap;
+  S.n = V.sh_n[task.x];
+  S.blk = V.imp.blk_of[ss[j] * V.imp.Q + task.z]; S.qn = V.imp.blks[S.blk].dst;
+  const int leaf = V.p_node[(size_t)S.c * V.smax + S.k] - (V.nleaf - 1);
+  S.delta = ((j + 1 < S.n) ? st[j + 1] : lz_edge(V, leaf + 1)) - st[j];
+  const int* fs = V.free_slot + (size_t)S.c * (V.smax + V.emax);
+  const int slot = fs[S.k];
+  S.en = lz_ent(V, S.c, slot, S.q0);
+  double* ent = lz_mat(V, S.c, slot, S.q0);
+  double* tmp = lz_mat(V, S.c, fs[V.smax + S.k], S.q0);
+  S.out = ((S.n - 1 - j) & 1) ? tmp : ent;     // the last step lands in the entry
+  S.in = ((S.n - 1 - j) & 1) ? ent : tmp;
   return S;
 }
 
-// operator j of every shadow leaf: M <- P_{Delta_j}(q_{j+1}) F_j M   (grid: tiles x (chain, leaf) x start sector)
+// operator j of every shadow leaf that has one: M <- P_{Delta_j}(q_{j+1}) F_j M   (persistent CTAs over the tile list of step j)
 template <bool CPLX>
-__global__ void __launch_bounds__(kLzThreads) lazy_leaf_step_kernel(LazyView V, int j, int NT) {
+__global__ void __launch_bounds__(kLzThreads) lazy_leaf_step_kernel(LazyView V, int j) {
   __shared__ LzSmem<CPLX> S;
-  const LzLeafTask T = lz_leaf_task(V, blockIdx.x, blockIdx.z);
-  if (!T.ok || j >= T.n) return;
-  const LzLeafStep st = lz_leaf_step(V, T, j);
-  const BlkDesc bd = V.imp.blks[st.blk];
-  const int M = bd.rows, K = bd.cols, N = V.imp.dim[T.q0];
-  const int m0 = (blockIdx.y / NT) * kLzTile, n0 = (blockIdx.y % NT) * kLzTile;
-  if (m0 >= M || n0 >= N) return;
-  const size_t en = lz_ent(V, T.c, T.slot, T.q0);
-  LzDiag dg; dg.delta = 0.0; dg.E = nullptr; dg.emin = 0.0; dg.kmax = 0;
-  if (j == 0) {
-    dg.delta = V.sh_tau[((size_t)T.c * V.emax + T.k) * V.cap] - T.a;
-    dg.E = V.imp.energy + V.imp.e_off[T.q0]; dg.emin = V.imp.e_min[T.q0]; dg.kmax = (int)V.ent_e[en];
+  const int cur = j % 3, nxt2 = (j + 2) % 3;
+  if (blockIdx.x == 0 && threadIdx.x == 0) { V.w_cnt[nxt2] = 0; V.w_cnt[3 + nxt2] = 0; }
+  const int n_items = V.w_cnt[3 + cur];
+  const int4* tiles = V.w_ltile + (size_t)cur * V.w_tile_cap;
+  const int4* tasks = V.w_ltask + (size_t)cur * V.w_task_cap;
+  for (int it = blockIdx.x; it < n_items; it += gridDim.x) {
+    const int4 tl = tiles[it];
+    const LzLeafStep st = lz_leaf_step(V, tasks[tl.x], j);
+    const BlkDesc bd = V.imp.blks[st.blk];
+    LzDiag dg; dg.delta = 0.0; dg.E = nullptr; dg.emin = 0.0; dg.kmax = 0;
+    if (j == 0) {
+      const int leaf = V.p_node[(size_t)st.c * V.smax + st.k] - (V.nleaf - 1);
+      dg.delta = V.sh_tau[((size_t)st.c * V.emax + st.k) * V.cap] - lz_edge(V, leaf);
+      dg.E = V.imp.energy + V.imp.e_off[st.q0]; dg.emin = V.imp.e_min[st.q0]; dg.kmax = (int)V.ent_e[st.en];
+    }
+    LzRowScale rs; rs.on = 1; rs.delta = st.delta; rs.E = V.imp.energy + V.imp.e_off[st.qn]; rs.emin = V.imp.e_min[st.qn];
+    lz_gemm_tile<CPLX>(S, tl.y, tl.z, bd.rows, V.imp.dim[st.q0], bd.cols, V.imp.store + bd.off, bd.ld, 1, j == 0 ? nullptr : st.in, V.ldm, dg,
+                       st.out, V.ldm, rs, &V.ent_k[st.en]);
+    __syncthreads();
   }
-  LzRowScale rs; rs.on = 1; rs.delta = st.delta; rs.E = V.imp.energy + V.imp.e_off[st.qn]; rs.emin = V.imp.e_min[st.qn];
-  lz_gemm_tile<CPLX>(S, m0, n0, M, N, K, V.imp.store + bd.off, bd.ld, 1, j == 0 ? nullptr : st.in, V.ldm, dg, st.out, V.ldm, rs, &V.ent_k[en]);
 }
 
+// common exponent and norm of the product of step j; the task moves on to step j + 1 (persistent CTAs over the task list)
 template <bool CPLX>
 __global__ void lazy_leaf_fix_kernel(LazyView V, int j) {
   __shared__ double red[32];
-  const LzLeafTask T = lz_leaf_task(V, blockIdx.x, blockIdx.y);
-  if (!T.ok || j >= T.n) return;
-  const LzLeafStep st = lz_leaf_step(V, T, j);
-  const size_t en = lz_ent(V, T.c, T.slot, T.q0);
-  int k = V.ent_k[en];
-  if (k == INT_MIN) k = 0;
-  LzRowScale rs; rs.on = 1; rs.delta = st.delta; rs.E = V.imp.energy + V.imp.e_off[st.qn]; rs.emin = V.imp.e_min[st.qn];
-  const double ss = lz_fix_entry<CPLX>(st.out, V.ldm, V.imp.dim[st.qn], V.imp.dim[T.q0], k, rs, red);
-  if (threadIdx.x == 0) {
-    V.ent_e[en] += k; V.ent_lg[en] += -st.delta * rs.emin * kLog2e; V.ent_k[en] = INT_MIN;
-    if (j == T.n - 1) { V.ent_nrm[en] = sqrt(ss); V.ent_valid[en] = 1; }
-    atomicAdd(V.n_products, 1ull);
+  const int cur = j % 3, nxt = (j + 1) % 3;
+  const int n_tasks = V.w_cnt[cur];
+  const int4* tasks = V.w_ltask + (size_t)cur * V.w_task_cap;
+  for (int ti = blockIdx.x; ti < n_tasks; ti += gridDim.x) {
+    const int4 task = tasks[ti];
+    const LzLeafStep st = lz_leaf_step(V, task, j);
+    int k = V.ent_k[st.en];
+    if (k == INT_MIN) k = 0;
+    LzRowScale rs; rs.on = 1; rs.delta = st.delta; rs.E = V.imp.energy + V.imp.e_off[st.qn]; rs.emin = V.imp.e_min[st.qn];
+    const double ss = lz_fix_entry<CPLX>(st.out, V.ldm, V.imp.dim[st.qn], V.imp.dim[st.q0], k, rs, red);
+    if (threadIdx.x == 0) {
+      V.ent_e[st.en] += k; V.ent_lg[st.en] += -st.delta * rs.emin * kLog2e; V.ent_k[st.en] = INT_MIN;
+      if (j == st.n - 1) { V.ent_nrm[st.en] = sqrt(ss); V.ent_valid[st.en] = 1; }
+      else {
+        const int t2 = atomicAdd(&V.w_cnt[nxt], 1);
+        V.w_ltask[(size_t)nxt * V.w_task_cap + t2] = make_int4(task.x, task.y, st.qn, 0);
+        const int blk = V.imp.blk_of[V.sh_sym[(size_t)task.x * V.cap + j + 1] * V.imp.Q + st.qn];
+        lz_push_tiles(&V.w_cnt[3 + nxt], V.w_ltile + (size_t)nxt * V.w_tile_cap, t2, V.imp.blks[blk].rows, V.imp.dim[st.q0]);
+      }
+      atomicAdd(V.n_products, 1ull);
+    }
+    __syncthreads();
   }
 }
 
@@ -564,71 +613,83 @@ __global__ void lazy_bound_kernel(LazyView V, double* bound_mant, long long* bou
 // ------------------------------------------------------------------------------------------------ dirty ancestors
 // mode 0: lazy round r -- only the entry that start sector order[r] needs at this node;  mode 1: every missing entry of the
 // node (completion of an accepted / undecided proposal, or -- gate = mask -- of a commit).
-struct LzNodeTask { int ok, c, slot, qin, sl, sr, mid; };
-__device__ __forceinline__ LzNodeTask lz_node_task(const LazyView& V, int y, int z, int level, int mode, int r, const int* gate, int gate_commit) {
-  LzNodeTask T; T.ok = 0;
-  T.c = y / V.smax;
-  const int di = y % V.smax;
-  if (di >= V.p_ndirty[T.c] || di < V.p_nleaf[T.c] || V.p_status[T.c] != 0) return T;
-  if (gate_commit ? (gate[T.c] == 0) : (V.decided[T.c] == 2)) return T;
-  const int node = V.p_node[(size_t)T.c * V.smax + di];
-  if (lz_level(node) != level) return T;
+// Plan of one (level, mode, r) step: one thread per candidate (chain, dirty ancestor of the level, sector) decides whether the
+// entry has to be multiplied now and appends it (two int4: {chain, slot, start sector, left slot}, {right slot, middle sector,
+// target sector, 0}) and its tiles to the node lists of parity `par`.
+__global__ void lazy_node_plan_kernel(LazyView V, int level, int mode, int r, const int* gate, int gate_commit, int par) {
+  const int nsec = mode == 0 ? 1 : V.imp.Q;
+  const long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (idx >= (long long)V.nC * V.emax * nsec) return;
+  const int z = (int)(idx % nsec), i = (int)((idx / nsec) % V.emax), c = (int)(idx / ((long long)nsec * V.emax));
+  if (V.p_status[c] != 0 || i >= V.p_lvl_cnt[(size_t)c * V.D + level]) return;
+  const int di = V.p_lvl_start[(size_t)c * V.D + level] + i;
+  if (di >= V.p_ndirty[c]) return;                             // nothing proposed since the last commit
+  if (gate_commit ? (gate[c] == 0) : (V.decided[c] == 2)) return;
+  const int node = V.p_node[(size_t)c * V.smax + di];
   int qin = z;
   if (mode == 0) {
-    if (r >= V.n_alive[T.c]) return T;
-    qin = V.order[(size_t)T.c * V.imp.Q + r];
+    if (r >= V.n_alive[c]) return;
+    qin = V.order[(size_t)c * V.imp.Q + r];
     int cur = 0;
-    for (int l = 0; l < level; ++l) {                      // walk from the root down to `node`
+    for (int l = 0; l < level; ++l) {                          // walk from the root down to `node`
       const int anc = (((node + 1) >> (level - l - 1)) - 1);   // ancestor of `node` at level l + 1
       const int left = 2 * cur + 1;
-      if (anc != left) { qin = V.ent_tgt[lz_ent(V, T.c, lz_slot(V, T.c, left), qin)]; if (qin < 0) return T; }
+      if (anc != left) { qin = V.ent_tgt[lz_ent(V, c, lz_slot(V, c, left), qin)]; if (qin < 0) return; }
       cur = anc;
     }
   }
-  T.slot = V.free_slot[(size_t)T.c * (V.smax + V.emax) + di];
-  const size_t en = lz_ent(V, T.c, T.slot, qin);
-  if (V.ent_tgt[en] < 0 || V.ent_valid[en]) return T;
-  T.sl = lz_slot(V, T.c, 2 * node + 1); T.sr = lz_slot(V, T.c, 2 * node + 2);
-  T.mid = V.ent_tgt[lz_ent(V, T.c, T.sl, qin)];
-  if (T.mid < 0) return T;
-  if (!V.ent_valid[lz_ent(V, T.c, T.sl, qin)] || !V.ent_valid[lz_ent(V, T.c, T.sr, T.mid)]) return T;
-  T.qin = qin; T.ok = 1;
-  return T;
+  const int slot = V.free_slot[(size_t)c * (V.smax + V.emax) + di];
+  const size_t en = lz_ent(V, c, slot, qin);
+  if (V.ent_tgt[en] < 0 || V.ent_valid[en]) return;
+  const int sl = lz_slot(V, c, 2 * node + 1), sr = lz_slot(V, c, 2 * node + 2);
+  const int mid = V.ent_tgt[lz_ent(V, c, sl, qin)];
+  if (mid < 0) return;
+  if (!V.ent_valid[lz_ent(V, c, sl, qin)] || !V.ent_valid[lz_ent(V, c, sr, mid)]) return;
+  const int tq = V.ent_tgt[lz_ent(V, c, sr, mid)];
+  const int ti = atomicAdd(&V.w_cnt[6 + par], 1);
+  int4* nt = V.w_ntask + ((size_t)par * V.w_task_cap + ti) * 2;
+  nt[0] = make_int4(c, slot, qin, sl); nt[1] = make_int4(sr, mid, tq, 0);
+  lz_push_tiles(&V.w_cnt[8 + par], V.w_ntile + (size_t)par * V.w_tile_cap, ti, V.imp.dim[tq], V.imp.dim[qin]);
 }
 
 template <bool CPLX>
-__global__ void __launch_bounds__(kLzThreads) lazy_node_gemm_kernel(LazyView V, int level, int mode, int r, const int* gate, int gate_commit, int NT) {
+__global__ void __launch_bounds__(kLzThreads) lazy_node_gemm_kernel(LazyView V, int par) {
   __shared__ LzSmem<CPLX> S;
-  const LzNodeTask T = lz_node_task(V, blockIdx.x, blockIdx.z, level, mode, r, gate, gate_commit);
-  if (!T.ok) return;
-  const int tq = V.ent_tgt[lz_ent(V, T.c, T.sr, T.mid)];
-  const int M = V.imp.dim[tq], K = V.imp.dim[T.mid], N = V.imp.dim[T.qin];
-  const int m0 = (blockIdx.y / NT) * kLzTile, n0 = (blockIdx.y % NT) * kLzTile;
-  if (m0 >= M || n0 >= N) return;
+  if (blockIdx.x == 0 && threadIdx.x == 0) { V.w_cnt[6 + (par ^ 1)] = 0; V.w_cnt[8 + (par ^ 1)] = 0; }
+  const int n_items = V.w_cnt[8 + par];
+  const int4* tiles = V.w_ntile + (size_t)par * V.w_tile_cap;
+  const int4* tasks = V.w_ntask + (size_t)par * V.w_task_cap * 2;
   LzDiag dg; dg.delta = 0.0; dg.E = nullptr; dg.emin = 0.0; dg.kmax = 0;
   LzRowScale rs; rs.on = 0; rs.delta = 0.0; rs.E = nullptr; rs.emin = 0.0;
-  lz_gemm_tile<CPLX>(S, m0, n0, M, N, K, lz_mat(V, T.c, T.sr, T.mid), 1, V.ldm, lz_mat(V, T.c, T.sl, T.qin), V.ldm, dg,
-                     lz_mat(V, T.c, T.slot, T.qin), V.ldm, rs, &V.ent_k[lz_ent(V, T.c, T.slot, T.qin)]);
+  for (int it = blockIdx.x; it < n_items; it += gridDim.x) {
+    const int4 tl = tiles[it];
+    const int4 t0 = tasks[2 * tl.x], t1 = tasks[2 * tl.x + 1];      // {c, slot, qin, sl}, {sr, mid, tq}
+    lz_gemm_tile<CPLX>(S, tl.y, tl.z, V.imp.dim[t1.z], V.imp.dim[t0.z], V.imp.dim[t1.y], lz_mat(V, t0.x, t1.x, t1.y), 1, V.ldm,
+                       lz_mat(V, t0.x, t0.w, t0.z), V.ldm, dg, lz_mat(V, t0.x, t0.y, t0.z), V.ldm, rs, &V.ent_k[lz_ent(V, t0.x, t0.y, t0.z)]);
+    __syncthreads();
+  }
 }
 
 template <bool CPLX>
-__global__ void lazy_node_fix_kernel(LazyView V, int level, int mode, int r, const int* gate, int gate_commit) {
+__global__ void lazy_node_fix_kernel(LazyView V, int par) {
   __shared__ double red[32];
-  const LzNodeTask T = lz_node_task(V, blockIdx.x, blockIdx.y, level, mode, r, gate, gate_commit);
-  if (!T.ok) return;
-  const size_t en = lz_ent(V, T.c, T.slot, T.qin), el = lz_ent(V, T.c, T.sl, T.qin), er = lz_ent(V, T.c, T.sr, T.mid);
-  const int tq = V.ent_tgt[er];
-  int k = V.ent_k[en];
-  if (k == INT_MIN) k = 0;
+  const int n_tasks = V.w_cnt[6 + par];
+  const int4* tasks = V.w_ntask + (size_t)par * V.w_task_cap * 2;
   LzRowScale rs; rs.on = 0; rs.delta = 0.0; rs.E = nullptr; rs.emin = 0.0;
-  const double ss = lz_fix_entry<CPLX>(lz_mat(V, T.c, T.slot, T.qin), V.ldm, V.imp.dim[tq], V.imp.dim[T.qin], k, rs, red);
-  __syncthreads();
-  if (threadIdx.x == 0) {
-    V.ent_e[en] = V.ent_e[el] + V.ent_e[er] + k; V.ent_lg[en] = V.ent_lg[el] + V.ent_lg[er];
-    V.ent_nrm[en] = sqrt(ss); V.ent_k[en] = INT_MIN;
-    __threadfence();
-    V.ent_valid[en] = 1;
-    atomicAdd(V.n_products, 1ull);
+  for (int ti = blockIdx.x; ti < n_tasks; ti += gridDim.x) {
+    const int4 t0 = tasks[2 * ti], t1 = tasks[2 * ti + 1];
+    const size_t en = lz_ent(V, t0.x, t0.y, t0.z), el = lz_ent(V, t0.x, t0.w, t0.z), er = lz_ent(V, t0.x, t1.x, t1.y);
+    int k = V.ent_k[en];
+    if (k == INT_MIN) k = 0;
+    const double ss = lz_fix_entry<CPLX>(lz_mat(V, t0.x, t0.y, t0.z), V.ldm, V.imp.dim[t1.z], V.imp.dim[t0.z], k, rs, red);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      V.ent_e[en] = V.ent_e[el] + V.ent_e[er] + k; V.ent_lg[en] = V.ent_lg[el] + V.ent_lg[er];
+      V.ent_nrm[en] = sqrt(ss); V.ent_k[en] = INT_MIN;
+      __threadfence();
+      V.ent_valid[en] = 1;
+      atomicAdd(V.n_products, 1ull);
+    }
   }
 }
 

@@ -12,6 +12,8 @@ struct ctqmc_chains {
   size_t bytes = 0;
   int lazy_rounds = 1;
   int NT = 1;                 // tiles per matrix side
+  int g_gemm = 1, g_fix = 1;  // persistent CTAs of the list-driven kernels (resident CTAs per SM x SMs)
+  int seq = 0;                // node steps enqueued so far: its parity selects the node work lists
   long long launches = 0;     // kernels enqueued by the most recent call
   cudaStream_t last_stream = nullptr;
 };
@@ -36,6 +38,10 @@ size_t chains_layout(LazyView& V, char* base) {
   V.term_re = bp.take<double>(nC * Q); V.term_im = bp.take<double>(nC * Q); V.term_e = bp.take<long long>(nC * Q);
   V.thr = bp.take<double>(nC); V.p_accept = bp.take<int>(nC);
   V.n_products = bp.take<unsigned long long>(1);
+  V.p_lvl_start = bp.take<int>(nC * (size_t)(V.D > 0 ? V.D : 1)); V.p_lvl_cnt = bp.take<int>(nC * (size_t)(V.D > 0 ? V.D : 1));
+  V.w_cnt = bp.take<int>(16);
+  V.w_ltask = bp.take<int4>(3 * (size_t)V.w_task_cap); V.w_ltile = bp.take<int4>(3 * (size_t)V.w_tile_cap);
+  V.w_ntask = bp.take<int4>(2 * 2 * (size_t)V.w_task_cap); V.w_ntile = bp.take<int4>(2 * (size_t)V.w_tile_cap);
   V.mats = bp.take<double>(nC * V.NN * (size_t)V.node_elems);
   return bp.off + 256;
 }
@@ -43,17 +49,18 @@ size_t chains_layout(LazyView& V, char* base) {
 // dirty ancestors, bottom-up: mode 0 = the entries start sector order[r] needs, mode 1 = every missing entry
 int chains_enqueue_levels(ctqmc_chains* ch, int mode, int r, const int* gate, int gate_commit, cudaStream_t st) {
   const LazyView& V = ch->V;
-  const unsigned tasks = (unsigned)((long long)V.nC * V.smax), nsec = mode == 0 ? 1u : (unsigned)V.imp.Q;
+  const long long cand = (long long)V.nC * V.emax * (mode == 0 ? 1 : V.imp.Q);
   for (int level = V.D - 1; level >= 0; --level) {
-    dim3 gg(tasks, (unsigned)(ch->NT * ch->NT), nsec), gf(tasks, nsec);
+    const int par = ch->seq++ & 1;
+    lazy_node_plan_kernel<<<(unsigned)((cand + 255) / 256), 256, 0, st>>>(V, level, mode, r, gate, gate_commit, par);
     if (V.imp.cplx) {
-      lazy_node_gemm_kernel<true><<<gg, kLzThreads, 0, st>>>(V, level, mode, r, gate, gate_commit, ch->NT);
-      lazy_node_fix_kernel<true><<<gf, 256, 0, st>>>(V, level, mode, r, gate, gate_commit);
+      lazy_node_gemm_kernel<true><<<ch->g_gemm, kLzThreads, 0, st>>>(V, par);
+      lazy_node_fix_kernel<true><<<ch->g_fix, 256, 0, st>>>(V, par);
     } else {
-      lazy_node_gemm_kernel<false><<<gg, kLzThreads, 0, st>>>(V, level, mode, r, gate, gate_commit, ch->NT);
-      lazy_node_fix_kernel<false><<<gf, 256, 0, st>>>(V, level, mode, r, gate, gate_commit);
+      lazy_node_gemm_kernel<false><<<ch->g_gemm, kLzThreads, 0, st>>>(V, par);
+      lazy_node_fix_kernel<false><<<ch->g_fix, 256, 0, st>>>(V, par);
     }
-    ch->launches += 2;
+    ch->launches += 3;
   }
   CU(cudaGetLastError());
   return 0;
@@ -83,7 +90,23 @@ extern "C" int ctqmc_chains_create(ctqmc_impurity* h, double beta, const ctqmc_c
   V.ldm = h->dev.dmax; V.node_elems = (long long)h->n_energy * V.ldm * (h->dev.cplx ? 2 : 1);
   ch->lazy_rounds = desc->lazy_rounds < h->dev.Q ? desc->lazy_rounds : h->dev.Q;
   ch->NT = (h->dev.dmax + kLzTile - 1) / kLzTile;
-  if ((long long)V.nC * V.smax > 2000000000LL) { delete ch; return fail(CTQMC_ERR_ARG, "n_chains * max_edits * (depth + 1) exceeds 2^31"); }
+  V.w_task_cap = (long long)V.nC * V.emax * h->dev.Q;
+  V.w_tile_cap = V.w_task_cap * ch->NT * ch->NT;
+  {
+    int occ_g = 1, occ_f = 1, sms = 1;
+    CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, h->device));
+    if (h->dev.cplx) {
+      CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_g, lazy_node_gemm_kernel<true>, kLzThreads, 0));
+      CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_f, lazy_node_fix_kernel<true>, 256, 0));
+    } else {
+      CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_g, lazy_node_gemm_kernel<false>, kLzThreads, 0));
+      CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_f, lazy_node_fix_kernel<false>, 256, 0));
+    }
+    ch->g_gemm = sms * (occ_g > 0 ? occ_g : 1); ch->g_fix = sms * (occ_f > 0 ? occ_f : 1);
+  }
+  if ((long long)V.nC * V.smax > 2000000000LL || V.w_tile_cap > 500000000LL) {
+    delete ch; return fail(CTQMC_ERR_ARG, "n_chains * max_edits * (depth + 1), or the work lists of n_chains * max_edits * sectors * tiles, exceed 2^31");
+  }
   ch->bytes = chains_layout(V, nullptr);
   cudaError_t e = cudaMalloc((void**)&ch->block, ch->bytes);
   if (e != cudaSuccess) {
@@ -140,11 +163,11 @@ extern "C" int ctqmc_chains_propose(ctqmc_chains* ch, const ctqmc_edit_batch* ed
   if (edits->n_edits == 0) E.offset = nullptr;
   lazy_prepare_kernel<<<(V.nC + 127) / 128, 128, 0, st>>>(V, E, log2_threshold);
   const unsigned ltasks = (unsigned)((long long)V.nC * V.emax);
-  dim3 gl(ltasks, (unsigned)Q), gs(ltasks, (unsigned)(ch->NT * ch->NT), (unsigned)Q);
+  dim3 gl(ltasks, (unsigned)Q);
   if (cx) lazy_leaf_init_kernel<true><<<gl, 256, 0, st>>>(V); else lazy_leaf_init_kernel<false><<<gl, 256, 0, st>>>(V);
   for (int j = 0; j < V.cap; ++j) {
-    if (cx) { lazy_leaf_step_kernel<true><<<gs, kLzThreads, 0, st>>>(V, j, ch->NT); lazy_leaf_fix_kernel<true><<<gl, 256, 0, st>>>(V, j); }
-    else    { lazy_leaf_step_kernel<false><<<gs, kLzThreads, 0, st>>>(V, j, ch->NT); lazy_leaf_fix_kernel<false><<<gl, 256, 0, st>>>(V, j); }
+    if (cx) { lazy_leaf_step_kernel<true><<<ch->g_gemm, kLzThreads, 0, st>>>(V, j); lazy_leaf_fix_kernel<true><<<ch->g_fix, 256, 0, st>>>(V, j); }
+    else    { lazy_leaf_step_kernel<false><<<ch->g_gemm, kLzThreads, 0, st>>>(V, j); lazy_leaf_fix_kernel<false><<<ch->g_fix, 256, 0, st>>>(V, j); }
   }
   const unsigned wg = (unsigned)(((long long)V.nC * 32 + 255) / 256);
   lazy_bound_kernel<<<wg, 256, 0, st>>>(V, bound_mant, (long long*)bound_exp2);
