@@ -616,40 +616,45 @@ __global__ void lazy_bound_kernel(LazyView V, double* bound_mant, long long* bou
 // Plan of one (level, mode, r) step: one thread per candidate (chain, dirty ancestor of the level, sector) decides whether the
 // entry has to be multiplied now and appends it (two int4: {chain, slot, start sector, left slot}, {right slot, middle sector,
 // target sector, 0}) and its tiles to the node lists of parity `par`.
-__global__ void lazy_node_plan_kernel(LazyView V, int level, int mode, int r, const int* gate, int gate_commit, int par) {
+__device__ __forceinline__ bool lz_node_candidate(const LazyView& V, int level, int mode, int r, const int* gate, int gate_commit,
+                                                  long long idx, int4& t0, int4& t1) {
   const int nsec = mode == 0 ? 1 : V.imp.Q;
-  const long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-  if (idx >= (long long)V.nC * V.emax * nsec) return;
+  if (idx >= (long long)V.nC * V.emax * nsec) return false;
   const int z = (int)(idx % nsec), i = (int)((idx / nsec) % V.emax), c = (int)(idx / ((long long)nsec * V.emax));
-  if (V.p_status[c] != 0 || i >= V.p_lvl_cnt[(size_t)c * V.D + level]) return;
+  if (V.p_status[c] != 0 || i >= V.p_lvl_cnt[(size_t)c * V.D + level]) return false;
   const int di = V.p_lvl_start[(size_t)c * V.D + level] + i;
-  if (di >= V.p_ndirty[c]) return;                             // nothing proposed since the last commit
-  if (gate_commit ? (gate[c] == 0) : (V.decided[c] == 2)) return;
+  if (di >= V.p_ndirty[c]) return false;                       // nothing proposed since the last commit
+  if (gate_commit ? (gate[c] == 0) : (V.decided[c] == 2)) return false;
   const int node = V.p_node[(size_t)c * V.smax + di];
   int qin = z;
   if (mode == 0) {
-    if (r >= V.n_alive[c]) return;
+    if (r >= V.n_alive[c]) return false;
     qin = V.order[(size_t)c * V.imp.Q + r];
     int cur = 0;
     for (int l = 0; l < level; ++l) {                          // walk from the root down to `node`
       const int anc = (((node + 1) >> (level - l - 1)) - 1);   // ancestor of `node` at level l + 1
       const int left = 2 * cur + 1;
-      if (anc != left) { qin = V.ent_tgt[lz_ent(V, c, lz_slot(V, c, left), qin)]; if (qin < 0) return; }
+      if (anc != left) { qin = V.ent_tgt[lz_ent(V, c, lz_slot(V, c, left), qin)]; if (qin < 0) return false; }
       cur = anc;
     }
   }
   const int slot = V.free_slot[(size_t)c * (V.smax + V.emax) + di];
   const size_t en = lz_ent(V, c, slot, qin);
-  if (V.ent_tgt[en] < 0 || V.ent_valid[en]) return;
+  if (V.ent_tgt[en] < 0 || V.ent_valid[en]) return false;
   const int sl = lz_slot(V, c, 2 * node + 1), sr = lz_slot(V, c, 2 * node + 2);
   const int mid = V.ent_tgt[lz_ent(V, c, sl, qin)];
-  if (mid < 0) return;
-  if (!V.ent_valid[lz_ent(V, c, sl, qin)] || !V.ent_valid[lz_ent(V, c, sr, mid)]) return;
-  const int tq = V.ent_tgt[lz_ent(V, c, sr, mid)];
+  if (mid < 0) return false;
+  if (!V.ent_valid[lz_ent(V, c, sl, qin)] || !V.ent_valid[lz_ent(V, c, sr, mid)]) return false;
+  t0 = make_int4(c, slot, qin, sl); t1 = make_int4(sr, mid, V.ent_tgt[lz_ent(V, c, sr, mid)], 0);
+  return true;
+}
+__global__ void lazy_node_plan_kernel(LazyView V, int level, int mode, int r, const int* gate, int gate_commit, int par) {
+  int4 t0, t1;
+  if (!lz_node_candidate(V, level, mode, r, gate, gate_commit, blockIdx.x * (long long)blockDim.x + threadIdx.x, t0, t1)) return;
   const int ti = atomicAdd(&V.w_cnt[6 + par], 1);
   int4* nt = V.w_ntask + ((size_t)par * V.w_task_cap + ti) * 2;
-  nt[0] = make_int4(c, slot, qin, sl); nt[1] = make_int4(sr, mid, tq, 0);
-  lz_push_tiles(&V.w_cnt[8 + par], V.w_ntile + (size_t)par * V.w_tile_cap, ti, V.imp.dim[tq], V.imp.dim[qin]);
+  nt[0] = t0; nt[1] = t1;
+  lz_push_tiles(&V.w_cnt[8 + par], V.w_ntile + (size_t)par * V.w_tile_cap, ti, V.imp.dim[t1.z], V.imp.dim[t0.z]);
 }
 
 template <bool CPLX>
@@ -690,6 +695,190 @@ __global__ void lazy_node_fix_kernel(LazyView V, int par) {
       V.ent_valid[en] = 1;
       atomicAdd(V.n_products, 1ull);
     }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------ small impurities
+// Sector dimensions <= 16 (configs 1 and 2): a 64 x 64 tensor-core tile would be all padding and a launch per operator all
+// latency.  One WARP owns a task and keeps both operands in shared memory (A k-major, B column-major, leading dimension 16);
+// lane l holds result elements l, l + 32, ... (row = e % M, column = e / M).  A shadow leaf is rebuilt in ONE launch (the warp
+// walks its operators), a dirty level in one launch (candidate test, product, common exponent and norm fused).  The arithmetic
+// is that of lz_gemm_tile + lz_fix_entry element by element; only the order of the contraction sum differs.
+constexpr int kLzSmall = 16;
+constexpr int kLzSmallWarps = 4;
+template <bool CPLX>
+struct LzSmallSmem { double A[CPLX ? 2 : 1][kLzSmall * kLzSmall]; double B[CPLX ? 2 : 1][kLzSmall * kLzSmall]; };
+
+template <bool CPLX>
+__device__ __forceinline__ void lz_small_product(const LzSmallSmem<CPLX>& S, int M, int N, int K, int lane, double (&cr)[8], double (&ci)[8]) {
+#pragma unroll
+  for (int u = 0; u < 8; ++u) {
+    cr[u] = 0.0; ci[u] = 0.0;
+    const int e = lane + 32 * u;
+    if (e < M * N) {
+      const int r = e % M, col = e / M;
+      for (int k = 0; k < K; ++k) {
+        const double ar = S.A[0][k * kLzSmall + r], br = S.B[0][col * kLzSmall + k];
+        cr[u] = fma(ar, br, cr[u]);
+        if (CPLX) {
+          const double ai = S.A[CPLX ? 1 : 0][k * kLzSmall + r], bi = S.B[CPLX ? 1 : 0][col * kLzSmall + k];
+          cr[u] = fma(-ai, bi, cr[u]);
+          ci[u] = fma(ar, bi, ci[u]); ci[u] = fma(ai, br, ci[u]);
+        }
+      }
+    }
+  }
+}
+
+// every shadow leaf of every chain, start to end: grid = ceil(chains * emax * Q / 4) CTAs of 4 warps
+template <bool CPLX>
+__global__ void __launch_bounds__(32 * kLzSmallWarps) lazy_leaf_small_kernel(LazyView V) {
+  constexpr int ES = CPLX ? 2 : 1;
+  __shared__ LzSmallSmem<CPLX> Sm[kLzSmallWarps];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const long long id = blockIdx.x * (long long)kLzSmallWarps + warp;
+  const int Q = V.imp.Q;
+  if (id >= (long long)V.nC * V.emax * Q) return;
+  const int y = (int)(id / Q), q0 = (int)(id % Q);
+  const LzLeafTask T = lz_leaf_task(V, y, q0);
+  if (!T.ok) return;
+  LzSmallSmem<CPLX>& S = Sm[warp];
+  const int d0 = V.imp.dim[q0];
+  const double* st = V.sh_tau + (size_t)y * V.cap;
+  const int* ss = V.sh_sym + (size_t)y * V.cap;
+  // first propagation P_{t1 - a}(q0) as the right operand
+  const double delta0 = (T.n ? st[0] : T.b) - T.a;
+  LzDiag dg; dg.delta = delta0; dg.E = V.imp.energy + V.imp.e_off[q0]; dg.emin = V.imp.e_min[q0];
+  int km = lane < d0 ? row_exp(prop_x(delta0, dg.E[lane], dg.emin)) : INT_MIN;
+  km = __reduce_max_sync(0xffffffffu, km);
+  dg.kmax = km;
+  for (int e = lane; e < kLzSmall * kLzSmall; e += 32) { S.B[0][e] = 0.0; if (CPLX) S.B[CPLX ? 1 : 0][e] = 0.0; }
+  __syncwarp();
+  double cr[8], ci[8];
+#pragma unroll
+  for (int u = 0; u < 8; ++u) { cr[u] = 0.0; ci[u] = 0.0; }
+  if (lane < d0) S.B[0][lane * kLzSmall + lane] = lz_diag_value(dg, lane);
+  __syncwarp();
+  long long e_acc = km;
+  double lg = -delta0 * dg.emin * kLog2e;
+  int q = q0, M = d0;                                     // rows of the current product
+  if (T.n == 0) {
+#pragma unroll
+    for (int u = 0; u < 8; ++u) { const int e = lane + 32 * u; if (e < d0 * d0) cr[u] = S.B[0][(e / d0) * kLzSmall + e % d0]; }
+  }
+  for (int j = 0; j < T.n; ++j) {
+    const BlkDesc bd = V.imp.blks[V.imp.blk_of[ss[j] * Q + q]];
+    const int qn = bd.dst, K = bd.cols;
+    M = bd.rows;
+    const double delta = ((j + 1 < T.n) ? st[j + 1] : T.b) - st[j];
+    const double* F = V.imp.store + bd.off;
+    for (int e = lane; e < M * K; e += 32) {
+      const int r = e / K, k = e % K;
+      const double* p = F + ((long long)r * bd.ld + k) * ES;
+      S.A[0][k * kLzSmall + r] = p[0]; if (CPLX) S.A[CPLX ? 1 : 0][k * kLzSmall + r] = p[1];
+    }
+    __syncwarp();
+    lz_small_product<CPLX>(S, M, d0, K, lane, cr, ci);
+    const double* En = V.imp.energy + V.imp.e_off[qn];
+    const double eminn = V.imp.e_min[qn];
+    int kr[8], wexp = INT_MIN;
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+      const int e = lane + 32 * u;
+      kr[u] = 0;
+      if (e < M * d0) {
+        const double x = prop_x(delta, En[e % M], eminn);
+        const double mr = exp2(__dsub_rn(x, floor(x)));
+        kr[u] = row_exp(x);
+        cr[u] *= mr; if (CPLX) ci[u] *= mr;
+        const double mx = fmax(fabs(cr[u]), fabs(ci[u]));
+        if (mx > 0.0) wexp = max(wexp, kr[u] + ilogb(mx));
+      }
+    }
+    wexp = __reduce_max_sync(0xffffffffu, wexp);
+    const int k = wexp == INT_MIN ? 0 : wexp;
+    __syncwarp();
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+      const int e = lane + 32 * u;
+      if (e < M * d0) {
+        cr[u] = lz_scale(cr[u], kr[u] - k); if (CPLX) ci[u] = lz_scale(ci[u], kr[u] - k);
+        S.B[0][(e / M) * kLzSmall + e % M] = cr[u]; if (CPLX) S.B[CPLX ? 1 : 0][(e / M) * kLzSmall + e % M] = ci[u];
+      }
+    }
+    __syncwarp();
+    e_acc += k; lg += -delta * eminn * kLog2e; q = qn;
+  }
+  double* Mx = lz_mat(V, T.c, T.slot, q0);
+  double sq = 0.0;
+#pragma unroll
+  for (int u = 0; u < 8; ++u) {
+    const int e = lane + 32 * u;
+    if (e < M * d0) {
+      double* p = Mx + ((long long)(e / M) * V.ldm + e % M) * ES;
+      p[0] = cr[u]; sq += cr[u] * cr[u];
+      if (CPLX) { p[1] = ci[u]; sq += ci[u] * ci[u]; }
+    }
+  }
+  sq = warp_sum(sq);
+  if (lane == 0) {
+    const size_t en = lz_ent(V, T.c, T.slot, q0);
+    V.ent_e[en] = e_acc; V.ent_lg[en] = lg; V.ent_nrm[en] = sqrt(sq); V.ent_valid[en] = 1;
+    if (T.n) atomicAdd(V.n_products, (unsigned long long)T.n);
+  }
+}
+
+// one dirty level: candidate test, product of the two children, common exponent, norm (one warp per candidate)
+template <bool CPLX>
+__global__ void __launch_bounds__(32 * kLzSmallWarps) lazy_node_small_kernel(LazyView V, int level, int mode, int r, const int* gate, int gate_commit) {
+  constexpr int ES = CPLX ? 2 : 1;
+  __shared__ LzSmallSmem<CPLX> Sm[kLzSmallWarps];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  int4 t0, t1;                                             // {c, slot, qin, sl}, {sr, mid, tq}
+  if (!lz_node_candidate(V, level, mode, r, gate, gate_commit, blockIdx.x * (long long)kLzSmallWarps + warp, t0, t1)) return;
+  LzSmallSmem<CPLX>& S = Sm[warp];
+  const int M = V.imp.dim[t1.z], K = V.imp.dim[t1.y], N = V.imp.dim[t0.z];
+  const double* R = lz_mat(V, t0.x, t1.x, t1.y);
+  const double* L = lz_mat(V, t0.x, t0.w, t0.z);
+  for (int e = lane; e < M * K; e += 32) {
+    const double* p = R + ((long long)(e / M) * V.ldm + e % M) * ES;
+    S.A[0][(e / M) * kLzSmall + e % M] = p[0]; if (CPLX) S.A[CPLX ? 1 : 0][(e / M) * kLzSmall + e % M] = p[1];
+  }
+  for (int e = lane; e < K * N; e += 32) {
+    const double* p = L + ((long long)(e / K) * V.ldm + e % K) * ES;
+    S.B[0][(e / K) * kLzSmall + e % K] = p[0]; if (CPLX) S.B[CPLX ? 1 : 0][(e / K) * kLzSmall + e % K] = p[1];
+  }
+  __syncwarp();
+  double cr[8], ci[8];
+  lz_small_product<CPLX>(S, M, N, K, lane, cr, ci);
+  int wexp = INT_MIN;
+#pragma unroll
+  for (int u = 0; u < 8; ++u) {
+    const double mx = fmax(fabs(cr[u]), fabs(ci[u]));
+    if (mx > 0.0) wexp = max(wexp, ilogb(mx));
+  }
+  wexp = __reduce_max_sync(0xffffffffu, wexp);
+  const int k = wexp == INT_MIN ? 0 : wexp;
+  double* Mx = lz_mat(V, t0.x, t0.y, t0.z);
+  double sq = 0.0;
+#pragma unroll
+  for (int u = 0; u < 8; ++u) {
+    const int e = lane + 32 * u;
+    if (e < M * N) {
+      const double vr = lz_scale(cr[u], -k), vi = CPLX ? lz_scale(ci[u], -k) : 0.0;
+      double* p = Mx + ((long long)(e / M) * V.ldm + e % M) * ES;
+      p[0] = vr; sq += vr * vr;
+      if (CPLX) { p[1] = vi; sq += vi * vi; }
+    }
+  }
+  sq = warp_sum(sq);
+  if (lane == 0) {
+    const size_t en = lz_ent(V, t0.x, t0.y, t0.z), el = lz_ent(V, t0.x, t0.w, t0.z), er = lz_ent(V, t0.x, t1.x, t1.y);
+    V.ent_e[en] = V.ent_e[el] + V.ent_e[er] + k; V.ent_lg[en] = V.ent_lg[el] + V.ent_lg[er];
+    V.ent_nrm[en] = sqrt(sq); V.ent_k[en] = INT_MIN;
+    __threadfence();
+    V.ent_valid[en] = 1;
+    atomicAdd(V.n_products, 1ull);
   }
 }
 

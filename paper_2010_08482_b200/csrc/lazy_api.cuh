@@ -14,6 +14,7 @@ struct ctqmc_chains {
   int NT = 1;                 // tiles per matrix side
   int g_gemm = 1, g_fix = 1;  // persistent CTAs of the list-driven kernels (resident CTAs per SM x SMs)
   int seq = 0;                // node steps enqueued so far: its parity selects the node work lists
+  bool small = false;         // every sector dimension <= kLzSmall: warp-per-task kernels (lazy.cuh, "small impurities")
   long long launches = 0;     // kernels enqueued by the most recent call
   cudaStream_t last_stream = nullptr;
 };
@@ -50,7 +51,13 @@ size_t chains_layout(LazyView& V, char* base) {
 int chains_enqueue_levels(ctqmc_chains* ch, int mode, int r, const int* gate, int gate_commit, cudaStream_t st) {
   const LazyView& V = ch->V;
   const long long cand = (long long)V.nC * V.emax * (mode == 0 ? 1 : V.imp.Q);
-  for (int level = V.D - 1; level >= 0; --level) {
+  for (int level = V.D - 1; level >= 0 && ch->small; --level) {
+    const unsigned g = (unsigned)((cand + kLzSmallWarps - 1) / kLzSmallWarps);
+    if (V.imp.cplx) lazy_node_small_kernel<true><<<g, 32 * kLzSmallWarps, 0, st>>>(V, level, mode, r, gate, gate_commit);
+    else            lazy_node_small_kernel<false><<<g, 32 * kLzSmallWarps, 0, st>>>(V, level, mode, r, gate, gate_commit);
+    ch->launches += 1;
+  }
+  for (int level = V.D - 1; level >= 0 && !ch->small; --level) {
     const int par = ch->seq++ & 1;
     lazy_node_plan_kernel<<<(unsigned)((cand + 255) / 256), 256, 0, st>>>(V, level, mode, r, gate, gate_commit, par);
     if (V.imp.cplx) {
@@ -90,6 +97,7 @@ extern "C" int ctqmc_chains_create(ctqmc_impurity* h, double beta, const ctqmc_c
   V.ldm = h->dev.dmax; V.node_elems = (long long)h->n_energy * V.ldm * (h->dev.cplx ? 2 : 1);
   ch->lazy_rounds = desc->lazy_rounds < h->dev.Q ? desc->lazy_rounds : h->dev.Q;
   ch->NT = (h->dev.dmax + kLzTile - 1) / kLzTile;
+  ch->small = h->dev.dmax <= kLzSmall;
   V.w_task_cap = (long long)V.nC * V.emax * h->dev.Q;
   V.w_tile_cap = V.w_task_cap * ch->NT * ch->NT;
   {
@@ -164,14 +172,18 @@ extern "C" int ctqmc_chains_propose(ctqmc_chains* ch, const ctqmc_edit_batch* ed
   lazy_prepare_kernel<<<(V.nC + 127) / 128, 128, 0, st>>>(V, E, log2_threshold);
   const unsigned ltasks = (unsigned)((long long)V.nC * V.emax);
   dim3 gl(ltasks, (unsigned)Q);
-  if (cx) lazy_leaf_init_kernel<true><<<gl, 256, 0, st>>>(V); else lazy_leaf_init_kernel<false><<<gl, 256, 0, st>>>(V);
-  for (int j = 0; j < V.cap; ++j) {
+  if (ch->small) {
+    const unsigned g = (unsigned)(((long long)ltasks * Q + kLzSmallWarps - 1) / kLzSmallWarps);
+    if (cx) lazy_leaf_small_kernel<true><<<g, 32 * kLzSmallWarps, 0, st>>>(V); else lazy_leaf_small_kernel<false><<<g, 32 * kLzSmallWarps, 0, st>>>(V);
+    ch->launches += 1;
+  } else if (cx) lazy_leaf_init_kernel<true><<<gl, 256, 0, st>>>(V); else lazy_leaf_init_kernel<false><<<gl, 256, 0, st>>>(V);
+  for (int j = 0; j < V.cap && !ch->small; ++j) {
     if (cx) { lazy_leaf_step_kernel<true><<<ch->g_gemm, kLzThreads, 0, st>>>(V, j); lazy_leaf_fix_kernel<true><<<ch->g_fix, 256, 0, st>>>(V, j); }
     else    { lazy_leaf_step_kernel<false><<<ch->g_gemm, kLzThreads, 0, st>>>(V, j); lazy_leaf_fix_kernel<false><<<ch->g_fix, 256, 0, st>>>(V, j); }
   }
   const unsigned wg = (unsigned)(((long long)V.nC * 32 + 255) / 256);
   lazy_bound_kernel<<<wg, 256, 0, st>>>(V, bound_mant, (long long*)bound_exp2);
-  ch->launches += 3 + 2 * V.cap;
+  ch->launches += ch->small ? 2 : 3 + 2 * V.cap;
   CU(cudaGetLastError());
   // lazy rounds: one start sector each, in order of decreasing bound
   for (int r = 0; r < ch->lazy_rounds; ++r) {
