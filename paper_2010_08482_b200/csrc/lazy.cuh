@@ -57,6 +57,7 @@ struct LazyView {
   // step kernel clears (j + 2) % 3), node lists over two (parity of the host's launch sequence number).
   int* w_cnt;                                                // [0..2] leaf tasks, [3..5] leaf tiles, [6..7] node tasks, [8..9] node tiles
   int4* w_ltask; int4* w_ltile; int4* w_ntask; int4* w_ntile;
+  int* w_larr; int* w_narr; double* w_part;                  // tiles of a task that have been rescaled; their partial sums of squares
   long long w_task_cap, w_tile_cap;                          // entries per buffer
 };
 
@@ -68,7 +69,7 @@ struct LazyEdits {
 __device__ __forceinline__ void lz_push_tiles(int* cnt, int4* tiles, int task, int M, int N) {
   const int tm = (M + kLzTile - 1) / kLzTile, tn = (N + kLzTile - 1) / kLzTile;
   const int base = atomicAdd(cnt, tm * tn);
-  for (int i = 0; i < tm * tn; ++i) tiles[base + i] = make_int4(task, (i / tn) * kLzTile, (i % tn) * kLzTile, 0);
+  for (int i = 0; i < tm * tn; ++i) tiles[base + i] = make_int4(task, (i / tn) * kLzTile, (i % tn) * kLzTile, i);
 }
 
 // ------------------------------------------------------------------------------------------------ small helpers
@@ -275,6 +276,35 @@ __device__ double lz_fix_entry(double* Mx, int ld, int rows, int cols, int k, Lz
   return lz_block_sum(ss, red);
 }
 
+// The same, one 64 x 64 tile per CTA (the rescale of a 295 x 295 product by one CTA was a third of a config-4 round).
+template <bool CPLX>
+__device__ double lz_fix_tile(double* Mx, int ld, int rows, int cols, int m0, int n0, int k, LzRowScale rs, double* red) {
+  constexpr int ES = CPLX ? 2 : 1;
+  double ss = 0.0;
+  for (int idx = threadIdx.x; idx < kLzTile * kLzTile; idx += blockDim.x) {
+    const int r = m0 + (idx & (kLzTile - 1)), c = n0 + idx / kLzTile;
+    if (r < rows && c < cols) {
+      const int sh = (rs.on ? row_exp(prop_x(rs.delta, rs.E[r], rs.emin)) : 0) - k;
+      double* p = Mx + ((long long)c * ld + r) * ES;
+      const double vr = lz_scale(p[0], sh); p[0] = vr; ss += vr * vr;
+      if (CPLX) { const double vi = lz_scale(p[1], sh); p[1] = vi; ss += vi * vi; }
+    }
+  }
+  return lz_block_sum(ss, red);
+}
+// Thread 0 of a CTA reports its tile (position `it` of the tile list, `ordinal` within its task).  The CTA that completes the
+// task gets the task's sum of squares, the partial sums added in tile order (so the norm does not depend on the schedule);
+// every other caller gets -1.
+__device__ __forceinline__ double lz_fix_arrive(double* part, int* arrived, int it, int ordinal, int ntiles, double ss) {
+  part[it] = ss;
+  __threadfence();
+  if (atomicAdd(arrived, 1) != ntiles - 1) return -1.0;
+  __threadfence();
+  double t = 0.0;
+  for (int i = 0; i < ntiles; ++i) t += ((volatile double*)part)[it - ordinal + i];
+  return t;
+}
+
 // ------------------------------------------------------------------------------------------------ creation
 __global__ void lazy_reset_kernel(LazyView V) {
   const long long n = (long long)V.nC * V.NN * V.imp.Q;
@@ -348,74 +378,78 @@ __global__ void lazy_replicate_kernel(LazyView V) {
 }
 
 // ------------------------------------------------------------------------------------------------ proposal: integer part
-// One thread per chain: validates the edits, builds the shadow leaves' operator lists, the dirty-node list (leaves first,
-// then their ancestors level by level) and the sector maps of every shadow entry.
+// One warp per chain.  Lane 0 validates the edits and builds the shadow leaves' operator lists and the dirty-node list (leaves
+// first, then their ancestors level by level); then the lanes share the sectors for the sector maps of every shadow entry.
 __global__ void lazy_prepare_kernel(LazyView V, LazyEdits E, const double* log2_thr) {
-  const int c = blockIdx.x * blockDim.x + threadIdx.x;
+  const int c = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
   if (c >= V.nC) return;
   const int Q = V.imp.Q, A = V.imp.A, cap = V.cap;
   int status = 0, n = 0;
   long long lo = 0;
-  if (E.offset) {
-    lo = E.offset[c];
-    const long long hi = E.offset[c + 1];
-    if (lo < 0 || hi < lo || hi > E.n_edits || hi - lo > V.emax) status = 2; else n = (int)(hi - lo);
-  }
   int* pn = V.p_node + (size_t)c * V.smax;
-  int nl = 0;
-  for (int e = 0; e < n && status == 0; ++e) {
-    const double t = E.tau[lo + e];
-    const int a = E.sym[lo + e], k = E.kind[lo + e];
-    if (!(t >= 0.0 && t < V.beta) || a < 0 || a >= A || (k != 1 && k != -1)) { status = 2; break; }
-    const int leaf = lz_leaf_of(V, t);
-    int pos = 0;
-    while (pos < nl && pn[pos] < leaf) ++pos;
-    if (pos < nl && pn[pos] == leaf) continue;
-    for (int i = nl; i > pos; --i) pn[i] = pn[i - 1];
-    pn[pos] = leaf; ++nl;
-  }
-  // shadow operator lists: removals first (first match in time order), then insertions after every operator with tau <= t
-  for (int k = 0; k < nl && status == 0; ++k) {
-    const int leaf = pn[k];
-    double* st = V.sh_tau + ((size_t)c * V.emax + k) * cap;
-    int* ss = V.sh_sym + ((size_t)c * V.emax + k) * cap;
-    int cnt = V.leaf_n[(size_t)c * V.nleaf + leaf];
-    for (int i = 0; i < cnt; ++i) { st[i] = V.leaf_tau[((size_t)c * V.nleaf + leaf) * cap + i]; ss[i] = V.leaf_sym[((size_t)c * V.nleaf + leaf) * cap + i]; }
-    for (int e = 0; e < n && status == 0; ++e) {
-      if (E.kind[lo + e] != -1 || lz_leaf_of(V, E.tau[lo + e]) != leaf) continue;
-      int i = 0;
-      while (i < cnt && !(st[i] == E.tau[lo + e] && ss[i] == E.sym[lo + e])) ++i;
-      if (i == cnt) { status = 3; break; }
-      for (; i + 1 < cnt; ++i) { st[i] = st[i + 1]; ss[i] = ss[i + 1]; }
-      --cnt;
+  int nl = 0, total = 0;
+  if (lane == 0) {
+    if (E.offset) {
+      lo = E.offset[c];
+      const long long hi = E.offset[c + 1];
+      if (lo < 0 || hi < lo || hi > E.n_edits || hi - lo > V.emax) status = 2; else n = (int)(hi - lo);
     }
     for (int e = 0; e < n && status == 0; ++e) {
-      if (E.kind[lo + e] != 1 || lz_leaf_of(V, E.tau[lo + e]) != leaf) continue;
-      if (cnt == cap) { status = 4; break; }
+      const double t = E.tau[lo + e];
+      const int a = E.sym[lo + e], k = E.kind[lo + e];
+      if (!(t >= 0.0 && t < V.beta) || a < 0 || a >= A || (k != 1 && k != -1)) { status = 2; break; }
+      const int leaf = lz_leaf_of(V, t);
       int pos = 0;
-      while (pos < cnt && st[pos] <= E.tau[lo + e]) ++pos;
-      for (int i = cnt; i > pos; --i) { st[i] = st[i - 1]; ss[i] = ss[i - 1]; }
-      st[pos] = E.tau[lo + e]; ss[pos] = E.sym[lo + e]; ++cnt;
+      while (pos < nl && pn[pos] < leaf) ++pos;
+      if (pos < nl && pn[pos] == leaf) continue;
+      for (int i = nl; i > pos; --i) pn[i] = pn[i - 1];
+      pn[pos] = leaf; ++nl;
     }
-    V.sh_n[(size_t)c * V.emax + k] = cnt;
-  }
-  if (status != 0) nl = 0;
-  if (c == 0) for (int i = 0; i < 6; ++i) V.w_cnt[i] = 0;      // leaf work lists of this proposal start empty
-  int total = nl;
-  for (int i = 0; i < nl; ++i) pn[i] += V.nleaf - 1;
-  {
-    int start = 0, cnt = nl;
-    for (int level = V.D - 1; level >= 0; --level) {
-      int prev = -1, nc = 0;
-      for (int i = start; i < start + cnt; ++i) { const int p = (pn[i] - 1) >> 1; if (p != prev) { pn[total + nc++] = p; prev = p; } }
-      V.p_lvl_start[(size_t)c * V.D + level] = total; V.p_lvl_cnt[(size_t)c * V.D + level] = nc;
-      start = total; total += nc; cnt = nc;
+    // shadow operator lists: removals first (first match in time order), then insertions after every operator with tau <= t
+    for (int k = 0; k < nl && status == 0; ++k) {
+      const int leaf = pn[k];
+      double* st = V.sh_tau + ((size_t)c * V.emax + k) * cap;
+      int* ss = V.sh_sym + ((size_t)c * V.emax + k) * cap;
+      int cnt = V.leaf_n[(size_t)c * V.nleaf + leaf];
+      for (int i = 0; i < cnt; ++i) { st[i] = V.leaf_tau[((size_t)c * V.nleaf + leaf) * cap + i]; ss[i] = V.leaf_sym[((size_t)c * V.nleaf + leaf) * cap + i]; }
+      for (int e = 0; e < n && status == 0; ++e) {
+        if (E.kind[lo + e] != -1 || lz_leaf_of(V, E.tau[lo + e]) != leaf) continue;
+        int i = 0;
+        while (i < cnt && !(st[i] == E.tau[lo + e] && ss[i] == E.sym[lo + e])) ++i;
+        if (i == cnt) { status = 3; break; }
+        for (; i + 1 < cnt; ++i) { st[i] = st[i + 1]; ss[i] = ss[i + 1]; }
+        --cnt;
+      }
+      for (int e = 0; e < n && status == 0; ++e) {
+        if (E.kind[lo + e] != 1 || lz_leaf_of(V, E.tau[lo + e]) != leaf) continue;
+        if (cnt == cap) { status = 4; break; }
+        int pos = 0;
+        while (pos < cnt && st[pos] <= E.tau[lo + e]) ++pos;
+        for (int i = cnt; i > pos; --i) { st[i] = st[i - 1]; ss[i] = ss[i - 1]; }
+        st[pos] = E.tau[lo + e]; ss[pos] = E.sym[lo + e]; ++cnt;
+      }
+      V.sh_n[(size_t)c * V.emax + k] = cnt;
     }
+    if (status != 0) nl = 0;
+    if (c == 0) for (int i = 0; i < 6; ++i) V.w_cnt[i] = 0;      // leaf work lists of this proposal start empty
+    total = nl;
+    for (int i = 0; i < nl; ++i) pn[i] += V.nleaf - 1;
+    {
+      int start = 0, cnt = nl;
+      for (int level = V.D - 1; level >= 0; --level) {
+        int prev = -1, nc = 0;
+        for (int i = start; i < start + cnt; ++i) { const int p = (pn[i] - 1) >> 1; if (p != prev) { pn[total + nc++] = p; prev = p; } }
+        V.p_lvl_start[(size_t)c * V.D + level] = total; V.p_lvl_cnt[(size_t)c * V.D + level] = nc;
+        start = total; total += nc; cnt = nc;
+      }
+    }
+    V.p_status[c] = status; V.p_nleaf[c] = nl; V.p_ndirty[c] = total;
+    V.decided[c] = status ? 2 : 0; V.decided_by[c] = 0; V.n_eval[c] = 0; V.n_alive[c] = 0;
+    V.thr[c] = log2_thr ? log2_thr[c] : -INFINITY;
   }
-  V.p_status[c] = status; V.p_nleaf[c] = nl; V.p_ndirty[c] = total;
-  V.decided[c] = status ? 2 : 0; V.decided_by[c] = 0; V.n_eval[c] = 0; V.n_alive[c] = 0;
-  V.thr[c] = log2_thr ? log2_thr[c] : -INFINITY;
-  // sector maps of the shadow entries (children come earlier in the list)
+  __syncwarp();
+  nl = __shfl_sync(0xffffffffu, nl, 0); total = __shfl_sync(0xffffffffu, total, 0);
+  // sector maps of the shadow entries (children come earlier in the list: a warp barrier after every entry)
   const int* fs = V.free_slot + (size_t)c * (V.smax + V.emax);
   for (int i = 0; i < total; ++i) {
     const int slot = fs[i], node = pn[i];
@@ -425,7 +459,7 @@ __global__ void lazy_prepare_kernel(LazyView V, LazyEdits E, const double* log2_
       sl = V.slot_of[(size_t)c * V.nnode + left]; sr = V.slot_of[(size_t)c * V.nnode + right];
       for (int j = 0; j < i; ++j) { if (pn[j] == left) sl = fs[j]; if (pn[j] == right) sr = fs[j]; }
     }
-    for (int q = 0; q < Q; ++q) {
+    for (int q = lane; q < Q; q += 32) {
       int tq = q;
       if (i < nl) {
         const int cnt = V.sh_n[(size_t)c * V.emax + i];
@@ -438,6 +472,7 @@ __global__ void lazy_prepare_kernel(LazyView V, LazyEdits E, const double* log2_
       const size_t en = lz_ent(V, c, slot, q);
       V.ent_tgt[en] = tq; V.ent_valid[en] = 0; V.ent_k[en] = INT_MIN; V.ent_e[en] = 0; V.ent_lg[en] = 0.0; V.ent_nrm[en] = 0.0;
     }
+    __syncwarp();
   }
 }
 
@@ -477,7 +512,7 @@ __global__ void lazy_leaf_init_kernel(LazyView V) {
   if (threadIdx.x == 0) {
     const size_t en = lz_ent(V, T.c, T.slot, T.q0); V.ent_e[en] = km; V.ent_lg[en] = -delta * emin * kLog2e;
     const int ti = atomicAdd(&V.w_cnt[0], 1);
-    V.w_ltask[ti] = make_int4((int)blockIdx.x, T.q0, T.q0, 0);
+    V.w_ltask[ti] = make_int4((int)blockIdx.x, T.q0, T.q0, 0); V.w_larr[ti] = 0;
     const int blk = V.imp.blk_of[V.sh_sym[((size_t)T.c * V.emax + T.k) * V.cap] * V.imp.Q + T.q0];
     lz_push_tiles(&V.w_cnt[3], V.w_ltile, ti, V.imp.blks[blk].rows, d);
   }
@@ -530,30 +565,39 @@ __global__ void __launch_bounds__(kLzThreads) lazy_leaf_step_kernel(LazyView V, 
   }
 }
 
-// common exponent and norm of the product of step j; the task moves on to step j + 1 (persistent CTAs over the task list)
+// common exponent and norm of the product of step j, tile by tile (persistent CTAs over the tile list); the CTA that finishes a
+// task's last tile closes the step and moves the task on to step j + 1
 template <bool CPLX>
 __global__ void lazy_leaf_fix_kernel(LazyView V, int j) {
   __shared__ double red[32];
   const int cur = j % 3, nxt = (j + 1) % 3;
-  const int n_tasks = V.w_cnt[cur];
+  const int n_items = V.w_cnt[3 + cur];
+  const int4* tiles = V.w_ltile + (size_t)cur * V.w_tile_cap;
   const int4* tasks = V.w_ltask + (size_t)cur * V.w_task_cap;
-  for (int ti = blockIdx.x; ti < n_tasks; ti += gridDim.x) {
-    const int4 task = tasks[ti];
+  for (int it = blockIdx.x; it < n_items; it += gridDim.x) {
+    const int4 tl = tiles[it];
+    const int4 task = tasks[tl.x];
     const LzLeafStep st = lz_leaf_step(V, task, j);
     int k = V.ent_k[st.en];
     if (k == INT_MIN) k = 0;
     LzRowScale rs; rs.on = 1; rs.delta = st.delta; rs.E = V.imp.energy + V.imp.e_off[st.qn]; rs.emin = V.imp.e_min[st.qn];
-    const double ss = lz_fix_entry<CPLX>(st.out, V.ldm, V.imp.dim[st.qn], V.imp.dim[st.q0], k, rs, red);
+    const int rows = V.imp.dim[st.qn], cols = V.imp.dim[st.q0];
+    const double part = lz_fix_tile<CPLX>(st.out, V.ldm, rows, cols, tl.y, tl.z, k, rs, red);
     if (threadIdx.x == 0) {
-      V.ent_e[st.en] += k; V.ent_lg[st.en] += -st.delta * rs.emin * kLog2e; V.ent_k[st.en] = INT_MIN;
-      if (j == st.n - 1) { V.ent_nrm[st.en] = sqrt(ss); V.ent_valid[st.en] = 1; }
-      else {
-        const int t2 = atomicAdd(&V.w_cnt[nxt], 1);
-        V.w_ltask[(size_t)nxt * V.w_task_cap + t2] = make_int4(task.x, task.y, st.qn, 0);
-        const int blk = V.imp.blk_of[V.sh_sym[(size_t)task.x * V.cap + j + 1] * V.imp.Q + st.qn];
-        lz_push_tiles(&V.w_cnt[3 + nxt], V.w_ltile + (size_t)nxt * V.w_tile_cap, t2, V.imp.blks[blk].rows, V.imp.dim[st.q0]);
+      const int nt = ((rows + kLzTile - 1) / kLzTile) * ((cols + kLzTile - 1) / kLzTile);
+      const double ss = lz_fix_arrive(V.w_part, &V.w_larr[(size_t)cur * V.w_task_cap + tl.x], it, tl.w, nt, part);
+      if (ss >= 0.0) {
+        V.ent_e[st.en] += k; V.ent_lg[st.en] += -st.delta * rs.emin * kLog2e; V.ent_k[st.en] = INT_MIN;
+        if (j == st.n - 1) { V.ent_nrm[st.en] = sqrt(ss); V.ent_valid[st.en] = 1; }
+        else {
+          const int t2 = atomicAdd(&V.w_cnt[nxt], 1);
+          V.w_ltask[(size_t)nxt * V.w_task_cap + t2] = make_int4(task.x, task.y, st.qn, 0);
+          V.w_larr[(size_t)nxt * V.w_task_cap + t2] = 0;
+          const int blk = V.imp.blk_of[V.sh_sym[(size_t)task.x * V.cap + j + 1] * V.imp.Q + st.qn];
+          lz_push_tiles(&V.w_cnt[3 + nxt], V.w_ltile + (size_t)nxt * V.w_tile_cap, t2, V.imp.blks[blk].rows, cols);
+        }
+        atomicAdd(V.n_products, 1ull);
       }
-      atomicAdd(V.n_products, 1ull);
     }
     __syncthreads();
   }
@@ -653,7 +697,7 @@ __global__ void lazy_node_plan_kernel(LazyView V, int level, int mode, int r, co
   if (!lz_node_candidate(V, level, mode, r, gate, gate_commit, blockIdx.x * (long long)blockDim.x + threadIdx.x, t0, t1)) return;
   const int ti = atomicAdd(&V.w_cnt[6 + par], 1);
   int4* nt = V.w_ntask + ((size_t)par * V.w_task_cap + ti) * 2;
-  nt[0] = t0; nt[1] = t1;
+  nt[0] = t0; nt[1] = t1; V.w_narr[(size_t)par * V.w_task_cap + ti] = 0;
   lz_push_tiles(&V.w_cnt[8 + par], V.w_ntile + (size_t)par * V.w_tile_cap, ti, V.imp.dim[t1.z], V.imp.dim[t0.z]);
 }
 
@@ -678,23 +722,30 @@ __global__ void __launch_bounds__(kLzThreads) lazy_node_gemm_kernel(LazyView V, 
 template <bool CPLX>
 __global__ void lazy_node_fix_kernel(LazyView V, int par) {
   __shared__ double red[32];
-  const int n_tasks = V.w_cnt[6 + par];
+  const int n_items = V.w_cnt[8 + par];
+  const int4* tiles = V.w_ntile + (size_t)par * V.w_tile_cap;
   const int4* tasks = V.w_ntask + (size_t)par * V.w_task_cap * 2;
   LzRowScale rs; rs.on = 0; rs.delta = 0.0; rs.E = nullptr; rs.emin = 0.0;
-  for (int ti = blockIdx.x; ti < n_tasks; ti += gridDim.x) {
-    const int4 t0 = tasks[2 * ti], t1 = tasks[2 * ti + 1];
+  for (int it = blockIdx.x; it < n_items; it += gridDim.x) {
+    const int4 tl = tiles[it];
+    const int4 t0 = tasks[2 * tl.x], t1 = tasks[2 * tl.x + 1];
     const size_t en = lz_ent(V, t0.x, t0.y, t0.z), el = lz_ent(V, t0.x, t0.w, t0.z), er = lz_ent(V, t0.x, t1.x, t1.y);
     int k = V.ent_k[en];
     if (k == INT_MIN) k = 0;
-    const double ss = lz_fix_entry<CPLX>(lz_mat(V, t0.x, t0.y, t0.z), V.ldm, V.imp.dim[t1.z], V.imp.dim[t0.z], k, rs, red);
-    __syncthreads();
+    const int rows = V.imp.dim[t1.z], cols = V.imp.dim[t0.z];
+    const double part = lz_fix_tile<CPLX>(lz_mat(V, t0.x, t0.y, t0.z), V.ldm, rows, cols, tl.y, tl.z, k, rs, red);
     if (threadIdx.x == 0) {
-      V.ent_e[en] = V.ent_e[el] + V.ent_e[er] + k; V.ent_lg[en] = V.ent_lg[el] + V.ent_lg[er];
-      V.ent_nrm[en] = sqrt(ss); V.ent_k[en] = INT_MIN;
-      __threadfence();
-      V.ent_valid[en] = 1;
-      atomicAdd(V.n_products, 1ull);
+      const int nt = ((rows + kLzTile - 1) / kLzTile) * ((cols + kLzTile - 1) / kLzTile);
+      const double ss = lz_fix_arrive(V.w_part, &V.w_narr[(size_t)par * V.w_task_cap + tl.x], it, tl.w, nt, part);
+      if (ss >= 0.0) {
+        V.ent_e[en] = V.ent_e[el] + V.ent_e[er] + k; V.ent_lg[en] = V.ent_lg[el] + V.ent_lg[er];
+        V.ent_nrm[en] = sqrt(ss); V.ent_k[en] = INT_MIN;
+        __threadfence();
+        V.ent_valid[en] = 1;
+        atomicAdd(V.n_products, 1ull);
+      }
     }
+    __syncthreads();
   }
 }
 
@@ -706,6 +757,7 @@ __global__ void lazy_node_fix_kernel(LazyView V, int par) {
 // is that of lz_gemm_tile + lz_fix_entry element by element; only the order of the contraction sum differs.
 constexpr int kLzSmall = 16;
 constexpr int kLzSmallWarps = 4;
+__host__ __device__ constexpr int lz_node_small_warps(bool cplx) { return cplx ? 4 : 8; }   // 32 KB of operands per CTA either way
 template <bool CPLX>
 struct LzSmallSmem { double A[CPLX ? 2 : 1][kLzSmall * kLzSmall]; double B[CPLX ? 2 : 1][kLzSmall * kLzSmall]; };
 
@@ -828,15 +880,34 @@ __global__ void __launch_bounds__(32 * kLzSmallWarps) lazy_leaf_small_kernel(Laz
   }
 }
 
-// one dirty level: candidate test, product of the two children, common exponent, norm (one warp per candidate)
+// the dirty ancestors of one chain, bottom-up (one CTA per chain; a level depends only on the chain's own lower levels, so a
+// CTA-wide barrier separates them): candidate test, product of the two children, common exponent, norm (one warp per candidate)
 template <bool CPLX>
-__global__ void __launch_bounds__(32 * kLzSmallWarps) lazy_node_small_kernel(LazyView V, int level, int mode, int r, const int* gate, int gate_commit) {
-  constexpr int ES = CPLX ? 2 : 1;
+__device__ __forceinline__ void lz_node_small(const LazyView& V, LzSmallSmem<CPLX>& S, int4 t0, int4 t1, int lane);
+
+template <bool CPLX>
+__global__ void __launch_bounds__(32 * lz_node_small_warps(CPLX)) lazy_node_small_kernel(LazyView V, int mode, int r, const int* gate, int gate_commit) {
+  constexpr int kLzSmallWarps = lz_node_small_warps(CPLX);
   __shared__ LzSmallSmem<CPLX> Sm[kLzSmallWarps];
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  int4 t0, t1;                                             // {c, slot, qin, sl}, {sr, mid, tq}
-  if (!lz_node_candidate(V, level, mode, r, gate, gate_commit, blockIdx.x * (long long)kLzSmallWarps + warp, t0, t1)) return;
-  LzSmallSmem<CPLX>& S = Sm[warp];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, c = blockIdx.x;
+  const int nsec = mode == 0 ? 1 : V.imp.Q;
+  if (V.p_status[c] != 0 || V.p_ndirty[c] == 0) return;
+  if (gate_commit ? (gate[c] == 0) : (V.decided[c] == 2)) return;
+  for (int level = V.D - 1; level >= 0; --level) {
+    const int n_cand = V.p_lvl_cnt[(size_t)c * V.D + level] * nsec;
+    for (int cand = warp; cand < n_cand; cand += kLzSmallWarps) {
+      int4 t0, t1;                                           // {c, slot, qin, sl}, {sr, mid, tq}
+      if (lz_node_candidate(V, level, mode, r, gate, gate_commit, ((long long)c * V.emax + cand / nsec) * nsec + cand % nsec, t0, t1))
+        lz_node_small<CPLX>(V, Sm[warp], t0, t1, lane);
+      __syncwarp();
+    }
+    __syncthreads();
+  }
+}
+
+template <bool CPLX>
+__device__ __forceinline__ void lz_node_small(const LazyView& V, LzSmallSmem<CPLX>& S, int4 t0, int4 t1, int lane) {
+  constexpr int ES = CPLX ? 2 : 1;
   const int M = V.imp.dim[t1.z], K = V.imp.dim[t1.y], N = V.imp.dim[t0.z];
   const double* R = lz_mat(V, t0.x, t1.x, t1.y);
   const double* L = lz_mat(V, t0.x, t0.w, t0.z);

@@ -43,6 +43,7 @@ size_t chains_layout(LazyView& V, char* base) {
   V.w_cnt = bp.take<int>(16);
   V.w_ltask = bp.take<int4>(3 * (size_t)V.w_task_cap); V.w_ltile = bp.take<int4>(3 * (size_t)V.w_tile_cap);
   V.w_ntask = bp.take<int4>(2 * 2 * (size_t)V.w_task_cap); V.w_ntile = bp.take<int4>(2 * (size_t)V.w_tile_cap);
+  V.w_larr = bp.take<int>(3 * (size_t)V.w_task_cap); V.w_narr = bp.take<int>(2 * (size_t)V.w_task_cap); V.w_part = bp.take<double>((size_t)V.w_tile_cap);
   V.mats = bp.take<double>(nC * V.NN * (size_t)V.node_elems);
   return bp.off + 256;
 }
@@ -51,10 +52,9 @@ size_t chains_layout(LazyView& V, char* base) {
 int chains_enqueue_levels(ctqmc_chains* ch, int mode, int r, const int* gate, int gate_commit, cudaStream_t st) {
   const LazyView& V = ch->V;
   const long long cand = (long long)V.nC * V.emax * (mode == 0 ? 1 : V.imp.Q);
-  for (int level = V.D - 1; level >= 0 && ch->small; --level) {
-    const unsigned g = (unsigned)((cand + kLzSmallWarps - 1) / kLzSmallWarps);
-    if (V.imp.cplx) lazy_node_small_kernel<true><<<g, 32 * kLzSmallWarps, 0, st>>>(V, level, mode, r, gate, gate_commit);
-    else            lazy_node_small_kernel<false><<<g, 32 * kLzSmallWarps, 0, st>>>(V, level, mode, r, gate, gate_commit);
+  if (ch->small && V.D > 0) {       // all levels in one launch, one CTA per chain
+    if (V.imp.cplx) lazy_node_small_kernel<true><<<V.nC, 32 * lz_node_small_warps(true), 0, st>>>(V, mode, r, gate, gate_commit);
+    else            lazy_node_small_kernel<false><<<V.nC, 32 * lz_node_small_warps(false), 0, st>>>(V, mode, r, gate, gate_commit);
     ch->launches += 1;
   }
   for (int level = V.D - 1; level >= 0 && !ch->small; --level) {
@@ -169,7 +169,7 @@ extern "C" int ctqmc_chains_propose(ctqmc_chains* ch, const ctqmc_edit_batch* ed
   LazyEdits E;
   E.offset = (const long long*)edits->offset; E.tau = edits->tau; E.sym = edits->symbol; E.kind = edits->kind; E.n_edits = edits->n_edits;
   if (edits->n_edits == 0) E.offset = nullptr;
-  lazy_prepare_kernel<<<(V.nC + 127) / 128, 128, 0, st>>>(V, E, log2_threshold);
+  lazy_prepare_kernel<<<(unsigned)(((long long)V.nC * 32 + 127) / 128), 128, 0, st>>>(V, E, log2_threshold);
   const unsigned ltasks = (unsigned)((long long)V.nC * V.emax);
   dim3 gl(ltasks, (unsigned)Q);
   if (ch->small) {
