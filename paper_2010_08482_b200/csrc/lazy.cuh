@@ -197,9 +197,13 @@ __device__ void lz_gemm_tile(LzSmem<CPLX>& S, int m0, int n0, int M, int N, int 
 #pragma unroll
       for (int x = 0; x < (CPLX ? 4 : 2); ++x) acc[mi][ni][x] = 0.0;
 
-  for (int k0 = 0; k0 < K; k0 += kLzKC) {
-    __syncthreads();
-    for (int idx = tid; idx < kLzTile * kLzKC; idx += kLzThreads) {
+  // the next K chunk travels from global memory to registers while the tensor cores work on the current one
+  constexpr int kPer = kLzTile * kLzKC / kLzThreads;      // staged values per thread, operand and chunk
+  double pa[kPer], pai[kPer], pb[kPer], pbi[kPer];
+  auto fetch = [&](int k0) {
+#pragma unroll
+    for (int u = 0; u < kPer; ++u) {
+      const int idx = tid + u * kLzThreads;
       int r, kk;
       if (a_cs == 1) { r = idx / kLzKC; kk = idx % kLzKC; } else { r = idx % kLzTile; kk = idx / kLzTile; }
       double vr = 0.0, vi = 0.0;
@@ -207,17 +211,28 @@ __device__ void lz_gemm_tile(LzSmem<CPLX>& S, int m0, int n0, int M, int N, int 
         const double* p = A + ((long long)(m0 + r) * a_rs + (long long)(k0 + kk) * a_cs) * ES;
         vr = p[0]; if (CPLX) vi = p[1];
       }
-      S.A[0][r][kk] = vr; if (CPLX) S.A[CPLX ? 1 : 0][r][kk] = vi;
-    }
-    for (int idx = tid; idx < kLzTile * kLzKC; idx += kLzThreads) {
-      const int kk = idx % kLzKC, nn = idx / kLzKC;
-      double vr = 0.0, vi = 0.0;
-      if (n0 + nn < N && k0 + kk < K) {
-        if (B) { const double* p = B + ((long long)(n0 + nn) * ldb + (long long)(k0 + kk) * b_ks) * ES; vr = p[0]; if (CPLX) vi = p[1]; }
-        else if (n0 + nn == k0 + kk) vr = lz_diag_value(dg, n0 + nn);
+      pa[u] = vr; pai[u] = vi;
+      const int kb = idx % kLzKC, nn = idx / kLzKC;
+      vr = 0.0; vi = 0.0;
+      if (n0 + nn < N && k0 + kb < K) {
+        if (B) { const double* p = B + ((long long)(n0 + nn) * ldb + (long long)(k0 + kb) * b_ks) * ES; vr = p[0]; if (CPLX) vi = p[1]; }
+        else if (n0 + nn == k0 + kb) vr = lz_diag_value(dg, n0 + nn);
       }
-      S.B[0][nn][kk] = vr; if (CPLX) S.B[CPLX ? 1 : 0][nn][kk] = vi;
+      pb[u] = vr; pbi[u] = vi;
     }
+  };
+  fetch(0);
+  for (int k0 = 0; k0 < K; k0 += kLzKC) {
+    __syncthreads();
+#pragma unroll
+    for (int u = 0; u < kPer; ++u) {
+      const int idx = tid + u * kLzThreads;
+      int r, kk;
+      if (a_cs == 1) { r = idx / kLzKC; kk = idx % kLzKC; } else { r = idx % kLzTile; kk = idx / kLzTile; }
+      S.A[0][r][kk] = pa[u]; if (CPLX) S.A[CPLX ? 1 : 0][r][kk] = pai[u];
+      S.B[0][idx / kLzKC][idx % kLzKC] = pb[u]; if (CPLX) S.B[CPLX ? 1 : 0][idx / kLzKC][idx % kLzKC] = pbi[u];
+    }
+    if (k0 + kLzKC < K) fetch(k0 + kLzKC);
     __syncthreads();
 #pragma unroll
     for (int ks = 0; ks < kLzKC; ks += 4) {
