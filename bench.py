@@ -628,7 +628,16 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-others", dest="others", action="store_false",
                     help="skip the short device-resident timings of the other BASELINE.json configs (about two minutes at N=1)")
+    ap.add_argument("--chains", default="", metavar="CFG,CHAINS,DEPTH,LEAF_CAPACITY,ROUNDS",
+                    help="only the chain-set row (SURVEY 8(f) 1-2) for this shape, e.g. 4,16,4,64,4: prints that row and exits")
     args = ap.parse_args()
+    if args.chains:
+        import torch
+        import paper_2010_08482_b200 as L
+        L.library()
+        c, n, depth, cap, rounds = (int(x) for x in args.chains.split(","))
+        print(json.dumps({"chains_row": measure_chains(L, torch, c, n, depth, rounds, 0, leaf_capacity=cap)}))
+        return
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))

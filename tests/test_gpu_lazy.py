@@ -67,14 +67,53 @@ def _check_traces(lib, torch, ch, oracles, imp, beta, label):
         assert d <= TOL * max(1.0, r["kappa"] * 1e-5), f"{label} chain {c}: stored root vs Eq. 65 from scratch {d:.3e}"
 
 
+def _gauge_twisted(base):
+    """The same impurity in a basis rotated by a diagonal unitary, |n> -> exp(i theta_n) |n>: every trace is unchanged, every
+    operator block becomes complex.  Gives the small-impurity kernels (sector dimensions <= 16) a complex case."""
+    import types
+    from workloads.rng import Stream
+    rng = Stream(515)
+    dims = np.asarray(base.dims, dtype=np.int64)
+    soff = np.concatenate([[0], np.cumsum(dims)])
+    phase = np.exp(2j * np.pi * np.array([rng.uniform() for _ in range(int(soff[-1]))]))
+    data = np.asarray(base.blk_data, dtype=np.complex128).copy()
+    for b in range(len(base.blk_symbol)):
+        qs, qd = int(base.blk_src[b]), int(base.blk_dst[b])
+        m, n = int(dims[qd]), int(dims[qs])
+        o = int(base.blk_offset[b])
+        blk = data[o:o + m * n].reshape((m, n), order="F")
+        blk *= phase[soff[qd]:soff[qd + 1], None] * np.conj(phase[soff[qs]:soff[qs + 1]])[None, :]
+        data[o:o + m * n] = blk.ravel(order="F")
+    return types.SimpleNamespace(dims=base.dims, energy=base.energy, n_symbols=base.n_symbols, is_complex=True, n_sectors=base.n_sectors,
+                                 beta=base.beta, blk_symbol=base.blk_symbol, blk_src=base.blk_src, blk_dst=base.blk_dst,
+                                 blk_offset=base.blk_offset, blk_data=data)
+
+
+def _real_part(base):
+    """Config 4's sectors and routing with the real parts of its operator blocks: not a physical impurity, but a real-valued
+    block-sparse operator set with sectors of up to 295 states -- the tiled chain-set kernels in real arithmetic.  (Config 3 in its
+    N-only basis would be the natural case, but fp64 does not determine its node norms to better than 1e-3: reading A8 (ii).)"""
+    import types
+    return types.SimpleNamespace(dims=base.dims, energy=base.energy, n_symbols=base.n_symbols, is_complex=False, n_sectors=base.n_sectors,
+                                 beta=base.beta, blk_symbol=base.blk_symbol, blk_src=base.blk_src, blk_dst=base.blk_dst,
+                                 blk_offset=base.blk_offset, blk_data=np.ascontiguousarray(np.asarray(base.blk_data).real, dtype=np.float64))
+
+
+# kernel families behind the cases: configs 1, 2 and 3 (fine sectors, 16 states at most) take the warp-per-task kernels, real;
+# "2twist" the same kernels, complex; config 4 the tiled kernels, complex; "4real" the tiled kernels, real
 @pytest.mark.parametrize("cfg,depth,n_chains,n_steps,lazy_rounds", [(1, 3, 6, 10, 1), (2, 5, 5, 8, 2), (2, 4, 3, 5, 0), (3, 4, 2, 4, 1),
-                                                                      (4, 3, 2, 7, 2)])
+                                                                      (4, 3, 2, 7, 2), ("2twist", 4, 3, 6, 1), ("4real", 3, 2, 5, 1)])
 def test_chains_follow_the_lazy_oracle(lib, torch_cuda, impurities, cfg, depth, n_chains, n_steps, lazy_rounds):
     from oracle import lazy_oracle as LZ
     from workloads import make_batch
     from workloads.rng import Stream
     torch = torch_cuda
-    imp = _imp_for(impurities, cfg)
+    if cfg == "2twist":
+        cfg, imp = 2, _gauge_twisted(impurities(2))
+    elif cfg == "4real":
+        cfg, imp = 4, _real_part(impurities(4))
+    else:
+        imp = _imp_for(impurities, cfg)
     beta = imp.beta
     h = lib.ctqmc_load_impurity(imp, 0)
     ch = None
