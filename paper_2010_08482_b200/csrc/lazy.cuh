@@ -55,7 +55,8 @@ struct LazyView {
   // CTAs that walk a compact list, so a step in which few chains (or none) have work costs a few microseconds instead of one
   // CTA per candidate.  Leaf lists rotate over three buffers (step j reads j % 3, the fix of step j fills (j + 1) % 3, the
   // step kernel clears (j + 2) % 3), node lists over two (parity of the host's launch sequence number).
-  int* w_cnt;                                                // [0..2] leaf tasks, [3..5] leaf tiles, [6..7] node tasks, [8..9] node tiles
+  int* w_cnt;                                                // [0..2] leaf tasks, [3..5] leaf tiles, [6..7] node tasks, [8..9] node tiles,
+                                                             // [10..12] / [13..14] next tile to hand out (leaf / node product kernels)
   int4* w_ltask; int4* w_ltile; int4* w_ntask; int4* w_ntile;
   int* w_larr; int* w_narr; double* w_part;                  // tiles of a task that have been rescaled; their partial sums of squares
   long long w_task_cap, w_tile_cap;                          // entries per buffer
@@ -159,8 +160,8 @@ __device__ inline int lz_block_max(int v, int* red) {
 // The largest binary exponent of the tile's non-zero results (plus the row exponent of the propagator) goes to *kmax_out.
 template <bool CPLX>
 struct LzSmem {
-  double A[CPLX ? 2 : 1][kLzTile][kLzKC + 1];
-  double B[CPLX ? 2 : 1][kLzTile][kLzKC + 1];
+  double A[CPLX ? 2 : 1][kLzTile][kLzKC + 4];   // row stride 20 doubles: the 16 lanes of a half-warp (rows g..g+3, k..k+3) hit 16 different banks
+  double B[CPLX ? 2 : 1][kLzTile][kLzKC + 4];
   double rowm[kLzTile];
   int rowk[kLzTile];
 };
@@ -446,7 +447,7 @@ __global__ void lazy_prepare_kernel(LazyView V, LazyEdits E, const double* log2_
       V.sh_n[(size_t)c * V.emax + k] = cnt;
     }
     if (status != 0) nl = 0;
-    if (c == 0) for (int i = 0; i < 6; ++i) V.w_cnt[i] = 0;      // leaf work lists of this proposal start empty
+    if (c == 0) for (int i = 0; i < 6; ++i) { V.w_cnt[i] = 0; if (i < 3) V.w_cnt[10 + i] = 0; }      // leaf work lists of this proposal start empty
     total = nl;
     for (int i = 0; i < nl; ++i) pn[i] += V.nleaf - 1;
     {
@@ -559,11 +560,16 @@ template <bool CPLX>
 __global__ void __launch_bounds__(kLzThreads) lazy_leaf_step_kernel(LazyView V, int j) {
   __shared__ LzSmem<CPLX> S;
   const int cur = j % 3, nxt2 = (j + 2) % 3;
-  if (blockIdx.x == 0 && threadIdx.x == 0) { V.w_cnt[nxt2] = 0; V.w_cnt[3 + nxt2] = 0; }
+  __shared__ int s_it;
+  if (blockIdx.x == 0 && threadIdx.x == 0) { V.w_cnt[nxt2] = 0; V.w_cnt[3 + nxt2] = 0; V.w_cnt[10 + nxt2] = 0; }
   const int n_items = V.w_cnt[3 + cur];
   const int4* tiles = V.w_ltile + (size_t)cur * V.w_tile_cap;
   const int4* tasks = V.w_ltask + (size_t)cur * V.w_task_cap;
-  for (int it = blockIdx.x; it < n_items; it += gridDim.x) {
+  for (;;) {                                                   // tiles differ in contraction length: handed out one by one
+    if (threadIdx.x == 0) s_it = atomicAdd(&V.w_cnt[10 + cur], 1);
+    __syncthreads();
+    const int it = s_it;
+    if (it >= n_items) break;
     const int4 tl = tiles[it];
     const LzLeafStep st = lz_leaf_step(V, tasks[tl.x], j);
     const BlkDesc bd = V.imp.blks[st.blk];
@@ -719,13 +725,18 @@ __global__ void lazy_node_plan_kernel(LazyView V, int level, int mode, int r, co
 template <bool CPLX>
 __global__ void __launch_bounds__(kLzThreads) lazy_node_gemm_kernel(LazyView V, int par) {
   __shared__ LzSmem<CPLX> S;
-  if (blockIdx.x == 0 && threadIdx.x == 0) { V.w_cnt[6 + (par ^ 1)] = 0; V.w_cnt[8 + (par ^ 1)] = 0; }
+  __shared__ int s_it;
+  if (blockIdx.x == 0 && threadIdx.x == 0) { V.w_cnt[6 + (par ^ 1)] = 0; V.w_cnt[8 + (par ^ 1)] = 0; V.w_cnt[13 + (par ^ 1)] = 0; }
   const int n_items = V.w_cnt[8 + par];
   const int4* tiles = V.w_ntile + (size_t)par * V.w_tile_cap;
   const int4* tasks = V.w_ntask + (size_t)par * V.w_task_cap * 2;
   LzDiag dg; dg.delta = 0.0; dg.E = nullptr; dg.emin = 0.0; dg.kmax = 0;
   LzRowScale rs; rs.on = 0; rs.delta = 0.0; rs.E = nullptr; rs.emin = 0.0;
-  for (int it = blockIdx.x; it < n_items; it += gridDim.x) {
+  for (;;) {
+    if (threadIdx.x == 0) s_it = atomicAdd(&V.w_cnt[13 + par], 1);
+    __syncthreads();
+    const int it = s_it;
+    if (it >= n_items) break;
     const int4 tl = tiles[it];
     const int4 t0 = tasks[2 * tl.x], t1 = tasks[2 * tl.x + 1];      // {c, slot, qin, sl}, {sr, mid, tq}
     lz_gemm_tile<CPLX>(S, tl.y, tl.z, V.imp.dim[t1.z], V.imp.dim[t0.z], V.imp.dim[t1.y], lz_mat(V, t0.x, t1.x, t1.y), 1, V.ldm,
