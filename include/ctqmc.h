@@ -311,6 +311,22 @@ int64_t ctqmc_density_size(const ctqmc_impurity* imp);
 int ctqmc_density_batch(ctqmc_impurity* imp, double beta, const ctqmc_batch* batch, const double* w_mant, const int64_t* w_exp2,
                         const int32_t* status, const double* weight, double* rho, void* cuda_stream);
 
+/* ctqmc_density_batch for callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses
+ * that forbid it): same arguments, same arithmetic, same kernel, but the per-string scratch lives in a file-scope device array
+ * of ctqmc_density_static_limit() = 64 MiB bytes (every GPU that loads the library holds it until the process exits) instead of
+ * the handle's arena.  The call allocates and frees nothing on the device and only enqueues on `cuda_stream`.
+ *   - A string needs (max_len + 5) * d_max^2 elements (x2 complex) + 2 * (max_len + 2) words of scratch; if that exceeds the
+ *     limit the call returns CTQMC_ERR_UNSUPPORTED and enqueues nothing (config 2 at max_len 300: 0.2 MB per string; config 4
+ *     does not fit -- use ctqmc_density_batch).  Fewer strings in flight than ctqmc_density_batch when the array is the limit.
+ *   - The first call on a device resolves the array's device address (cudaGetSymbolAddress, once per device): make that call
+ *     outside a graph capture.
+ *   - Every call on a device shares the ONE array, which keeps the last call's contents (nothing in it has to start at zero:
+ *     a string only reads what it has written).  Calls that overlap on the GPU -- different streams, or this call concurrent
+ *     with itself from two host threads -- RACE on it; order them on one stream or with events. */
+int64_t ctqmc_density_static_limit(void);
+int ctqmc_density_batch_static(ctqmc_impurity* imp, double beta, const ctqmc_batch* batch, const double* w_mant, const int64_t* w_exp2,
+                               const int32_t* status, const double* weight, double* rho, void* cuda_stream);
+
 /* Thread-local description of the last error on this thread ("" if none). */
 const char* ctqmc_last_error(void);
 

@@ -26,7 +26,7 @@ CTQMC_CHAIN_OK, CTQMC_CHAIN_BAD_EDIT, CTQMC_CHAIN_NOT_FOUND, CTQMC_CHAIN_LEAF_FU
 EXPORTS = ["ctqmc_load_impurity", "ctqmc_free_impurity", "ctqmc_set_option", "ctqmc_trace_batch", "ctqmc_bound_batch",
            "ctqmc_trace_batch_host", "ctqmc_bound_batch_host", "ctqmc_last_stats", "ctqmc_last_timing", "ctqmc_measure_fp64_peak", "ctqmc_last_error",
            "ctqmc_chains_create", "ctqmc_chains_destroy", "ctqmc_chains_propose", "ctqmc_chains_commit", "ctqmc_chains_trace",
-           "ctqmc_chains_stats", "ctqmc_density_size", "ctqmc_density_batch"]
+           "ctqmc_chains_stats", "ctqmc_density_size", "ctqmc_density_batch", "ctqmc_density_static_limit", "ctqmc_density_batch_static"]
 
 
 class CtqmcError(RuntimeError):
@@ -105,6 +105,10 @@ def library() -> C.CDLL:
         lib.ctqmc_density_size.restype = i64
         lib.ctqmc_density_batch.argtypes = [vp, dbl, C.POINTER(_Batch), vp, vp, vp, vp, vp, vp]
         lib.ctqmc_density_batch.restype = C.c_int
+        lib.ctqmc_density_static_limit.argtypes = []
+        lib.ctqmc_density_static_limit.restype = i64
+        lib.ctqmc_density_batch_static.argtypes = [vp, dbl, C.POINTER(_Batch), vp, vp, vp, vp, vp, vp]
+        lib.ctqmc_density_batch_static.restype = C.c_int
         _lib = lib
     return _lib
 
@@ -408,4 +412,25 @@ def ctqmc_density_batch(imp: ImpurityHandle, beta: float, offset, symbol, tau, w
     b = _dev_batch(offset, symbol, tau, max_len)
     _check(library().ctqmc_density_batch(imp.ptr, float(beta), C.byref(b), w_mant.data_ptr(), w_exp2.data_ptr(), status.data_ptr(),
                                          weight.data_ptr() if weight is not None else None, rho.data_ptr(), _stream_ptr(stream)))
+    return rho
+
+
+def ctqmc_density_static_limit() -> int:
+    return int(library().ctqmc_density_static_limit())
+
+
+def ctqmc_density_batch_static(imp: ImpurityHandle, beta: float, offset, symbol, tau, w_mant, w_exp2, status, rho, weight=None,
+                               stream=None, max_len=None):
+    """ctqmc_density_batch with its scratch in the library's fixed device array (no cudaMalloc / cudaFree; include/ctqmc.h).
+    Nothing is created here either: `rho` is the caller's (zeroed before the first call).  Raises CtqmcError
+    (CTQMC_ERR_UNSUPPORTED) when one string's prefix products exceed ctqmc_density_static_limit() bytes."""
+    import torch
+    n = ctqmc_density_size(imp) * (2 if imp.is_complex else 1)
+    assert rho.is_cuda and rho.dtype == torch.float64 and rho.numel() == n and rho.is_contiguous()
+    assert w_mant.dtype == torch.float64 and w_exp2.dtype == torch.int64 and status.dtype == torch.int32
+    if weight is not None:
+        assert weight.is_cuda and weight.dtype == torch.float64 and weight.numel() == offset.numel() - 1
+    b = _dev_batch(offset, symbol, tau, max_len)
+    _check(library().ctqmc_density_batch_static(imp.ptr, float(beta), C.byref(b), w_mant.data_ptr(), w_exp2.data_ptr(), status.data_ptr(),
+                                                weight.data_ptr() if weight is not None else None, rho.data_ptr(), _stream_ptr(stream)))
     return rho

@@ -1430,3 +1430,4 @@ extern "C" const char* ctqmc_last_error(void) { return g_err.c_str(); }
 
 #include "lazy_api.cuh"
 #include "density_api.cuh"
+#include "density_static_api.cuh"
