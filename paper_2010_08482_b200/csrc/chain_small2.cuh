@@ -4,6 +4,9 @@
 //     zeros, stored TRANSPOSED in shared memory, so a chain step is the same fully unrolled DP-term dot product for every
 //     string whatever sectors it is in -- no data-dependent loop bounds, no index arithmetic;
 //   * a group of DP lanes owns one configuration (lane = row of the carried matrix), 32/DP configurations per warp.
+//   * small batches (P.split): the whole warp owns ONE configuration -- its 32/DP groups share validation and routing (start
+//     sectors dealt over all lanes) and take the surviving start sectors' chains round-robin, so the latency of a launch is that of
+//     a third (DP = 9) or an eighth (DP = 4) of one configuration's chains instead of all of them.
 // Padded rows carry exact zeros (their operator rows are zero), so results are those of the unpadded product.
 #pragma once
 #include <climits>
@@ -19,6 +22,7 @@ struct Small2Params {
   const int2* binfo;        // [n_blocks] {dst sector, rows << 16 | cols}
   int n_blocks;
   int literal;
+  int split;                // 1: one warp per configuration (small batches), 0: one group of DP lanes per configuration
   double* mant; long long* exp2; uint8_t* survive; int* status;
   Counters* cnt;
 };
@@ -60,11 +64,18 @@ __global__ void __launch_bounds__(512) small2_trace_kernel(Small2Params P) {
   const int lg = lane - grp * DP;
   const unsigned mask = (DP == 32 ? 0xffffffffu : ((1u << DP) - 1u)) << (grp * DP);
   const int grp_in_cta = (threadIdx.x >> 5) * GPW + grp;
-  const int groups_per_cta = (blockDim.x >> 5) * GPW;
   const size_t gbytes = small2_group_bytes(Q, DP);
   double* Xa = reinterpret_cast<double*>(s_groups + (size_t)grp_in_cta * gbytes);
   double* Xb = Xa + DP * DP;
-  double* t_re = Xb + DP * DP;
+  // the lanes that share a configuration: this group, or (split) every group of the warp; the per-configuration tables then live
+  // in the shared-memory region of the warp's first group
+  const bool split = P.split != 0;
+  const int sub = split ? grp : 0, nsub = split ? GPW : 1;
+  const int cl = sub * DP + lg, ncl = nsub * DP;
+  const unsigned cmask = split ? ((GPW * DP == 32) ? 0xffffffffu : ((1u << (GPW * DP)) - 1u)) : mask;
+  const int slot_in_cta = split ? (int)(threadIdx.x >> 5) : grp_in_cta;
+  const int groups_per_cta = split ? (int)(blockDim.x >> 5) : (int)(blockDim.x >> 5) * GPW;      // configurations in flight per CTA
+  double* t_re = reinterpret_cast<double*>(s_groups + (size_t)(split ? (threadIdx.x >> 5) * GPW : grp_in_cta) * gbytes) + 2 * DP * DP;
   double* t_lg = t_re + Q;
   long long* t_e = reinterpret_cast<long long*>(t_lg + Q);
   int* s_c = reinterpret_cast<int*>(t_e + Q);
@@ -74,7 +85,7 @@ __global__ void __launch_bounds__(512) small2_trace_kernel(Small2Params P) {
 
   const long long n_groups = (long long)gridDim.x * groups_per_cta;
   unsigned long long st_strings = 0, st_flops = 0, st_exp = 0, st_pmacs = 0;
-  for (long long b = (long long)blockIdx.x * groups_per_cta + grp_in_cta; b < P.bv.B; b += n_groups) {
+  for (long long b = (long long)blockIdx.x * groups_per_cta + slot_in_cta; b < P.bv.B; b += n_groups) {
     const long long lo = P.bv.offset[b];
     const long long hi_off = P.bv.offset[b + 1];
     const bool off_ok = lo >= 0 && hi_off >= lo && hi_off <= P.bv.n_ops && hi_off - lo <= (long long)P.bv.max_len;
@@ -85,25 +96,25 @@ __global__ void __launch_bounds__(512) small2_trace_kernel(Small2Params P) {
 
     // ---- validation (reading A7)
     bool ok = off_ok;
-    for (int i = lg; i < L; i += DP) {
+    for (int i = cl; i < L; i += ncl) {
       const int a = __ldg(sym + i);
       const double t = __ldg(tau + i);
       const double prev = i ? __ldg(tau + i - 1) : 0.0;
       ok = ok && (a >= 0) && (a < A) && (t >= prev) && (t < beta);
     }
-    ok = __all_sync(mask, ok);
+    ok = __all_sync(cmask, ok);
     if (!ok) {
-      if (lg == 0) {
+      if (cl == 0) {
         const double nan = __longlong_as_double(0x7ff8000000000000LL);
         P.mant[2 * b] = nan; P.mant[2 * b + 1] = nan; P.exp2[b] = 0; P.status[b] = 2;
       }
-      if (P.survive) for (int q0 = lg; q0 < Q; q0 += DP) P.survive[b * Q + q0] = 0;
+      if (P.survive) for (int q0 = cl; q0 < Q; q0 += ncl) P.survive[b * Q + q0] = 0;
       continue;
     }
 
     // ---- routing (a2): start sectors dealt to the lanes of the group
     bool any_surv = false;
-    for (int q0 = lg; q0 < Q; q0 += DP) {
+    for (int q0 = cl; q0 < Q; q0 += ncl) {
       int q = q0, dmin = s_dim[q0], rpos = 0, qmin = q0;
       double lgv = 0.0;
       bool alive = true;
@@ -140,18 +151,18 @@ __global__ void __launch_bounds__(512) small2_trace_kernel(Small2Params P) {
       if (P.survive) P.survive[b * Q + q0] = alive ? 1 : 0;
       any_surv = any_surv || alive;
     }
-    any_surv = __any_sync(mask, any_surv);
-    __syncwarp(mask);
-    if (lg == 0) {   // compact list of the start sectors that have a chain: every group of the warp then runs its
+    any_surv = __any_sync(cmask, any_surv);
+    __syncwarp(cmask);
+    if (cl == 0) {   // compact list of the start sectors that have a chain: every group of the warp then runs its
       int ns = 0;    // si-th chain at the same time (a `continue` over q0 would serialise the groups of a warp)
       for (int q0 = 0; q0 < Q; ++q0) if (s_c[q0] > 0) s_sv[ns++] = q0;
       s_sv[Q] = ns;
     }
-    __syncwarp(mask);
+    __syncwarp(cmask);
     const int n_chain = s_sv[Q];
 
     // ---- chains of the surviving start sectors (a3, a4, a5)
-    for (int si = 0; si < n_chain; ++si) {
+    for (int si = sub; si < n_chain; si += nsub) {
       const int q0 = s_sv[si];
       const int c = s_c[q0];
       int q = s_qs[q0];
@@ -226,10 +237,10 @@ __global__ void __launch_bounds__(512) small2_trace_kernel(Small2Params P) {
       }
       if (lg == 0) { t_re[q0] = dead ? 0.0 : tr; t_e[q0] = dead ? 0 : e2; }
     }
-    __syncwarp(mask);
+    __syncwarp(cmask);
 
     // ---- sector sum with exponent alignment (a5): q0 ascending, Neumaier-compensated, normalised to [1, 2)
-    if (lg == 0) {
+    if (cl == 0) {
       bool any_nz = false;
       long long emax = 0;
       for (int q0 = 0; q0 < Q; ++q0) {
@@ -262,7 +273,7 @@ __global__ void __launch_bounds__(512) small2_trace_kernel(Small2Params P) {
       }
       P.status[b] = any_surv ? 0 : 1;
     }
-    __syncwarp(mask);
+    __syncwarp(cmask);
   }
   if (lg == 0 && st_strings) {
     atomicAdd(&P.cnt->n_strings, st_strings);

@@ -1022,14 +1022,19 @@ extern "C" int ctqmc_trace_batch(ctqmc_impurity* h, double beta, const ctqmc_bat
       s2.mant = mant; s2.exp2 = (long long*)exp2; s2.survive = survive; s2.status = status; s2.cnt = a.cnt_total;
       // CTA size: small batches are latency-bound, so they are spread over all SMs in ONE wave: warps per CTA =
       // ceil(configurations per SM / configurations per warp), at most the configured maximum
-      const int gpw = 32 / h->small2_dp, max_warps = h->small2_threads / 32;
+      // small batches: one WARP per configuration (its groups share the start sectors) while every configuration still gets a
+      // resident warp of its own (with two rounds of warps the gain is gone: measured on config 2 at 4096, 0.273 against 0.227 ms)
+      const int max_warps = h->small2_threads / 32;
+      s2.split = (32 / h->small2_dp > 1 && B <= (long long)h->sm_count * max_warps) ? 1 : 0;
+      const int gpw = s2.split ? 1 : 32 / h->small2_dp;
       long long per_sm = (B + h->sm_count - 1) / h->sm_count;
       int warps = (int)((per_sm + gpw - 1) / gpw);
       if (warps < 2) warps = 2;
       if (warps > max_warps) warps = max_warps;
       const int threads = 32 * warps;
       const long long gpc = (long long)warps * gpw;
-      const size_t smem = small2_common_bytes(h->dev.Q, h->dev.A, h->n_blocks, h->small2_dp) + (size_t)gpc * small2_group_bytes(h->dev.Q, h->small2_dp);
+      const size_t smem = small2_common_bytes(h->dev.Q, h->dev.A, h->n_blocks, h->small2_dp) +
+                          (size_t)warps * (32 / h->small2_dp) * small2_group_bytes(h->dev.Q, h->small2_dp);
       if (h->small2_occ[warps] == 0) {
         int occ = 0;
         CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, pick_small2(h->small2_dp), threads, smem));
