@@ -37,6 +37,12 @@ __host__ __device__ inline size_t small2_group_bytes(int Q, int DP) {
   return (b + 15) / 16 * 16;
 }
 
+// split mode: per warp, the carried matrices of its 32/DP groups and ONE set of per-configuration tables
+__host__ __device__ inline size_t small2_warp_bytes(int Q, int DP) {
+  size_t b = (size_t)(32 / DP) * 2 * DP * DP * 8 + (size_t)Q * (8 * 3) + (size_t)Q * 4 * 4 + 16;
+  return (b + 15) / 16 * 16;
+}
+
 template <int DP>
 __global__ void __launch_bounds__(512) small2_trace_kernel(Small2Params P) {
   constexpr int GPW = 32 / DP;                       // groups (configurations) per warp
@@ -49,7 +55,15 @@ __global__ void __launch_bounds__(512) small2_trace_kernel(Small2Params P) {
   int* s_dim = reinterpret_cast<int*>(s_binfo + nb);
   short* s_blkof = reinterpret_cast<short*>(s_dim + Q);
   unsigned char* s_groups = ssm2 + small2_common_bytes(Q, A, nb, DP);
-  for (int i = threadIdx.x; i < nb * DP * DP; i += blockDim.x) s_ft[i] = P.ftpad[i];
+  // operator store -> shared memory, 8 loads in flight per thread (a plain copy loop waits for every load before the next one:
+  // 90 us of a 64-thread CTA's launch on config 2, cold L2)
+  for (int i0 = threadIdx.x; i0 < nb * DP * DP; i0 += 8 * blockDim.x) {
+    double v[8];
+#pragma unroll
+    for (int u = 0; u < 8; ++u) { const int i = i0 + u * blockDim.x; v[u] = i < nb * DP * DP ? __ldg(P.ftpad + i) : 0.0; }
+#pragma unroll
+    for (int u = 0; u < 8; ++u) { const int i = i0 + u * blockDim.x; if (i < nb * DP * DP) s_ft[i] = v[u]; }
+  }
   for (int i = threadIdx.x; i < Q * DP; i += blockDim.x) {
     const int q = i / DP, r = i - q * DP;
     s_de[i] = (r < P.imp.dim[q]) ? __dsub_rn(P.imp.energy[P.imp.e_off[q] + r], P.imp.e_min[q]) : 0.0;
@@ -65,17 +79,20 @@ __global__ void __launch_bounds__(512) small2_trace_kernel(Small2Params P) {
   const unsigned mask = (DP == 32 ? 0xffffffffu : ((1u << DP) - 1u)) << (grp * DP);
   const int grp_in_cta = (threadIdx.x >> 5) * GPW + grp;
   const size_t gbytes = small2_group_bytes(Q, DP);
-  double* Xa = reinterpret_cast<double*>(s_groups + (size_t)grp_in_cta * gbytes);
+  const bool split = P.split != 0;
+  const size_t wbytes = small2_warp_bytes(Q, DP);
+  double* Xa = split ? reinterpret_cast<double*>(s_groups + (size_t)(threadIdx.x >> 5) * wbytes) + (size_t)grp * 2 * DP * DP
+                     : reinterpret_cast<double*>(s_groups + (size_t)grp_in_cta * gbytes);
   double* Xb = Xa + DP * DP;
   // the lanes that share a configuration: this group, or (split) every group of the warp; the per-configuration tables then live
-  // in the shared-memory region of the warp's first group
-  const bool split = P.split != 0;
+  // once per warp (small2_warp_bytes)
   const int sub = split ? grp : 0, nsub = split ? GPW : 1;
   const int cl = sub * DP + lg, ncl = nsub * DP;
   const unsigned cmask = split ? ((GPW * DP == 32) ? 0xffffffffu : ((1u << (GPW * DP)) - 1u)) : mask;
   const int slot_in_cta = split ? (int)(threadIdx.x >> 5) : grp_in_cta;
   const int groups_per_cta = split ? (int)(blockDim.x >> 5) : (int)(blockDim.x >> 5) * GPW;      // configurations in flight per CTA
-  double* t_re = reinterpret_cast<double*>(s_groups + (size_t)(split ? (threadIdx.x >> 5) * GPW : grp_in_cta) * gbytes) + 2 * DP * DP;
+  double* t_re = split ? reinterpret_cast<double*>(s_groups + (size_t)(threadIdx.x >> 5) * wbytes) + (size_t)GPW * 2 * DP * DP
+                       : reinterpret_cast<double*>(s_groups + (size_t)grp_in_cta * gbytes) + 2 * DP * DP;
   double* t_lg = t_re + Q;
   long long* t_e = reinterpret_cast<long long*>(t_lg + Q);
   int* s_c = reinterpret_cast<int*>(t_e + Q);
@@ -112,44 +129,58 @@ __global__ void __launch_bounds__(512) small2_trace_kernel(Small2Params P) {
       continue;
     }
 
-    // ---- routing (a2): start sectors dealt to the lanes of the group
+    // ---- routing (a2): start sectors dealt to the lanes that share the configuration, two independent walks per lane and pass
+    //      (integer only: the exponent of exp(-Delta Emin) is summed by the chain pass, for the strings that have a chain)
     bool any_surv = false;
-    for (int q0 = cl; q0 < Q; q0 += ncl) {
-      int q = q0, dmin = s_dim[q0], rpos = 0, qmin = q0;
-      double lgv = 0.0;
-      bool alive = true;
-      const double t0 = L ? __ldg(tau) : 0.0;
-      double tcur = t0;
-      // operator string one step ahead in registers: the loads overlap the table look-ups of the current step
+    for (int qa0 = cl; qa0 < Q; qa0 += 2 * ncl) {
+      const int qb0 = qa0 + ncl;
+      const bool has_b = qb0 < Q;
+      int qa = qa0, qb = has_b ? qb0 : 0;
+      int dmin_a = s_dim[qa0], dmin_b = s_dim[qb], rpos_a = 0, rpos_b = 0, qmin_a = qa0, qmin_b = qb;
+      bool alive_a = true, alive_b = has_b;
       int sym_nx = L ? __ldg(sym) : 0;
-      double tau_nx = (L > 1) ? __ldg(tau + 1) : 0.0;
       for (int i = 0; i < L; ++i) {
         const int sym_c = sym_nx;
-        const double tau_c1 = tau_nx;
         if (i + 1 < L) sym_nx = __ldg(sym + i + 1);
-        if (i + 2 < L) tau_nx = __ldg(tau + i + 2);
-        const int blk = s_blkof[sym_c * Q + q];
-        if (blk < 0) { alive = false; break; }
-        const int qn = s_binfo[blk].x;
-        const int dn = s_dim[qn];
-        const double tnext = (i + 1 < L) ? tau_c1 : beta + t0;
-        lgv -= (tnext - tcur) * s_emin[qn] * kLog2e;
-        tcur = tnext;
-        if (i + 1 < L && dn < dmin) { dmin = dn; rpos = i + 1; qmin = qn; }
-        q = qn;
-      }
-      if (L == 0) lgv = -beta * s_emin[q0] * kLog2e;
-      int c = -1;
-      if (alive) {
-        c = 0;
-        if (q == q0) {
-          if (P.literal) { c = s_dim[q0]; s_r[q0] = 0; s_qs[q0] = q0; }
-          else { c = dmin; s_r[q0] = rpos; s_qs[q0] = qmin; }
+        if (alive_a) {
+          const int blk = s_blkof[sym_c * Q + qa];
+          if (blk < 0) alive_a = false;
+          else {
+            const int2 bi = s_binfo[blk];
+            const int dn = bi.y >> 16;                        // rows of the block = dimension of its target sector
+            if (i + 1 < L && dn < dmin_a) { dmin_a = dn; rpos_a = i + 1; qmin_a = bi.x; }
+            qa = bi.x;
+          }
         }
+        if (alive_b) {
+          const int blk = s_blkof[sym_c * Q + qb];
+          if (blk < 0) alive_b = false;
+          else {
+            const int2 bi = s_binfo[blk];
+            const int dn = bi.y >> 16;
+            if (i + 1 < L && dn < dmin_b) { dmin_b = dn; rpos_b = i + 1; qmin_b = bi.x; }
+            qb = bi.x;
+          }
+        }
+        if (!alive_a && !alive_b) break;
       }
-      s_c[q0] = c; t_lg[q0] = lgv; t_re[q0] = 0.0; t_e[q0] = 0;
-      if (P.survive) P.survive[b * Q + q0] = alive ? 1 : 0;
-      any_surv = any_surv || alive;
+#pragma unroll
+      for (int w = 0; w < 2; ++w) {
+        if (w == 1 && !has_b) break;
+        const int q0 = w ? qb0 : qa0, q = w ? qb : qa;
+        const bool alive = w ? alive_b : alive_a;
+        int c = -1;
+        if (alive) {
+          c = 0;
+          if (q == q0) {
+            if (P.literal) { c = s_dim[q0]; s_r[q0] = 0; s_qs[q0] = q0; }
+            else { c = w ? dmin_b : dmin_a; s_r[q0] = w ? rpos_b : rpos_a; s_qs[q0] = w ? qmin_b : qmin_a; }
+          }
+        }
+        s_c[q0] = c; t_lg[q0] = 0.0; t_re[q0] = 0.0; t_e[q0] = 0;
+        if (P.survive) P.survive[b * Q + q0] = alive ? 1 : 0;
+        any_surv = any_surv || alive;
+      }
     }
     any_surv = __any_sync(cmask, any_surv);
     __syncwarp(cmask);
@@ -169,11 +200,12 @@ __global__ void __launch_bounds__(512) small2_trace_kernel(Small2Params P) {
       const int r = s_r[q0];
       double* X = Xa;      // X[n * DP + k]: column n of the carried matrix, padded rows are zero
       double* Xn = Xb;
-      double tr = 0.0;
+      double tr = 0.0, lgv = 0.0;
       long long e2 = 0;
       bool dead = false;
       if (L == 0) {        // empty configuration: Tr P_beta(q0) (reading A7)
         if (lg == 0) for (int n = 0; n < c; ++n) tr += exp(-beta * s_de[q * DP + n]);
+        lgv = -beta * s_emin[q0] * kLog2e;
       } else {
         for (int n = 0; n < c; ++n) X[n * DP + lg] = (lg == n) ? 1.0 : 0.0;
         __syncwarp(mask);
@@ -192,6 +224,7 @@ __global__ void __launch_bounds__(512) small2_trace_kernel(Small2Params P) {
           const int2 bi = s_binfo[blk];
           const int qn = bi.x;
           const double delta = wrap ? (beta - ta + tb) : (tb - ta);
+          lgv -= delta * s_emin[qn] * kLog2e;
           // this lane's row of F (transposed store: consecutive lanes read consecutive doubles)
           const double* ft = s_ft + (size_t)blk * (DP * DP) + lg;
           double f[DP];
@@ -235,7 +268,7 @@ __global__ void __launch_bounds__(512) small2_trace_kernel(Small2Params P) {
         }
         __syncwarp(mask);
       }
-      if (lg == 0) { t_re[q0] = dead ? 0.0 : tr; t_e[q0] = dead ? 0 : e2; }
+      if (lg == 0) { t_re[q0] = dead ? 0.0 : tr; t_e[q0] = dead ? 0 : e2; t_lg[q0] = lgv; }
     }
     __syncwarp(cmask);
 

@@ -1034,7 +1034,8 @@ extern "C" int ctqmc_trace_batch(ctqmc_impurity* h, double beta, const ctqmc_bat
       const int threads = 32 * warps;
       const long long gpc = (long long)warps * gpw;
       const size_t smem = small2_common_bytes(h->dev.Q, h->dev.A, h->n_blocks, h->small2_dp) +
-                          (size_t)warps * (32 / h->small2_dp) * small2_group_bytes(h->dev.Q, h->small2_dp);
+                          (s2.split ? (size_t)warps * small2_warp_bytes(h->dev.Q, h->small2_dp)
+                                    : (size_t)warps * (32 / h->small2_dp) * small2_group_bytes(h->dev.Q, h->small2_dp));
       if (h->small2_occ[warps] == 0) {
         int occ = 0;
         CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, pick_small2(h->small2_dp), threads, smem));
