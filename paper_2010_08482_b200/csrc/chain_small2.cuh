@@ -11,6 +11,7 @@
 #pragma once
 #include <climits>
 
+#include "chain_large.cuh"
 #include "chain_small.cuh"
 
 namespace ctqmc {
@@ -55,14 +56,25 @@ __global__ void __launch_bounds__(512) small2_trace_kernel(Small2Params P) {
   int* s_dim = reinterpret_cast<int*>(s_binfo + nb);
   short* s_blkof = reinterpret_cast<short*>(s_dim + Q);
   unsigned char* s_groups = ssm2 + small2_common_bytes(Q, A, nb, DP);
-  // operator store -> shared memory, 8 loads in flight per thread (a plain copy loop waits for every load before the next one:
-  // 90 us of a 64-thread CTA's launch on config 2, cold L2)
-  for (int i0 = threadIdx.x; i0 < nb * DP * DP; i0 += 8 * blockDim.x) {
-    double v[8];
-#pragma unroll
-    for (int u = 0; u < 8; ++u) { const int i = i0 + u * blockDim.x; v[u] = i < nb * DP * DP ? __ldg(P.ftpad + i) : 0.0; }
-#pragma unroll
-    for (int u = 0; u < 8; ++u) { const int i = i0 + u * blockDim.x; if (i < nb * DP * DP) s_ft[i] = v[u]; }
+  // operator store -> shared memory with 1-D bulk copies (cp.async.bulk) issued by one thread and awaited on an mbarrier: a plain
+  // copy loop waits for every load before the next one (90 us of a 64-thread CTA's launch on config 2 with a cold L2; 8 loads in
+  // flight per thread still left 23 us).  The odd last double, if any, is copied by hand.
+  __shared__ __align__(8) unsigned long long fill_bar;
+  const unsigned ft_bytes = (unsigned)((size_t)nb * DP * DP * 8), ft_bulk = ft_bytes & ~15u;
+  if (threadIdx.x == 0) {
+    mbar_init(&fill_bar, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    if (ft_bulk) {
+      mbar_expect_tx(&fill_bar, ft_bulk);
+      for (unsigned o = 0; o < ft_bulk; o += 32768u) {
+        const unsigned n = ft_bulk - o < 32768u ? ft_bulk - o : 32768u;
+        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                     ::"r"(smem_u32(reinterpret_cast<unsigned char*>(s_ft) + o)), "l"(reinterpret_cast<const unsigned char*>(P.ftpad) + o), "r"(n),
+                       "r"(smem_u32(&fill_bar)) : "memory");
+      }
+    }
+    if (ft_bulk != ft_bytes) s_ft[nb * DP * DP - 1] = P.ftpad[nb * DP * DP - 1];
   }
   for (int i = threadIdx.x; i < Q * DP; i += blockDim.x) {
     const int q = i / DP, r = i - q * DP;
@@ -71,6 +83,8 @@ __global__ void __launch_bounds__(512) small2_trace_kernel(Small2Params P) {
   for (int i = threadIdx.x; i < Q; i += blockDim.x) { s_emin[i] = P.imp.e_min[i]; s_dim[i] = P.imp.dim[i]; }
   for (int i = threadIdx.x; i < nb; i += blockDim.x) s_binfo[i] = P.binfo[i];
   for (int i = threadIdx.x; i < A * Q; i += blockDim.x) s_blkof[i] = (short)P.imp.blk_of[i];
+  __syncthreads();                                   // fill_bar is initialised for everyone
+  if (ft_bulk) mbar_wait(&fill_bar, 0);
   __syncthreads();
 
   const int lane = threadIdx.x & 31, grp = lane / DP;
