@@ -16,6 +16,21 @@
 
 namespace ctqmc {
 
+// 2^f for f in [0, 1] as sqrt(2) exp((f - 1/2) ln 2), Taylor to degree 14 (|(f - 1/2) ln 2| <= 0.347: remainder 5e-18), Horner with
+// the coefficients as constant-bank operands: 16 FP64 instructions.  The library's exp2 costs 45 on this path (range reduction
+// for arbitrary arguments, 22 UMOV re-materialising its constants every step, a special-case branch).
+__constant__ double kExp2Taylor[15] = {1.0, 0.6931471805599453, 0.24022650695910072, 0.05550410866482158, 0.009618129107628477,
+                                       0.0013333558146428443, 0.0001540353039338161, 1.5252733804059841e-05, 1.321548679014431e-06,
+                                       1.01780860092397e-07, 7.054911620801123e-09, 4.4455382718708116e-10, 2.5678435993488206e-11,
+                                       1.3691488853904128e-12, 6.778726354822545e-14};
+__device__ __forceinline__ double exp2_unit(double f) {
+  const double t = f - 0.5;
+  double p = kExp2Taylor[14];
+#pragma unroll
+  for (int k = 13; k >= 0; --k) p = fma(p, t, kExp2Taylor[k]);
+  return p * 1.4142135623730951;
+}
+
 struct Small2Params {
   DevImp imp;
   BatchView bv;
@@ -224,56 +239,100 @@ __global__ void __launch_bounds__(512) small2_trace_kernel(Small2Params P) {
         for (int n = 0; n < c; ++n) X[n * DP + lg] = (lg == n) ? 1.0 : 0.0;
         __syncwarp(mask);
         unsigned long long macs = 0, nexp = 0;
-        int i = r;
-        int sym_nx = __ldg(sym + i);
-        double ta_nx = __ldg(tau + i), tb_nx = __ldg(tau + ((i + 1 < L) ? i + 1 : 0));
-        for (int j = 0; j < L; ++j) {
-          const int sym_c = sym_nx;
-          const double ta = ta_nx, tb = tb_nx;
-          const bool wrap = i + 1 >= L;
-          i = wrap ? 0 : i + 1;
-          sym_nx = __ldg(sym + i);                     // next step's operator, in flight during this step
-          ta_nx = __ldg(tau + i); tb_nx = __ldg(tau + ((i + 1 < L) ? i + 1 : 0));
-          const int blk = s_blkof[sym_c * Q + q];
-          const int2 bi = s_binfo[blk];
-          const int qn = bi.x;
-          const double delta = wrap ? (beta - ta + tb) : (tb - ta);
-          lgv -= delta * s_emin[qn] * kLog2e;
-          // this lane's row of F (transposed store: consecutive lanes read consecutive doubles)
-          const double* ft = s_ft + (size_t)blk * (DP * DP) + lg;
-          double f[DP];
-#pragma unroll
-          for (int k = 0; k < DP; ++k) f[k] = ft[k * DP];
-          // propagator of this row: 2^x = mantissa in [1, 2) times 2^kr  (prop_x with the pre-subtracted energy)
-          const double x = __dmul_rn(__dmul_rn(-delta, s_de[qn * DP + lg]), kLog2e);
-          const double mr = exp2(__dsub_rn(x, floor(x)));
-          const int kr = row_exp(x);
-          int wexp = INT_MIN;
-          for (int n = 0; n < c; ++n) {
-            const double* xs = X + n * DP;
+        // One column (the string passes through a one-state sector: most strings of configs 1 and 2) has a loop of its own -- this
+        // lane's entry stays in a register between the product and the rescale, 32-bit counters, one new tau per step -- taken when
+        // every group that is at this point of the warp together with this one has one column too: groups on different loops would
+        // run one after the other.  Both loops do the same arithmetic in the same order, so the choice never changes a result.
+        const unsigned together = __activemask();
+        if (__all_sync(together, c == 1)) {
+          unsigned macs32 = 0, nexp32 = 0;
+          int cur = r, nx = (r + 1 >= L) ? 0 : r + 1;         // this step's operator and the next one (cyclically)
+          int sym_c = __ldg(sym + cur);
+          double ta = __ldg(tau + cur), tb = __ldg(tau + nx);
+          for (int j = 0; j < L; ++j) {
+            const bool wrap = cur + 1 >= L;
+            const double delta = wrap ? (beta - ta + tb) : (tb - ta);
+            const int nn = (nx + 1 >= L) ? 0 : nx + 1;
+            const int sym_n = __ldg(sym + nx);               // next step's operator, in flight during this step
+            const double tb_n = __ldg(tau + nn);
+            const int blk = s_blkof[sym_c * Q + q];
+            const int2 bi = s_binfo[blk];
+            const int qn = bi.x;
+            lgv -= delta * s_emin[qn] * kLog2e;
+            const double* ft = s_ft + (size_t)blk * (DP * DP) + lg;
             double a0 = 0.0, a1 = 0.0;
 #pragma unroll
-            for (int k = 0; k + 1 < DP; k += 2) { a0 = fma(f[k], xs[k], a0); a1 = fma(f[k + 1], xs[k + 1], a1); }
-            if (DP & 1) a0 = fma(f[DP - 1], xs[DP - 1], a0);
-            const double v = (a0 + a1) * mr;
-            Xn[n * DP + lg] = v;
-            if (v != 0.0) wexp = max(wexp, kr + ilogb_fast(v));
+            for (int k = 0; k + 1 < DP; k += 2) { a0 = fma(ft[k * DP], X[k], a0); a1 = fma(ft[(k + 1) * DP], X[k + 1], a1); }
+            if (DP & 1) a0 = fma(ft[(DP - 1) * DP], X[DP - 1], a0);
+            const double x = __dmul_rn(__dmul_rn(-delta, s_de[qn * DP + lg]), kLog2e);
+            const int kr = row_exp(x);
+            double v = (a0 + a1) * exp2_unit(__dsub_rn(x, floor(x)));
+            const int kmax = __reduce_max_sync(mask, v != 0.0 ? kr + ilogb_fast(v) : INT_MIN);
+            if (kmax == INT_MIN) { dead = true; break; }
+            e2 += kmax;
+            const int sh = kr - kmax;
+            v = (sh > 1022 || sh < -1022) ? scalbn(v, max(sh, -2200)) : v * pow2i(sh);
+            Xn[lg] = v;
+            __syncwarp(mask);
+            double* tmp = X; X = Xn; Xn = tmp;
+            macs32 += (unsigned)(bi.y >> 16) * (unsigned)(bi.y & 0xffff);
+            nexp32 += (unsigned)(bi.y >> 16);
+            q = qn;
+            cur = nx; nx = nn; sym_c = sym_n; ta = tb; tb = tb_n;
           }
-          const int kmax = __reduce_max_sync(mask, wexp);
-          if (kmax == INT_MIN) { dead = true; break; }
-          e2 += kmax;
-          const int sh = kr - kmax;
-          if (sh > 1022 || sh < -1022) {
-            for (int n = 0; n < c; ++n) Xn[n * DP + lg] = scalbn(Xn[n * DP + lg], max(sh, -2200));
-          } else {
-            const double sc = pow2i(sh);
-            for (int n = 0; n < c; ++n) Xn[n * DP + lg] *= sc;
+          macs = macs32; nexp = nexp32;
+        } else {
+          int i = r;
+          int sym_nx = __ldg(sym + i);
+          double ta_nx = __ldg(tau + i), tb_nx = __ldg(tau + ((i + 1 < L) ? i + 1 : 0));
+          for (int j = 0; j < L; ++j) {
+            const int sym_c = sym_nx;
+            const double ta = ta_nx, tb = tb_nx;
+            const bool wrap = i + 1 >= L;
+            i = wrap ? 0 : i + 1;
+            sym_nx = __ldg(sym + i);                     // next step's operator, in flight during this step
+            ta_nx = __ldg(tau + i); tb_nx = __ldg(tau + ((i + 1 < L) ? i + 1 : 0));
+            const int blk = s_blkof[sym_c * Q + q];
+            const int2 bi = s_binfo[blk];
+            const int qn = bi.x;
+            const double delta = wrap ? (beta - ta + tb) : (tb - ta);
+            lgv -= delta * s_emin[qn] * kLog2e;
+            // this lane's row of F (transposed store: consecutive lanes read consecutive doubles)
+            const double* ft = s_ft + (size_t)blk * (DP * DP) + lg;
+            double f[DP];
+  #pragma unroll
+            for (int k = 0; k < DP; ++k) f[k] = ft[k * DP];
+            // propagator of this row: 2^x = mantissa in [1, 2) times 2^kr  (prop_x with the pre-subtracted energy)
+            const double x = __dmul_rn(__dmul_rn(-delta, s_de[qn * DP + lg]), kLog2e);
+            const double mr = exp2_unit(__dsub_rn(x, floor(x)));
+            const int kr = row_exp(x);
+            int wexp = INT_MIN;
+            for (int n = 0; n < c; ++n) {
+              const double* xs = X + n * DP;
+              double a0 = 0.0, a1 = 0.0;
+  #pragma unroll
+              for (int k = 0; k + 1 < DP; k += 2) { a0 = fma(f[k], xs[k], a0); a1 = fma(f[k + 1], xs[k + 1], a1); }
+              if (DP & 1) a0 = fma(f[DP - 1], xs[DP - 1], a0);
+              const double v = (a0 + a1) * mr;
+              Xn[n * DP + lg] = v;
+              if (v != 0.0) wexp = max(wexp, kr + ilogb_fast(v));
+            }
+            const int kmax = __reduce_max_sync(mask, wexp);
+            if (kmax == INT_MIN) { dead = true; break; }
+            e2 += kmax;
+            const int sh = kr - kmax;
+            if (sh > 1022 || sh < -1022) {
+              for (int n = 0; n < c; ++n) Xn[n * DP + lg] = scalbn(Xn[n * DP + lg], max(sh, -2200));
+            } else {
+              const double sc = pow2i(sh);
+              for (int n = 0; n < c; ++n) Xn[n * DP + lg] *= sc;
+            }
+            __syncwarp(mask);
+            double* tmp = X; X = Xn; Xn = tmp;
+            macs += (unsigned long long)(bi.y >> 16) * (unsigned long long)(bi.y & 0xffff);
+            nexp += (unsigned long long)(bi.y >> 16);
+            q = qn;
           }
-          __syncwarp(mask);
-          double* tmp = X; X = Xn; Xn = tmp;
-          macs += (unsigned long long)(bi.y >> 16) * (unsigned long long)(bi.y & 0xffff);
-          nexp += (unsigned long long)(bi.y >> 16);
-          q = qn;
         }
         if (lg == 0) {
           if (!dead) for (int n = 0; n < c; ++n) tr += X[n * DP + n];
