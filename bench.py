@@ -569,7 +569,7 @@ def run_ours(args, rank: int, world: int, local_rank: int):
                                     "cfg4": measure_chains(L, torch, 4, 16, 4, 4, local_rank, leaf_capacity=64)}
         next_rows["split_precision"] = measure_split(L, torch, 64, 3, local_rank, pk)
         next_rows["density"] = {"cfg2": measure_density(L, torch, 2, 4096, 3, local_rank),
-                                "cfg4": measure_density(L, torch, 4, 16, 2, local_rank)}
+                                "cfg4": measure_density(L, torch, 4, 64, 2, local_rank)}
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()

@@ -321,7 +321,8 @@ int ctqmc_density_batch(ctqmc_impurity* imp, double beta, const ctqmc_batch* bat
  *   - The first call on a device resolves the array's device address (cudaGetSymbolAddress, once per device): make that call
  *     outside a graph capture.
  *   - Every call on a device shares the ONE array, which keeps the last call's contents (nothing in it has to start at zero:
- *     a string only reads what it has written).  Calls that overlap on the GPU -- different streams, or this call concurrent
+ *     a string only reads what it has written; the kernel's work counter, a second static word, is zeroed by every call on
+ *     its stream).  Calls that overlap on the GPU -- different streams, or this call concurrent
  *     with itself from two host threads -- RACE on it; order them on one stream or with events. */
 int64_t ctqmc_density_static_limit(void);
 int ctqmc_density_batch_static(ctqmc_impurity* imp, double beta, const ctqmc_batch* batch, const double* w_mant, const int64_t* w_exp2,

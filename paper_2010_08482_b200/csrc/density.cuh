@@ -27,6 +27,7 @@ struct DensityParams {
   long long slot_doubles;
   int ldm;                       // leading dimension of every scratch matrix (= d_max)
   int Lcap;                      // steps a slot can hold (= max_len)
+  int* work;                     // next (configuration, start sector) candidate to hand out; zeroed before the launch
 };
 
 __host__ __device__ inline long long density_slot_doubles(int dmax, int Lcap, int es) {
@@ -110,7 +111,15 @@ __global__ void __launch_bounds__(kLzThreads) density_kernel(DensityParams P) {
   long long* eG = reinterpret_cast<long long*>(Cb + mat);          // [Lcap + 1]
   int* qs = reinterpret_cast<int*>(eG + P.Lcap + 1);               // [Lcap + 1] sectors q_0 .. q_L
   const long long nS = P.bv.B * Q;
-  for (long long s = blockIdx.x; s < nS; s += gridDim.x) {
+  __shared__ int s_next;
+  // candidates are handed out one by one: few of them survive and close, and the survivors differ in length by an order of
+  // magnitude -- with a fixed stride the SMs were busy a third of the launch (config 4, profiles/r02_density.md)
+  for (;;) {
+    __syncthreads();
+    if (threadIdx.x == 0) s_next = atomicAdd(P.work, 1);
+    __syncthreads();
+    const long long s = s_next;
+    if (s >= nS) break;
     const long long b = s / Q;
     const int q0 = (int)(s - b * Q);
     if (P.status[b] != 0) continue;

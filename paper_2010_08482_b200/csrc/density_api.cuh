@@ -48,6 +48,8 @@ extern "C" int ctqmc_density_batch(ctqmc_impurity* h, double beta, const ctqmc_b
   dp.imp = h->dev; dp.bv = make_view(batch, beta, 0, B, Lcap); dp.w_mant = w_mant; dp.w_exp2 = (const long long*)w_exp2; dp.status = status;
   dp.weight = weight; dp.rho = rho; dp.rho_off = h->d_rho_off; dp.scratch = (double*)a.base; dp.slot_doubles = (long long)(slot_bytes / sizeof(double));
   dp.ldm = h->dev.dmax; dp.Lcap = Lcap;
+  dp.work = reinterpret_cast<int*>(a.base + (size_t)grid * slot_bytes);        // the 256 spare bytes behind the slots
+  CU(cudaMemsetAsync(dp.work, 0, sizeof(int), st));
   if (h->dev.cplx) density_kernel<true><<<(unsigned)grid, kLzThreads, 0, st>>>(dp);
   else             density_kernel<false><<<(unsigned)grid, kLzThreads, 0, st>>>(dp);
   h->last_stream = st; h->last_launches = 1;

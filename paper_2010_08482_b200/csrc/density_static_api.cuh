@@ -10,16 +10,18 @@
 namespace ctqmc {
 constexpr size_t kDensityStaticBytes = 64ull << 20;       // 64 MiB per GPU that loads the library, held until the process exits
 static __device__ __align__(256) double g_density_static_scratch[kDensityStaticBytes / sizeof(double)];
+static __device__ int g_density_static_work;              // the kernel's work counter (zeroed by every call, on its stream)
 }  // namespace ctqmc
 
 namespace {
 constexpr int kStaticMaxDevices = 64;
 double* g_density_static_ptr[kStaticMaxDevices] = {};
+int* g_density_static_work_ptr[kStaticMaxDevices] = {};
 std::mutex g_density_static_mu;
 
 // Device address of the array on `device` (which must be current).  In host code the array's name is only a stand-in for the
 // symbol, not an address a kernel can use: resolved once per device with cudaGetSymbolAddress.
-int density_static_address(int device, double** out) {
+int density_static_address(int device, double** out, int** work) {
   if (device < 0 || device >= kStaticMaxDevices) return fail(CTQMC_ERR_ARG, "device ordinal %d out of range for the static scratch table", device);
   std::lock_guard<std::mutex> lock(g_density_static_mu);
   if (!g_density_static_ptr[device]) {
@@ -29,9 +31,16 @@ int density_static_address(int device, double** out) {
       cudaGetLastError();
       return fail(CTQMC_ERR_CUDA, "cudaGetSymbolAddress(static density scratch) on device %d: %s", device, cudaGetErrorString(e));
     }
+    void* w = nullptr;
+    e = cudaGetSymbolAddress(&w, g_density_static_work);
+    if (e != cudaSuccess || !w) {
+      cudaGetLastError();
+      return fail(CTQMC_ERR_CUDA, "cudaGetSymbolAddress(static density work counter) on device %d: %s", device, cudaGetErrorString(e));
+    }
+    g_density_static_work_ptr[device] = (int*)w;
     g_density_static_ptr[device] = (double*)p;
   }
-  *out = g_density_static_ptr[device];
+  *out = g_density_static_ptr[device]; *work = g_density_static_work_ptr[device];
   return 0;
 }
 }  // namespace
@@ -58,20 +67,22 @@ extern "C" int ctqmc_density_batch_static(ctqmc_impurity* h, double beta, const 
                 "use ctqmc_density_batch", Lcap, h->dev.dmax, slot_bytes, kDensityStaticBytes);
   CU(cudaSetDevice(h->device));
   double* scratch = nullptr;
-  rc = density_static_address(h->device, &scratch);
+  int* work = nullptr;
+  rc = density_static_address(h->device, &scratch, &work);
   if (rc) return rc;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   long long grid = 2LL * h->sm_count;
   const long long nS = B * h->dev.Q, fit = (long long)(kDensityStaticBytes / slot_bytes);
   if (grid > nS) grid = nS;
   if (grid > fit) grid = fit;
-  // Nothing in the scratch has to start at zero: every element a string reads (prefix products, carried matrices, exponent and
+  // Nothing in the scratch itself has to start at zero: every element a string reads (prefix products, carried matrices, exponent and
   // sector tables of its slot) it has written before, and the product tiles are bounds-guarded.  The array keeps the last
   // call's contents; two calls that overlap on the GPU (different streams) would share slots and race.
   DensityParams dp;
   dp.imp = h->dev; dp.bv = make_view(batch, beta, 0, B, Lcap); dp.w_mant = w_mant; dp.w_exp2 = (const long long*)w_exp2; dp.status = status;
   dp.weight = weight; dp.rho = rho; dp.rho_off = h->d_rho_off; dp.scratch = scratch; dp.slot_doubles = (long long)(slot_bytes / sizeof(double));
-  dp.ldm = h->dev.dmax; dp.Lcap = Lcap;
+  dp.ldm = h->dev.dmax; dp.Lcap = Lcap; dp.work = work;
+  CU(cudaMemsetAsync(work, 0, sizeof(int), st));          // the one word that must start at zero
   if (h->dev.cplx) density_kernel<true><<<(unsigned)grid, kLzThreads, 0, st>>>(dp);
   else             density_kernel<false><<<(unsigned)grid, kLzThreads, 0, st>>>(dp);
   h->last_stream = st; h->last_launches = 1;
