@@ -16,6 +16,8 @@
 
 namespace ctqmc {
 
+constexpr int kDnMaxQ = 1024;      // sectors the hand-out order is built for (more: configuration-major order)
+
 struct DensityParams {
   DevImp imp;
   BatchView bv;
@@ -112,6 +114,18 @@ __global__ void __launch_bounds__(kLzThreads) density_kernel(DensityParams P) {
   int* qs = reinterpret_cast<int*>(eG + P.Lcap + 1);               // [Lcap + 1] sectors q_0 .. q_L
   const long long nS = P.bv.B * Q;
   __shared__ int s_next;
+  // start sectors in order of decreasing dimension (the cost of a string grows with the square of it): the heavy strings are
+  // handed out first, the tail of the launch is made of light ones
+  __shared__ short s_qord[kDnMaxQ];
+  const bool ordered = Q <= kDnMaxQ;
+  if (ordered) {
+    for (int q = threadIdx.x; q < Q; q += blockDim.x) {
+      const int d = P.imp.dim[q];
+      int rank = 0;
+      for (int p = 0; p < Q; ++p) { const int dp = P.imp.dim[p]; rank += (dp > d) || (dp == d && p < q); }
+      s_qord[rank] = (short)q;
+    }
+  }
   // candidates are handed out one by one: few of them survive and close, and the survivors differ in length by an order of
   // magnitude -- with a fixed stride the SMs were busy a third of the launch (config 4, profiles/r02_density.md)
   for (;;) {
@@ -120,8 +134,8 @@ __global__ void __launch_bounds__(kLzThreads) density_kernel(DensityParams P) {
     __syncthreads();
     const long long s = s_next;
     if (s >= nS) break;
-    const long long b = s / Q;
-    const int q0 = (int)(s - b * Q);
+    const long long b = ordered ? s % P.bv.B : s / Q;
+    const int q0 = ordered ? (int)s_qord[s / P.bv.B] : (int)(s - b * Q);
     if (P.status[b] != 0) continue;
     const double wr = P.w_mant[2 * b], wi = P.w_mant[2 * b + 1];
     if ((wr == 0.0 && wi == 0.0) || !isfinite(wr) || !isfinite(wi)) continue;
