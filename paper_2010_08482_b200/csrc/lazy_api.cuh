@@ -98,7 +98,7 @@ extern "C" int ctqmc_chains_create(ctqmc_impurity* h, double beta, const ctqmc_c
   ch->lazy_rounds = desc->lazy_rounds < h->dev.Q ? desc->lazy_rounds : h->dev.Q;
   ch->NT = (h->dev.dmax + kLzTile - 1) / kLzTile;
   ch->small = h->dev.dmax <= kLzSmall;
-  V.w_task_cap = (long long)V.nC * V.emax * h->dev.Q;
+  V.w_task_cap = ch->small ? 1 : (long long)V.nC * V.emax * h->dev.Q;      // small impurities never build work lists
   V.w_tile_cap = V.w_task_cap * ch->NT * ch->NT;
   {
     int occ_g = 1, occ_f = 1, sms = 1;
