@@ -90,3 +90,22 @@ def test_density_edge_cases(lib, torch_cuda, impurities):
     for q in range(imp.n_sectors):
         blk = rho1[off2[q]:off2[q + 1]].reshape((int(imp.dims[q]),) * 2, order="F")
         assert np.abs(blk - np.diag(p[off[q]:off[q + 1]] / p.sum())).max() <= 1e-14
+
+
+def test_density_at_bench_size_has_the_weight_sum_as_its_trace(lib, torch_cuda, impurities):
+    """BASELINE's batch of config 2 (4096 configurations, the launch bench.py times): pin D1 -- every contributing configuration
+    adds a matrix of unit trace -- holds at any size, so trace(rho) must equal the sum of the weights of the configurations with
+    status 0 and a non-zero weight; the first 16 configurations are also compared with the oracle element by element."""
+    from oracle import density_oracle as D
+    from workloads import Batch, make_batch
+    imp = impurities(2)
+    n = 4096
+    batch = make_batch(2, n)
+    weight = [1.0 if b % 5 else -1.0 for b in range(n)]
+    rho, status, mant = _run(lib, torch_cuda, imp, batch, weight)
+    wsum = sum(w for b, w in enumerate(weight) if status[b] == 0 and (mant[b] != 0).any())
+    assert abs(_trace_of(imp, rho) - wsum) <= 1e-10 * n
+    head = Batch.from_lists(imp.beta, [batch.config(b) for b in range(16)])
+    rho16, _, _ = _run(lib, torch_cuda, imp, head, weight[:16])
+    want = D.density_batch(imp, head.beta, head.offset, head.symbol, head.tau, weight[:16])
+    assert np.abs(rho16 - want).max() <= 1e-9 * np.abs(want).max()

@@ -267,3 +267,60 @@ def test_chain_set_products_are_logarithmic_and_create_reports_oom(lib, torch_cu
     finally:
         ch.destroy()
         h.free()
+
+
+def test_chain_sets_at_bench_size_agree_with_the_stateless_trace(lib, torch_cuda, impurities):
+    """The launch configuration bench.py times (config 2, 1024 chains, depth 6, leaf capacity 32, two lazy rounds): after loading a
+    BASELINE configuration per chain and three Metropolis rounds of pair moves, the stored root of EVERY chain must equal
+    ctqmc_trace_batch of the host's mirror of its configuration (a path that is itself held to the oracle on every output of config
+    2), and a sample of chains is compared with oracle.trace_oracle directly.  A property that holds at any size."""
+    from oracle import trace_oracle as O
+    from workloads import Batch, apply_move, make_batch, random_pair_move
+    from workloads.rng import Stream
+    torch = torch_cuda
+    imp = impurities(2)
+    beta, nC, nf = imp.beta, 1024, imp.n_symbols // 2
+    h = lib.ctqmc_load_impurity(imp, 0)
+    ch = lib.ctqmc_chains_create(h, beta, nC, 6, leaf_capacity=32, max_edits=8, lazy_rounds=2)
+    try:
+        ops = [_ops_of(make_batch(2, 1, start=c % 64), 0) for c in range(nC)]
+        ones = torch.ones(nC, dtype=torch.int32, device="cuda")
+        for k in range(max((len(s) + 7) // 8 for s in ops)):
+            out = lib.ctqmc_chains_propose(ch, *_edits(torch, [(s[8 * k:8 * k + 8], []) for s in ops]))
+            lib.ctqmc_chains_commit(ch, ones)
+        assert (out["status"] == 0).all().item()
+        rngs = [Stream(880000 + c) for c in range(nC)]
+        n_acc = 0
+        for _ in range(3):
+            moves = [random_pair_move(rngs[c], nf, beta, ops[c]) for c in range(nC)]
+            u = torch.tensor([max(rngs[c].uniform(), 1e-300) for c in range(nC)], dtype=torch.float64, device="cuda")
+            mant, exp2 = lib.ctqmc_chains_trace(ch)
+            thr = torch.log2(torch.hypot(mant[:, 0], mant[:, 1])) + exp2.to(torch.float64) + torch.log2(u)
+            out = lib.ctqmc_chains_propose(ch, *_edits(torch, moves), thr)
+            lib.ctqmc_chains_commit(ch)
+            torch.cuda.synchronize()
+            acc, st = out["accept"].cpu().numpy(), out["status"].cpu().numpy()
+            assert (st == 0).all()
+            for c in range(nC):
+                if acc[c]:
+                    ops[c] = apply_move(ops[c], *moves[c])
+            n_acc += int(acc.sum())
+        assert 0 < n_acc < 3 * nC
+        mant, exp2 = lib.ctqmc_chains_trace(ch)
+        batch = Batch.from_lists(beta, [([a for _, a in s], [t for t, _ in s]) for s in ops])
+        off, sym, tau = (torch.from_numpy(x).cuda() for x in (batch.offset, batch.symbol, batch.tau))
+        m2, e2, _, status = lib.ctqmc_trace_batch(h, beta, off, sym, tau, max_len=int(np.diff(batch.offset).max()))
+        torch.cuda.synchronize()
+        mant, exp2, m2, e2 = mant.cpu().numpy(), exp2.cpu().numpy(), m2.cpu().numpy(), e2.cpu().numpy()
+        assert (status.cpu().numpy() == 0).all()
+        worst = 0.0
+        for c in range(nC):
+            assert m2[c, 0] != 0.0, c                      # an accepted configuration has a non-zero weight
+            worst = max(worst, rel_diff(complex(*mant[c]), int(exp2[c]), complex(*m2[c]), int(e2[c])))
+        assert worst <= TOL, worst
+        for c in range(0, nC, 128):
+            r = _exact(imp, beta, ops[c])
+            assert rel_diff(complex(*mant[c]), int(exp2[c]), r["mant"], r["exp2"]) <= TOL * max(1.0, r["kappa"] * 1e-5), c
+    finally:
+        ch.destroy()
+        h.free()
