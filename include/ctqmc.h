@@ -169,6 +169,11 @@ int ctqmc_trace_batch(ctqmc_impurity* imp, double beta, const ctqmc_batch* batch
  *   bound_mant [B], bound_exp2 [B]                   bound = mant * 2^exp2, mant in [1,2) or 0
  *   sector_bound_mant [B][Q], sector_bound_exp2 [B][Q]   or NULL: B(q0), zero where q0 does not survive
  *   status [B]                                        as for ctqmc_trace_batch
+ *
+ * Conditioning signal: the ratio bound / |w_loc| of the Frobenius bound (norm_kind 0, segment_len 1) to the trace of the same
+ * batch is an upper estimate of the cancellation in the final sector sum and chain products (reading A8: the oracle's
+ * kappa); a caller that sees ratios beyond ~1e6 has lost that many digits of the 1e-9 bar and should label its sectors with every
+ * conserved quantum number.
  */
 int ctqmc_bound_batch(ctqmc_impurity* imp, double beta, const ctqmc_batch* batch, int norm_kind, int segment_len,
                       double* bound_mant, int64_t* bound_exp2, double* sector_bound_mant, int64_t* sector_bound_exp2,
