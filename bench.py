@@ -566,7 +566,7 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         # SURVEY 8(f) rows built beyond the stateless batch path: the incremental lazy trace over many chains (f1, f2) and the
         # density-matrix accumulation (f3), each on a small-sector and a mid-size complex config
         next_rows["lazy_chains"] = {"cfg2": measure_chains(L, torch, 2, 1024, 6, 8, local_rank),
-                                    "cfg4": measure_chains(L, torch, 4, 16, 4, 4, local_rank, leaf_capacity=64)}
+                                    "cfg4": measure_chains(L, torch, 4, 16, 5, 4, local_rank, leaf_capacity=32)}
         next_rows["split_precision"] = measure_split(L, torch, 64, 3, local_rank, pk)
         next_rows["density"] = {"cfg2": measure_density(L, torch, 2, 4096, 3, local_rank),
                                 "cfg4": measure_density(L, torch, 4, 64, 2, local_rank)}
