@@ -297,13 +297,36 @@ template <bool CPLX>
 __device__ double lz_fix_tile(double* Mx, int ld, int rows, int cols, int m0, int n0, int k, LzRowScale rs, double* red) {
   constexpr int ES = CPLX ? 2 : 1;
   double ss = 0.0;
-  for (int idx = threadIdx.x; idx < kLzTile * kLzTile; idx += blockDim.x) {
-    const int r = m0 + (idx & (kLzTile - 1)), c = n0 + idx / kLzTile;
-    if (r < rows && c < cols) {
-      const int sh = (rs.on ? row_exp(prop_x(rs.delta, rs.E[r], rs.emin)) : 0) - k;
-      double* p = Mx + ((long long)c * ld + r) * ES;
-      const double vr = lz_scale(p[0], sh); p[0] = vr; ss += vr * vr;
-      if (CPLX) { const double vi = lz_scale(p[1], sh); p[1] = vi; ss += vi * vi; }
+  // blockDim.x is a multiple of the tile height: a thread stays on one row, whose shift is computed once
+  const int r_fixed = m0 + (threadIdx.x & (kLzTile - 1));
+  const int sh_fixed = ((rs.on && r_fixed < rows) ? row_exp(prop_x(rs.delta, rs.E[r_fixed], rs.emin)) : 0) - k;
+  // eight loads in flight per thread (a load-scale-store loop waits for every load: the stores may alias the next load)
+  constexpr int kBatch = 8;
+  const int r = r_fixed;
+  for (int c0 = n0 + (int)(threadIdx.x / kLzTile); c0 < n0 + kLzTile; c0 += kBatch * (int)(blockDim.x / kLzTile)) {
+    double vr[kBatch], vi[kBatch];
+#pragma unroll
+    for (int u = 0; u < kBatch; ++u) {
+      const int c = c0 + u * (int)(blockDim.x / kLzTile);
+      vr[u] = 0.0; vi[u] = 0.0;
+      if (r < rows && c < cols && c < n0 + kLzTile) {
+        const double* p = Mx + ((long long)c * ld + r) * ES;
+        if (CPLX) { const double2 z = *reinterpret_cast<const double2*>(p); vr[u] = z.x; vi[u] = z.y; } else vr[u] = p[0];
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < kBatch; ++u) {
+      const int c = c0 + u * (int)(blockDim.x / kLzTile);
+      if (r < rows && c < cols && c < n0 + kLzTile) {
+        double* p = Mx + ((long long)c * ld + r) * ES;
+        const double xr = lz_scale(vr[u], sh_fixed);
+        ss += xr * xr;
+        if (CPLX) {
+          const double xi = lz_scale(vi[u], sh_fixed);
+          ss += xi * xi;
+          *reinterpret_cast<double2*>(p) = make_double2(xr, xi);
+        } else p[0] = xr;
+      }
     }
   }
   return lz_block_sum(ss, red);
