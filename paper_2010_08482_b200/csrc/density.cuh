@@ -37,32 +37,76 @@ __host__ __device__ inline long long density_slot_doubles(int dmax, int Lcap, in
   return (long long)Lcap * mat + 5 * mat + 2LL * (Lcap + 2);      // G_i, X ping-pong, Y ping-pong, C, exponents + sectors
 }
 
-// dst = diag(2^x) src brought to a common exponent (reading A5); returns that exponent (INT_MIN: src vanishes)
+// dst = diag(2^x) src brought to a common exponent (reading A5); returns that exponent (INT_MIN: src vanishes).  The mantissa and
+// the exponent of every row's propagator factor are computed once per row into `rowm` / `rowk` (shared memory, >= rows entries:
+// the kernel lends the operand stage of its product tile), and the scaling pass keeps four loads in flight per thread (a
+// load-scale-store loop is serialised by the possible aliasing of its stores with the next load).
 template <bool CPLX>
 __device__ int dn_propagate(const double* src, double* dst, int ld, int rows, int cols, double delta, const double* E, double emin,
-                            int* redi) {
+                            int* redi, double* rowm, int* rowk) {
   constexpr int ES = CPLX ? 2 : 1;
+  const int n = rows * cols;
+  if (n <= (int)blockDim.x) {          // small impurities: one element per thread, nothing to amortise
+    const int r = threadIdx.x % rows, c = threadIdx.x / rows;
+    const bool on = (int)threadIdx.x < n;
+    double vr = 0.0, vi = 0.0, m = 1.0;
+    int kr = 0, km = INT_MIN;
+    if (on) {
+      const double* p = src + ((long long)c * ld + r) * ES;
+      vr = p[0]; if (CPLX) vi = p[1];
+      const double x = prop_x(delta, E[r], emin);
+      m = exp2(__dsub_rn(x, floor(x))); kr = row_exp(x);
+      const double mx = CPLX ? fmax(fabs(vr), fabs(vi)) : fabs(vr);
+      if (mx > 0.0) km = kr + ilogb(mx * m);
+    }
+    km = lz_block_max(km, redi);
+    const int k = km == INT_MIN ? 0 : km;
+    if (on) {
+      double* o = dst + ((long long)c * ld + r) * ES;
+      o[0] = lz_scale(vr * m, kr - k);
+      if (CPLX) o[1] = lz_scale(vi * m, kr - k);
+    }
+    __syncthreads();
+    return km;
+  }
+  __syncthreads();
+  for (int r = threadIdx.x; r < rows; r += blockDim.x) {
+    const double x = prop_x(delta, E[r], emin);
+    rowm[r] = exp2(__dsub_rn(x, floor(x))); rowk[r] = row_exp(x);
+  }
+  __syncthreads();
   int km = INT_MIN;
-  for (int idx = threadIdx.x; idx < rows * cols; idx += blockDim.x) {
+  for (int idx = threadIdx.x; idx < n; idx += blockDim.x) {
     const int r = idx % rows, c = idx / rows;
     const double* p = src + ((long long)c * ld + r) * ES;
     const double mx = CPLX ? fmax(fabs(p[0]), fabs(p[1])) : fabs(p[0]);
-    if (mx > 0.0) {
-      const double x = prop_x(delta, E[r], emin);
-      km = max(km, row_exp(x) + ilogb(mx * exp2(__dsub_rn(x, floor(x)))));
-    }
+    if (mx > 0.0) km = max(km, rowk[r] + ilogb(mx * rowm[r]));
   }
   km = lz_block_max(km, redi);
   const int k = km == INT_MIN ? 0 : km;
-  for (int idx = threadIdx.x; idx < rows * cols; idx += blockDim.x) {
-    const int r = idx % rows, c = idx / rows;
-    const double x = prop_x(delta, E[r], emin);
-    const double m = exp2(__dsub_rn(x, floor(x)));
-    const int sh = row_exp(x) - k;
-    const double* p = src + ((long long)c * ld + r) * ES;
-    double* o = dst + ((long long)c * ld + r) * ES;
-    o[0] = lz_scale(p[0] * m, sh);
-    if (CPLX) o[1] = lz_scale(p[1] * m, sh);
+  constexpr int kBatch = 4;
+  for (int idx0 = threadIdx.x; idx0 < n; idx0 += kBatch * blockDim.x) {
+    double vr[kBatch], vi[kBatch];
+#pragma unroll
+    for (int u = 0; u < kBatch; ++u) {
+      const int idx = idx0 + u * blockDim.x;
+      vr[u] = 0.0; vi[u] = 0.0;
+      if (idx < n) {
+        const double* p = src + ((long long)(idx / rows) * ld + idx % rows) * ES;
+        vr[u] = p[0]; if (CPLX) vi[u] = p[1];
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < kBatch; ++u) {
+      const int idx = idx0 + u * blockDim.x;
+      if (idx < n) {
+        const int r = idx % rows;
+        const int sh = rowk[r] - k;
+        double* o = dst + ((long long)(idx / rows) * ld + r) * ES;
+        o[0] = lz_scale(vr[u] * rowm[r], sh);
+        if (CPLX) o[1] = lz_scale(vi[u] * rowm[r], sh);
+      }
+    }
   }
   __syncthreads();
   return km;
@@ -72,11 +116,25 @@ __device__ int dn_propagate(const double* src, double* dst, int ld, int rows, in
 template <bool CPLX>
 __device__ void dn_rescale(double* Mx, int ld, int rows, int cols, int k) {
   constexpr int ES = CPLX ? 2 : 1;
-  for (int idx = threadIdx.x; idx < rows * cols; idx += blockDim.x) {
-    const int r = idx % rows, c = idx / rows;
-    double* p = Mx + ((long long)c * ld + r) * ES;
-    p[0] = lz_scale(p[0], -k);
-    if (CPLX) p[1] = lz_scale(p[1], -k);
+  const int n = rows * cols;
+  constexpr int kBatch = 4;
+  for (int idx0 = threadIdx.x; idx0 < n; idx0 += kBatch * blockDim.x) {
+    double vr[kBatch], vi[kBatch];
+#pragma unroll
+    for (int u = 0; u < kBatch; ++u) {
+      const int idx = idx0 + u * blockDim.x;
+      vr[u] = 0.0; vi[u] = 0.0;
+      if (idx < n) { const double* p = Mx + ((long long)(idx / rows) * ld + idx % rows) * ES; vr[u] = p[0]; if (CPLX) vi[u] = p[1]; }
+    }
+#pragma unroll
+    for (int u = 0; u < kBatch; ++u) {
+      const int idx = idx0 + u * blockDim.x;
+      if (idx < n) {
+        double* p = Mx + ((long long)(idx / rows) * ld + idx % rows) * ES;
+        p[0] = lz_scale(vr[u], -k);
+        if (CPLX) p[1] = lz_scale(vi[u], -k);
+      }
+    }
   }
   __syncthreads();
 }
@@ -103,6 +161,11 @@ __global__ void __launch_bounds__(kLzThreads) density_kernel(DensityParams P) {
   constexpr int ES = CPLX ? 2 : 1;
   __shared__ LzSmem<CPLX> S;
   __shared__ int s_k, s_ok, redi[32];
+  // per-row propagator factors of dn_propagate live in the operand stage of the product tile (idle between products):
+  // kLzMaxDim doubles + kLzMaxDim ints = 6 KB of its 10 KB
+  static_assert(sizeof(S.A[0]) >= kLzMaxDim * (sizeof(double) + sizeof(int)), "row table does not fit the operand stage");
+  double* rowm = &S.A[0][0][0];
+  int* rowk = reinterpret_cast<int*>(rowm + kLzMaxDim);
   const int Q = P.imp.Q, ld = P.ldm;
   const long long mat = (long long)ld * ld * ES;
   double* base = P.scratch + (size_t)blockIdx.x * P.slot_doubles;
@@ -192,7 +255,7 @@ __global__ void __launch_bounds__(kLzThreads) density_kernel(DensityParams P) {
       double* Gi = Gs + (long long)i * mat;
       dn_gemm<CPLX>(S, bd.rows, d0, bd.cols, P.imp.store + bd.off, bd.ld, 1, X, ld, 1, Gi, ld, &s_k);
       if (threadIdx.x == 0) eG[i] = ex;
-      const int k = dn_propagate<CPLX>(Gi, Xn, ld, bd.rows, d0, delta, P.imp.energy + P.imp.e_off[qn], P.imp.e_min[qn], redi);
+      const int k = dn_propagate<CPLX>(Gi, Xn, ld, bd.rows, d0, delta, P.imp.energy + P.imp.e_off[qn], P.imp.e_min[qn], redi, rowm, rowk);
       if (k == INT_MIN) { dead = true; break; }
       ex += k;
       lg += -delta * P.imp.e_min[qn] * kLog2e;
@@ -233,7 +296,7 @@ __global__ void __launch_bounds__(kLzThreads) density_kernel(DensityParams P) {
       }
       __syncthreads();
       if (i == 0) break;
-      const int k1 = dn_propagate<CPLX>(Y, Y, ld, dn, d0, delta, E, emin, redi);
+      const int k1 = dn_propagate<CPLX>(Y, Y, ld, dn, d0, delta, E, emin, redi, rowm, rowk);
       if (k1 == INT_MIN) break;                                     // nothing left to carry back
       ey += k1;
       // Y_{i-1}^T = F_i^T Y': F_i is row-major (dim q_i x dim q_{i-1}), its transpose has row stride 1 and column stride ld
